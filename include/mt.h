@@ -1,0 +1,193 @@
+/*
+ * mt.h — C-ABI of libmagtile: the data-parallel hot path of MagTense (arxiv 2107.05364) on B200.
+ *
+ * Citations are `/root/reference/PAPER.md` line numbers + section / equation; formulas the paper
+ * only cites (Smith 2010, Nielsen 2019, refs PAPER.md:286-287) are those derived in
+ * SURVEY.md Appendix A and restated in DESIGN.md.
+ *
+ * Conventions (all entry points)
+ *  - Return value: 0 (MT_OK) or a negative MT_ERR_* code.  Nothing throws or aborts across the
+ *    ABI.  `mt_last_error(ctx)` returns a ctx-owned, NUL-terminated description of the last
+ *    failure (valid until the next failing call on that ctx).
+ *  - Unless a parameter is documented as HOST, every array pointer is a DEVICE pointer owned by
+ *    the caller (e.g. a torch tensor's data_ptr()); the library never frees or retains it beyond
+ *    the call.  The library owns only small workspaces inside `mt_ctx` (staged magnetisation,
+ *    Runge-Kutta stages, reduction scratch), released by mt_destroy.
+ *  - All work is enqueued on the ctx's stream (a `cudaStream_t` passed as void*, e.g.
+ *    torch.cuda.current_stream().cuda_stream; NULL = legacy default stream).  Calls are
+ *    ASYNCHRONOUS with respect to the host except mt_integrate and the *_host variants, which
+ *    synchronise the stream before returning.
+ *  - Layouts.  Vectors are structure-of-arrays fp64 `[B][3][n]` (B = batch of independent
+ *    magnetisation states, component-major, tile index fastest).  The tensor is six planes
+ *    `[6][n_rows][ld]` of MT_F32 or MT_F64 elements in component order xx, xy, xz, yy, yz, zz;
+ *    row i = TARGET tile (field point = its centre), column j = SOURCE tile;
+ *    ld >= n is the row pitch in elements and must make rows 16-byte aligned (ld % 4 == 0 for
+ *    MT_F32, ld % 2 == 0 for MT_F64); the base pointer must be 16-byte aligned.  Index arithmetic
+ *    is 64-bit throughout (a plane of n = 65,536 has 2^32 elements).
+ *  - There is no CPU fallback: every entry point fails with MT_ERR_CUDA when no device is usable.
+ */
+#ifndef MT_H_
+#define MT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- error codes ------------------------------------------------------------------------------ */
+#define MT_OK 0
+#define MT_ERR_INVALID_ARG (-1)       /* null / misaligned pointer, ld < n, n <= 0, bad dtype, batch < 1 */
+#define MT_ERR_CUDA (-2)              /* launch / allocation failure; text in mt_last_error            */
+#define MT_ERR_SINGULAR_GEOMETRY (-3) /* reserved for callers that read *status_flag (see assembly)    */
+#define MT_ERR_STEP_UNDERFLOW (-4)    /* DP45 step size fell below 16 ulp of t                          */
+#define MT_ERR_MAX_STEPS (-5)         /* integrator hit max_steps before t_end                          */
+#define MT_ERR_UNIMPLEMENTED (-6)
+
+/* ---- element types of the stored tensor ("stored as a float (4 byte)") ---------- */
+#define MT_F32 0
+#define MT_F64 1
+
+/* ---- integrator methods ------------------------------------------------------------------------ */
+#define MT_RK4 0  /* classical fixed-step Runge-Kutta (BASELINE.json config 2)                          */
+#define MT_DP45 1 /* Dormand-Prince 5(4): "explicit Runge-Kutta (4,5)" PAPER.md:143, "ODE45" :181       */
+
+typedef struct mt_ctx mt_ctx;
+
+/* Create a context bound to CUDA device `device` and stream `cuda_stream` (HOST call).
+ * *out receives the handle.  Errors: MT_ERR_INVALID_ARG (out == NULL), MT_ERR_CUDA.              */
+int mt_create(mt_ctx** out, int device, void* cuda_stream);
+
+/* Synchronise the stream, free all workspaces and the context.  NULL is accepted.                */
+int mt_destroy(mt_ctx* ctx);
+
+/* Description of the last error on this ctx ("" if none).  NULL ctx returns a static string.     */
+const char* mt_last_error(const mt_ctx* ctx);
+
+/* Library version string and the SM architecture the kernels were compiled for ("sm_100a").      */
+const char* mt_version(void);
+
+/* ---- A0. Tile-geometry buffer ("subdivides the region into N tiles"; PAPER.md:126
+ * cuboid or tetrahedron; PAPER.md:27 space-dependent Ms).  DEVICE pointers, caller-owned.         */
+typedef struct {
+  int64_t n;             /* number of tiles                                                        */
+  const int32_t* type;   /* [n]     0 = axis-aligned cuboid, 1 = tetrahedron                       */
+  const double* center;  /* [n][3]  evaluation point: cuboid centre / tetrahedron centroid         */
+  const double* size;    /* [n][3]  full edge lengths (cuboids; ignored for tetrahedra)            */
+  const double* verts;   /* [n][4][3] tetrahedron vertices, any orientation (ignored for cuboids);
+                            may be NULL when no tile has type 1                                    */
+  const double* Ms;      /* [n]     saturation magnetisation per tile (not used by assembly)       */
+} mt_tiles;
+
+/* ---- A1-A3. Analytic assembly of the demagnetisation tensor (Eq. 9 PAPER.md:78;
+ * "computed only once, at the beginning of the simulation" PAPER.md:143).
+ * Writes rows [row_begin, row_end) : out[c][i - row_begin][j] = N^{c}_{ij}, the field at the
+ * centre of tile i of tile j carrying unit uniform magnetisation, H = -N.M, evaluated from the
+ * closed forms in fp64 for EVERY pair (no translation-invariance shortcut) and rounded to nearest
+ * when dtype == MT_F32.  The band form is the multi-GPU shard unit and lets n = 65,536 be checked
+ * in slices.  `out` is [6][row_end-row_begin][ld].
+ * status_flag (DEVICE int32, may be NULL): OR-ed with 1 if any block came out non-finite — a
+ * target centre lying on a source face or edge segment (genuine singularity, Q8); the
+ * caller zeroes it before and reads it after synchronising.
+ * Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA.                                                        */
+int mt_assemble_tensor(mt_ctx* ctx, const mt_tiles* tiles, int dtype, int64_t row_begin,
+                       int64_t row_end, void* out, int64_t ld, int32_t* status_flag);
+
+/* ---- A4 / A7. Demagnetising field (Eq. 9 PAPER.md:78 with the sign and Ms reading DESIGN.md Q1;
+ * "the most time consuming part" PAPER.md:17,122,138; moved to CUDA PAPER.md:145,223):
+ *     Hd[b][a][i] = - sum_j sum_c N^{ac}_{ij} Ms[j] m[b][c][j],   i in [0, n_rows)
+ * N is [6][n_rows][ld] (n_rows == n for the full tensor; a row band gives the band's field),
+ * Ms [n], m [batch][3][n], Hd [batch][3][n_rows], 1 <= batch <= 8.  For MT_F32 the product
+ * Ms*m is rounded to fp32 once, products are fp32 and accumulation is fp32 over at most 128
+ * consecutive terms per lane then fp64 (Q19); for MT_F64 everything is fp64.  The
+ * reduction order is fixed: results are bitwise reproducible run to run.
+ * Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA.                                                        */
+int mt_demag_field(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                   const double* Ms, const double* m, int batch, double* Hd);
+
+/* Same operation with HOST vectors: m_host -> device, field, Hd -> Hd_host, stream synchronised
+ * before returning (the end-to-end path bench.py times).  N and Ms stay DEVICE pointers (the
+ * tensor is assembled on the device and never leaves it).  Pinned host memory recommended.       */
+int mt_demag_field_host(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows,
+                        int64_t ld, const double* Ms, const double* m_host, int batch,
+                        double* Hd_host);
+
+/* ---- A5 / A6. Effective field and Landau-Lifshitz right-hand side ------------------------------
+ * H_eff = H_d + H_exch + H_anis + H_a                                   (Eq. 17)
+ *   H_exch,i = c_ex,i * sum_{dir} (m_{i+} - 2 m_i + m_{i-}) * inv_d2[dir]   (Eq. 12 PAPER.md:94;
+ *              3-point stencil PAPER.md:181; a missing neighbour (-1) is replaced by m_i:
+ *              Neumann, Eq. 3)
+ *   H_anis,i = c_an,i (m_i . e_i) e_i                                    (Eq. 16)
+ *   H_a                                                                   (Eq. 7,  PAPER.md:70)
+ * dm/dt = -gamma m x H_eff - alpha_ll m x (m x H_eff)                    (Eq. 1,  PAPER.md:33)
+ * gamma and alpha_ll are the two prefactors exactly as written in Eq. 1 (Q5).
+ * A NULL array pointer selects the scalar / constant beside it; nbr == NULL disables exchange;
+ * N == NULL disables the demagnetising term.  The tensor must be square here (n rows).           */
+typedef struct {
+  int64_t n;
+  const void* N;         /* [6][n][ld] or NULL                                                     */
+  int dtype;             /* MT_F32 | MT_F64                                                        */
+  int64_t ld;
+  const double* Ms;      /* [n]                                                                    */
+  const int32_t* nbr;    /* [n][6]  -x,+x,-y,+y,-z,+z neighbour index or -1; NULL = no exchange    */
+  double inv_d2[3];      /* 1/dx^2, 1/dy^2, 1/dz^2                                                 */
+  const double* c_ex;    /* [n] 2A/(mu0 Ms) per tile, or NULL -> c_ex_scalar                       */
+  double c_ex_scalar;
+  const double* c_an;    /* [n] 2K/(mu0 Ms) per tile, or NULL -> c_an_scalar                       */
+  double c_an_scalar;
+  const double* easy;    /* [n][3] unit easy axes, or NULL -> easy_const                           */
+  double easy_const[3];
+  const double* H_a;     /* [n][3] applied field, or NULL -> H_a_const                             */
+  double H_a_const[3];
+  double gamma, alpha_ll;
+  const double* vol;     /* [n] tile volumes: weights of <m> (A10); NULL = plain mean              */
+} mt_problem;
+
+/* dmdt[b][3][n] (required) and Heff[b][3][n] (optional, NULL to skip) for m[b][3][n].
+ * Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA.                                                        */
+int mt_llg_rhs(mt_ctx* ctx, const mt_problem* prob, const double* m, int batch, double* dmdt,
+               double* Heff_or_null);
+
+/* ---- A8-A10. Time integration ("explicit Runge-Kutta (4,5)" PAPER.md:143; RK4 per BASELINE
+ * config 2; observables <m>(t) as plotted in Fig. 6).                               */
+typedef struct {
+  int method;            /* MT_RK4 | MT_DP45                                                       */
+  double dt;             /* RK4: the step; DP45: initial step (<= 0: 1e-3)                         */
+  double t_end;
+  int64_t max_steps;     /* <= 0: unlimited                                                        */
+  double rtol, atol;     /* DP45: err = max |e| / (atol + rtol max(|m|, |m_new|)), accept if <= 1  */
+  double torque_tol;     /* stop when max_i |m_i x H_eff,i| <= torque_tol (Eq. 2);
+                            <= 0: off                                                              */
+  int renormalize;       /* 1: m_i <- m_i/|m_i| after every (accepted) step (Q10)        */
+  int64_t sample_every;  /* RK4: write a sample every k steps (0: never)                           */
+  double sample_dt;      /* DP45: land exactly on t0 + k*sample_dt and sample there (0: never)     */
+} mt_integrator_opts;
+
+typedef struct {
+  int64_t accepted, rejected, rhs_calls, n_samples;
+  double t, dt_last, max_torque;
+} mt_integrator_result;
+
+/* Advance m_inout[batch][3][n] (DEVICE) from *t_inout (HOST) towards opts->t_end.  All states of
+ * the batch share the step sequence.  samples (DEVICE, may be NULL) is [sample_cap][1+3*batch]:
+ * t, then <m_x>,<m_y>,<m_z> per state.  host_out (HOST) receives the counters.  Synchronises the
+ * stream before returning.  Resumable: (m, t, dt_last) is the whole state.
+ * Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA, MT_ERR_STEP_UNDERFLOW, MT_ERR_MAX_STEPS (the state
+ * reached so far is still written back).                                                          */
+int mt_integrate(mt_ctx* ctx, const mt_problem* prob, const mt_integrator_opts* opts,
+                 double* m_inout, int batch, double* t_inout, double* samples, int64_t sample_cap,
+                 mt_integrator_result* host_out);
+
+/* ---- instrumentation --------------------------------------------------------------------------- */
+/* Number of kernels this ctx has launched since creation (bench.py's gpu_launches).              */
+int64_t mt_launch_count(const mt_ctx* ctx);
+
+/* Tuning / A-B testing hook: selects the demag kernel variant (0 = default choice by shape,
+ * 1 = register-streaming LDG kernel, 2 = TMA bulk-tensor pipeline).  Returns MT_OK or
+ * MT_ERR_INVALID_ARG.  Results of all variants agree to rounding; each is deterministic.          */
+int mt_set_demag_variant(mt_ctx* ctx, int variant);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MT_H_ */

@@ -1,0 +1,282 @@
+"""Thin ctypes binding of libmagtile.so — same names as include/mt.h, argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels behind the C-ABI; this module only turns torch
+tensors into device pointers and fills the C structs.  PyTorch is used for device memory and
+streams, nothing else.  There is no fallback: importing works without a GPU (so that the symbol
+check can run on CPU), but `load()` raises if the library is missing and `mt_create` raises if no
+CUDA device is usable.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libmagtile.so")
+
+MT_OK = 0
+MT_ERR_INVALID_ARG, MT_ERR_CUDA, MT_ERR_SINGULAR_GEOMETRY = -1, -2, -3
+MT_ERR_STEP_UNDERFLOW, MT_ERR_MAX_STEPS, MT_ERR_UNIMPLEMENTED = -4, -5, -6
+MT_F32, MT_F64 = 0, 1
+MT_RK4, MT_DP45 = 0, 1
+COMPONENTS = ("xx", "xy", "xz", "yy", "yz", "zz")
+EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assemble_tensor",
+           "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_launch_count",
+           "mt_set_demag_variant")
+
+
+class MtError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"libmagtile error {code}: {msg}")
+        self.code = code
+
+
+class _Tiles(C.Structure):
+    _fields_ = [("n", C.c_int64), ("type", C.c_void_p), ("center", C.c_void_p), ("size", C.c_void_p),
+                ("verts", C.c_void_p), ("Ms", C.c_void_p)]
+
+
+class _Problem(C.Structure):
+    _fields_ = [
+        ("n", C.c_int64), ("N", C.c_void_p), ("dtype", C.c_int), ("ld", C.c_int64), ("Ms", C.c_void_p),
+        ("nbr", C.c_void_p), ("inv_d2", C.c_double * 3),
+        ("c_ex", C.c_void_p), ("c_ex_scalar", C.c_double),
+        ("c_an", C.c_void_p), ("c_an_scalar", C.c_double),
+        ("easy", C.c_void_p), ("easy_const", C.c_double * 3),
+        ("H_a", C.c_void_p), ("H_a_const", C.c_double * 3),
+        ("gamma", C.c_double), ("alpha_ll", C.c_double), ("vol", C.c_void_p),
+    ]
+
+
+class _Opts(C.Structure):
+    _fields_ = [
+        ("method", C.c_int), ("dt", C.c_double), ("t_end", C.c_double), ("max_steps", C.c_int64),
+        ("rtol", C.c_double), ("atol", C.c_double), ("torque_tol", C.c_double),
+        ("renormalize", C.c_int), ("sample_every", C.c_int64), ("sample_dt", C.c_double),
+    ]
+
+
+class _Result(C.Structure):
+    _fields_ = [("accepted", C.c_int64), ("rejected", C.c_int64), ("rhs_calls", C.c_int64),
+                ("n_samples", C.c_int64), ("t", C.c_double), ("dt_last", C.c_double),
+                ("max_torque", C.c_double)]
+
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """dlopen the in-tree library; fails loudly when it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: run `python -m paper_2107_05364_b200.build` "
+                              "(there is no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        lib.mt_last_error.restype = C.c_char_p
+        lib.mt_last_error.argtypes = [C.c_void_p]
+        lib.mt_version.restype = C.c_char_p
+        lib.mt_launch_count.restype = C.c_int64
+        lib.mt_launch_count.argtypes = [C.c_void_p]
+        lib.mt_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_void_p]
+        lib.mt_destroy.argtypes = [C.c_void_p]
+        lib.mt_set_demag_variant.argtypes = [C.c_void_p, C.c_int]
+        lib.mt_assemble_tensor.argtypes = [C.c_void_p, C.POINTER(_Tiles), C.c_int, C.c_int64, C.c_int64,
+                                           C.c_void_p, C.c_int64, C.c_void_p]
+        lib.mt_demag_field.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64,
+                                       C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
+        lib.mt_demag_field_host.argtypes = lib.mt_demag_field.argtypes
+        lib.mt_llg_rhs.argtypes = [C.c_void_p, C.POINTER(_Problem), C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
+        lib.mt_integrate.argtypes = [C.c_void_p, C.POINTER(_Problem), C.POINTER(_Opts), C.c_void_p, C.c_int,
+                                     C.POINTER(C.c_double), C.c_void_p, C.c_int64, C.POINTER(_Result)]
+        _lib = lib
+    return _lib
+
+
+def _ptr(t, dtype=None):
+    """Device (or pinned host) pointer of a contiguous torch tensor; None -> NULL."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if not t.is_contiguous():
+        raise ValueError("tensor must be contiguous")
+    if dtype is not None and t.dtype != dtype:
+        raise ValueError(f"expected {dtype}, got {t.dtype}")
+    return t.data_ptr()
+
+
+def torch_dtype(dtype: int):
+    return torch.float32 if dtype == MT_F32 else torch.float64
+
+
+class Context:
+    """Owns an mt_ctx bound to a device and a torch stream."""
+
+    def __init__(self, device: int = 0, stream: torch.cuda.Stream | None = None):
+        if not torch.cuda.is_available():
+            raise MtError(MT_ERR_CUDA, "no CUDA device: libmagtile has no CPU fallback")
+        self.lib = load()
+        self.device = device
+        self.stream = stream if stream is not None else torch.cuda.current_stream(device)
+        h = C.c_void_p()
+        rc = self.lib.mt_create(C.byref(h), device, C.c_void_p(self.stream.cuda_stream))
+        if rc != MT_OK:
+            raise MtError(rc, "mt_create failed")
+        self.h = h
+
+    def check(self, rc: int, allow=()):
+        if rc != MT_OK and rc not in allow:
+            raise MtError(rc, self.lib.mt_last_error(self.h).decode())
+        return rc
+
+    def close(self):
+        if getattr(self, "h", None):
+            self.lib.mt_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def launches(self) -> int:
+        return int(self.lib.mt_launch_count(self.h))
+
+
+def mt_create(device: int = 0, stream=None) -> Context:
+    return Context(device, stream)
+
+
+def mt_destroy(ctx: Context):
+    ctx.close()
+
+
+def mt_version() -> str:
+    return load().mt_version().decode()
+
+
+def mt_launch_count(ctx: Context) -> int:
+    return ctx.launches
+
+
+def mt_set_demag_variant(ctx: Context, variant: int):
+    ctx.check(ctx.lib.mt_set_demag_variant(ctx.h, variant))
+
+
+@dataclass
+class Tiles:
+    """A0: device-resident tile geometry (torch tensors on the ctx's device)."""
+    type: torch.Tensor      # [n] int32
+    center: torch.Tensor    # [n, 3] float64
+    size: torch.Tensor      # [n, 3] float64
+    verts: torch.Tensor | None  # [n, 4, 3] float64 or None
+    Ms: torch.Tensor        # [n] float64
+
+    @property
+    def n(self) -> int:
+        return int(self.type.shape[0])
+
+    def _c(self) -> _Tiles:
+        return _Tiles(self.n, _ptr(self.type, torch.int32), _ptr(self.center, torch.float64),
+                      _ptr(self.size, torch.float64), _ptr(self.verts, torch.float64),
+                      _ptr(self.Ms, torch.float64))
+
+
+def mt_assemble_tensor(ctx: Context, tiles: Tiles, dtype: int, row_begin: int, row_end: int,
+                       out: torch.Tensor, ld: int, status_flag: torch.Tensor | None = None):
+    """out: [6, row_end-row_begin, ld] tensor of the matching dtype on the device."""
+    t = tiles._c()
+    ctx.check(ctx.lib.mt_assemble_tensor(ctx.h, C.byref(t), dtype, row_begin, row_end,
+                                         _ptr(out, torch_dtype(dtype)), ld, _ptr(status_flag, torch.int32)))
+
+
+def mt_demag_field(ctx: Context, N: torch.Tensor, dtype: int, n: int, n_rows: int, ld: int,
+                   Ms: torch.Tensor, m: torch.Tensor, batch: int, Hd: torch.Tensor):
+    ctx.check(ctx.lib.mt_demag_field(ctx.h, _ptr(N, torch_dtype(dtype)), dtype, n, n_rows, ld,
+                                     _ptr(Ms, torch.float64), _ptr(m, torch.float64), batch,
+                                     _ptr(Hd, torch.float64)))
+
+
+def mt_demag_field_host(ctx: Context, N: torch.Tensor, dtype: int, n: int, n_rows: int, ld: int,
+                        Ms: torch.Tensor, m_host: torch.Tensor, batch: int, Hd_host: torch.Tensor):
+    """m_host / Hd_host are HOST tensors (pinned recommended); synchronises before returning."""
+    if m_host.is_cuda or Hd_host.is_cuda:
+        raise ValueError("mt_demag_field_host takes host tensors")
+    ctx.check(ctx.lib.mt_demag_field_host(ctx.h, _ptr(N, torch_dtype(dtype)), dtype, n, n_rows, ld,
+                                          _ptr(Ms, torch.float64), _ptr(m_host, torch.float64), batch,
+                                          _ptr(Hd_host, torch.float64)))
+
+
+@dataclass
+class Problem:
+    """mt_problem: tensor + local-term parameters.  Scalars or device tensors for c_ex, c_an;
+    3-vectors or [n, 3] device tensors for easy, H_a."""
+    n: int
+    Ms: torch.Tensor
+    N: torch.Tensor | None = None
+    dtype: int = MT_F32
+    ld: int = 0
+    nbr: torch.Tensor | None = None
+    inv_d2: tuple = (0.0, 0.0, 0.0)
+    c_ex: object = 0.0
+    c_an: object = 0.0
+    easy: object = (0.0, 0.0, 1.0)
+    H_a: object = (0.0, 0.0, 0.0)
+    gamma: float = 1.0
+    alpha_ll: float = 0.0
+    vol: torch.Tensor | None = None
+
+    def _c(self) -> _Problem:
+        s = _Problem()
+        s.n = self.n
+        s.N = _ptr(self.N, torch_dtype(self.dtype)) if self.N is not None else None
+        s.dtype, s.ld = self.dtype, self.ld
+        s.Ms = _ptr(self.Ms, torch.float64)
+        s.nbr = _ptr(self.nbr, torch.int32)
+        s.inv_d2 = (C.c_double * 3)(*self.inv_d2)
+        for name in ("c_ex", "c_an"):
+            v = getattr(self, name)
+            if isinstance(v, torch.Tensor):
+                setattr(s, name, _ptr(v, torch.float64))
+            else:
+                setattr(s, name, None)
+                setattr(s, name + "_scalar", float(v))
+        for name in ("easy", "H_a"):
+            v = getattr(self, name)
+            if isinstance(v, torch.Tensor):
+                setattr(s, name, _ptr(v, torch.float64))
+            else:
+                setattr(s, name, None)
+                setattr(s, name + "_const", (C.c_double * 3)(*[float(x) for x in v]))
+        s.gamma, s.alpha_ll = float(self.gamma), float(self.alpha_ll)
+        s.vol = _ptr(self.vol, torch.float64)
+        return s
+
+
+def mt_llg_rhs(ctx: Context, prob: Problem, m: torch.Tensor, batch: int, dmdt: torch.Tensor,
+               heff: torch.Tensor | None = None):
+    p = prob._c()
+    ctx.check(ctx.lib.mt_llg_rhs(ctx.h, C.byref(p), _ptr(m, torch.float64), batch,
+                                 _ptr(dmdt, torch.float64), _ptr(heff, torch.float64)))
+
+
+def mt_integrate(ctx: Context, prob: Problem, m: torch.Tensor, batch: int, t0: float, *, method: int,
+                 dt: float, t_end: float, max_steps: int = 0, rtol: float = 1e-6, atol: float = 1e-8,
+                 torque_tol: float = 0.0, renormalize: bool = True, sample_every: int = 0,
+                 sample_dt: float = 0.0, samples: torch.Tensor | None = None, allow=()):
+    """Advances m in place; returns (t, result dict, return code)."""
+    p = prob._c()
+    o = _Opts(method, dt, t_end, max_steps, rtol, atol, torque_tol, int(renormalize), sample_every, sample_dt)
+    res = _Result()
+    t = C.c_double(t0)
+    cap = int(samples.shape[0]) if samples is not None else 0
+    rc = ctx.check(ctx.lib.mt_integrate(ctx.h, C.byref(p), C.byref(o), _ptr(m, torch.float64), batch,
+                                        C.byref(t), _ptr(samples, torch.float64), cap, C.byref(res)),
+                   allow=allow)
+    return t.value, {k: getattr(res, k) for k, _ in _Result._fields_}, rc

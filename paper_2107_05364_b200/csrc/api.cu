@@ -1,0 +1,492 @@
+// api.cu — the extern "C" boundary declared in include/mt.h: argument validation, workspace
+// management and the host-side drivers of the integrators (A8 RK4 with CUDA graphs, A9 DP45).
+#include <math.h>
+#include <string.h>
+
+#include <new>
+
+#include "mt_internal.cuh"
+
+namespace {
+
+inline int64_t round_up(int64_t x, int64_t m) { return (x + m - 1) / m * m; }
+inline size_t elem_size(int dtype) { return dtype == MT_F32 ? 4 : 8; }
+
+int check_tensor_args(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld) {
+  if (dtype != MT_F32 && dtype != MT_F64) return mt_fail(ctx, MT_ERR_INVALID_ARG, "unknown dtype %d", dtype);
+  if (n <= 0 || n_rows <= 0) return mt_fail(ctx, MT_ERR_INVALID_ARG, "n and n_rows must be positive");
+  if (ld < n) return mt_fail(ctx, MT_ERR_INVALID_ARG, "ld (%lld) < n (%lld)", (long long)ld, (long long)n);
+  const int64_t vec = dtype == MT_F32 ? 4 : 2;
+  if (ld % vec) return mt_fail(ctx, MT_ERR_INVALID_ARG, "ld must be a multiple of %lld elements", (long long)vec);
+  if (!N || ((uintptr_t)N & 15)) return mt_fail(ctx, MT_ERR_INVALID_ARG, "tensor pointer null or not 16-byte aligned");
+  return MT_OK;
+}
+
+int ensure_Mst(mt_ctx* ctx, int dtype, int batch, int64_t npad) {
+  const size_t need = (size_t)batch * 3 * npad * elem_size(dtype);
+  if (ctx->Mst_bytes >= need && ctx->Mst[0]) return MT_OK;
+  for (int k = 0; k < 2; ++k) {
+    size_t cur = ctx->Mst[k] ? ctx->Mst_bytes : 0;
+    int rc = mt_ensure_ws(ctx, &ctx->Mst[k], &cur, need);
+    if (rc) return rc;
+  }
+  ctx->Mst_bytes = need;
+  return MT_OK;
+}
+
+void fill_problem(EpiArgs& e, const mt_problem* p, int batch) {
+  memset(&e, 0, sizeof(e));
+  e.mode = 1;
+  e.batch = batch;
+  e.n = p->n;
+  e.n_rows = p->n;
+  e.Ms = p->Ms;
+  e.nbr = p->nbr;
+  for (int a = 0; a < 3; ++a) {
+    e.inv_d2[a] = p->inv_d2[a];
+    e.easy_c[a] = p->easy_const[a];
+    e.H_a_c[a] = p->H_a_const[a];
+  }
+  e.c_ex = p->c_ex;
+  e.c_ex_s = p->c_ex_scalar;
+  e.c_an = p->c_an;
+  e.c_an_s = p->c_an_scalar;
+  e.easy = p->easy;
+  e.H_a = p->H_a;
+  e.gamma = p->gamma;
+  e.alpha = p->alpha_ll;
+  e.M_dtype = p->dtype;
+}
+
+int check_problem(mt_ctx* ctx, const mt_problem* p, int batch) {
+  if (!p) return mt_fail(ctx, MT_ERR_INVALID_ARG, "problem is NULL");
+  if (p->n <= 0 || !p->Ms) return mt_fail(ctx, MT_ERR_INVALID_ARG, "problem needs n > 0 and Ms");
+  if (batch < 1 || batch > MT_MAX_BATCH) return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
+  if (p->N) return check_tensor_args(ctx, p->N, p->dtype, p->n, p->n, p->ld);
+  return MT_OK;
+}
+
+// one evaluation of the fused right-hand side: field of the staged M (ctx->Mst[src]) + epilogue
+int eval_rhs(mt_ctx* ctx, const mt_problem* p, int64_t npad, int src, const EpiArgs& e) {
+  if (p->N) return mt_launch_demag(ctx, p->N, p->dtype, p->n, p->n, p->ld, ctx->Mst[src], npad, e);
+  return mt_launch_local_only(ctx, e);
+}
+
+const double DP_A[7][6] = {
+    {0, 0, 0, 0, 0, 0},
+    {1.0 / 5, 0, 0, 0, 0, 0},
+    {3.0 / 40, 9.0 / 40, 0, 0, 0, 0},
+    {44.0 / 45, -56.0 / 15, 32.0 / 9, 0, 0, 0},
+    {19372.0 / 6561, -25360.0 / 2187, 64448.0 / 6561, -212.0 / 729, 0, 0},
+    {9017.0 / 3168, -355.0 / 33, 46732.0 / 5247, 49.0 / 176, -5103.0 / 18656, 0},
+    {35.0 / 384, 0, 500.0 / 1113, 125.0 / 192, -2187.0 / 6784, 11.0 / 84}};
+const double DP_E[7] = {35.0 / 384 - 5179.0 / 57600,       0.0,
+                        500.0 / 1113 - 7571.0 / 16695,     125.0 / 192 - 393.0 / 640,
+                        -2187.0 / 6784 + 92097.0 / 339200, 11.0 / 84 - 187.0 / 2100,
+                        -1.0 / 40};
+
+inline double bits_to_double(unsigned long long b) {
+  double d;
+  memcpy(&d, &b, 8);
+  return d;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* mt_version(void) { return "magtile-b200 0.1 (sm_100a)"; }
+
+int mt_create(mt_ctx** out, int device, void* cuda_stream) {
+  if (!out) return MT_ERR_INVALID_ARG;
+  *out = nullptr;
+  int count = 0;
+  if (cudaGetDeviceCount(&count) != cudaSuccess || device < 0 || device >= count) return MT_ERR_CUDA;
+  if (cudaSetDevice(device) != cudaSuccess) return MT_ERR_CUDA;
+  mt_ctx* c = new (std::nothrow) mt_ctx;
+  if (!c) return MT_ERR_CUDA;
+  memset(c, 0, sizeof(*c));
+  c->device = device;
+  c->stream = (cudaStream_t)cuda_stream;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, device) != cudaSuccess) {
+    delete c;
+    return MT_ERR_CUDA;
+  }
+  c->num_sms = prop.multiProcessorCount;
+  if (cudaMalloc((void**)&c->dscal, 8 * sizeof(unsigned long long)) != cudaSuccess ||
+      cudaMallocHost((void**)&c->hscal, 8 * sizeof(unsigned long long)) != cudaSuccess) {
+    delete c;
+    return MT_ERR_CUDA;
+  }
+  *out = c;
+  return MT_OK;
+}
+
+int mt_destroy(mt_ctx* c) {
+  if (!c) return MT_OK;
+  cudaSetDevice(c->device);
+  cudaStreamSynchronize(c->stream);
+  cudaFree(c->Mst[0]);
+  cudaFree(c->Mst[1]);
+  cudaFree(c->partial);
+  cudaFree(c->rk);
+  cudaFree(c->dscal);
+  cudaFree(c->stage_io);
+  cudaFreeHost(c->hscal);
+  cudaFreeHost(c->pinned_io);
+  delete c;
+  return MT_OK;
+}
+
+const char* mt_last_error(const mt_ctx* c) { return c ? c->err : "mt_ctx is NULL"; }
+
+int64_t mt_launch_count(const mt_ctx* c) { return c ? c->launches : 0; }
+
+int mt_set_demag_variant(mt_ctx* c, int variant) {
+  if (!c || variant < 0 || variant > 2) return MT_ERR_INVALID_ARG;
+  c->variant = variant;
+  return MT_OK;
+}
+
+int mt_assemble_tensor(mt_ctx* ctx, const mt_tiles* t, int dtype, int64_t row_begin, int64_t row_end,
+                       void* out, int64_t ld, int32_t* status_flag) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  if (!t || !t->type || !t->center || !t->size) return mt_fail(ctx, MT_ERR_INVALID_ARG, "tiles incomplete");
+  if (row_begin < 0 || row_end < row_begin || row_end > t->n)
+    return mt_fail(ctx, MT_ERR_INVALID_ARG, "row band [%lld, %lld) outside [0, %lld)", (long long)row_begin,
+                   (long long)row_end, (long long)t->n);
+  if (row_end == row_begin) return MT_OK;
+  int rc = check_tensor_args(ctx, out, dtype, t->n, row_end - row_begin, ld);
+  if (rc) return rc;
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  return mt_launch_assemble(ctx, t, dtype, row_begin, row_end, out, ld, status_flag);
+}
+
+int mt_demag_field(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                   const double* Ms, const double* m, int batch, double* Hd) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_tensor_args(ctx, N, dtype, n, n_rows, ld);
+  if (rc) return rc;
+  if (!Ms || !m || !Hd) return mt_fail(ctx, MT_ERR_INVALID_ARG, "Ms, m and Hd must be non-NULL");
+  if (batch < 1 || batch > MT_MAX_BATCH) return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  const int64_t npad = round_up(n, MT_COL_CHUNK);
+  rc = ensure_Mst(ctx, dtype, batch, npad);
+  if (rc) return rc;
+  rc = mt_launch_stage_M(ctx, dtype, Ms, m, batch, n, npad, ctx->Mst[0]);
+  if (rc) return rc;
+  EpiArgs e;
+  memset(&e, 0, sizeof(e));
+  e.mode = 0;
+  e.batch = batch;
+  e.n = n;
+  e.n_rows = n_rows;
+  e.Hd = Hd;
+  return mt_launch_demag(ctx, N, dtype, n, n_rows, ld, ctx->Mst[0], npad, e);
+}
+
+int mt_demag_field_host(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                        const double* Ms, const double* m_host, int batch, double* Hd_host) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  if (!m_host || !Hd_host) return mt_fail(ctx, MT_ERR_INVALID_ARG, "host vectors must be non-NULL");
+  if (batch < 1 || batch > MT_MAX_BATCH || n <= 0 || n_rows <= 0)
+    return mt_fail(ctx, MT_ERR_INVALID_ARG, "bad batch / n / n_rows");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  const size_t in_b = (size_t)batch * 3 * n * sizeof(double), out_b = (size_t)batch * 3 * n_rows * sizeof(double);
+  int rc = mt_ensure_ws(ctx, (void**)&ctx->stage_io, &ctx->stage_io_bytes, in_b + out_b);
+  if (rc) return rc;
+  double* d_m = ctx->stage_io;
+  double* d_h = ctx->stage_io + (size_t)batch * 3 * n;
+  MT_CUDA_OK(ctx, cudaMemcpyAsync(d_m, m_host, in_b, cudaMemcpyHostToDevice, ctx->stream));
+  rc = mt_demag_field(ctx, N, dtype, n, n_rows, ld, Ms, d_m, batch, d_h);
+  if (rc) return rc;
+  MT_CUDA_OK(ctx, cudaMemcpyAsync(Hd_host, d_h, out_b, cudaMemcpyDeviceToHost, ctx->stream));
+  MT_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  return MT_OK;
+}
+
+int mt_llg_rhs(mt_ctx* ctx, const mt_problem* p, const double* m, int batch, double* dmdt, double* Heff) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_problem(ctx, p, batch);
+  if (rc) return rc;
+  if (!m || !dmdt) return mt_fail(ctx, MT_ERR_INVALID_ARG, "m and dmdt must be non-NULL");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  const int64_t npad = round_up(p->n, MT_COL_CHUNK);
+  if (p->N) {
+    rc = ensure_Mst(ctx, p->dtype, batch, npad);
+    if (rc) return rc;
+    rc = mt_launch_stage_M(ctx, p->dtype, p->Ms, m, batch, p->n, npad, ctx->Mst[0]);
+    if (rc) return rc;
+  }
+  EpiArgs e;
+  fill_problem(e, p, batch);
+  e.y = m;
+  e.k_out = dmdt;
+  e.heff_out = Heff;
+  return eval_rhs(ctx, p, npad, 0, e);
+}
+
+int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, double* m, int batch,
+                 double* t_inout, double* samples, int64_t sample_cap, mt_integrator_result* res) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_problem(ctx, p, batch);
+  if (rc) return rc;
+  if (!o || !m || !t_inout || !res) return mt_fail(ctx, MT_ERR_INVALID_ARG, "opts, m, t and result must be non-NULL");
+  if (o->method != MT_RK4 && o->method != MT_DP45) return mt_fail(ctx, MT_ERR_INVALID_ARG, "unknown method %d", o->method);
+  if (o->method == MT_RK4 && !(o->dt > 0)) return mt_fail(ctx, MT_ERR_INVALID_ARG, "RK4 needs dt > 0");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  cudaStream_t st = ctx->stream;
+  const int64_t n = p->n, sv = (int64_t)batch * 3 * n;  // doubles per state vector
+  const int64_t npad = round_up(n, MT_COL_CHUNK);
+  const int64_t stride = 1 + 3 * (int64_t)batch;
+  memset(res, 0, sizeof(*res));
+  // workspace: k1..k7, two scratch states, candidate state
+  rc = mt_ensure_ws(ctx, (void**)&ctx->rk, &ctx->rk_bytes, (size_t)(7 + 3) * sv * sizeof(double));
+  if (rc) return rc;
+  double* k[7];
+  for (int s = 0; s < 7; ++s) k[s] = ctx->rk + (int64_t)s * sv;
+  double* ya = ctx->rk + 7 * sv;
+  double* yb = ctx->rk + 8 * sv;
+  double* mc = ctx->rk + 9 * sv;
+  if (p->N) {
+    rc = ensure_Mst(ctx, p->dtype, batch, npad);
+    if (rc) return rc;
+    rc = mt_launch_stage_M(ctx, p->dtype, p->Ms, m, batch, n, npad, ctx->Mst[0]);
+    if (rc) return rc;
+  }
+  unsigned long long* d_err = ctx->dscal;
+  unsigned long long* d_tq = ctx->dscal + 1;
+  double t = *t_inout;
+  const double t0 = t;
+  int status = MT_OK;
+  EpiArgs base;
+  fill_problem(base, p, batch);
+  base.M_out = nullptr;
+  base.npad = npad;
+
+  if (o->method == MT_RK4) {
+    // ---- A8: classical RK4; the four fused launches of a step are replayed from a CUDA graph ----
+    const double dt = o->dt;
+    int64_t nsteps = (int64_t)llround((o->t_end - t) / dt);
+    if (nsteps < 0) nsteps = 0;
+    bool hit_max = false;
+    if (o->max_steps > 0 && nsteps > o->max_steps) { nsteps = o->max_steps; hit_max = true; }
+    const bool want_tq = o->torque_tol > 0;
+    auto stage1 = [&]() -> int {  // k1 = f(m); ya = m + dt/2 k1
+      EpiArgs e = base;
+      e.y = m; e.k_out = k[0]; e.torque_bits = want_tq ? d_tq : nullptr;
+      e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[0]; e.coef[0] = 1.0; e.base = m; e.h = 0.5 * dt; e.y_out = ya;
+      e.M_out = p->N ? ctx->Mst[1] : nullptr;
+      return eval_rhs(ctx, p, npad, 0, e);
+    };
+    auto stages234 = [&]() -> int {
+      int r;
+      EpiArgs e = base;  // stage 2: k2 = f(ya); yb = m + dt/2 k2
+      e.y = ya; e.k_out = k[1];
+      e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[1]; e.coef[0] = 1.0; e.base = m; e.h = 0.5 * dt; e.y_out = yb;
+      e.M_out = p->N ? ctx->Mst[0] : nullptr;
+      if ((r = eval_rhs(ctx, p, npad, 1, e))) return r;
+      e = base;  // stage 3: k3 = f(yb); ya = m + dt k3
+      e.y = yb; e.k_out = k[2];
+      e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[2]; e.coef[0] = 1.0; e.base = m; e.h = dt; e.y_out = ya;
+      e.M_out = p->N ? ctx->Mst[1] : nullptr;
+      if ((r = eval_rhs(ctx, p, npad, 0, e))) return r;
+      e = base;  // stage 4: k4 = f(ya); m <- m + dt/6 (k1 + 2 k2 + 2 k3 + k4), renormalised, restaged
+      e.y = ya; e.k_out = k[3];
+      e.do_comb = 1; e.ncomb = 4;
+      for (int s = 0; s < 4; ++s) e.kptr[s] = k[s];
+      e.coef[0] = 1.0; e.coef[1] = 2.0; e.coef[2] = 2.0; e.coef[3] = 1.0;
+      e.base = m; e.h = dt / 6.0; e.y_out = m; e.renorm = o->renormalize;
+      e.M_out = p->N ? ctx->Mst[0] : nullptr;
+      return eval_rhs(ctx, p, npad, 1, e);
+    };
+    auto sample_if_due = [&](int64_t done) -> int {
+      if (o->sample_every > 0 && done % o->sample_every == 0 && samples && res->n_samples < sample_cap) {
+        int r = mt_launch_mean(ctx, m, p->vol, batch, n, t0 + (double)done * dt, samples + res->n_samples * stride);
+        if (r) return r;
+        res->n_samples++;
+      }
+      return MT_OK;
+    };
+    int64_t done = 0;
+    if (want_tq) {
+      // the stop test (Eq. 2) needs the torque of every step's first stage: one host
+      // read per step; a satisfied test leaves m untouched
+      while (done < nsteps) {
+        MT_CUDA_OK(ctx, cudaMemsetAsync(d_tq, 0, 8, st));
+        if ((rc = stage1())) return rc;
+        MT_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hscal, d_tq, 8, cudaMemcpyDeviceToHost, st));
+        MT_CUDA_OK(ctx, cudaStreamSynchronize(st));
+        res->max_torque = bits_to_double(ctx->hscal[0]);
+        if (res->max_torque <= o->torque_tol) break;
+        if ((rc = stages234())) return rc;
+        done++;
+        if ((rc = sample_if_due(done))) return rc;
+      }
+    } else {
+      // `chunk` steps are captured once into a CUDA graph and replayed (every buffer is back in its
+      // role after a step).  The first chunk runs eagerly: it sizes the workspaces, which must not be
+      // allocated under capture.
+      int64_t chunk = o->sample_every > 0 ? o->sample_every : 64;
+      if (chunk > 256) chunk = 256;
+      while (o->sample_every > 0 && o->sample_every % chunk) chunk--;  // chunk divides sample_every
+      cudaGraph_t graph = nullptr;
+      cudaGraphExec_t exec = nullptr;
+      int64_t graph_launches = 0;
+      while (done < nsteps && !rc) {
+        if (done >= chunk && done % chunk == 0 && nsteps - done >= chunk) {
+          if (!exec) {
+            const int64_t l0 = ctx->launches;
+            MT_CUDA_OK(ctx, cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+            int r = MT_OK;
+            for (int64_t s = 0; s < chunk && !r; ++s) {
+              r = stage1();
+              if (!r) r = stages234();
+            }
+            cudaError_t ce = cudaStreamEndCapture(st, &graph);
+            graph_launches = ctx->launches - l0;
+            ctx->launches = l0;  // captured, not yet launched
+            if (r) { if (graph) cudaGraphDestroy(graph); return r; }
+            MT_CUDA_OK(ctx, ce);
+            MT_CUDA_OK(ctx, cudaGraphInstantiate(&exec, graph, 0));
+          }
+          cudaError_t ce = cudaGraphLaunch(exec, st);
+          if (ce != cudaSuccess) { rc = mt_fail(ctx, MT_ERR_CUDA, "cudaGraphLaunch: %s", cudaGetErrorString(ce)); break; }
+          ctx->launches += graph_launches;
+          done += chunk;
+        } else {
+          if ((rc = stage1())) break;
+          if ((rc = stages234())) break;
+          done++;
+        }
+        rc = sample_if_due(done);
+      }
+      if (exec) cudaGraphExecDestroy(exec);
+      if (graph) cudaGraphDestroy(graph);
+      if (rc) return rc;
+    }
+    res->rhs_calls = 4 * done;
+    res->accepted = done;
+    res->dt_last = dt;
+    t = t0 + (double)done * dt;
+    if (hit_max && done == nsteps) status = MT_ERR_MAX_STEPS;
+  } else {
+    // ---- A9: Dormand-Prince 5(4) with FSAL; the controller runs on the host, one 16-byte read per
+    // attempted step (at the sizes where the step is milliseconds this is noise) ----------
+    double dt = o->dt > 0 ? o->dt : 1e-3;
+    int64_t next_sample = 1;
+    // k1 = f(m)
+    {
+      MT_CUDA_OK(ctx, cudaMemsetAsync(d_tq, 0, 8, st));
+      EpiArgs e = base;
+      e.y = m; e.k_out = k[0]; e.torque_bits = d_tq;
+      if ((rc = eval_rhs(ctx, p, npad, 0, e))) return rc;
+      MT_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hscal, d_tq, 8, cudaMemcpyDeviceToHost, st));
+      MT_CUDA_OK(ctx, cudaStreamSynchronize(st));
+      res->max_torque = bits_to_double(ctx->hscal[0]);
+      res->rhs_calls = 1;
+    }
+    while (t < o->t_end) {
+      if (o->torque_tol > 0 && res->max_torque <= o->torque_tol) break;
+      if (o->max_steps > 0 && res->accepted + res->rejected >= o->max_steps) { status = MT_ERR_MAX_STEPS; break; }
+      double t_target = o->t_end;
+      bool hit_sample = false;
+      if (o->sample_dt > 0) {
+        const double ts = t0 + (double)next_sample * o->sample_dt;
+        if (ts <= t_target) { t_target = ts; hit_sample = true; }
+      }
+      double h = dt;
+      bool clipped = false;
+      if (t + h >= t_target) { h = t_target - t; clipped = true; }
+      const double h_min = 16.0 * 2.220446049250313e-16 * fmax(fabs(t), fabs(o->t_end));
+      if (h <= h_min) {
+        if (clipped) {
+          t = t_target;
+          if (hit_sample) {
+            if (samples && res->n_samples < sample_cap) {
+              if ((rc = mt_launch_mean(ctx, m, p->vol, batch, n, t, samples + res->n_samples * stride))) return rc;
+              res->n_samples++;
+            }
+            next_sample++;
+          }
+          continue;
+        }
+        status = MT_ERR_STEP_UNDERFLOW;
+        break;
+      }
+      // y2 = m + h a21 k1 (k1 is known: no field evaluation to fuse with).  The staged-M buffers
+      // alternate: every evaluation reads Mst[src] and stages its successor state into the other one.
+      // Ms*m itself is only needed for the very first k1: FSAL supplies k1 afterwards.
+      int src = 0;
+      {
+        EpiArgs e = base;
+        e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[0]; e.coef[0] = DP_A[1][0]; e.base = m; e.h = h; e.y_out = ya;
+        e.M_out = p->N ? ctx->Mst[src ^ 1] : nullptr;
+        if ((rc = mt_launch_combine(ctx, e))) return rc;
+        src ^= 1;
+      }
+      double* yin = ya;
+      double* yout = yb;
+      for (int s = 1; s <= 5; ++s) {  // evaluation of k_{s+1} at y_{s+1}, then y_{s+2}
+        EpiArgs e = base;
+        e.y = yin; e.k_out = k[s];
+        e.do_comb = 1; e.ncomb = s + 1;
+        for (int j = 0; j <= s; ++j) { e.kptr[j] = k[j]; e.coef[j] = DP_A[s + 1][j]; }
+        e.base = m; e.h = h; e.y_out = yout;
+        e.M_out = p->N ? ctx->Mst[src ^ 1] : nullptr;
+        if ((rc = eval_rhs(ctx, p, npad, src, e))) return rc;
+        src ^= 1;
+        double* tmp = yin; yin = yout; yout = tmp;
+      }
+      // yin now holds y7 = the 5th-order solution; k7 = f(y7) with error estimate, torque and the
+      // (renormalised) candidate state + its staged M
+      MT_CUDA_OK(ctx, cudaMemsetAsync(d_err, 0, 16, st));
+      {
+        EpiArgs e = base;
+        e.y = yin; e.k_out = k[6]; e.torque_bits = d_tq;
+        e.nerr = 7;
+        for (int j = 0; j < 7; ++j) { e.eptr[j] = k[j]; e.ecoef[j] = DP_E[j]; }
+        e.ebase = m; e.atol = o->atol; e.rtol = o->rtol; e.err_bits = d_err; e.h = h;
+        e.do_comb = 1; e.ncomb = 0; e.base = yin; e.y_out = mc; e.renorm = o->renormalize;
+        e.M_out = nullptr;
+        if ((rc = eval_rhs(ctx, p, npad, src, e))) return rc;
+      }
+      MT_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hscal, d_err, 16, cudaMemcpyDeviceToHost, st));
+      MT_CUDA_OK(ctx, cudaStreamSynchronize(st));
+      res->rhs_calls += 6;
+      const double err = bits_to_double(ctx->hscal[0]);
+      const double tq7 = bits_to_double(ctx->hscal[1]);
+      double fac = err > 0 ? 0.9 * pow(err, -0.2) : 5.0;
+      fac = fmin(5.0, fmax(0.2, fac));
+      if (err <= 1.0) {
+        t = clipped ? t_target : t + h;
+        MT_CUDA_OK(ctx, cudaMemcpyAsync(m, mc, (size_t)sv * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        double* tmp = k[0]; k[0] = k[6]; k[6] = tmp;  // FSAL
+        res->max_torque = tq7;
+        res->accepted++;
+        res->dt_last = h;
+        if (clipped && hit_sample) {
+          if (samples && res->n_samples < sample_cap) {
+            if ((rc = mt_launch_mean(ctx, m, p->vol, batch, n, t, samples + res->n_samples * stride))) return rc;
+            res->n_samples++;
+          }
+          next_sample++;
+        }
+        dt = clipped ? fmax(dt, h * fac) : h * fac;
+      } else {
+        res->rejected++;
+        dt = h * fmin(1.0, fac);
+        if (!(err == err)) { status = MT_ERR_STEP_UNDERFLOW; mt_fail(ctx, status, "non-finite error estimate"); break; }
+      }
+    }
+  }
+  MT_CUDA_OK(ctx, cudaStreamSynchronize(st));
+  res->t = t;
+  *t_inout = t;
+  if (status == MT_ERR_MAX_STEPS) mt_fail(ctx, status, "max_steps reached at t = %g", t);
+  if (status == MT_ERR_STEP_UNDERFLOW && !ctx->err[0]) mt_fail(ctx, status, "step size underflow at t = %g", t);
+  return status;
+}
+
+}  // extern "C"

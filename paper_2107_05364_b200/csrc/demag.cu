@@ -1,0 +1,374 @@
+// demag.cu — A4/A7: H_d = -N.(Ms m), register-streaming variant ("LDG"), plus the small O(N)
+// kernels around it: staging of Ms*m in the tensor's dtype, split-column reduction, local-only
+// right-hand side, stage combine and the <m> observable (A10).
+//
+// Kernel shape (HBM-bound): one warp owns one target row i and streams the
+// six component rows N^{c}_{i,*} once with 128-bit non-allocating loads; the staged vector
+// M = Ms*m (same dtype as the tensor) comes through L1/L2.  fp32 tensors accumulate in short fp32
+// runs (8 vector iterations = 96 products per accumulator) flushed into fp64; fp64 tensors use
+// DFMA directly.  The warp reduces with a fixed xor-butterfly (bitwise reproducible) and lanes
+// 0..B-1 run the fused epilogue (epilogue.cuh).  For small n the columns are split over
+// gridDim.y and a second kernel adds the partials in a fixed order.
+#include <stdarg.h>
+
+#include "epilogue.cuh"
+
+int mt_fail(mt_ctx* ctx, int code, const char* fmt, ...) {
+  if (ctx) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+    va_end(ap);
+  }
+  return code;
+}
+
+int mt_ensure_ws(mt_ctx* ctx, void** p, size_t* cur, size_t need) {
+  if (*cur >= need && *p) return MT_OK;
+  if (*p) {
+    MT_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+    MT_CUDA_OK(ctx, cudaFree(*p));
+    *p = nullptr;
+    *cur = 0;
+  }
+  MT_CUDA_OK(ctx, cudaMalloc(p, need));
+  *cur = need;
+  return MT_OK;
+}
+
+namespace {
+
+template <typename T> struct VecOf;
+template <> struct VecOf<float> { typedef float4 type; static constexpr int W = 4; };
+template <> struct VecOf<double> { typedef double2 type; static constexpr int W = 2; };
+
+// streaming (read-once) 128-bit loads: do not allocate in L1
+__device__ __forceinline__ float4 ld_stream(const float4* p) {
+  float4 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];"
+               : "=f"(r.x), "=f"(r.y), "=f"(r.z), "=f"(r.w) : "l"(p));
+  return r;
+}
+__device__ __forceinline__ double2 ld_stream(const double2* p) {
+  double2 r;
+  asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0, %1}, [%2];" : "=d"(r.x), "=d"(r.y) : "l"(p));
+  return r;
+}
+
+template <typename A>
+__device__ __forceinline__ void fma_block(A acc[3], float xx, float xy, float xz, float yy, float yz,
+                                          float zz, float mx, float my, float mz) {
+  acc[0] = fmaf(xx, mx, fmaf(xy, my, fmaf(xz, mz, acc[0])));
+  acc[1] = fmaf(xy, mx, fmaf(yy, my, fmaf(yz, mz, acc[1])));
+  acc[2] = fmaf(xz, mx, fmaf(yz, my, fmaf(zz, mz, acc[2])));
+}
+__device__ __forceinline__ void fma_block(double acc[3], double xx, double xy, double xz, double yy,
+                                          double yz, double zz, double mx, double my, double mz) {
+  acc[0] = fma(xx, mx, fma(xy, my, fma(xz, mz, acc[0])));
+  acc[1] = fma(xy, mx, fma(yy, my, fma(yz, mz, acc[1])));
+  acc[2] = fma(xz, mx, fma(yz, my, fma(zz, mz, acc[2])));
+}
+
+__device__ __forceinline__ void vec_fma(float acc[3], const float4 v[6], const float4 m[3]) {
+  fma_block(acc, v[0].x, v[1].x, v[2].x, v[3].x, v[4].x, v[5].x, m[0].x, m[1].x, m[2].x);
+  fma_block(acc, v[0].y, v[1].y, v[2].y, v[3].y, v[4].y, v[5].y, m[0].y, m[1].y, m[2].y);
+  fma_block(acc, v[0].z, v[1].z, v[2].z, v[3].z, v[4].z, v[5].z, m[0].z, m[1].z, m[2].z);
+  fma_block(acc, v[0].w, v[1].w, v[2].w, v[3].w, v[4].w, v[5].w, m[0].w, m[1].w, m[2].w);
+}
+__device__ __forceinline__ void vec_fma(double acc[3], const double2 v[6], const double2 m[3]) {
+  fma_block(acc, v[0].x, v[1].x, v[2].x, v[3].x, v[4].x, v[5].x, m[0].x, m[1].x, m[2].x);
+  fma_block(acc, v[0].y, v[1].y, v[2].y, v[3].y, v[4].y, v[5].y, m[0].y, m[1].y, m[2].y);
+}
+
+template <typename T>
+struct DemagArgs {
+  const T* N;
+  int64_t n, n_rows, ld, plane;  // plane = n_rows * ld
+  const T* M;                    // [B][3][npad]
+  int64_t npad;
+  int64_t vec_per_split;         // full vectors per column split
+  int nsplit;
+  double* partial;               // [nsplit][B][3][n_rows] when nsplit > 1
+};
+
+constexpr int kWarps = 8;
+constexpr int kFlush = 8;  // fp32: vector iterations per fp32 run
+
+template <typename T, int B>
+__global__ void __launch_bounds__(kWarps * 32) demag_ldg_kernel(DemagArgs<T> a, EpiArgs e) {
+  typedef typename VecOf<T>::type V;
+  constexpr int W = VecOf<T>::W;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t row = (int64_t)blockIdx.x * kWarps + warp;
+  if (row >= a.n_rows) return;
+  const int split = blockIdx.y;
+  const int64_t nvec = a.n / W;
+  const int64_t v0 = (int64_t)split * a.vec_per_split;
+  const int64_t v1 = min(nvec, v0 + a.vec_per_split);
+  const V* p[6];
+#pragma unroll
+  for (int c = 0; c < 6; ++c) p[c] = reinterpret_cast<const V*>(a.N + c * a.plane + row * a.ld);
+  const V* mp = reinterpret_cast<const V*>(a.M);
+  const int64_t mstride = a.npad / W;  // vectors per component row of M
+
+  double acc[B][3];
+#pragma unroll
+  for (int b = 0; b < B; ++b) acc[b][0] = acc[b][1] = acc[b][2] = 0.0;
+
+  for (int64_t vb = v0 + lane; vb < v1; vb += 32 * kFlush) {
+    T run[B][3];
+#pragma unroll
+    for (int b = 0; b < B; ++b) run[b][0] = run[b][1] = run[b][2] = T(0);
+#pragma unroll 2
+    for (int it = 0; it < kFlush; ++it) {
+      const int64_t v = vb + (int64_t)it * 32;
+      if (v < v1) {
+        V t[6];
+#pragma unroll
+        for (int c = 0; c < 6; ++c) t[c] = ld_stream(p[c] + v);
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+          V m[3];
+#pragma unroll
+          for (int c = 0; c < 3; ++c) m[c] = __ldg(mp + (b * 3 + c) * mstride + v);
+          vec_fma(run[b], t, m);
+        }
+      }
+    }
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+      acc[b][0] += (double)run[b][0];
+      acc[b][1] += (double)run[b][1];
+      acc[b][2] += (double)run[b][2];
+    }
+  }
+  // scalar tail (n not a multiple of the vector width): last split, one lane per leftover column
+  if (split == a.nsplit - 1) {
+    const int64_t j = nvec * W + lane;
+    if (j < a.n) {
+#pragma unroll
+      for (int b = 0; b < B; ++b) {
+        T t[6], m[3];
+#pragma unroll
+        for (int c = 0; c < 6; ++c) t[c] = a.N[c * a.plane + row * a.ld + j];
+#pragma unroll
+        for (int c = 0; c < 3; ++c) m[c] = a.M[(b * 3 + c) * a.npad + j];
+        T run[3] = {T(0), T(0), T(0)};
+        fma_block(run, t[0], t[1], t[2], t[3], t[4], t[5], m[0], m[1], m[2]);
+        acc[b][0] += (double)run[0];
+        acc[b][1] += (double)run[1];
+        acc[b][2] += (double)run[2];
+      }
+    }
+  }
+  // fixed-order butterfly: every lane ends with the same, reproducible sum
+#pragma unroll
+  for (int b = 0; b < B; ++b)
+#pragma unroll
+    for (int c = 0; c < 3; ++c)
+#pragma unroll
+      for (int off = 16; off > 0; off >>= 1) acc[b][c] += __shfl_xor_sync(0xffffffffu, acc[b][c], off);
+
+  if (a.nsplit > 1) {
+    if (lane == 0) {
+#pragma unroll
+      for (int b = 0; b < B; ++b)
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+          a.partial[(((int64_t)split * B + b) * 3 + c) * a.n_rows + row] = acc[b][c];
+    }
+    return;
+  }
+  // lanes 0..B-1 each finish one state (static selection keeps acc[][] in registers)
+  double hd[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+  for (int b = 0; b < B; ++b)
+    if (lane == b) {
+      hd[0] = -acc[b][0];
+      hd[1] = -acc[b][1];
+      hd[2] = -acc[b][2];
+    }
+  if (lane < B) row_epilogue(e, row, lane, hd);
+}
+
+// second pass for nsplit > 1: add the partials in split order, then the epilogue
+__global__ void __launch_bounds__(256) demag_reduce_kernel(const double* partial, int nsplit, int B,
+                                                           int64_t n_rows, EpiArgs e) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= n_rows * B) return;
+  const int b = (int)(idx / n_rows);
+  const int64_t row = idx % n_rows;
+  double hd[3];
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    double s = 0.0;
+    for (int sp = 0; sp < nsplit; ++sp) s += partial[(((int64_t)sp * B + b) * 3 + c) * n_rows + row];
+    hd[c] = -s;
+  }
+  row_epilogue(e, row, b, hd);
+}
+
+__global__ void __launch_bounds__(256) local_only_kernel(EpiArgs e) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= e.n * e.batch) return;
+  const double hd[3] = {0.0, 0.0, 0.0};
+  row_epilogue(e, idx % e.n, (int)(idx / e.n), hd);
+}
+
+__global__ void __launch_bounds__(256) combine_kernel(EpiArgs e) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= e.n * e.batch) return;
+  stage_combine(e, idx % e.n, (int)(idx / e.n), nullptr);
+}
+
+// M[b][c][j] = T(Ms[j] * m[b][c][j]), zero in the padding j in [n, npad)
+template <typename T>
+__global__ void __launch_bounds__(256) stage_M_kernel(const double* __restrict__ Ms, const double* __restrict__ m,
+                                                      int64_t n, int64_t npad, int rows /* B*3 */, T* __restrict__ M) {
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int r = blockIdx.y;
+  if (j >= npad || r >= rows) return;
+  M[(int64_t)r * npad + j] = j < n ? (T)(Ms[j] * m[(int64_t)r * n + j]) : T(0);
+}
+
+// A10: <m_c> of state b = sum_i w_i m_i / sum_i w_i; one block per (c, b), fixed-order tree.
+__global__ void __launch_bounds__(1024) mean_kernel(const double* __restrict__ m, const double* __restrict__ vol,
+                                                    int64_t n, int batch, double t, double* __restrict__ out) {
+  __shared__ double sh[1024], shw[1024];
+  const int c = blockIdx.x, b = blockIdx.y;
+  const double* v = m + ((int64_t)b * 3 + c) * n;
+  double s = 0.0, w = 0.0;
+  for (int64_t i = threadIdx.x; i < n; i += 1024) {
+    const double wi = vol ? vol[i] : 1.0;
+    s += wi * v[i];
+    w += wi;
+  }
+  sh[threadIdx.x] = s;
+  shw[threadIdx.x] = w;
+  __syncthreads();
+  for (int off = 512; off > 0; off >>= 1) {
+    if ((int)threadIdx.x < off) {
+      sh[threadIdx.x] += sh[threadIdx.x + off];
+      shw[threadIdx.x] += shw[threadIdx.x + off];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    out[1 + b * 3 + c] = sh[0] / shw[0];
+    if (c == 0 && b == 0) out[0] = t;
+  }
+}
+
+template <typename T, int B>
+int launch_ldg_T(mt_ctx* ctx, const DemagArgs<T>& a, const EpiArgs& e) {
+  dim3 grid((unsigned)((a.n_rows + kWarps - 1) / kWarps), (unsigned)a.nsplit);
+  demag_ldg_kernel<T, B><<<grid, kWarps * 32, 0, ctx->stream>>>(a, e);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  if (a.nsplit > 1) {
+    const int64_t tot = a.n_rows * B;
+    demag_reduce_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(a.partial, a.nsplit, B, a.n_rows, e);
+    ctx->launches++;
+    MT_CUDA_OK(ctx, cudaGetLastError());
+  }
+  return MT_OK;
+}
+
+template <typename T>
+int launch_ldg(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
+               int64_t npad, const EpiArgs& e) {
+  constexpr int W = VecOf<T>::W;
+  DemagArgs<T> a;
+  a.N = (const T*)N;
+  a.n = n;
+  a.n_rows = n_rows;
+  a.ld = ld;
+  a.plane = n_rows * ld;
+  a.M = (const T*)Mst;
+  a.npad = npad;
+  // split the columns when the rows alone cannot fill the machine twice over
+  const int64_t ctas = (n_rows + kWarps - 1) / kWarps;
+  const int64_t want = 2LL * ctx->num_sms;
+  int nsplit = 1;
+  const int64_t nvec = n / W;
+  if (ctas < want) {
+    nsplit = (int)((want + ctas - 1) / ctas);
+    const int64_t max_split = (nvec + 255) / 256;  // keep >= 256 vectors per split
+    if (nsplit > max_split) nsplit = (int)(max_split > 0 ? max_split : 1);
+    if (nsplit > 64) nsplit = 64;
+  }
+  int64_t vps = (nvec + nsplit - 1) / nsplit;
+  vps = (vps + 31) / 32 * 32;
+  if (vps == 0) vps = 32;
+  nsplit = (int)((nvec + vps - 1) / vps);
+  if (nsplit < 1) nsplit = 1;
+  a.vec_per_split = vps;
+  a.nsplit = nsplit;
+  a.partial = nullptr;
+  if (nsplit > 1) {
+    const size_t need = (size_t)nsplit * e.batch * 3 * n_rows * sizeof(double);
+    int rc = mt_ensure_ws(ctx, (void**)&ctx->partial, &ctx->partial_bytes, need);
+    if (rc) return rc;
+    a.partial = ctx->partial;
+  }
+  switch (e.batch) {
+    case 1: return launch_ldg_T<T, 1>(ctx, a, e);
+    case 2: return launch_ldg_T<T, 2>(ctx, a, e);
+    case 3: return launch_ldg_T<T, 3>(ctx, a, e);
+    case 4: return launch_ldg_T<T, 4>(ctx, a, e);
+    case 5: return launch_ldg_T<T, 5>(ctx, a, e);
+    case 6: return launch_ldg_T<T, 6>(ctx, a, e);
+    case 7: return launch_ldg_T<T, 7>(ctx, a, e);
+    case 8: return launch_ldg_T<T, 8>(ctx, a, e);
+  }
+  return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
+}
+
+}  // namespace
+
+int mt_launch_stage_M(mt_ctx* ctx, int dtype, const double* Ms, const double* m, int batch, int64_t n,
+                      int64_t npad, void* M_out) {
+  dim3 grid((unsigned)((npad + 255) / 256), (unsigned)(batch * 3));
+  if (dtype == MT_F32)
+    stage_M_kernel<float><<<grid, 256, 0, ctx->stream>>>(Ms, m, n, npad, batch * 3, (float*)M_out);
+  else
+    stage_M_kernel<double><<<grid, 256, 0, ctx->stream>>>(Ms, m, n, npad, batch * 3, (double*)M_out);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+int mt_launch_demag(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                    const void* Mst, int64_t npad, const EpiArgs& epi) {
+  if (ctx->variant != 1) {
+    int rc = mt_launch_demag_tma(ctx, N, dtype, n, n_rows, ld, Mst, npad, epi);
+    if (rc != MT_ERR_UNIMPLEMENTED) return rc;
+    if (ctx->variant == 2) return rc;
+  }
+  if (dtype == MT_F32) return launch_ldg<float>(ctx, N, n, n_rows, ld, Mst, npad, epi);
+  return launch_ldg<double>(ctx, N, n, n_rows, ld, Mst, npad, epi);
+}
+
+int mt_launch_local_only(mt_ctx* ctx, const EpiArgs& epi) {
+  const int64_t tot = epi.n * epi.batch;
+  local_only_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(epi);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+int mt_launch_combine(mt_ctx* ctx, const EpiArgs& epi) {
+  const int64_t tot = epi.n * epi.batch;
+  combine_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(epi);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+int mt_launch_mean(mt_ctx* ctx, const double* m, const double* vol, int batch, int64_t n, double t,
+                   double* sample_row) {
+  mean_kernel<<<dim3(3, (unsigned)batch), 1024, 0, ctx->stream>>>(m, vol, n, batch, t, sample_row);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
