@@ -135,6 +135,7 @@ int mt_destroy(mt_ctx* c) {
   cudaFree(c->stage_io);
   cudaFreeHost(c->hscal);
   cudaFreeHost(c->pinned_io);
+  if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
   delete c;
   return MT_OK;
 }
@@ -337,14 +338,19 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       while (done < nsteps && !rc) {
         if (done >= chunk && done % chunk == 0 && nsteps - done >= chunk) {
           if (!exec) {
+            // capture on a private stream (the caller's may be the legacy default stream, which cannot
+            // be captured); the instantiated graph is then launched on the caller's stream
+            if (!ctx->cap_stream) MT_CUDA_OK(ctx, cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
             const int64_t l0 = ctx->launches;
-            MT_CUDA_OK(ctx, cudaStreamBeginCapture(st, cudaStreamCaptureModeThreadLocal));
+            MT_CUDA_OK(ctx, cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal));
+            ctx->stream = ctx->cap_stream;
             int r = MT_OK;
             for (int64_t s = 0; s < chunk && !r; ++s) {
               r = stage1();
               if (!r) r = stages234();
             }
-            cudaError_t ce = cudaStreamEndCapture(st, &graph);
+            ctx->stream = st;
+            cudaError_t ce = cudaStreamEndCapture(ctx->cap_stream, &graph);
             graph_launches = ctx->launches - l0;
             ctx->launches = l0;  // captured, not yet launched
             if (r) { if (graph) cudaGraphDestroy(graph); return r; }

@@ -13,6 +13,7 @@
 struct mt_ctx {
   int device;
   cudaStream_t stream;
+  cudaStream_t cap_stream;  // private stream for CUDA-graph capture
   int num_sms;
   int variant;  // 0 auto, 1 LDG, 2 TMA
   int64_t launches;

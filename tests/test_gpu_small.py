@@ -33,12 +33,12 @@ def check_tensor(N_gpu, N_ref, dtype, n):
         assert np.max(row_err / row_nrm) <= TOL_ASM
         assert H.rel_l2(got, N_ref) <= TOL_ASM
     else:
+        # fp32 planes = round-to-nearest of the fp64 closed form: within 1 fp32 ulp of the rounded
+        # oracle value, or (entries that are differences of O(1) terms down at fp64 resolution, e.g.
+        # symmetry zeros) within the 1e-15 absolute floor of any fp64 evaluation
         ulp = H.f32_ulp_distance(got, N_ref)
-        # entries whose exact value is below fp64 resolution of the O(1) terms they are differences of
-        # (|N| < 1e-13) round to +-tiny either way; measure those absolutely
-        big = np.abs(N_ref) > 1e-12
-        assert ulp[big].max() <= 1
-        assert np.max(np.abs(got[~big].astype(np.float64) - N_ref[~big])) < 1e-12 if (~big).any() else True
+        ok = (ulp <= 1) | (np.abs(got.astype(np.float64) - N_ref) < 1e-15)
+        assert ok.all(), f"{(~ok).sum()} entries off; worst ulp {ulp[~ok].max()}"
     # padding columns are zero
     if N_gpu.shape[2] > n:
         assert torch.count_nonzero(N_gpu[:, :, n:]).item() == 0
