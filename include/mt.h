@@ -182,6 +182,16 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* prob, const mt_integrator_opts* 
 /* Number of kernels this ctx has launched since creation (bench.py's gpu_launches).              */
 int64_t mt_launch_count(const mt_ctx* ctx);
 
+/* Per-kernel timing for the roofline (bench.py): between mt_profile_begin and mt_profile_end every
+ * launch of the demag field kernel (the dominant kernel of A4-A7; for small n its fixed-order second
+ * pass is included) is bracketed by CUDA events recorded on the ctx's stream, at most 1024 launches
+ * (later ones are not timed).  mt_profile_end synchronises the stream and returns the summed device
+ * time in milliseconds and the number of launches timed (HOST pointers).  Not for use while a CUDA
+ * graph is being replayed by mt_integrate (captured launches are not bracketed).
+ * Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA.                                                         */
+int mt_profile_begin(mt_ctx* ctx);
+int mt_profile_end(mt_ctx* ctx, double* total_ms, int64_t* launches);
+
 /* Tuning / A-B testing hook: selects the demag kernel variant (0 = default choice by shape,
  * 1 = register-streaming LDG kernel, 2 = TMA bulk-tensor pipeline).  Returns MT_OK or
  * MT_ERR_INVALID_ARG.  Results of all variants agree to rounding; each is deterministic.          */

@@ -25,7 +25,7 @@ MT_RK4, MT_DP45 = 0, 1
 COMPONENTS = ("xx", "xy", "xz", "yy", "yz", "zz")
 EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assemble_tensor",
            "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_launch_count",
-           "mt_set_demag_variant")
+           "mt_set_demag_variant", "mt_profile_begin", "mt_profile_end")
 
 
 class MtError(RuntimeError):
@@ -84,6 +84,8 @@ def load() -> C.CDLL:
         lib.mt_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_void_p]
         lib.mt_destroy.argtypes = [C.c_void_p]
         lib.mt_set_demag_variant.argtypes = [C.c_void_p, C.c_int]
+        lib.mt_profile_begin.argtypes = [C.c_void_p]
+        lib.mt_profile_end.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         lib.mt_assemble_tensor.argtypes = [C.c_void_p, C.POINTER(_Tiles), C.c_int, C.c_int64, C.c_int64,
                                            C.c_void_p, C.c_int64, C.c_void_p]
         lib.mt_demag_field.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64,
@@ -167,6 +169,17 @@ def mt_launch_count(ctx: Context) -> int:
 
 def mt_set_demag_variant(ctx: Context, variant: int):
     ctx.check(ctx.lib.mt_set_demag_variant(ctx.h, variant))
+
+
+def mt_profile_begin(ctx: Context):
+    ctx.check(ctx.lib.mt_profile_begin(ctx.h))
+
+
+def mt_profile_end(ctx: Context):
+    """Returns (summed device time of the demag field kernel in ms, launches timed)."""
+    ms, cnt = C.c_double(0.0), C.c_int64(0)
+    ctx.check(ctx.lib.mt_profile_end(ctx.h, C.byref(ms), C.byref(cnt)))
+    return ms.value, cnt.value
 
 
 @dataclass

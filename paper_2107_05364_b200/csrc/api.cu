@@ -136,6 +136,10 @@ int mt_destroy(mt_ctx* c) {
   cudaFreeHost(c->hscal);
   cudaFreeHost(c->pinned_io);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
+  if (c->prof_ev) {
+    for (int k = 0; k < 2 * MT_PROF_CAP; ++k) cudaEventDestroy(c->prof_ev[k]);
+    delete[] c->prof_ev;
+  }
   delete c;
   return MT_OK;
 }
@@ -143,6 +147,35 @@ int mt_destroy(mt_ctx* c) {
 const char* mt_last_error(const mt_ctx* c) { return c ? c->err : "mt_ctx is NULL"; }
 
 int64_t mt_launch_count(const mt_ctx* c) { return c ? c->launches : 0; }
+
+int mt_profile_begin(mt_ctx* c) {
+  if (!c) return MT_ERR_INVALID_ARG;
+  MT_CUDA_OK(c, cudaSetDevice(c->device));
+  if (!c->prof_ev) {
+    c->prof_ev = new (std::nothrow) cudaEvent_t[2 * MT_PROF_CAP];
+    if (!c->prof_ev) return mt_fail(c, MT_ERR_CUDA, "out of host memory");
+    for (int k = 0; k < 2 * MT_PROF_CAP; ++k) MT_CUDA_OK(c, cudaEventCreate(&c->prof_ev[k]));
+  }
+  c->prof_count = 0;
+  c->prof_on = 1;
+  return MT_OK;
+}
+
+int mt_profile_end(mt_ctx* c, double* total_ms, int64_t* launches) {
+  if (!c || !total_ms || !launches) return MT_ERR_INVALID_ARG;
+  *total_ms = 0.0;
+  *launches = 0;
+  if (!c->prof_on) return mt_fail(c, MT_ERR_INVALID_ARG, "mt_profile_end without mt_profile_begin");
+  c->prof_on = 0;
+  MT_CUDA_OK(c, cudaStreamSynchronize(c->stream));
+  for (int k = 0; k < c->prof_count; ++k) {
+    float ms = 0.f;
+    MT_CUDA_OK(c, cudaEventElapsedTime(&ms, c->prof_ev[2 * k], c->prof_ev[2 * k + 1]));
+    *total_ms += ms;
+  }
+  *launches = c->prof_count;
+  return MT_OK;
+}
 
 int mt_set_demag_variant(mt_ctx* c, int variant) {
   if (!c || variant < 0 || variant > 2) return MT_ERR_INVALID_ARG;
@@ -344,12 +377,15 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
             const int64_t l0 = ctx->launches;
             MT_CUDA_OK(ctx, cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal));
             ctx->stream = ctx->cap_stream;
+            const int prof_saved = ctx->prof_on;
+            ctx->prof_on = 0;  // timing events must not become graph nodes
             int r = MT_OK;
             for (int64_t s = 0; s < chunk && !r; ++s) {
               r = stage1();
               if (!r) r = stages234();
             }
             ctx->stream = st;
+            ctx->prof_on = prof_saved;
             cudaError_t ce = cudaStreamEndCapture(ctx->cap_stream, &graph);
             graph_launches = ctx->launches - l0;
             ctx->launches = l0;  // captured, not yet launched

@@ -338,8 +338,8 @@ int mt_launch_stage_M(mt_ctx* ctx, int dtype, const double* Ms, const double* m,
   return MT_OK;
 }
 
-int mt_launch_demag(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
-                    const void* Mst, int64_t npad, const EpiArgs& epi) {
+static int launch_demag_variant(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                                const void* Mst, int64_t npad, const EpiArgs& epi) {
   if (ctx->variant != 1) {
     int rc = mt_launch_demag_tma(ctx, N, dtype, n, n_rows, ld, Mst, npad, epi);
     if (rc != MT_ERR_UNIMPLEMENTED) return rc;
@@ -347,6 +347,18 @@ int mt_launch_demag(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_
   }
   if (dtype == MT_F32) return launch_ldg<float>(ctx, N, n, n_rows, ld, Mst, npad, epi);
   return launch_ldg<double>(ctx, N, n, n_rows, ld, Mst, npad, epi);
+}
+
+int mt_launch_demag(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                    const void* Mst, int64_t npad, const EpiArgs& epi) {
+  const bool prof = ctx->prof_on && ctx->prof_ev && ctx->prof_count < MT_PROF_CAP;
+  if (prof) MT_CUDA_OK(ctx, cudaEventRecord(ctx->prof_ev[2 * ctx->prof_count], ctx->stream));
+  const int rc = launch_demag_variant(ctx, N, dtype, n, n_rows, ld, Mst, npad, epi);
+  if (prof) {
+    MT_CUDA_OK(ctx, cudaEventRecord(ctx->prof_ev[2 * ctx->prof_count + 1], ctx->stream));
+    ctx->prof_count++;
+  }
+  return rc;
 }
 
 int mt_launch_local_only(mt_ctx* ctx, const EpiArgs& epi) {

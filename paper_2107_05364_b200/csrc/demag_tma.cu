@@ -1,8 +1,410 @@
-// demag_tma.cu — A4/A7, TMA bulk-tensor pipeline variant (placeholder until the pipeline lands:
-// reports MT_ERR_UNIMPLEMENTED so that the dispatcher falls back to the register-streaming kernel).
-#include "mt_internal.cuh"
+// demag_tma.cu — A4/A7, TMA bulk-tensor pipeline variant of H_d = -N.(Ms m) ("demag_tma").
+//
+// PAPER.md:17,122,138 name this product as the dominant cost; PAPER.md:145 moves it to CUDA.  The
+// kernel is HBM-bound: per call it must stream the six component planes once.
+//
+// Shape.  A persistent grid of P = (#SMs) CTAs.  The work is the flattened space of tiles
+// (row group g of RT target rows) x (column chunk k of CT source columns); CTA c owns the contiguous
+// range [T c / P, T (c+1) / P) of it, so every SM streams the same number of bytes (+-1 tile) whatever
+// n is.  One producer thread issues, per tile, ONE 3-D TMA box {CT, RT, 6} of the tensor (all six
+// planes; out-of-range rows/columns are zero-filled by the hardware, which is the ragged-tail
+// handling) and one 2-D box {CT, 3B} of the staged magnetisation M into a ring of STAGES shared
+// memory buffers guarded by full/empty mbarriers; eight consumer warps (warp w owns rows
+// w*RW .. w*RW+RW-1 of the group) multiply out of shared memory.  The producer is lane 0 of warp 0,
+// which tops the ring up (non-blocking probe of the empty barriers) before each of its own tiles:
+// a ninth warp would cap every thread at 168 registers (three warps on one SM sub-partition), too
+// few for the B = 8 accumulators.  Bytes in flight per SM = the ring
+// (up to ~200 KB), independent of registers and occupancy.
+//
+// Arithmetic (Q19): fp32 tensors: fp32 products, fp32 partial sums over ONE tile (at most
+// CT/32*4*3 = 96 terms per lane), then fp64; fp64 tensors: DFMA throughout.  Lanes are combined
+// with a fixed xor butterfly; a group finished inside one CTA goes straight to the fused epilogue
+// (epilogue.cuh); a group split between CTAs leaves per-CTA partial sums that a small second kernel
+// adds in CTA order — no atomics, bitwise reproducible for a given (n, n_rows, #SMs).
+#include <cuda.h>
 
-int mt_launch_demag_tma(mt_ctx*, const void*, int, int64_t, int64_t, int64_t, const void*, int64_t,
-                        const EpiArgs&) {
-  return MT_ERR_UNIMPLEMENTED;
+#include "epilogue.cuh"
+
+namespace {
+
+constexpr int kConsumerWarps = 8;
+constexpr int kThreads = kConsumerWarps * 32;
+
+template <typename T> struct Vec;
+template <> struct Vec<float> { typedef float4 type; static constexpr int W = 4; };
+template <> struct Vec<double> { typedef double2 type; static constexpr int W = 2; };
+
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_test(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(ok)
+      : "r"(bar), "r"(parity)
+      : "memory");
+  return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* map, int c0, int c1, int c2,
+                                            uint32_t bar, uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%2, %3, %4}], [%5], %6;" ::"r"(dst),
+      "l"(map), "r"(c0), "r"(c1), "r"(c2), "r"(bar), "l"(policy)
+      : "memory");
+}
+__device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* map, int c0, int c1, uint32_t bar,
+                                            uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%2, %3}], [%4], %5;" ::"r"(dst),
+      "l"(map), "r"(c0), "r"(c1), "r"(bar), "l"(policy)
+      : "memory");
+}
+
+__device__ __forceinline__ void fma3(float acc[3], const float4 v[6], const float4 m[3]) {
+#define MT_BLK(q)                                                            \
+  acc[0] = fmaf(v[0].q, m[0].q, fmaf(v[1].q, m[1].q, fmaf(v[2].q, m[2].q, acc[0]))); \
+  acc[1] = fmaf(v[1].q, m[0].q, fmaf(v[3].q, m[1].q, fmaf(v[4].q, m[2].q, acc[1]))); \
+  acc[2] = fmaf(v[2].q, m[0].q, fmaf(v[4].q, m[1].q, fmaf(v[5].q, m[2].q, acc[2])));
+  MT_BLK(x) MT_BLK(y) MT_BLK(z) MT_BLK(w)
+#undef MT_BLK
+}
+__device__ __forceinline__ void fma3(double acc[3], const double2 v[6], const double2 m[3]) {
+#define MT_BLK(q)                                                        \
+  acc[0] = fma(v[0].q, m[0].q, fma(v[1].q, m[1].q, fma(v[2].q, m[2].q, acc[0]))); \
+  acc[1] = fma(v[1].q, m[0].q, fma(v[3].q, m[1].q, fma(v[4].q, m[2].q, acc[1]))); \
+  acc[2] = fma(v[2].q, m[0].q, fma(v[4].q, m[1].q, fma(v[5].q, m[2].q, acc[2])));
+  MT_BLK(x) MT_BLK(y)
+#undef MT_BLK
+}
+
+struct TmaArgs {
+  int64_t n_rows;
+  int64_t groups;   // ceil(n_rows / RT)
+  int64_t chunks;   // ceil(n / CT)
+  int64_t tiles;    // groups * chunks
+  double* partial;  // [P][2][RT][B][3]
+};
+
+__host__ __device__ __forceinline__ int64_t range_begin(int64_t tiles, int64_t P, int64_t c) {
+  return (int64_t)(((unsigned __int128)tiles * (unsigned __int128)c) / (unsigned __int128)P);
+}
+
+template <typename T, int B, int RW, int CT, int STAGES>
+struct TmaCfg {
+  static constexpr int RT = kConsumerWarps * RW;
+  static constexpr int W = Vec<T>::W;
+  static constexpr int VPL = CT / (32 * W);  // 16-byte vectors per lane per row-plane per tile
+  static constexpr size_t tensor_bytes = (size_t)6 * RT * CT * sizeof(T);
+  static constexpr size_t m_bytes = (size_t)3 * B * CT * sizeof(T);
+  static constexpr size_t stage_bytes = tensor_bytes + m_bytes;
+  static constexpr size_t smem_bytes = STAGES * stage_bytes + 2 * STAGES * sizeof(uint64_t) + 128;
+  static_assert(CT % (32 * W) == 0, "tile width must be a whole number of warp-wide vectors");
+  static_assert(tensor_bytes % 128 == 0 && m_bytes % 128 == 0, "TMA destinations must stay 128-byte aligned");
+};
+
+template <typename T, int B, int RW, int CT, int STAGES>
+__global__ void __launch_bounds__(kThreads, 1)
+    demag_tma_kernel(const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmM, TmaArgs a,
+                     EpiArgs e) {
+  typedef TmaCfg<T, B, RW, CT, STAGES> Cfg;
+  typedef typename Vec<T>::type V;
+  constexpr int RT = Cfg::RT, VPL = Cfg::VPL;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  unsigned char* smem = (unsigned char*)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+  uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::stage_bytes);
+  const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t P = gridDim.x, c = blockIdx.x;
+  const int64_t t0 = range_begin(a.tiles, P, c), t1 = range_begin(a.tiles, P, c + 1);
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, kConsumerWarps);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (t0 >= t1) return;
+
+  // ===== producer state (used by lane 0 of warp 0 only) =====
+  uint64_t pol_stream = 0, pol_keep = 0;
+  int p_stage = 0;
+  uint32_t p_phase = 0;
+  int64_t p_t = t0, p_g = t0 / a.chunks, p_k = t0 % a.chunks;
+  const bool is_producer = (threadIdx.x == 0);
+  if (is_producer) {
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+  }
+  // issues tiles until the ring is full or a slot is still being read; `must` = tile index that has to
+  // be in flight on return (blocking wait for its slot if necessary)
+  auto top_up = [&](int64_t must) {
+    while (p_t < t1) {
+      if (!mbar_test(empty0 + 8 * p_stage, p_phase ^ 1)) {
+        if (p_t > must) break;
+        mbar_wait(empty0 + 8 * p_stage, p_phase ^ 1);
+      }
+      const uint32_t dst = smem_u32(smem + (size_t)p_stage * Cfg::stage_bytes);
+      mbar_expect_tx(full0 + 8 * p_stage, (uint32_t)Cfg::stage_bytes);
+      tma_load_3d(dst, &tmN, (int)(p_k * CT), (int)(p_g * RT), 0, full0 + 8 * p_stage, pol_stream);
+      tma_load_2d(dst + (uint32_t)Cfg::tensor_bytes, &tmM, (int)(p_k * CT), 0, full0 + 8 * p_stage, pol_keep);
+      if (++p_stage == STAGES) { p_stage = 0; p_phase ^= 1; }
+      if (++p_k == a.chunks) { p_k = 0; ++p_g; }
+      ++p_t;
+    }
+  };
+
+  // ===== consumers =====
+  double acc[RW][B][3];
+#pragma unroll
+  for (int r = 0; r < RW; ++r)
+#pragma unroll
+    for (int b = 0; b < B; ++b) acc[r][b][0] = acc[r][b][1] = acc[r][b][2] = 0.0;
+  int stage = 0;
+  uint32_t phase = 0;
+  int64_t g = t0 / a.chunks, k = t0 % a.chunks;
+  const int64_t g_first = g;
+  bool head_in_range = (k == 0);  // the current group's first chunk belongs to this CTA
+  for (int64_t t = t0; t < t1; ++t) {
+    if (is_producer) top_up(t);
+    __syncwarp();
+    mbar_wait(full0 + 8 * stage, phase);
+    const T* tile = (const T*)(smem + (size_t)stage * Cfg::stage_bytes);
+    const T* mt = (const T*)(smem + (size_t)stage * Cfg::stage_bytes + Cfg::tensor_bytes);
+    T run[RW][B][3];
+#pragma unroll
+    for (int r = 0; r < RW; ++r)
+#pragma unroll
+      for (int b = 0; b < B; ++b) run[r][b][0] = run[r][b][1] = run[r][b][2] = T(0);
+#pragma unroll
+    for (int v = 0; v < VPL; ++v) {
+      const int col = (v * 32 + lane) * Cfg::W;
+      V tv[RW][6];
+#pragma unroll
+      for (int r = 0; r < RW; ++r)
+#pragma unroll
+        for (int cc = 0; cc < 6; ++cc)
+          tv[r][cc] = *(const V*)(tile + ((size_t)cc * RT + (warp * RW + r)) * CT + col);
+#pragma unroll
+      for (int b = 0; b < B; ++b) {
+        V mv[3];
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc) mv[cc] = *(const V*)(mt + (size_t)(b * 3 + cc) * CT + col);
+#pragma unroll
+        for (int r = 0; r < RW; ++r) fma3(run[r][b], tv[r], mv);
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+    if (++stage == STAGES) { stage = 0; phase ^= 1; }
+#pragma unroll
+    for (int r = 0; r < RW; ++r)
+#pragma unroll
+      for (int b = 0; b < B; ++b) {
+        acc[r][b][0] += (double)run[r][b][0];
+        acc[r][b][1] += (double)run[r][b][1];
+        acc[r][b][2] += (double)run[r][b][2];
+      }
+    const bool group_done = (k + 1 == a.chunks);
+    if (group_done || t + 1 == t1) {
+      // fixed-order butterfly: every lane ends with the same sums
+#pragma unroll
+      for (int r = 0; r < RW; ++r)
+#pragma unroll
+        for (int b = 0; b < B; ++b)
+#pragma unroll
+          for (int cc = 0; cc < 3; ++cc)
+#pragma unroll
+            for (int off = 16; off > 0; off >>= 1)
+              acc[r][b][cc] += __shfl_xor_sync(0xffffffffu, acc[r][b][cc], off);
+      const bool whole = head_in_range && group_done;
+#pragma unroll
+      for (int r = 0; r < RW; ++r) {
+        const int rg = warp * RW + r;
+        const int64_t row = g * RT + rg;
+        double s[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+        for (int b = 0; b < B; ++b)
+          if (lane == b) { s[0] = acc[r][b][0]; s[1] = acc[r][b][1]; s[2] = acc[r][b][2]; }
+        if (lane < B && row < a.n_rows) {
+          if (whole) {
+            const double hd[3] = {-s[0], -s[1], -s[2]};
+            row_epilogue(e, row, lane, hd);
+          } else {
+            const int slot = (g == g_first) ? 0 : 1;
+            double* p = a.partial + ((((int64_t)c * 2 + slot) * RT + rg) * B + lane) * 3;
+            p[0] = s[0]; p[1] = s[1]; p[2] = s[2];
+          }
+        }
+      }
+#pragma unroll
+      for (int r = 0; r < RW; ++r)
+#pragma unroll
+        for (int b = 0; b < B; ++b) acc[r][b][0] = acc[r][b][1] = acc[r][b][2] = 0.0;
+    }
+    if (group_done) { k = 0; ++g; head_in_range = true; } else { ++k; }
+  }
+}
+
+// second pass: groups that were split between CTAs — add the per-CTA partial sums in CTA order
+template <int RT>
+__global__ void __launch_bounds__(256) demag_tma_fixup_kernel(TmaArgs a, int64_t P, int B, EpiArgs e) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= a.n_rows * B) return;
+  const int b = (int)(idx / a.n_rows);
+  const int64_t row = idx % a.n_rows;
+  const int64_t g = row / RT;
+  const int rg = (int)(row % RT);
+  const int64_t tb = g * a.chunks, te = tb + a.chunks;  // tiles of this group
+  // CTA that owns tile t: the c with begin(c) <= t < begin(c+1)
+  auto owner = [&](int64_t t) {
+    int64_t c = (int64_t)(((unsigned __int128)t * (unsigned __int128)P) / (unsigned __int128)a.tiles);
+    while (c + 1 < P && range_begin(a.tiles, P, c + 1) <= t) ++c;
+    while (c > 0 && range_begin(a.tiles, P, c) > t) --c;
+    return c;
+  };
+  const int64_t c_lo = owner(tb), c_hi = owner(te - 1);
+  if (c_lo == c_hi) return;  // finished inside one CTA: epilogue already done there
+  double s[3] = {0.0, 0.0, 0.0};
+  for (int64_t c = c_lo; c <= c_hi; ++c) {
+    const int64_t cb = range_begin(a.tiles, P, c), ce = range_begin(a.tiles, P, c + 1);
+    if (cb >= ce) continue;
+    const int slot = (cb / a.chunks == g) ? 0 : 1;
+    const double* p = a.partial + ((((int64_t)c * 2 + slot) * RT + rg) * B + b) * 3;
+    s[0] += p[0]; s[1] += p[1]; s[2] += p[2];
+  }
+  const double hd[3] = {-s[0], -s[1], -s[2]};
+  row_epilogue(e, row, b, hd);
+}
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_fn() {
+  static EncodeTiledFn fn = nullptr;
+  static bool tried = false;
+  if (!tried) {
+    tried = true;
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess &&
+        q == cudaDriverEntryPointSuccess)
+      fn = (EncodeTiledFn)p;
+  }
+  return fn;
+}
+
+int make_map(mt_ctx* ctx, CUtensorMap* out, int dtype, const void* base, int rank, const uint64_t* dims,
+             const uint64_t* strides_bytes, const uint32_t* box) {
+  EncodeTiledFn fn = encode_fn();
+  if (!fn) return mt_fail(ctx, MT_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
+  const cuuint32_t ones[3] = {1, 1, 1};
+  CUresult r = fn(out, dtype == MT_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64,
+                  (cuuint32_t)rank, const_cast<void*>(base), (const cuuint64_t*)dims, (const cuuint64_t*)strides_bytes,
+                  (const cuuint32_t*)box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                  CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) return mt_fail(ctx, MT_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
+  return MT_OK;
+}
+
+template <typename T, int B, int RW, int CT, int STAGES>
+int launch_cfg(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
+               int64_t npad, const EpiArgs& e) {
+  typedef TmaCfg<T, B, RW, CT, STAGES> Cfg;
+  constexpr int RT = Cfg::RT;
+  static_assert(Cfg::smem_bytes <= 227 * 1024, "ring does not fit shared memory");
+  const int64_t P = ctx->num_sms;
+  TmaArgs a;
+  a.n_rows = n_rows;
+  a.groups = (n_rows + RT - 1) / RT;
+  a.chunks = (n + CT - 1) / CT;
+  a.tiles = a.groups * a.chunks;
+  const size_t need = (size_t)P * 2 * RT * B * 3 * sizeof(double);
+  int rc = mt_ensure_ws(ctx, (void**)&ctx->partial, &ctx->partial_bytes, need);
+  if (rc) return rc;
+  a.partial = ctx->partial;
+  alignas(64) CUtensorMap tmN, tmM;
+  {
+    const uint64_t dims[3] = {(uint64_t)n, (uint64_t)n_rows, 6};
+    const uint64_t strides[2] = {(uint64_t)ld * sizeof(T), (uint64_t)n_rows * (uint64_t)ld * sizeof(T)};
+    const uint32_t box[3] = {CT, RT, 6};
+    if ((rc = make_map(ctx, &tmN, dtype, N, 3, dims, strides, box))) return rc;
+  }
+  {
+    const uint64_t dims[2] = {(uint64_t)npad, (uint64_t)(3 * B)};
+    const uint64_t strides[1] = {(uint64_t)npad * sizeof(T)};
+    const uint32_t box[2] = {CT, 3 * B};
+    if ((rc = make_map(ctx, &tmM, dtype, Mst, 2, dims, strides, box))) return rc;
+  }
+  auto kern = demag_tma_kernel<T, B, RW, CT, STAGES>;
+  static bool attr_set = false;
+  if (!attr_set) {
+    MT_CUDA_OK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes));
+    attr_set = true;
+  }
+  kern<<<(unsigned)P, kThreads, Cfg::smem_bytes, ctx->stream>>>(tmN, tmM, a, e);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  const int64_t tot = n_rows * B;
+  demag_tma_fixup_kernel<RT><<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(a, P, B, e);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+template <typename T>
+int launch_T(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
+             int64_t npad, const EpiArgs& e) {
+  constexpr int CT1 = 1024 / sizeof(T);  // 1 KB of one row-plane per tile
+  switch (e.batch) {
+    case 1: return launch_cfg<T, 1, 1, CT1, 4>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+    case 2: return launch_cfg<T, 2, 1, CT1, 4>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+    case 3: return launch_cfg<T, 3, 1, CT1, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+    case 4: return launch_cfg<T, 4, 1, CT1, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+    case 5: return launch_cfg<T, 5, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+    case 6: return launch_cfg<T, 6, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+    case 7: return launch_cfg<T, 7, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+    case 8: return launch_cfg<T, 8, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+  }
+  return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
+}
+
+}  // namespace
+
+// Returns MT_ERR_UNIMPLEMENTED when the shape is better served by the register-streaming kernel
+// (too few tiles to give every SM a share); the dispatcher then falls back to it.
+int mt_launch_demag_tma(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                        const void* Mst, int64_t npad, const EpiArgs& e) {
+  if (ctx->variant != 2) {
+    const int64_t tiles = ((n_rows + 7) / 8) * ((n * (dtype == MT_F32 ? 4 : 8) + 1023) / 1024);
+    if (tiles < 16LL * ctx->num_sms) return MT_ERR_UNIMPLEMENTED;
+  }
+  if (dtype == MT_F32) return launch_T<float>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+  return launch_T<double>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
 }

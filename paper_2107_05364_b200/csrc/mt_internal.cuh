@@ -37,7 +37,12 @@ struct mt_ctx {
   int64_t tm_n, tm_rows, tm_ld;
   alignas(64) unsigned char tm_desc[128];
   int tm_valid;
+  // per-kernel timing of the demag field kernel (mt_profile_begin / mt_profile_end)
+  int prof_on;
+  int prof_count;
+  cudaEvent_t* prof_ev;  // MT_PROF_CAP pairs, created lazily
 };
+#define MT_PROF_CAP 1024
 
 int mt_fail(mt_ctx* ctx, int code, const char* fmt, ...);
 #define MT_CUDA_OK(ctx, expr)                                                                  \
