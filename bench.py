@@ -27,6 +27,10 @@ if ROOT not in sys.path:
 METRIC = "demag_Hd_evals_per_s"
 UNIT = "evals/s"
 HBM_FALLBACK_GBS = 6650.0  # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture (profiles/); key = (config, tensor dtype, n_gpus)
+NCU_TRAFFIC_BYTES = {(5, "f32", 1): 103.082310e9 + 5.798656e6}
+NCU_TRAFFIC_SOURCE = "profiles/r01b_demag_tma_f32_b1_ncu_full.md"
 
 
 def parse_args():
@@ -180,6 +184,7 @@ def main():
     import numpy as np
     import torch
     from paper_2107_05364_b200 import binding as B
+    from paper_2107_05364_b200 import sharding as S
     from paper_2107_05364_b200 import workloads as W
     from tests import harness as H
 
@@ -201,7 +206,7 @@ def main():
         B.mt_set_demag_variant(ctx, args.variant)
     tiles = H.dev_tiles(w, dev)
     # rows of this rank (§8e: the tensor is sharded by target rows; no collective in assembly)
-    r0, r1 = rank * n // world, (rank + 1) * n // world
+    r0, r1 = S.row_band(rank, world, n)
     rows = r1 - r0
     ld = W.leading_dim(n, dtype)
     N = torch.empty((6, rows, ld), dtype=B.torch_dtype(code), device=dev)
@@ -230,34 +235,47 @@ def main():
     m_all = torch.from_numpy(w.m).to(dev)              # [8, 3, n]
     m1 = m_all[:1].contiguous()
     Hd1 = torch.empty((1, 3, rows), dtype=torch.float64, device=dev)
-    Hd_full = torch.empty((world, 3 * rows), dtype=torch.float64, device=dev) if world > 1 else None
+    gather_scratch = (torch.empty((world, 1, 3, S.max_band_rows(world, n)), dtype=torch.float64, device=dev)
+                      if world > 1 else None)
 
     def step_field():
         B.mt_demag_field(ctx, N, code, n, rows, ld, tiles.Ms, m1, 1, Hd1)
         if dist is not None:  # the one real exchange step: every rank needs the whole field / next m
-            dist.all_gather_into_tensor(Hd_full.view(-1), Hd1.view(-1))
+            S.all_gather_field(dist, Hd1, n, rank, world, scratch=gather_scratch)
 
-    def timed(fn, warmup, steps, clocks=False):
+    kernel_ms = {}
+
+    def timed(fn, warmup, steps, clocks=False, tag=None):
+        """CUDA-event time per step (max over ranks).  With `tag`, the library also brackets every
+        launch of the demag field kernel with its own events on the launching stream
+        (mt_profile_begin/end): kernel_ms[tag] = that kernel's average device time per launch."""
         for _ in range(warmup):
             fn()
         barrier()
         sampler = ClockSampler(local_rank) if (clocks and rank == 0) else None
         e0, e1 = ev(), ev()
         l0 = ctx.launches
+        if tag:
+            B.mt_profile_begin(ctx)
         e0.record()
         for _ in range(steps):
             fn()
         e1.record()
         barrier()
+        if tag:
+            tot, cnt = B.mt_profile_end(ctx)
+            kernel_ms[tag] = tot / max(1, cnt)
         ms = e0.elapsed_time(e1) / steps
         if dist is not None:
-            t = torch.tensor([ms], device=dev)
+            t = torch.tensor([ms, kernel_ms.get(tag, 0.0)], device=dev)
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+            ms = float(t[0].item())
+            if tag:
+                kernel_ms[tag] = float(t[1].item())
         return ms, (ctx.launches - l0), (sampler.stop() if sampler else None)
 
     K, Wm = max(1, args.steps), max(3, args.warmup)
-    ms_step, launches, clocks = timed(step_field, Wm, K, clocks=True)
+    ms_step, launches, clocks = timed(step_field, Wm, K, clocks=True, tag="b1")
     value = 1000.0 / ms_step
 
     out = {
@@ -273,11 +291,15 @@ def main():
     s = 4 if dtype == "f32" else 8
     alg_bytes = 6.0 * rows * n * s + 3.0 * n * s + 24.0 * rows
     peak, peak_src = peak_hbm()
-    achieved = alg_bytes / (ms_step * 1e-3) / 1e9
+    achieved = alg_bytes / (kernel_ms["b1"] * 1e-3) / 1e9
     out["roofline"] = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                       "traffic": None, "peak_source": peak_src, "kernel": "demag field kernel (per rank)",
+                       "traffic": NCU_TRAFFIC_BYTES.get((args.config, dtype, world)) if not args.grid else None,
+                       "traffic_source": NCU_TRAFFIC_SOURCE,
+                       "peak_source": peak_src, "kernel": "demag field kernel (per rank), batch 1",
+                       "kernel_ms": kernel_ms["b1"], "kernel_share_of_step": kernel_ms["b1"] / ms_step,
                        "algorithmic_bytes_per_launch": alg_bytes,
-                       "note": "duration = CUDA-event time of the whole mt_demag_field step (staging kernel included)"}
+                       "note": "duration = CUDA events recorded by the library on the launching stream around "
+                               "the demag field kernel only (mt_profile_begin/end), averaged over the timed steps"}
     out["assembly"] = {"pairs_per_s": rows * n / (asm_ms * 1e-3) * world, "ms": asm_ms, "pairs": rows * n * world,
                        "launches": asm_launches, "dtype": dtype, "every_pair_evaluated": True}
 
@@ -304,11 +326,13 @@ def main():
 
         def step_b8():
             B.mt_demag_field(ctx, N, code, n, rows, ld, tiles.Ms, m_all, 8, Hd8)
-        ms_b8, _, _ = timed(step_b8, 3, max(5, K // 4))
-        out["batch8"] = {"state_evals_per_s": 8000.0 / ms_b8, "ms": ms_b8,
-                         "achieved_gbs": alg_bytes / (ms_b8 * 1e-3) / 1e9}
+        ms_b8, _, _ = timed(step_b8, 3, max(5, K // 4), tag="b8")
+        alg_b8 = 6.0 * rows * n * s + 8 * 3.0 * n * s + 8 * 24.0 * rows
+        out["batch8"] = {"state_evals_per_s": 8000.0 / ms_b8, "ms": ms_b8, "kernel_ms": kernel_ms["b8"],
+                         "achieved_gbs": alg_b8 / (kernel_ms["b8"] * 1e-3) / 1e9,
+                         "frac": alg_b8 / (kernel_ms["b8"] * 1e-3) / 1e9 / peak}
         if rank == 0 and world == 1:
-            out["cpu_baseline"] = oracle_sample(w, band_rows=64, calls=3)
+            out["cpu_baseline"] = oracle_sample(w, band_rows=4096, calls=6)
     if rank == 0:
         print(json.dumps(out))
     ctx.close()
