@@ -22,13 +22,17 @@ int check_tensor_args(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t 
   return MT_OK;
 }
 
+// The two staged-M buffers always have room for MT_MAX_BATCH states (the batched kernels' TMA boxes
+// may cover rows beyond 3*batch; what they read there is never used) and start out zeroed.
 int ensure_Mst(mt_ctx* ctx, int dtype, int batch, int64_t npad) {
-  const size_t need = (size_t)batch * 3 * npad * elem_size(dtype);
+  (void)batch;
+  const size_t need = (size_t)MT_MAX_BATCH * 3 * npad * elem_size(dtype);
   if (ctx->Mst_bytes >= need && ctx->Mst[0]) return MT_OK;
   for (int k = 0; k < 2; ++k) {
     size_t cur = ctx->Mst[k] ? ctx->Mst_bytes : 0;
     int rc = mt_ensure_ws(ctx, &ctx->Mst[k], &cur, need);
     if (rc) return rc;
+    MT_CUDA_OK(ctx, cudaMemsetAsync(ctx->Mst[k], 0, need, ctx->stream));
   }
   ctx->Mst_bytes = need;
   return MT_OK;

@@ -17,7 +17,9 @@
 // (up to ~200 KB), independent of registers and occupancy.
 //
 // Arithmetic (Q19): fp32 tensors: fp32 products, fp32 partial sums over ONE tile (at most
-// CT/32*4*3 = 96 terms per lane), then fp64; fp64 tensors: DFMA throughout.  Lanes are combined
+// CT/32*4*3 = 96 terms per lane), then fp64; fp64 tensors: DFMA throughout.  Batches of 5..8 states
+// on fp32 tensors use `demag_tma_f32x2_kernel` below (packed FFMA2, the only way to the full FP32
+// rate on sm_100a: a three-register FFMA issues every other cycle per scheduler).  Lanes are combined
 // with a fixed xor butterfly; a group finished inside one CTA goes straight to the fused epilogue
 // (epilogue.cuh); a group split between CTAs leaves per-CTA partial sums that a small second kernel
 // adds in CTA order — no atomics, bitwise reproducible for a given (n, n_rows, #SMs).
@@ -101,6 +103,9 @@ __device__ __forceinline__ void fma3(double acc[3], const double2 v[6], const do
 #undef MT_BLK
 }
 
+template <typename T, bool Direct> struct RunSel { typedef T type; };
+template <typename T> struct RunSel<T, true> { typedef char type; };
+
 struct TmaArgs {
   int64_t n_rows;
   int64_t groups;   // ceil(n_rows / RT)
@@ -113,9 +118,10 @@ __host__ __device__ __forceinline__ int64_t range_begin(int64_t tiles, int64_t P
   return (int64_t)(((unsigned __int128)tiles * (unsigned __int128)c) / (unsigned __int128)P);
 }
 
-template <typename T, int B, int RW, int CT, int STAGES>
+template <typename T, int B, int RW, int CT_, int STAGES>
 struct TmaCfg {
   static constexpr int RT = kConsumerWarps * RW;
+  static constexpr int CT = CT_;
   static constexpr int W = Vec<T>::W;
   static constexpr int VPL = CT / (32 * W);  // 16-byte vectors per lane per row-plane per tile
   static constexpr size_t tensor_bytes = (size_t)6 * RT * CT * sizeof(T);
@@ -196,11 +202,20 @@ __global__ void __launch_bounds__(kThreads, 1)
     mbar_wait(full0 + 8 * stage, phase);
     const T* tile = (const T*)(smem + (size_t)stage * Cfg::stage_bytes);
     const T* mt = (const T*)(smem + (size_t)stage * Cfg::stage_bytes + Cfg::tensor_bytes);
-    T run[RW][B][3];
+    // fp32: a short fp32 run per tile, flushed into the fp64 accumulators below; fp64: the
+    // accumulators themselves (no second register set)
+    constexpr bool kDirect = (sizeof(T) == 8);
+    typedef typename RunSel<T, kDirect>::type RunT;
+    RunT run_store[kDirect ? 1 : RW][kDirect ? 1 : B][3];
+    auto run_of = [&](int r, int b) -> T* {
+      if constexpr (kDirect) return (T*)acc[r][b]; else return (T*)run_store[r][b];
+    };
+    if constexpr (!kDirect) {
 #pragma unroll
-    for (int r = 0; r < RW; ++r)
+      for (int r = 0; r < RW; ++r)
 #pragma unroll
-      for (int b = 0; b < B; ++b) run[r][b][0] = run[r][b][1] = run[r][b][2] = T(0);
+        for (int b = 0; b < B; ++b) run_store[r][b][0] = run_store[r][b][1] = run_store[r][b][2] = RunT(0);
+    }
 #pragma unroll
     for (int v = 0; v < VPL; ++v) {
       const int col = (v * 32 + lane) * Cfg::W;
@@ -216,20 +231,22 @@ __global__ void __launch_bounds__(kThreads, 1)
 #pragma unroll
         for (int cc = 0; cc < 3; ++cc) mv[cc] = *(const V*)(mt + (size_t)(b * 3 + cc) * CT + col);
 #pragma unroll
-        for (int r = 0; r < RW; ++r) fma3(run[r][b], tv[r], mv);
+        for (int r = 0; r < RW; ++r) fma3(run_of(r, b), tv[r], mv);
       }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(empty0 + 8 * stage);
     if (++stage == STAGES) { stage = 0; phase ^= 1; }
+    if constexpr (!kDirect) {
 #pragma unroll
-    for (int r = 0; r < RW; ++r)
+      for (int r = 0; r < RW; ++r)
 #pragma unroll
-      for (int b = 0; b < B; ++b) {
-        acc[r][b][0] += (double)run[r][b][0];
-        acc[r][b][1] += (double)run[r][b][1];
-        acc[r][b][2] += (double)run[r][b][2];
-      }
+        for (int b = 0; b < B; ++b) {
+          acc[r][b][0] += (double)run_store[r][b][0];
+          acc[r][b][1] += (double)run_store[r][b][1];
+          acc[r][b][2] += (double)run_store[r][b][2];
+        }
+    }
     const bool group_done = (k + 1 == a.chunks);
     if (group_done || t + 1 == t1) {
       // fixed-order butterfly: every lane ends with the same sums
@@ -266,6 +283,178 @@ __global__ void __launch_bounds__(kThreads, 1)
       for (int r = 0; r < RW; ++r)
 #pragma unroll
         for (int b = 0; b < B; ++b) acc[r][b][0] = acc[r][b][1] = acc[r][b][2] = 0.0;
+    }
+    if (group_done) { k = 0; ++g; head_in_range = true; } else { ++k; }
+  }
+}
+
+// ---- fp32 tensors, batches of 5..8 states: packed-FMA consumer -------------------------------------
+// Same ring, same work split, same fix-up as above; what differs is the arithmetic of a tile.  At
+// B = 8 a tile block (24 B) carries 72 FMAs: at the HBM rate that is 67 FMA/clk/SM, above what
+// three-register FFMA sustains (64/clk/SM), so the products are issued as FFMA2 (fma.rn.f32x2): the
+// two halves of a 64-bit register pair are two adjacent source columns, so an LDS.128 of a plane row
+// and an LDS.128 of a component of M are each two ready-made operands.  Each (row, state, component)
+// sum therefore lives in an even-column/odd-column pair of fp32 accumulators (2 rows x 8 states x 3
+// x 2 = 96 registers), which leaves no room for per-lane fp64 accumulators; instead, every kFlush
+// tiles (<= 96 terms per fp32 accumulator, Q19) and at the end of a row group the 48 fp32
+// sums of a lane are combined across the warp by a transposing butterfly (24+12+6+3+3 shuffles) after
+// which lane l holds the three components of (row l>>4, state (l>>1)&7) and adds them to three fp64
+// accumulators.  The order is fixed: bitwise reproducible.
+constexpr int kB8 = 8, kB8RW = 2, kB8CT = 128, kB8Flush = 16;
+
+__device__ __forceinline__ void ffma2(unsigned long long& d, unsigned long long a, unsigned long long b) {
+  asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b));
+}
+__device__ __forceinline__ float sum_halves(unsigned long long v) {
+  float lo, hi;
+  asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+  return lo + hi;
+}
+
+template <int STAGES>
+__global__ void __launch_bounds__(kThreads, 1)
+    demag_tma_f32x2_kernel(const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmM,
+                           TmaArgs a, EpiArgs e) {
+  typedef TmaCfg<float, kB8, kB8RW, kB8CT, STAGES> Cfg;
+  constexpr int RT = Cfg::RT, RW = kB8RW, B = kB8, CT = kB8CT;
+  static_assert(Cfg::VPL == 1 && RW * B == 16, "lane mapping of the transposing butterfly");
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  unsigned char* smem = (unsigned char*)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
+  uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::stage_bytes);
+  const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t P = gridDim.x, c = blockIdx.x;
+  const int64_t t0 = range_begin(a.tiles, P, c), t1 = range_begin(a.tiles, P, c + 1);
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, kConsumerWarps);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (t0 >= t1) return;
+
+  // producer (lane 0 of warp 0), as in demag_tma_kernel
+  uint64_t pol_stream = 0, pol_keep = 0;
+  int p_stage = 0;
+  uint32_t p_phase = 0;
+  int64_t p_t = t0, p_g = t0 / a.chunks, p_k = t0 % a.chunks;
+  const bool is_producer = (threadIdx.x == 0);
+  if (is_producer) {
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+  }
+  auto top_up = [&](int64_t must) {
+    while (p_t < t1) {
+      if (!mbar_test(empty0 + 8 * p_stage, p_phase ^ 1)) {
+        if (p_t > must) break;
+        mbar_wait(empty0 + 8 * p_stage, p_phase ^ 1);
+      }
+      const uint32_t dst = smem_u32(smem + (size_t)p_stage * Cfg::stage_bytes);
+      mbar_expect_tx(full0 + 8 * p_stage, (uint32_t)Cfg::stage_bytes);
+      tma_load_3d(dst, &tmN, (int)(p_k * CT), (int)(p_g * RT), 0, full0 + 8 * p_stage, pol_stream);
+      tma_load_2d(dst + (uint32_t)Cfg::tensor_bytes, &tmM, (int)(p_k * CT), 0, full0 + 8 * p_stage, pol_keep);
+      if (++p_stage == STAGES) { p_stage = 0; p_phase ^= 1; }
+      if (++p_k == a.chunks) { p_k = 0; ++p_g; }
+      ++p_t;
+    }
+  };
+
+  unsigned long long run[RW][B][3];  // {even-column sum, odd-column sum}
+#pragma unroll
+  for (int r = 0; r < RW; ++r)
+#pragma unroll
+    for (int b = 0; b < B; ++b) run[r][b][0] = run[r][b][1] = run[r][b][2] = 0ull;
+  double acc[3] = {0.0, 0.0, 0.0};  // of (row lane>>4, state (lane>>1)&7)
+  int since_flush = 0;
+  int stage = 0;
+  uint32_t phase = 0;
+  int64_t g = t0 / a.chunks, k = t0 % a.chunks;
+  const int64_t g_first = g;
+  bool head_in_range = (k == 0);
+  for (int64_t t = t0; t < t1; ++t) {
+    if (is_producer) top_up(t);
+    __syncwarp();
+    mbar_wait(full0 + 8 * stage, phase);
+    const float* tile = (const float*)(smem + (size_t)stage * Cfg::stage_bytes);
+    const float* mt = (const float*)(smem + (size_t)stage * Cfg::stage_bytes + Cfg::tensor_bytes);
+    const int col = lane * 4;
+    ulonglong2 tv[RW][6];
+#pragma unroll
+    for (int r = 0; r < RW; ++r)
+#pragma unroll
+      for (int cc = 0; cc < 6; ++cc)
+        tv[r][cc] = *(const ulonglong2*)(tile + ((size_t)cc * RT + (warp * RW + r)) * CT + col);
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+      ulonglong2 mv[3];
+#pragma unroll
+      for (int cc = 0; cc < 3; ++cc) mv[cc] = *(const ulonglong2*)(mt + (size_t)(b * 3 + cc) * CT + col);
+#pragma unroll
+      for (int r = 0; r < RW; ++r) {
+        // planes xx, xy, xz, yy, yz, zz = 0..5; columns {0,1} in .x, {2,3} in .y
+        ffma2(run[r][b][0], tv[r][0].x, mv[0].x); ffma2(run[r][b][0], tv[r][0].y, mv[0].y);
+        ffma2(run[r][b][0], tv[r][1].x, mv[1].x); ffma2(run[r][b][0], tv[r][1].y, mv[1].y);
+        ffma2(run[r][b][0], tv[r][2].x, mv[2].x); ffma2(run[r][b][0], tv[r][2].y, mv[2].y);
+        ffma2(run[r][b][1], tv[r][1].x, mv[0].x); ffma2(run[r][b][1], tv[r][1].y, mv[0].y);
+        ffma2(run[r][b][1], tv[r][3].x, mv[1].x); ffma2(run[r][b][1], tv[r][3].y, mv[1].y);
+        ffma2(run[r][b][1], tv[r][4].x, mv[2].x); ffma2(run[r][b][1], tv[r][4].y, mv[2].y);
+        ffma2(run[r][b][2], tv[r][2].x, mv[0].x); ffma2(run[r][b][2], tv[r][2].y, mv[0].y);
+        ffma2(run[r][b][2], tv[r][4].x, mv[1].x); ffma2(run[r][b][2], tv[r][4].y, mv[1].y);
+        ffma2(run[r][b][2], tv[r][5].x, mv[2].x); ffma2(run[r][b][2], tv[r][5].y, mv[2].y);
+      }
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+    if (++stage == STAGES) { stage = 0; phase ^= 1; }
+    const bool group_done = (k + 1 == a.chunks);
+    const bool emit = group_done || t + 1 == t1;
+    if (++since_flush == kB8Flush || emit) {
+      since_flush = 0;
+      // val[(r*8 + b)*3 + cc]; halving steps keep the lower or upper half of the index space by one
+      // lane bit each, so that after offsets 16, 8, 4, 2 lane l owns (r*8 + b) == l >> 1
+      float val[48];
+#pragma unroll
+      for (int r = 0; r < RW; ++r)
+#pragma unroll
+        for (int b = 0; b < B; ++b)
+#pragma unroll
+          for (int cc = 0; cc < 3; ++cc) {
+            val[(r * B + b) * 3 + cc] = sum_halves(run[r][b][cc]);
+            run[r][b][cc] = 0ull;
+          }
+#pragma unroll
+      for (int half = 24, off = 16; half >= 3; half >>= 1, off >>= 1) {
+        const bool upper = (lane & off) != 0;
+#pragma unroll
+        for (int i = 0; i < half; ++i) {
+          const float keep = upper ? val[i + half] : val[i];
+          const float send = upper ? val[i] : val[i + half];
+          val[i] = keep + __shfl_xor_sync(0xffffffffu, send, off);
+        }
+      }
+#pragma unroll
+      for (int cc = 0; cc < 3; ++cc) {
+        val[cc] += __shfl_xor_sync(0xffffffffu, val[cc], 1);
+        acc[cc] += (double)val[cc];
+      }
+    }
+    if (emit) {
+      const int rg = warp * RW + (lane >> 4), b = (lane >> 1) & 7;
+      const int64_t row = g * RT + rg;
+      if (!(lane & 1) && b < e.batch && row < a.n_rows) {
+        if (head_in_range && group_done) {
+          const double hd[3] = {-acc[0], -acc[1], -acc[2]};
+          row_epilogue(e, row, b, hd);
+        } else {
+          const int slot = (g == g_first) ? 0 : 1;
+          double* p = a.partial + ((((int64_t)c * 2 + slot) * RT + rg) * e.batch + b) * 3;
+          p[0] = acc[0]; p[1] = acc[1]; p[2] = acc[2];
+        }
+      }
+      acc[0] = acc[1] = acc[2] = 0.0;
     }
     if (group_done) { k = 0; ++g; head_in_range = true; } else { ++k; }
   }
@@ -333,19 +522,19 @@ int make_map(mt_ctx* ctx, CUtensorMap* out, int dtype, const void* base, int ran
   return MT_OK;
 }
 
-template <typename T, int B, int RW, int CT, int STAGES>
-int launch_cfg(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
-               int64_t npad, const EpiArgs& e) {
-  typedef TmaCfg<T, B, RW, CT, STAGES> Cfg;
+// Cfg = tile geometry; kern = the kernel instantiated for it; m_rows = rows of the staged-M box (3 B)
+template <typename T, typename Cfg, typename Kern>
+int launch_tiles(mt_ctx* ctx, Kern kern, bool* attr_set, int m_rows, const void* N, int dtype, int64_t n,
+                 int64_t n_rows, int64_t ld, const void* Mst, int64_t npad, const EpiArgs& e) {
   constexpr int RT = Cfg::RT;
   static_assert(Cfg::smem_bytes <= 227 * 1024, "ring does not fit shared memory");
   const int64_t P = ctx->num_sms;
   TmaArgs a;
   a.n_rows = n_rows;
   a.groups = (n_rows + RT - 1) / RT;
-  a.chunks = (n + CT - 1) / CT;
+  a.chunks = (n + Cfg::CT - 1) / Cfg::CT;
   a.tiles = a.groups * a.chunks;
-  const size_t need = (size_t)P * 2 * RT * B * 3 * sizeof(double);
+  const size_t need = (size_t)P * 2 * RT * e.batch * 3 * sizeof(double);
   int rc = mt_ensure_ws(ctx, (void**)&ctx->partial, &ctx->partial_bytes, need);
   if (rc) return rc;
   a.partial = ctx->partial;
@@ -353,29 +542,46 @@ int launch_cfg(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows,
   {
     const uint64_t dims[3] = {(uint64_t)n, (uint64_t)n_rows, 6};
     const uint64_t strides[2] = {(uint64_t)ld * sizeof(T), (uint64_t)n_rows * (uint64_t)ld * sizeof(T)};
-    const uint32_t box[3] = {CT, RT, 6};
+    const uint32_t box[3] = {(uint32_t)Cfg::CT, (uint32_t)RT, 6};
     if ((rc = make_map(ctx, &tmN, dtype, N, 3, dims, strides, box))) return rc;
   }
   {
-    const uint64_t dims[2] = {(uint64_t)npad, (uint64_t)(3 * B)};
+    // the staged-M buffers always hold MT_MAX_BATCH states (rows beyond 3*batch: zero or stale, unused)
+    const uint64_t dims[2] = {(uint64_t)npad, (uint64_t)(3 * MT_MAX_BATCH)};
     const uint64_t strides[1] = {(uint64_t)npad * sizeof(T)};
-    const uint32_t box[2] = {CT, 3 * B};
+    const uint32_t box[2] = {(uint32_t)Cfg::CT, (uint32_t)m_rows};
     if ((rc = make_map(ctx, &tmM, dtype, Mst, 2, dims, strides, box))) return rc;
   }
-  auto kern = demag_tma_kernel<T, B, RW, CT, STAGES>;
-  static bool attr_set = false;
-  if (!attr_set) {
+  if (!*attr_set) {
     MT_CUDA_OK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes));
-    attr_set = true;
+    *attr_set = true;
   }
   kern<<<(unsigned)P, kThreads, Cfg::smem_bytes, ctx->stream>>>(tmN, tmM, a, e);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
-  const int64_t tot = n_rows * B;
-  demag_tma_fixup_kernel<RT><<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(a, P, B, e);
+  const int64_t tot = n_rows * e.batch;
+  demag_tma_fixup_kernel<RT><<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(a, P, e.batch, e);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   return MT_OK;
+}
+
+template <typename T, int B, int RW, int CT, int STAGES>
+int launch_cfg(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
+               int64_t npad, const EpiArgs& e) {
+  static bool attr_set = false;
+  return launch_tiles<T, TmaCfg<T, B, RW, CT, STAGES>>(ctx, demag_tma_kernel<T, B, RW, CT, STAGES>, &attr_set, 3 * B,
+                                                        N, dtype, n, n_rows, ld, Mst, npad, e);
+}
+
+// fp32, 5 <= batch <= 8: packed-FMA kernel (states beyond `batch` are computed on unused rows of M
+// and dropped)
+int launch_f32x2(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld, const void* Mst, int64_t npad,
+                 const EpiArgs& e) {
+  static bool attr_set = false;
+  constexpr int STAGES = 3;
+  return launch_tiles<float, TmaCfg<float, kB8, kB8RW, kB8CT, STAGES>>(ctx, demag_tma_f32x2_kernel<STAGES>, &attr_set,
+                                                                      3 * kB8, N, MT_F32, n, n_rows, ld, Mst, npad, e);
 }
 
 template <typename T>
@@ -387,10 +593,18 @@ int launch_T(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, i
     case 2: return launch_cfg<T, 2, 1, CT1, 4>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
     case 3: return launch_cfg<T, 3, 1, CT1, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
     case 4: return launch_cfg<T, 4, 1, CT1, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
-    case 5: return launch_cfg<T, 5, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
-    case 6: return launch_cfg<T, 6, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
-    case 7: return launch_cfg<T, 7, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
-    case 8: return launch_cfg<T, 8, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+  }
+  if (e.batch >= 5 && e.batch <= MT_MAX_BATCH) {
+    if constexpr (sizeof(T) == 4) {
+      return launch_f32x2(ctx, N, n, n_rows, ld, Mst, npad, e);
+    } else {
+      switch (e.batch) {
+        case 5: return launch_cfg<T, 5, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+        case 6: return launch_cfg<T, 6, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+        case 7: return launch_cfg<T, 7, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+        case 8: return launch_cfg<T, 8, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+      }
+    }
   }
   return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
 }

@@ -36,7 +36,7 @@ def field(ctx, N, dtype, n, n_rows, ld, Ms, m_np):
 @pytest.mark.parametrize("grid,dtype,batch", [
     ((1, 1, 1), "f64", 1), ((3, 1, 1), "f32", 2), ((7, 5, 3), "f32", 1), ((7, 5, 3), "f64", 4),
     ((33, 31, 1), "f32", 3), ((16, 12, 4), "f32", 8), ((16, 12, 4), "f64", 8), ((41, 11, 3), "f32", 5),
-    ((41, 11, 3), "f64", 6), ((50, 30, 2), "f32", 7), ((50, 30, 2), "f32", 1)])
+    ((41, 11, 3), "f64", 6), ((41, 11, 3), "f32", 6), ((50, 30, 2), "f32", 7), ((50, 30, 2), "f32", 1)])
 def test_tma_field_matches_oracle(ctx, oracle, grid, dtype, batch):
     nx, ny, nz = grid
     n = nx * ny * nz
