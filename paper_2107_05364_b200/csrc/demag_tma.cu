@@ -30,6 +30,17 @@
 namespace {
 
 constexpr int kConsumerWarps = 8;
+// shape of the packed-FMA batched kernel (see demag_tma_f32x2_kernel)
+#ifndef MT_B8_WARPS
+#define MT_B8_WARPS 8   /* measured at N = 32,768, B = 8 (r01): 8/128/3 4.55 ms; 12/64/4 5.04; 8/64/6 6.2 */
+#define MT_B8_CT 128
+#define MT_B8_STAGES 3
+#endif
+#ifndef MT_B4_WARPS
+#define MT_B4_WARPS 8
+#define MT_B4_CT 128
+#define MT_B4_STAGES 4
+#endif
 constexpr int kThreads = kConsumerWarps * 32;
 
 template <typename T> struct Vec;
@@ -118,9 +129,10 @@ __host__ __device__ __forceinline__ int64_t range_begin(int64_t tiles, int64_t P
   return (int64_t)(((unsigned __int128)tiles * (unsigned __int128)c) / (unsigned __int128)P);
 }
 
-template <typename T, int B, int RW, int CT_, int STAGES>
+template <typename T, int B, int RW, int CT_, int STAGES, int WARPS_ = kConsumerWarps>
 struct TmaCfg {
-  static constexpr int RT = kConsumerWarps * RW;
+  static constexpr int WARPS = WARPS_;
+  static constexpr int RT = WARPS_ * RW;
   static constexpr int CT = CT_;
   static constexpr int W = Vec<T>::W;
   static constexpr int VPL = CT / (32 * W);  // 16-byte vectors per lane per row-plane per tile
@@ -128,7 +140,7 @@ struct TmaCfg {
   static constexpr size_t m_bytes = (size_t)3 * B * CT * sizeof(T);
   static constexpr size_t stage_bytes = tensor_bytes + m_bytes;
   static constexpr size_t smem_bytes = STAGES * stage_bytes + 2 * STAGES * sizeof(uint64_t) + 128;
-  static_assert(CT % (32 * W) == 0, "tile width must be a whole number of warp-wide vectors");
+  static_assert(CT % 64 == 0, "tile width must be a whole number of warp-wide 8-byte vectors");
   static_assert(tensor_bytes % 128 == 0 && m_bytes % 128 == 0, "TMA destinations must stay 128-byte aligned");
 };
 
@@ -300,7 +312,7 @@ __global__ void __launch_bounds__(kThreads, 1)
 // sums of a lane are combined across the warp by a transposing butterfly (24+12+6+3+3 shuffles) after
 // which lane l holds the three components of (row l>>4, state (l>>1)&7) and adds them to three fp64
 // accumulators.  The order is fixed: bitwise reproducible.
-constexpr int kB8 = 8, kB8RW = 2, kB8CT = 128, kB8Flush = 16;
+constexpr int kPackRW = 2;  // rows per consumer warp of the packed-FMA kernel
 
 __device__ __forceinline__ void ffma2(unsigned long long& d, unsigned long long a, unsigned long long b) {
   asm("fma.rn.f32x2 %0, %1, %2, %0;" : "+l"(d) : "l"(a), "l"(b));
@@ -310,14 +322,23 @@ __device__ __forceinline__ float sum_halves(unsigned long long v) {
   asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
   return lo + hi;
 }
+// NP column pairs per lane: 1 (LDS.64, CT = 64) or 2 (LDS.128, CT = 128)
+template <int NP> struct PairVec;
+template <> struct PairVec<1> { unsigned long long p[1]; };
+template <> struct alignas(16) PairVec<2> { unsigned long long p[2]; };
 
-template <int STAGES>
-__global__ void __launch_bounds__(kThreads, 1)
+template <int B, int WARPS, int CT, int STAGES>
+__global__ void __launch_bounds__(WARPS * 32, 1)
     demag_tma_f32x2_kernel(const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmM,
                            TmaArgs a, EpiArgs e) {
-  typedef TmaCfg<float, kB8, kB8RW, kB8CT, STAGES> Cfg;
-  constexpr int RT = Cfg::RT, RW = kB8RW, B = kB8, CT = kB8CT;
-  static_assert(Cfg::VPL == 1 && RW * B == 16, "lane mapping of the transposing butterfly");
+  typedef TmaCfg<float, B, kPackRW, CT, STAGES, WARPS> Cfg;
+  constexpr int RT = Cfg::RT, RW = kPackRW;
+  constexpr int NV = RW * B * 3;                 // fp32 sums per lane
+  constexpr int kOwnShift = (B == 8) ? 1 : 2;    // lane l ends up owning (row, state) index l >> kOwnShift
+  constexpr int NP = CT / 64;            // column pairs per lane
+  constexpr int kFlush = 96 / (3 * NP);  // tiles per fp32 run: <= 96 terms per accumulator
+  static_assert((NP == 1 || NP == 2) && (B == 4 || B == 8), "lane mapping of the transposing butterfly");
+  typedef PairVec<NP> PV;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char* smem = (unsigned char*)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
   uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::stage_bytes);
@@ -329,7 +350,7 @@ __global__ void __launch_bounds__(kThreads, 1)
   if (threadIdx.x == 0) {
     for (int s = 0; s < STAGES; ++s) {
       mbar_init(full0 + 8 * s, 1);
-      mbar_init(empty0 + 8 * s, kConsumerWarps);
+      mbar_init(empty0 + 8 * s, WARPS);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -380,42 +401,44 @@ __global__ void __launch_bounds__(kThreads, 1)
     mbar_wait(full0 + 8 * stage, phase);
     const float* tile = (const float*)(smem + (size_t)stage * Cfg::stage_bytes);
     const float* mt = (const float*)(smem + (size_t)stage * Cfg::stage_bytes + Cfg::tensor_bytes);
-    const int col = lane * 4;
-    ulonglong2 tv[RW][6];
+    const int col = lane * (2 * NP);
+    PV tv[RW][6];
 #pragma unroll
     for (int r = 0; r < RW; ++r)
 #pragma unroll
       for (int cc = 0; cc < 6; ++cc)
-        tv[r][cc] = *(const ulonglong2*)(tile + ((size_t)cc * RT + (warp * RW + r)) * CT + col);
+        tv[r][cc] = *(const PV*)(tile + ((size_t)cc * RT + (warp * RW + r)) * CT + col);
 #pragma unroll
     for (int b = 0; b < B; ++b) {
-      ulonglong2 mv[3];
+      PV mv[3];
 #pragma unroll
-      for (int cc = 0; cc < 3; ++cc) mv[cc] = *(const ulonglong2*)(mt + (size_t)(b * 3 + cc) * CT + col);
+      for (int cc = 0; cc < 3; ++cc) mv[cc] = *(const PV*)(mt + (size_t)(b * 3 + cc) * CT + col);
 #pragma unroll
-      for (int r = 0; r < RW; ++r) {
-        // planes xx, xy, xz, yy, yz, zz = 0..5; columns {0,1} in .x, {2,3} in .y
-        ffma2(run[r][b][0], tv[r][0].x, mv[0].x); ffma2(run[r][b][0], tv[r][0].y, mv[0].y);
-        ffma2(run[r][b][0], tv[r][1].x, mv[1].x); ffma2(run[r][b][0], tv[r][1].y, mv[1].y);
-        ffma2(run[r][b][0], tv[r][2].x, mv[2].x); ffma2(run[r][b][0], tv[r][2].y, mv[2].y);
-        ffma2(run[r][b][1], tv[r][1].x, mv[0].x); ffma2(run[r][b][1], tv[r][1].y, mv[0].y);
-        ffma2(run[r][b][1], tv[r][3].x, mv[1].x); ffma2(run[r][b][1], tv[r][3].y, mv[1].y);
-        ffma2(run[r][b][1], tv[r][4].x, mv[2].x); ffma2(run[r][b][1], tv[r][4].y, mv[2].y);
-        ffma2(run[r][b][2], tv[r][2].x, mv[0].x); ffma2(run[r][b][2], tv[r][2].y, mv[0].y);
-        ffma2(run[r][b][2], tv[r][4].x, mv[1].x); ffma2(run[r][b][2], tv[r][4].y, mv[1].y);
-        ffma2(run[r][b][2], tv[r][5].x, mv[2].x); ffma2(run[r][b][2], tv[r][5].y, mv[2].y);
-      }
+      for (int r = 0; r < RW; ++r)
+#pragma unroll
+        for (int q = 0; q < NP; ++q) {
+          // planes xx, xy, xz, yy, yz, zz = 0..5; p[q] = columns {2q, 2q+1} of the lane
+          ffma2(run[r][b][0], tv[r][0].p[q], mv[0].p[q]);
+          ffma2(run[r][b][1], tv[r][1].p[q], mv[0].p[q]);
+          ffma2(run[r][b][2], tv[r][2].p[q], mv[0].p[q]);
+          ffma2(run[r][b][0], tv[r][1].p[q], mv[1].p[q]);
+          ffma2(run[r][b][1], tv[r][3].p[q], mv[1].p[q]);
+          ffma2(run[r][b][2], tv[r][4].p[q], mv[1].p[q]);
+          ffma2(run[r][b][0], tv[r][2].p[q], mv[2].p[q]);
+          ffma2(run[r][b][1], tv[r][4].p[q], mv[2].p[q]);
+          ffma2(run[r][b][2], tv[r][5].p[q], mv[2].p[q]);
+        }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(empty0 + 8 * stage);
     if (++stage == STAGES) { stage = 0; phase ^= 1; }
     const bool group_done = (k + 1 == a.chunks);
     const bool emit = group_done || t + 1 == t1;
-    if (++since_flush == kB8Flush || emit) {
+    if (++since_flush == kFlush || emit) {
       since_flush = 0;
       // val[(r*8 + b)*3 + cc]; halving steps keep the lower or upper half of the index space by one
       // lane bit each, so that after offsets 16, 8, 4, 2 lane l owns (r*8 + b) == l >> 1
-      float val[48];
+      float val[NV];
 #pragma unroll
       for (int r = 0; r < RW; ++r)
 #pragma unroll
@@ -426,7 +449,7 @@ __global__ void __launch_bounds__(kThreads, 1)
             run[r][b][cc] = 0ull;
           }
 #pragma unroll
-      for (int half = 24, off = 16; half >= 3; half >>= 1, off >>= 1) {
+      for (int half = NV / 2, off = 16; half >= 3; half >>= 1, off >>= 1) {
         const bool upper = (lane & off) != 0;
 #pragma unroll
         for (int i = 0; i < half; ++i) {
@@ -437,14 +460,16 @@ __global__ void __launch_bounds__(kThreads, 1)
       }
 #pragma unroll
       for (int cc = 0; cc < 3; ++cc) {
-        val[cc] += __shfl_xor_sync(0xffffffffu, val[cc], 1);
+#pragma unroll
+        for (int off = 1 << (kOwnShift - 1); off > 0; off >>= 1) val[cc] += __shfl_xor_sync(0xffffffffu, val[cc], off);
         acc[cc] += (double)val[cc];
       }
     }
     if (emit) {
-      const int rg = warp * RW + (lane >> 4), b = (lane >> 1) & 7;
+      const int own = lane >> kOwnShift;  // == r * B + b
+      const int rg = warp * RW + own / B, b = own % B;
       const int64_t row = g * RT + rg;
-      if (!(lane & 1) && b < e.batch && row < a.n_rows) {
+      if (!(lane & ((1 << kOwnShift) - 1)) && b < e.batch && row < a.n_rows) {
         if (head_in_range && group_done) {
           const double hd[3] = {-acc[0], -acc[1], -acc[2]};
           row_epilogue(e, row, b, hd);
@@ -556,7 +581,7 @@ int launch_tiles(mt_ctx* ctx, Kern kern, bool* attr_set, int m_rows, const void*
     MT_CUDA_OK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes));
     *attr_set = true;
   }
-  kern<<<(unsigned)P, kThreads, Cfg::smem_bytes, ctx->stream>>>(tmN, tmM, a, e);
+  kern<<<(unsigned)P, Cfg::WARPS * 32, Cfg::smem_bytes, ctx->stream>>>(tmN, tmM, a, e);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   const int64_t tot = n_rows * e.batch;
@@ -576,29 +601,35 @@ int launch_cfg(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows,
 
 // fp32, 5 <= batch <= 8: packed-FMA kernel (states beyond `batch` are computed on unused rows of M
 // and dropped)
+template <int B, int WARPS, int CT, int STAGES>
+int launch_f32x2_shape(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
+                       int64_t npad, const EpiArgs& e) {
+  static bool attr_set = false;
+  return launch_tiles<float, TmaCfg<float, B, kPackRW, CT, STAGES, WARPS>>(
+      ctx, demag_tma_f32x2_kernel<B, WARPS, CT, STAGES>, &attr_set, 3 * B, N, MT_F32, n, n_rows, ld, Mst, npad, e);
+}
+
+// fp32, 3 <= batch <= 8: packed-FMA kernels for 4 or 8 states (states beyond `batch` are computed on
+// unused rows of M and dropped)
 int launch_f32x2(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld, const void* Mst, int64_t npad,
                  const EpiArgs& e) {
-  static bool attr_set = false;
-  constexpr int STAGES = 3;
-  return launch_tiles<float, TmaCfg<float, kB8, kB8RW, kB8CT, STAGES>>(ctx, demag_tma_f32x2_kernel<STAGES>, &attr_set,
-                                                                      3 * kB8, N, MT_F32, n, n_rows, ld, Mst, npad, e);
+  if (e.batch <= 4) return launch_f32x2_shape<4, MT_B4_WARPS, MT_B4_CT, MT_B4_STAGES>(ctx, N, n, n_rows, ld, Mst, npad, e);
+  return launch_f32x2_shape<8, MT_B8_WARPS, MT_B8_CT, MT_B8_STAGES>(ctx, N, n, n_rows, ld, Mst, npad, e);
 }
 
 template <typename T>
 int launch_T(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
              int64_t npad, const EpiArgs& e) {
   constexpr int CT1 = 1024 / sizeof(T);  // 1 KB of one row-plane per tile
-  switch (e.batch) {
-    case 1: return launch_cfg<T, 1, 1, CT1, 4>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
-    case 2: return launch_cfg<T, 2, 1, CT1, 4>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
-    case 3: return launch_cfg<T, 3, 1, CT1, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
-    case 4: return launch_cfg<T, 4, 1, CT1, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
-  }
-  if (e.batch >= 5 && e.batch <= MT_MAX_BATCH) {
+  if (e.batch == 1) return launch_cfg<T, 1, 1, CT1, 4>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+  if (e.batch == 2) return launch_cfg<T, 2, 1, CT1, 4>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+  if (e.batch >= 3 && e.batch <= MT_MAX_BATCH) {
     if constexpr (sizeof(T) == 4) {
       return launch_f32x2(ctx, N, n, n_rows, ld, Mst, npad, e);
     } else {
       switch (e.batch) {
+        case 3: return launch_cfg<T, 3, 1, CT1, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+        case 4: return launch_cfg<T, 4, 1, CT1, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
         case 5: return launch_cfg<T, 5, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
         case 6: return launch_cfg<T, 6, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
         case 7: return launch_cfg<T, 7, 2, CT1 / 2, 3>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
