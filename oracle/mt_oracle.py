@@ -260,6 +260,33 @@ def energy(prob: Problem, m, vol=None) -> float:
     return float(lib().mto_energy(C.byref(cp), _p(m), _p(v)))
 
 
+def energy_terms(prob: Problem, m, vol=None) -> np.ndarray:
+    """(E_demag, E_exch, E_anis, E_zeeman) of one state — Eq. 8, 11, 15, 6 through the fields."""
+    m = _f64(m).reshape(3, prob.n)
+    cp = prob._c()
+    v = _f64(vol) if vol is not None else None
+    out = np.empty(4)
+    lib().mto_energy_terms(C.byref(cp), _p(m), _p(v), _p(out))
+    return out
+
+
+def field_sweep(prob: Problem, m0, fields, *, vol=None, **integrate_kw):
+    """F4, the loop of the paper's hysteresis experiment ("the applied field is changed
+    in steps ... for each field the system is relaxed"): for every applied field H_a in `fields`
+    ([k][3]) in order, integrate from the previous end state over [0, t_end] with `integrate_kw`,
+    then record <m> (volume weighted) and the four energy terms.  Returns (m_end, rows [k][3+4])."""
+    import dataclasses
+    m = _f64(m0).copy().reshape(3, prob.n)
+    rows = []
+    for Hk in np.asarray(fields, dtype=np.float64).reshape(-1, 3):
+        pk = dataclasses.replace(prob, H_a=tuple(float(x) for x in Hk))
+        m, _, _ = integrate(pk, m, weights=vol, **integrate_kw)
+        w = np.ones(prob.n) if vol is None else _f64(vol)
+        mean = (m * w).sum(axis=1) / w.sum()
+        rows.append(np.concatenate([mean, energy_terms(pk, m, vol)]))
+    return m, np.array(rows)
+
+
 def dp45_tableau():
     c, a, b5, b4 = np.empty(7), np.empty(42), np.empty(7), np.empty(7)
     lib().mto_dp45_tableau(_p(c), _p(a), _p(b5), _p(b4))
