@@ -178,6 +178,34 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* prob, const mt_integrator_opts* 
                  double* m_inout, int batch, double* t_inout, double* samples, int64_t sample_cap,
                  mt_integrator_result* host_out);
 
+/* ---- F4. Energy terms and the field-sweep (hysteresis) loop -------------------------------------
+ * Free energy of Eq. 4 split into its terms, each evaluated through the field it
+ * generates, for state b (Ms_i V_i weights; V = prob->vol, NULL: 1):
+ *   E_out[b][0] = -(1/2) sum_i Ms_i V_i m_i . H_d,i      demagnetisation, Eq. 8
+ *   E_out[b][1] = -(1/2) sum_i Ms_i V_i m_i . H_exch,i   exchange,        Eq. 11
+ *   E_out[b][2] = -(1/2) sum_i Ms_i V_i m_i . H_anis,i   anisotropy,      Eq. 15 (up to its
+ *                                                         m-independent constant)
+ *   E_out[b][3] = -      sum_i Ms_i V_i m_i . H_a,i      Zeeman,          Eq. 6
+ *   E_out[b][4] = their sum.
+ * In units of mu0 x (field unit)^2 x (length unit)^3.  One pass of the fused field kernel (same
+ * arithmetic as mt_llg_rhs) and a fixed-order reduction: bitwise reproducible.  E_out is a DEVICE
+ * array [batch][5]; asynchronous.  Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA.                        */
+int mt_energy(mt_ctx* ctx, const mt_problem* prob, const double* m, int batch, double* E_out);
+
+/* The loop of the paper's hysteresis experiment (mumag standard problem 2: "the
+ * applied field is changed in steps" and the system relaxed at each): for f = 0 .. n_fields-1 the
+ * uniform applied field is set to fields_host[f][0..2] (HOST array; prob->H_a must be NULL),
+ * m_inout is integrated with `opts` from t = 0 to opts->t_end (or to opts->torque_tol) starting
+ * from the previous field's end state, and row f of `rows` (DEVICE, [n_fields][batch][8]) receives
+ * <m_x>, <m_y>, <m_z>, E_demag, E_exch, E_anis, E_zeeman, E_total of every state.  res_host (HOST,
+ * may be NULL) receives the counters summed over the sweep (t = total simulated time).
+ * Synchronises the stream before returning.  MT_ERR_MAX_STEPS from a field step is not fatal (the
+ * sweep continues, as the paper relaxes a fixed time per field) and is returned at the end only if
+ * it was the last step's status.  Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA, MT_ERR_STEP_UNDERFLOW.  */
+int mt_field_sweep(mt_ctx* ctx, const mt_problem* prob, const mt_integrator_opts* opts,
+                   const double* fields_host, int64_t n_fields, double* m_inout, int batch,
+                   double* rows, mt_integrator_result* res_host);
+
 /* ---- instrumentation --------------------------------------------------------------------------- */
 /* Number of kernels this ctx has launched since creation (bench.py's gpu_launches).              */
 int64_t mt_launch_count(const mt_ctx* ctx);

@@ -24,7 +24,8 @@ MT_F32, MT_F64 = 0, 1
 MT_RK4, MT_DP45 = 0, 1
 COMPONENTS = ("xx", "xy", "xz", "yy", "yz", "zz")
 EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assemble_tensor",
-           "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_launch_count",
+           "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_energy",
+           "mt_field_sweep", "mt_launch_count",
            "mt_set_demag_variant", "mt_profile_begin", "mt_profile_end")
 
 
@@ -94,6 +95,9 @@ def load() -> C.CDLL:
         lib.mt_llg_rhs.argtypes = [C.c_void_p, C.POINTER(_Problem), C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         lib.mt_integrate.argtypes = [C.c_void_p, C.POINTER(_Problem), C.POINTER(_Opts), C.c_void_p, C.c_int,
                                      C.POINTER(C.c_double), C.c_void_p, C.c_int64, C.POINTER(_Result)]
+        lib.mt_energy.argtypes = [C.c_void_p, C.POINTER(_Problem), C.c_void_p, C.c_int, C.c_void_p]
+        lib.mt_field_sweep.argtypes = [C.c_void_p, C.POINTER(_Problem), C.POINTER(_Opts), C.c_void_p, C.c_int64,
+                                       C.c_void_p, C.c_int, C.c_void_p, C.POINTER(_Result)]
         _lib = lib
     return _lib
 
@@ -293,3 +297,25 @@ def mt_integrate(ctx: Context, prob: Problem, m: torch.Tensor, batch: int, t0: f
                                         C.byref(t), _ptr(samples, torch.float64), cap, C.byref(res)),
                    allow=allow)
     return t.value, {k: getattr(res, k) for k, _ in _Result._fields_}, rc
+
+
+def mt_energy(ctx: Context, prob: Problem, m: torch.Tensor, batch: int, E_out: torch.Tensor):
+    """E_out[batch][5] (device): E_demag, E_exch, E_anis, E_zeeman, E_total."""
+    p = prob._c()
+    ctx.check(ctx.lib.mt_energy(ctx.h, C.byref(p), _ptr(m, torch.float64), batch, _ptr(E_out, torch.float64)))
+
+
+def mt_field_sweep(ctx: Context, prob: Problem, fields, m: torch.Tensor, batch: int, rows: torch.Tensor, *,
+                   method: int, dt: float, t_end: float, max_steps: int = 0, rtol: float = 1e-6,
+                   atol: float = 1e-8, torque_tol: float = 0.0, renormalize: bool = True, allow=()):
+    """fields: host sequence [k][3]; rows (device) [k][batch][8]; m advanced in place.  Returns the
+    summed counters and the return code."""
+    p = prob._c()
+    o = _Opts(method, dt, t_end, max_steps, rtol, atol, torque_tol, int(renormalize), 0, 0.0)
+    flat = [float(x) for row in fields for x in row]
+    nf = len(flat) // 3
+    arr = (C.c_double * max(1, len(flat)))(*flat)
+    res = _Result()
+    rc = ctx.check(ctx.lib.mt_field_sweep(ctx.h, C.byref(p), C.byref(o), arr, nf, _ptr(m, torch.float64), batch,
+                                          _ptr(rows, torch.float64), C.byref(res)), allow=allow)
+    return {k: getattr(res, k) for k, _ in _Result._fields_}, rc

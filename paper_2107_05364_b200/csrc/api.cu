@@ -135,6 +135,7 @@ int mt_destroy(mt_ctx* c) {
   cudaFree(c->Mst[1]);
   cudaFree(c->partial);
   cudaFree(c->rk);
+  cudaFree(c->edens);
   cudaFree(c->dscal);
   cudaFree(c->stage_io);
   cudaFreeHost(c->hscal);
@@ -263,6 +264,69 @@ int mt_llg_rhs(mt_ctx* ctx, const mt_problem* p, const double* m, int batch, dou
   e.k_out = dmdt;
   e.heff_out = Heff;
   return eval_rhs(ctx, p, npad, 0, e);
+}
+
+int mt_energy(mt_ctx* ctx, const mt_problem* p, const double* m, int batch, double* E_out) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_problem(ctx, p, batch);
+  if (rc) return rc;
+  if (!m || !E_out) return mt_fail(ctx, MT_ERR_INVALID_ARG, "m and E_out must be non-NULL");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  const int64_t npad = round_up(p->n, MT_COL_CHUNK);
+  rc = mt_ensure_ws(ctx, (void**)&ctx->edens, &ctx->edens_bytes, (size_t)batch * 4 * p->n * sizeof(double));
+  if (rc) return rc;
+  if (p->N) {
+    if ((rc = ensure_Mst(ctx, p->dtype, batch, npad))) return rc;
+    if ((rc = mt_launch_stage_M(ctx, p->dtype, p->Ms, m, batch, p->n, npad, ctx->Mst[0]))) return rc;
+  }
+  EpiArgs e;
+  fill_problem(e, p, batch);
+  e.y = m;
+  e.e_dens = ctx->edens;
+  e.vol = p->vol;
+  if ((rc = eval_rhs(ctx, p, npad, 0, e))) return rc;
+  return mt_launch_energy_reduce(ctx, ctx->edens, batch, p->n, E_out);
+}
+
+int mt_field_sweep(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, const double* fields_host,
+                   int64_t n_fields, double* m, int batch, double* rows, mt_integrator_result* res_host) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_problem(ctx, p, batch);
+  if (rc) return rc;
+  if (!o || !fields_host || n_fields < 0 || !m || !rows)
+    return mt_fail(ctx, MT_ERR_INVALID_ARG, "opts, fields, m and rows must be non-NULL");
+  if (p->H_a) return mt_fail(ctx, MT_ERR_INVALID_ARG, "mt_field_sweep sets the uniform applied field: H_a must be NULL");
+  const int64_t stride = 8 * (int64_t)batch;
+  mt_problem pk = *p;
+  mt_integrator_result total;
+  memset(&total, 0, sizeof(total));
+  for (int64_t f = 0; f < n_fields; ++f) {
+    for (int a = 0; a < 3; ++a) pk.H_a_const[a] = fields_host[3 * f + a];
+    double t = 0.0;
+    mt_integrator_result r;
+    rc = mt_integrate(ctx, &pk, o, m, batch, &t, nullptr, 0, &r);
+    total.accepted += r.accepted; total.rejected += r.rejected; total.rhs_calls += r.rhs_calls;
+    total.t += r.t; total.dt_last = r.dt_last; total.max_torque = r.max_torque;
+    if (rc && rc != MT_ERR_MAX_STEPS) break;
+    // row f: per state <m_x>, <m_y>, <m_z> (A10) then E_demag, E_exch, E_anis, E_zeeman, E_total.  The
+    // mean kernel writes t into its slot 0, so it gets a scratch row of 1 + 3 B doubles and the means
+    // are copied behind it; the energies are written in place.
+    double* row = rows + f * stride;
+    if ((rc = mt_ensure_ws(ctx, (void**)&ctx->stage_io, &ctx->stage_io_bytes, (size_t)(1 + 8 * batch) * sizeof(double)))) break;
+    double* scratch = ctx->stage_io;
+    if ((rc = mt_launch_mean(ctx, m, p->vol, batch, p->n, t, scratch))) break;
+    if ((rc = mt_energy(ctx, &pk, m, batch, scratch + 1 + 3 * batch))) break;
+    for (int b = 0; b < batch && !rc; ++b) {
+      if (cudaMemcpyAsync(row + 8 * b, scratch + 1 + 3 * b, 3 * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream) != cudaSuccess ||
+          cudaMemcpyAsync(row + 8 * b + 3, scratch + 1 + 3 * batch + 5 * b, 5 * sizeof(double), cudaMemcpyDeviceToDevice, ctx->stream) != cudaSuccess)
+        rc = mt_fail(ctx, MT_ERR_CUDA, "cudaMemcpyAsync failed in mt_field_sweep");
+    }
+    if (rc) break;
+    // the scratch row is reused by the next field: order is kept by the stream
+  }
+  if (cudaStreamSynchronize(ctx->stream) != cudaSuccess && !rc) rc = mt_fail(ctx, MT_ERR_CUDA, "stream synchronise failed");
+  if (res_host) *res_host = total;
+  return rc;
 }
 
 int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, double* m, int batch,

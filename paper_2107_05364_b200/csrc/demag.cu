@@ -259,6 +259,28 @@ __global__ void __launch_bounds__(1024) mean_kernel(const double* __restrict__ m
   }
 }
 
+// F4: E[b][term] = sum_i e_dens[b][term][i] (one block per (term, b), fixed-order tree: bitwise
+// reproducible); the total is added by the last launch's thread 0 of term 0 in a second tiny kernel.
+__global__ void __launch_bounds__(1024) energy_reduce_kernel(const double* __restrict__ e_dens, int64_t n,
+                                                             double* __restrict__ out) {
+  __shared__ double sh[1024];
+  const int term = blockIdx.x, b = blockIdx.y;
+  const double* v = e_dens + ((int64_t)b * 4 + term) * n;
+  double s = 0.0;
+  for (int64_t i = threadIdx.x; i < n; i += 1024) s += v[i];
+  sh[threadIdx.x] = s;
+  __syncthreads();
+  for (int off = 512; off > 0; off >>= 1) {
+    if ((int)threadIdx.x < off) sh[threadIdx.x] += sh[threadIdx.x + off];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) out[b * 5 + term] = sh[0];
+}
+__global__ void energy_total_kernel(int batch, double* __restrict__ out) {
+  const int b = threadIdx.x;
+  if (b < batch) out[b * 5 + 4] = ((out[b * 5] + out[b * 5 + 1]) + out[b * 5 + 2]) + out[b * 5 + 3];
+}
+
 template <typename T, int B>
 int launch_ldg_T(mt_ctx* ctx, const DemagArgs<T>& a, const EpiArgs& e) {
   dim3 grid((unsigned)((a.n_rows + kWarps - 1) / kWarps), (unsigned)a.nsplit);
@@ -380,6 +402,16 @@ int mt_launch_combine(mt_ctx* ctx, const EpiArgs& epi) {
 int mt_launch_mean(mt_ctx* ctx, const double* m, const double* vol, int batch, int64_t n, double t,
                    double* sample_row) {
   mean_kernel<<<dim3(3, (unsigned)batch), 1024, 0, ctx->stream>>>(m, vol, n, batch, t, sample_row);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+int mt_launch_energy_reduce(mt_ctx* ctx, const double* e_dens, int batch, int64_t n, double* E_out) {
+  energy_reduce_kernel<<<dim3(4, (unsigned)batch), 1024, 0, ctx->stream>>>(e_dens, n, E_out);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  energy_total_kernel<<<1, 32, 0, ctx->stream>>>(batch, E_out);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   return MT_OK;

@@ -68,6 +68,7 @@ __device__ __forceinline__ void row_epilogue(const EpiArgs& e, int64_t i, int b,
   const double* y = e.y + sb;
   const double mi[3] = {y[i], y[n + i], y[2 * n + i]};
   double H[3] = {hd[0], hd[1], hd[2]};
+  double ed[4] = {0.0, 0.0, 0.0, 0.0};  // m.H_d, m.H_exch, m.H_anis, m.H_a (only used for e.e_dens)
   // exchange: Eq. 12, 3-point stencil, Neumann ghost = self
   if (e.nbr) {
     const double cex = e.c_ex ? e.c_ex[i] : e.c_ex_s;
@@ -84,6 +85,7 @@ __device__ __forceinline__ void row_epilogue(const EpiArgs& e, int64_t i, int b,
     }
 #pragma unroll
     for (int a = 0; a < 3; ++a) H[a] += cex * hx[a];
+    ed[1] = cex * (mi[0] * hx[0] + mi[1] * hx[1] + mi[2] * hx[2]);
   }
   // uniaxial anisotropy: Eq. 16; applied field: Eq. 7
   {
@@ -97,6 +99,19 @@ __device__ __forceinline__ void row_epilogue(const EpiArgs& e, int64_t i, int b,
     const double me = mi[0] * ax[0] + mi[1] * ax[1] + mi[2] * ax[2];
 #pragma unroll
     for (int a = 0; a < 3; ++a) H[a] += can * me * ax[a] + ha[a];
+    ed[2] = can * me * me;
+    ed[3] = mi[0] * ha[0] + mi[1] * ha[1] + mi[2] * ha[2];
+  }
+  // F4: energy densities of the four terms (Eq. 8, 11, 15, 6: PAPER.md:74, 89, 110, 66), each through
+  // its field: -(1/2) Ms V m.H for the terms quadratic in m, -Ms V m.H_a for the Zeeman term
+  if (e.e_dens) {
+    ed[0] = mi[0] * hd[0] + mi[1] * hd[1] + mi[2] * hd[2];
+    const double w = e.Ms[i] * (e.vol ? e.vol[i] : 1.0);
+    double* eo = e.e_dens + (int64_t)b * 4 * n;
+    eo[i] = -0.5 * w * ed[0];
+    eo[n + i] = -0.5 * w * ed[1];
+    eo[2 * n + i] = -0.5 * w * ed[2];
+    eo[3 * n + i] = -w * ed[3];
   }
   // Landau-Lifshitz: Eq. 1
   double mxH[3], mxmxH[3], k[3];
@@ -104,9 +119,11 @@ __device__ __forceinline__ void row_epilogue(const EpiArgs& e, int64_t i, int b,
   cross3(mi, mxH, mxmxH);
 #pragma unroll
   for (int a = 0; a < 3; ++a) k[a] = -e.gamma * mxH[a] - e.alpha * mxmxH[a];
-  double* ko = e.k_out + sb;
+  if (e.k_out) {
+    double* ko = e.k_out + sb;
 #pragma unroll
-  for (int a = 0; a < 3; ++a) ko[a * n + i] = k[a];
+    for (int a = 0; a < 3; ++a) ko[a * n + i] = k[a];
+  }
   if (e.heff_out) {
     double* ho = e.heff_out + sb;
 #pragma unroll

@@ -25,6 +25,8 @@ struct mt_ctx {
   size_t partial_bytes;
   double* rk;  // integrator stages + scratch states
   size_t rk_bytes;
+  double* edens;  // [B][4][n] energy densities (mt_energy)
+  size_t edens_bytes;
   unsigned long long* dscal;  // device scalars: [0] err bits, [1] torque bits
   unsigned long long* hscal;  // pinned host mirror
   double* stage_io;           // device staging for the *_host entry points
@@ -76,6 +78,8 @@ struct EpiArgs {
   double gamma, alpha;
   double* k_out;     // dm/dt [B][3][n]
   double* heff_out;  // optional
+  double* e_dens;    // optional [B][4][n]: per-tile energy of the demag, exchange, anisotropy, Zeeman terms
+  const double* vol; // tile volumes for e_dens (NULL: 1)
   unsigned long long* torque_bits;  // optional: atomicMax of |y x H_eff| (bits of a non-negative double)
   // stage combine: y_out = base + h * sum_j coef[j] * kptr[j]; optional renormalisation; optional
   // staging of Ms*y_out in the tensor's dtype for the next field evaluation
@@ -109,6 +113,8 @@ int mt_launch_combine(mt_ctx* ctx, const EpiArgs& epi);     // stage combine wit
 int mt_launch_mean(mt_ctx* ctx, const double* m, const double* vol, int batch, int64_t n, double t,
                    double* sample_row);
 int mt_ensure_ws(mt_ctx* ctx, void** p, size_t* cur, size_t need);
+// E_out[b][5] = fixed-order sums over tiles of e_dens[b][0..3][n], then their total
+int mt_launch_energy_reduce(mt_ctx* ctx, const double* e_dens, int batch, int64_t n, double* E_out);
 
 // launchers (assemble.cu)
 int mt_launch_assemble(mt_ctx* ctx, const mt_tiles* t, int dtype, int64_t r0, int64_t r1, void* out,
