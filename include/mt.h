@@ -112,6 +112,49 @@ int mt_demag_field_host(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_
                         int64_t ld, const double* Ms, const double* m_host, int batch,
                         double* Hd_host);
 
+/* ---- F1. Thresholded tensor (section 4.3.1) -------------------------------------
+ * "removing all elements of the tensor smaller than a given threshold value ... allows the
+ * demagnetization tensor ... to be allocated as a sparse matrix".  Layout ("bitmap
+ * rows"): for plane c and target row i, mask[(c*n_rows + i)*nw + w] holds one bit per source column
+ * (bit l of word w = column 32 w + l, 1 = kept) and the kept values are packed in column order from
+ * vals[row_ptr[c*n_rows + i]].  nw = mt_sparse_mask_words(n) (a multiple of 4; padding words zero).
+ * All three arrays are DEVICE memory owned by the caller.                                           */
+typedef struct {
+  int64_t n, n_rows;
+  int dtype;               /* MT_F32 | MT_F64: element type of vals                                  */
+  int64_t nw;              /* mask words per (plane, row)                                            */
+  const int64_t* row_ptr;  /* [6*n_rows + 1] offsets into vals (elements); last = number kept        */
+  const uint32_t* mask;    /* [6][n_rows][nw]                                                        */
+  const void* vals;        /* [row_ptr[6*n_rows]]                                                    */
+} mt_sparse_tensor;
+
+int64_t mt_sparse_mask_words(int64_t n);
+
+/* Threshold value for a fraction X in [0, 1] ("for a threshold of 20% the absolute
+ * smallest fifth of the elements larger than zero in the tensor is truncated to zero"): with the
+ * non-zero elements of the dense 3n x 3n matrix sorted by absolute value (off-diagonal components,
+ * stored once, count twice: DESIGN.md Q20), *tau_host = the element of rank floor(X*count), i.e.
+ * the smallest value kept; entries with |v| < tau are the ones removed (ties with tau are kept);
+ * +inf when X*count >= count.  *count_host (may be NULL) = number of non-zero elements counted.
+ * N is the dense DEVICE tensor [6][n_rows][ld].  Exact (integer radix select on the bit patterns);
+ * synchronises the stream.  Errors: MT_ERR_INVALID_ARG (fraction outside [0,1], ...), MT_ERR_CUDA. */
+int mt_threshold_value(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                       double fraction, double* tau_host, int64_t* count_host);
+
+/* Compression, two calls: mt_sparse_count fills row_ptr (DEVICE, [6*n_rows+1]) for threshold tau and
+ * returns the number of kept entries in *nnz_host (synchronises); the caller allocates mask
+ * ([6*n_rows*nw] uint32) and vals ([nnz] of dtype), then mt_sparse_fill writes them (asynchronous).
+ * An entry is kept iff it is non-zero and not |v| < tau.                                            */
+int mt_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                    double tau, int64_t* row_ptr, int64_t* nnz_host);
+int mt_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                   double tau, const int64_t* row_ptr, uint32_t* mask, void* vals);
+
+/* mt_demag_field on the thresholded tensor: Hd[b][a][i] = - sum over kept entries; same arithmetic
+ * rules (fp32 runs of at most 96 terms, then fp64), fixed reduction order.                          */
+int mt_demag_field_sparse(mt_ctx* ctx, const mt_sparse_tensor* S, const double* Ms, const double* m,
+                          int batch, double* Hd);
+
 /* ---- A5 / A6. Effective field and Landau-Lifshitz right-hand side ------------------------------
  * H_eff = H_d + H_exch + H_anis + H_a                                   (Eq. 17)
  *   H_exch,i = c_ex,i * sum_{dir} (m_{i+} - 2 m_i + m_{i-}) * inv_d2[dir]   (Eq. 12 PAPER.md:94;
@@ -141,6 +184,8 @@ typedef struct {
   double H_a_const[3];
   double gamma, alpha_ll;
   const double* vol;     /* [n] tile volumes: weights of <m> (A10); NULL = plain mean              */
+  const mt_sparse_tensor* N_sparse; /* HOST pointer or NULL: when set, the demagnetising term uses this
+                            thresholded tensor (F1) instead of N (N may then be NULL)  */
 } mt_problem;
 
 /* dmdt[b][3][n] (required) and Heff[b][3][n] (optional, NULL to skip) for m[b][3][n].

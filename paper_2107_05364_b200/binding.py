@@ -25,7 +25,8 @@ MT_RK4, MT_DP45 = 0, 1
 COMPONENTS = ("xx", "xy", "xz", "yy", "yz", "zz")
 EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assemble_tensor",
            "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_energy",
-           "mt_field_sweep", "mt_launch_count",
+           "mt_field_sweep", "mt_sparse_mask_words", "mt_threshold_value", "mt_sparse_count",
+           "mt_sparse_fill", "mt_demag_field_sparse", "mt_launch_count",
            "mt_set_demag_variant", "mt_profile_begin", "mt_profile_end")
 
 
@@ -48,8 +49,13 @@ class _Problem(C.Structure):
         ("c_an", C.c_void_p), ("c_an_scalar", C.c_double),
         ("easy", C.c_void_p), ("easy_const", C.c_double * 3),
         ("H_a", C.c_void_p), ("H_a_const", C.c_double * 3),
-        ("gamma", C.c_double), ("alpha_ll", C.c_double), ("vol", C.c_void_p),
+        ("gamma", C.c_double), ("alpha_ll", C.c_double), ("vol", C.c_void_p), ("N_sparse", C.c_void_p),
     ]
+
+
+class _Sparse(C.Structure):
+    _fields_ = [("n", C.c_int64), ("n_rows", C.c_int64), ("dtype", C.c_int), ("nw", C.c_int64),
+                ("row_ptr", C.c_void_p), ("mask", C.c_void_p), ("vals", C.c_void_p)]
 
 
 class _Opts(C.Structure):
@@ -95,6 +101,16 @@ def load() -> C.CDLL:
         lib.mt_llg_rhs.argtypes = [C.c_void_p, C.POINTER(_Problem), C.c_void_p, C.c_int, C.c_void_p, C.c_void_p]
         lib.mt_integrate.argtypes = [C.c_void_p, C.POINTER(_Problem), C.POINTER(_Opts), C.c_void_p, C.c_int,
                                      C.POINTER(C.c_double), C.c_void_p, C.c_int64, C.POINTER(_Result)]
+        lib.mt_sparse_mask_words.restype = C.c_int64
+        lib.mt_sparse_mask_words.argtypes = [C.c_int64]
+        lib.mt_threshold_value.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64,
+                                           C.c_double, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+        lib.mt_sparse_count.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64,
+                                        C.c_double, C.c_void_p, C.POINTER(C.c_int64)]
+        lib.mt_sparse_fill.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64,
+                                       C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.mt_demag_field_sparse.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p, C.c_void_p, C.c_int,
+                                              C.c_void_p]
         lib.mt_energy.argtypes = [C.c_void_p, C.POINTER(_Problem), C.c_void_p, C.c_int, C.c_void_p]
         lib.mt_field_sweep.argtypes = [C.c_void_p, C.POINTER(_Problem), C.POINTER(_Opts), C.c_void_p, C.c_int64,
                                        C.c_void_p, C.c_int, C.c_void_p, C.POINTER(_Result)]
@@ -248,9 +264,13 @@ class Problem:
     gamma: float = 1.0
     alpha_ll: float = 0.0
     vol: torch.Tensor | None = None
+    N_sparse: object = None  # SparseTensor (F1): used for the demagnetising term instead of N
 
     def _c(self) -> _Problem:
         s = _Problem()
+        if self.N_sparse is not None:
+            self._sparse_c = self.N_sparse._c()  # keep the struct alive while the call runs
+            s.N_sparse = C.addressof(self._sparse_c)
         s.n = self.n
         s.N = _ptr(self.N, torch_dtype(self.dtype)) if self.N is not None else None
         s.dtype, s.ld = self.dtype, self.ld
@@ -319,3 +339,54 @@ def mt_field_sweep(ctx: Context, prob: Problem, fields, m: torch.Tensor, batch: 
     rc = ctx.check(ctx.lib.mt_field_sweep(ctx.h, C.byref(p), C.byref(o), arr, nf, _ptr(m, torch.float64), batch,
                                           _ptr(rows, torch.float64), C.byref(res)), allow=allow)
     return {k: getattr(res, k) for k, _ in _Result._fields_}, rc
+
+
+@dataclass
+class SparseTensor:
+    """mt_sparse_tensor (F1): bitmap rows of a thresholded tensor; device tensors owned here."""
+    n: int
+    n_rows: int
+    dtype: int
+    nw: int
+    row_ptr: torch.Tensor  # [6*n_rows + 1] int64
+    mask: torch.Tensor     # [6, n_rows, nw] int32 (bit patterns of uint32)
+    vals: torch.Tensor     # [nnz]
+    nnz: int = 0
+    tau: float = 0.0
+
+    def _c(self) -> _Sparse:
+        return _Sparse(self.n, self.n_rows, self.dtype, self.nw, _ptr(self.row_ptr, torch.int64),
+                       _ptr(self.mask, torch.int32), _ptr(self.vals, torch_dtype(self.dtype)))
+
+    def nbytes(self) -> int:
+        return self.row_ptr.numel() * 8 + self.mask.numel() * 4 + self.vals.numel() * self.vals.element_size()
+
+
+def mt_threshold_value(ctx: Context, N: torch.Tensor, dtype: int, n: int, n_rows: int, ld: int, fraction: float):
+    """Returns (tau, number of non-zero elements counted with multiplicity)."""
+    tau, cnt = C.c_double(), C.c_int64()
+    ctx.check(ctx.lib.mt_threshold_value(ctx.h, _ptr(N, torch_dtype(dtype)), dtype, n, n_rows, ld, float(fraction),
+                                         C.byref(tau), C.byref(cnt)))
+    return tau.value, cnt.value
+
+
+def mt_sparse_build(ctx: Context, N: torch.Tensor, dtype: int, n: int, n_rows: int, ld: int, tau: float) -> SparseTensor:
+    """mt_sparse_count + allocation (torch) + mt_sparse_fill."""
+    dev = N.device
+    row_ptr = torch.empty(6 * n_rows + 1, dtype=torch.int64, device=dev)
+    nnz = C.c_int64()
+    ctx.check(ctx.lib.mt_sparse_count(ctx.h, _ptr(N, torch_dtype(dtype)), dtype, n, n_rows, ld, float(tau),
+                                      _ptr(row_ptr), C.byref(nnz)))
+    nw = int(ctx.lib.mt_sparse_mask_words(n))
+    mask = torch.empty((6, n_rows, nw), dtype=torch.int32, device=dev)
+    vals = torch.empty(max(1, nnz.value), dtype=torch_dtype(dtype), device=dev)
+    ctx.check(ctx.lib.mt_sparse_fill(ctx.h, _ptr(N, torch_dtype(dtype)), dtype, n, n_rows, ld, float(tau),
+                                     _ptr(row_ptr), _ptr(mask), _ptr(vals)))
+    return SparseTensor(n, n_rows, dtype, nw, row_ptr, mask, vals, nnz=nnz.value, tau=float(tau))
+
+
+def mt_demag_field_sparse(ctx: Context, S: SparseTensor, Ms: torch.Tensor, m: torch.Tensor, batch: int,
+                          Hd: torch.Tensor):
+    s = S._c()
+    ctx.check(ctx.lib.mt_demag_field_sparse(ctx.h, C.byref(s), _ptr(Ms, torch.float64), _ptr(m, torch.float64),
+                                            batch, _ptr(Hd, torch.float64)))

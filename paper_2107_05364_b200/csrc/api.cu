@@ -38,6 +38,18 @@ int ensure_Mst(mt_ctx* ctx, int dtype, int batch, int64_t npad) {
   return MT_OK;
 }
 
+inline bool has_demag(const mt_problem* p) { return p->N != nullptr || p->N_sparse != nullptr; }
+inline int demag_dtype(const mt_problem* p) { return p->N_sparse ? p->N_sparse->dtype : p->dtype; }
+
+int check_sparse(mt_ctx* ctx, const mt_sparse_tensor* s) {
+  if (!s) return mt_fail(ctx, MT_ERR_INVALID_ARG, "sparse tensor is NULL");
+  if (s->dtype != MT_F32 && s->dtype != MT_F64) return mt_fail(ctx, MT_ERR_INVALID_ARG, "unknown dtype %d", s->dtype);
+  if (s->n <= 0 || s->n_rows <= 0) return mt_fail(ctx, MT_ERR_INVALID_ARG, "n and n_rows must be positive");
+  if (s->nw != mt_sparse_mask_words(s->n)) return mt_fail(ctx, MT_ERR_INVALID_ARG, "nw must be mt_sparse_mask_words(n)");
+  if (!s->row_ptr || !s->mask) return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and mask must be non-NULL");
+  return MT_OK;
+}
+
 void fill_problem(EpiArgs& e, const mt_problem* p, int batch) {
   memset(&e, 0, sizeof(e));
   e.mode = 1;
@@ -59,19 +71,27 @@ void fill_problem(EpiArgs& e, const mt_problem* p, int batch) {
   e.H_a = p->H_a;
   e.gamma = p->gamma;
   e.alpha = p->alpha_ll;
-  e.M_dtype = p->dtype;
+  e.M_dtype = demag_dtype(p);
 }
 
 int check_problem(mt_ctx* ctx, const mt_problem* p, int batch) {
   if (!p) return mt_fail(ctx, MT_ERR_INVALID_ARG, "problem is NULL");
   if (p->n <= 0 || !p->Ms) return mt_fail(ctx, MT_ERR_INVALID_ARG, "problem needs n > 0 and Ms");
   if (batch < 1 || batch > MT_MAX_BATCH) return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
+  if (p->N_sparse) {
+    int rc = check_sparse(ctx, p->N_sparse);
+    if (rc) return rc;
+    if (p->N_sparse->n != p->n || p->N_sparse->n_rows != p->n)
+      return mt_fail(ctx, MT_ERR_INVALID_ARG, "sparse tensor must be n x n");
+    return MT_OK;
+  }
   if (p->N) return check_tensor_args(ctx, p->N, p->dtype, p->n, p->n, p->ld);
   return MT_OK;
 }
 
 // one evaluation of the fused right-hand side: field of the staged M (ctx->Mst[src]) + epilogue
 int eval_rhs(mt_ctx* ctx, const mt_problem* p, int64_t npad, int src, const EpiArgs& e) {
+  if (p->N_sparse) return mt_launch_demag_sparse(ctx, p->N_sparse, ctx->Mst[src], npad, e);
   if (p->N) return mt_launch_demag(ctx, p->N, p->dtype, p->n, p->n, p->ld, ctx->Mst[src], npad, e);
   return mt_launch_local_only(ctx, e);
 }
@@ -252,10 +272,10 @@ int mt_llg_rhs(mt_ctx* ctx, const mt_problem* p, const double* m, int batch, dou
   if (!m || !dmdt) return mt_fail(ctx, MT_ERR_INVALID_ARG, "m and dmdt must be non-NULL");
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
   const int64_t npad = round_up(p->n, MT_COL_CHUNK);
-  if (p->N) {
-    rc = ensure_Mst(ctx, p->dtype, batch, npad);
+  if (has_demag(p)) {
+    rc = ensure_Mst(ctx, demag_dtype(p), batch, npad);
     if (rc) return rc;
-    rc = mt_launch_stage_M(ctx, p->dtype, p->Ms, m, batch, p->n, npad, ctx->Mst[0]);
+    rc = mt_launch_stage_M(ctx, demag_dtype(p), p->Ms, m, batch, p->n, npad, ctx->Mst[0]);
     if (rc) return rc;
   }
   EpiArgs e;
@@ -264,6 +284,108 @@ int mt_llg_rhs(mt_ctx* ctx, const mt_problem* p, const double* m, int batch, dou
   e.k_out = dmdt;
   e.heff_out = Heff;
   return eval_rhs(ctx, p, npad, 0, e);
+}
+
+int64_t mt_sparse_mask_words(int64_t n) { return n <= 0 ? 0 : round_up((n + 31) / 32, 4); }
+
+int mt_threshold_value(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                       double fraction, double* tau_host, int64_t* count_host) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_tensor_args(ctx, N, dtype, n, n_rows, ld);
+  if (rc) return rc;
+  if (!tau_host || !(fraction >= 0.0 && fraction <= 1.0))
+    return mt_fail(ctx, MT_ERR_INVALID_ARG, "fraction must be in [0, 1] and tau_host non-NULL");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  // MSB-first radix select over the bit pattern of |v| (sign bit cleared: 31 / 63 significant bits),
+  // 11-bit digits; each pass is one stream of the tensor and one 16 KB histogram read.
+  const int bits = dtype == MT_F32 ? 32 : 64;
+  const int kDigit = 11, kBins = 1 << kDigit;
+  unsigned long long* d_hist = nullptr;
+  MT_CUDA_OK(ctx, cudaMalloc((void**)&d_hist, kBins * sizeof(unsigned long long)));
+  unsigned long long* h_hist = new (std::nothrow) unsigned long long[kBins];
+  if (!h_hist) { cudaFree(d_hist); return mt_fail(ctx, MT_ERR_CUDA, "out of host memory"); }
+  unsigned long long prefix = 0, k = 0, count = 0;
+  bool all_removed = false;
+  int hi = bits;  // bits [hi, bits) of the key are fixed to `prefix`
+  cudaError_t ce = cudaSuccess;
+  while (hi > 0 && !all_removed) {
+    const int width = hi >= kDigit ? kDigit : hi;
+    const int shift = hi - width;
+    if ((ce = cudaMemsetAsync(d_hist, 0, kBins * sizeof(unsigned long long), ctx->stream)) != cudaSuccess) break;
+    if ((rc = mt_launch_select_hist(ctx, N, dtype, n, n_rows, ld, prefix, hi, shift, width, d_hist))) break;
+    if ((ce = cudaMemcpyAsync(h_hist, d_hist, kBins * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream)) != cudaSuccess) break;
+    if ((ce = cudaStreamSynchronize(ctx->stream)) != cudaSuccess) break;
+    if (hi == bits) {  // first pass: total number of non-zero elements, and the rank to find
+      for (int b = 0; b < kBins; ++b) count += h_hist[b];
+      k = (unsigned long long)floor(fraction * (double)count);
+      if (k >= count) { all_removed = true; break; }
+    }
+    int b = 0;
+    while (b < (1 << width) - 1 && k >= h_hist[b]) { k -= h_hist[b]; ++b; }
+    prefix = (prefix << width) | (unsigned long long)b;
+    hi = shift;
+  }
+  cudaFree(d_hist);
+  delete[] h_hist;
+  if (rc) return rc;
+  MT_CUDA_OK(ctx, ce);
+  if (count_host) *count_host = (int64_t)count;
+  if (all_removed) {
+    *tau_host = INFINITY;
+  } else if (dtype == MT_F32) {
+    const uint32_t u = (uint32_t)prefix;
+    float f;
+    memcpy(&f, &u, 4);
+    *tau_host = (double)f;
+  } else {
+    *tau_host = bits_to_double(prefix);
+  }
+  return MT_OK;
+}
+
+int mt_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
+                    int64_t* row_ptr, int64_t* nnz_host) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_tensor_args(ctx, N, dtype, n, n_rows, ld);
+  if (rc) return rc;
+  if (!row_ptr || !nnz_host) return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and nnz_host must be non-NULL");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  if ((rc = mt_launch_sparse_count(ctx, N, dtype, n, n_rows, ld, tau, row_ptr))) return rc;
+  MT_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hscal, row_ptr + 6 * n_rows, 8, cudaMemcpyDeviceToHost, ctx->stream));
+  MT_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  *nnz_host = (int64_t)ctx->hscal[0];
+  return MT_OK;
+}
+
+int mt_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
+                   const int64_t* row_ptr, uint32_t* mask, void* vals) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_tensor_args(ctx, N, dtype, n, n_rows, ld);
+  if (rc) return rc;
+  if (!row_ptr || !mask) return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and mask must be non-NULL");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  return mt_launch_sparse_fill(ctx, N, dtype, n, n_rows, ld, tau, row_ptr, mt_sparse_mask_words(n), mask, vals);
+}
+
+int mt_demag_field_sparse(mt_ctx* ctx, const mt_sparse_tensor* S, const double* Ms, const double* m, int batch,
+                          double* Hd) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_sparse(ctx, S);
+  if (rc) return rc;
+  if (!Ms || !m || !Hd) return mt_fail(ctx, MT_ERR_INVALID_ARG, "Ms, m and Hd must be non-NULL");
+  if (batch < 1 || batch > MT_MAX_BATCH) return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  const int64_t npad = round_up(S->n, MT_COL_CHUNK);
+  if ((rc = ensure_Mst(ctx, S->dtype, batch, npad))) return rc;
+  if ((rc = mt_launch_stage_M(ctx, S->dtype, Ms, m, batch, S->n, npad, ctx->Mst[0]))) return rc;
+  EpiArgs e;
+  memset(&e, 0, sizeof(e));
+  e.mode = 0;
+  e.batch = batch;
+  e.n = S->n;
+  e.n_rows = S->n_rows;
+  e.Hd = Hd;
+  return mt_launch_demag_sparse(ctx, S, ctx->Mst[0], npad, e);
 }
 
 int mt_energy(mt_ctx* ctx, const mt_problem* p, const double* m, int batch, double* E_out) {
@@ -275,9 +397,9 @@ int mt_energy(mt_ctx* ctx, const mt_problem* p, const double* m, int batch, doub
   const int64_t npad = round_up(p->n, MT_COL_CHUNK);
   rc = mt_ensure_ws(ctx, (void**)&ctx->edens, &ctx->edens_bytes, (size_t)batch * 4 * p->n * sizeof(double));
   if (rc) return rc;
-  if (p->N) {
-    if ((rc = ensure_Mst(ctx, p->dtype, batch, npad))) return rc;
-    if ((rc = mt_launch_stage_M(ctx, p->dtype, p->Ms, m, batch, p->n, npad, ctx->Mst[0]))) return rc;
+  if (has_demag(p)) {
+    if ((rc = ensure_Mst(ctx, demag_dtype(p), batch, npad))) return rc;
+    if ((rc = mt_launch_stage_M(ctx, demag_dtype(p), p->Ms, m, batch, p->n, npad, ctx->Mst[0]))) return rc;
   }
   EpiArgs e;
   fill_problem(e, p, batch);
@@ -351,10 +473,10 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
   double* ya = ctx->rk + 7 * sv;
   double* yb = ctx->rk + 8 * sv;
   double* mc = ctx->rk + 9 * sv;
-  if (p->N) {
-    rc = ensure_Mst(ctx, p->dtype, batch, npad);
+  if (has_demag(p)) {
+    rc = ensure_Mst(ctx, demag_dtype(p), batch, npad);
     if (rc) return rc;
-    rc = mt_launch_stage_M(ctx, p->dtype, p->Ms, m, batch, n, npad, ctx->Mst[0]);
+    rc = mt_launch_stage_M(ctx, demag_dtype(p), p->Ms, m, batch, n, npad, ctx->Mst[0]);
     if (rc) return rc;
   }
   unsigned long long* d_err = ctx->dscal;
@@ -379,7 +501,7 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       EpiArgs e = base;
       e.y = m; e.k_out = k[0]; e.torque_bits = want_tq ? d_tq : nullptr;
       e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[0]; e.coef[0] = 1.0; e.base = m; e.h = 0.5 * dt; e.y_out = ya;
-      e.M_out = p->N ? ctx->Mst[1] : nullptr;
+      e.M_out = has_demag(p) ? ctx->Mst[1] : nullptr;
       return eval_rhs(ctx, p, npad, 0, e);
     };
     auto stages234 = [&]() -> int {
@@ -387,12 +509,12 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       EpiArgs e = base;  // stage 2: k2 = f(ya); yb = m + dt/2 k2
       e.y = ya; e.k_out = k[1];
       e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[1]; e.coef[0] = 1.0; e.base = m; e.h = 0.5 * dt; e.y_out = yb;
-      e.M_out = p->N ? ctx->Mst[0] : nullptr;
+      e.M_out = has_demag(p) ? ctx->Mst[0] : nullptr;
       if ((r = eval_rhs(ctx, p, npad, 1, e))) return r;
       e = base;  // stage 3: k3 = f(yb); ya = m + dt k3
       e.y = yb; e.k_out = k[2];
       e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[2]; e.coef[0] = 1.0; e.base = m; e.h = dt; e.y_out = ya;
-      e.M_out = p->N ? ctx->Mst[1] : nullptr;
+      e.M_out = has_demag(p) ? ctx->Mst[1] : nullptr;
       if ((r = eval_rhs(ctx, p, npad, 0, e))) return r;
       e = base;  // stage 4: k4 = f(ya); m <- m + dt/6 (k1 + 2 k2 + 2 k3 + k4), renormalised, restaged
       e.y = ya; e.k_out = k[3];
@@ -400,7 +522,7 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       for (int s = 0; s < 4; ++s) e.kptr[s] = k[s];
       e.coef[0] = 1.0; e.coef[1] = 2.0; e.coef[2] = 2.0; e.coef[3] = 1.0;
       e.base = m; e.h = dt / 6.0; e.y_out = m; e.renorm = o->renormalize;
-      e.M_out = p->N ? ctx->Mst[0] : nullptr;
+      e.M_out = has_demag(p) ? ctx->Mst[0] : nullptr;
       return eval_rhs(ctx, p, npad, 1, e);
     };
     auto sample_if_due = [&](int64_t done) -> int {
@@ -532,7 +654,7 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       {
         EpiArgs e = base;
         e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[0]; e.coef[0] = DP_A[1][0]; e.base = m; e.h = h; e.y_out = ya;
-        e.M_out = p->N ? ctx->Mst[src ^ 1] : nullptr;
+        e.M_out = has_demag(p) ? ctx->Mst[src ^ 1] : nullptr;
         if ((rc = mt_launch_combine(ctx, e))) return rc;
         src ^= 1;
       }
@@ -544,7 +666,7 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
         e.do_comb = 1; e.ncomb = s + 1;
         for (int j = 0; j <= s; ++j) { e.kptr[j] = k[j]; e.coef[j] = DP_A[s + 1][j]; }
         e.base = m; e.h = h; e.y_out = yout;
-        e.M_out = p->N ? ctx->Mst[src ^ 1] : nullptr;
+        e.M_out = has_demag(p) ? ctx->Mst[src ^ 1] : nullptr;
         if ((rc = eval_rhs(ctx, p, npad, src, e))) return rc;
         src ^= 1;
         double* tmp = yin; yin = yout; yout = tmp;

@@ -122,3 +122,12 @@ int mt_launch_assemble(mt_ctx* ctx, const mt_tiles* t, int dtype, int64_t r0, in
 // TMA variant (demag_tma.cu)
 int mt_launch_demag_tma(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
                         const void* Mst, int64_t npad, const EpiArgs& epi);
+// thresholded tensor (sparse.cu)
+int mt_launch_select_hist(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                          unsigned long long prefix, int prefix_shift, int shift, int width,
+                          unsigned long long* hist);
+int mt_launch_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
+                           int64_t* row_ptr);
+int mt_launch_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
+                          const int64_t* row_ptr, int64_t nw, uint32_t* mask, void* vals);
+int mt_launch_demag_sparse(mt_ctx* ctx, const mt_sparse_tensor* s, const void* Mst, int64_t npad, const EpiArgs& epi);

@@ -1,0 +1,316 @@
+// sparse.cu — F1: thresholded ("sparse") demagnetisation tensor, PAPER.md:235-243 (§4.3.1).
+//
+// "the demagnetization tensor can be reduced in size by removing all elements of the
+// tensor smaller than a given threshold value ... This also allows the demagnetization tensor, which
+// normally is a dense matrix, to be allocated as a sparse matrix, thus saving memory, which is
+// especially important when doing CUDA calculations."  PAPER.md:239 defines the threshold as a
+// fraction of the non-zero elements sorted by absolute value (reading DESIGN.md Q20).
+//
+// Three pieces:
+//  1. threshold selection: the k-th smallest |v| among the non-zero elements, by an MSB-first radix
+//     select over the bit patterns of |v| (which order like unsigned integers): one streaming pass of
+//     the dense tensor per 11-bit digit, integer histogram in shared memory -> exact and reproducible.
+//  2. compression to BITMAP ROWS: per (plane, row) a bit per column (1 = kept) and the kept values
+//     packed in column order.  Unlike CSR (4-byte column index per 4-byte value: no saving until more
+//     than half of the entries are gone — the slowdown at small thresholds PAPER.md:241 reports) the
+//     index costs 1/32 of a dense fp32 row, so HBM bytes per evaluation fall as (1 - X) + 3 %.
+//  3. the field kernel on that layout (A4-A7 semantics, same fused epilogue): one warp per target row;
+//     a 32-column chunk is one mask word per plane (uniform load), lane l owns column 32 c + l and
+//     fetches its value at offset popc(mask & lanes-below) of the chunk's packed run.
+#include "epilogue.cuh"
+
+namespace {
+
+constexpr int kDigitBits = 11;
+constexpr int kBins = 1 << kDigitBits;
+
+template <typename T> struct KeyOf;
+template <> struct KeyOf<float> {
+  typedef uint32_t type;
+  static constexpr int bits = 32;
+  __device__ static __forceinline__ uint32_t key(float v) { return __float_as_uint(v) & 0x7fffffffu; }
+};
+template <> struct KeyOf<double> {
+  typedef unsigned long long type;
+  static constexpr int bits = 64;
+  __device__ static __forceinline__ unsigned long long key(double v) {
+    return (unsigned long long)__double_as_longlong(v) & 0x7fffffffffffffffull;
+  }
+};
+
+// hist[d] += multiplicity of every non-zero element whose key has the given prefix above `shift+width`
+// and digit d at `shift`; planes xy, xz, yz (1, 2, 4) count twice (Q20).
+template <typename T>
+__global__ void __launch_bounds__(512) select_hist_kernel(const T* __restrict__ N, int64_t n, int64_t n_rows,
+                                                          int64_t ld, typename KeyOf<T>::type prefix,
+                                                          int prefix_shift, int shift, int width,
+                                                          unsigned long long* __restrict__ hist) {
+  typedef typename KeyOf<T>::type K;
+  __shared__ unsigned long long sh[kBins];
+  for (int k = threadIdx.x; k < kBins; k += blockDim.x) sh[k] = 0ull;
+  __syncthreads();
+  const int64_t rows_total = 6 * n_rows;
+  const K dmask = (K)((1u << width) - 1u);
+  for (int64_t r = blockIdx.x; r < rows_total; r += gridDim.x) {
+    const int plane = (int)(r / n_rows);
+    const unsigned long long w = (plane == 1 || plane == 2 || plane == 4) ? 2ull : 1ull;
+    const T* row = N + r * ld;
+    for (int64_t j = threadIdx.x; j < n; j += blockDim.x) {
+      const K key = KeyOf<T>::key(row[j]);
+      if (key == 0) continue;
+      if (prefix_shift < KeyOf<T>::bits && (key >> prefix_shift) != prefix) continue;
+      atomicAdd(&sh[(unsigned)((key >> shift) & dmask)], w);
+    }
+  }
+  __syncthreads();
+  for (int k = threadIdx.x; k < kBins; k += blockDim.x)
+    if (sh[k]) atomicAdd(&hist[k], sh[k]);
+}
+
+template <typename T> __device__ __forceinline__ bool kept(T v, T tau) { return v != T(0) && !(fabs(v) < tau); }
+
+// counts[plane * n_rows + i] = kept entries of row i of the plane; one warp per (plane, row)
+template <typename T>
+__global__ void __launch_bounds__(256) sparse_count_kernel(const T* __restrict__ N, int64_t n, int64_t n_rows,
+                                                           int64_t ld, T tau, int64_t* __restrict__ counts) {
+  const int64_t r = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (r >= 6 * n_rows) return;
+  const T* row = N + r * ld;
+  int c = 0;
+  for (int64_t j = lane; j < n; j += 32) c += kept(row[j], tau) ? 1 : 0;
+#pragma unroll
+  for (int off = 16; off > 0; off >>= 1) c += __shfl_xor_sync(0xffffffffu, c, off);
+  if (lane == 0) counts[r] = c;
+}
+
+// in-place exclusive scan of len+1 int64 (slot len receives the total); one block, sequential chunks
+__global__ void __launch_bounds__(1024) scan_kernel(int64_t* __restrict__ a, int64_t len) {
+  __shared__ int64_t sh[1024];
+  __shared__ int64_t carry;
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  for (int64_t base = 0; base < len; base += 1024) {
+    const int64_t i = base + threadIdx.x;
+    const int64_t v = i < len ? a[i] : 0;
+    sh[threadIdx.x] = v;
+    __syncthreads();
+    for (int off = 1; off < 1024; off <<= 1) {
+      const int64_t t = (int)threadIdx.x >= off ? sh[threadIdx.x - off] : 0;
+      __syncthreads();
+      sh[threadIdx.x] += t;
+      __syncthreads();
+    }
+    if (i < len) a[i] = carry + sh[threadIdx.x] - v;
+    __syncthreads();
+    if (threadIdx.x == 1023) carry += sh[1023];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) a[len] = carry;
+}
+
+// mask[(plane * n_rows + i) * nw + c] bit l = entry (i, 32 c + l) kept; kept values packed from
+// vals[row_ptr[plane * n_rows + i]] in column order.  One warp per (plane, row).
+template <typename T>
+__global__ void __launch_bounds__(256) sparse_fill_kernel(const T* __restrict__ N, int64_t n, int64_t n_rows,
+                                                          int64_t ld, T tau, const int64_t* __restrict__ row_ptr,
+                                                          int64_t nw, uint32_t* __restrict__ mask,
+                                                          T* __restrict__ vals) {
+  const int64_t r = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (r >= 6 * n_rows) return;
+  const T* row = N + r * ld;
+  uint32_t* mrow = mask + r * nw;
+  T* out = vals + row_ptr[r];
+  int64_t off = 0;
+  for (int64_t c = 0; c < nw; ++c) {
+    const int64_t j = c * 32 + lane;
+    const T v = j < n ? row[j] : T(0);
+    const bool k = kept(v, tau);
+    const uint32_t word = __ballot_sync(0xffffffffu, k);
+    if (k) out[off + __popc(word & ((1u << lane) - 1u))] = v;
+    if (lane == 0) mrow[c] = word;
+    off += __popc(word);
+  }
+}
+
+// ---- field kernel on bitmap rows (A4-A7 on the thresholded tensor) ---------------------------------
+// nw (mask words per row-plane) is a multiple of kUnroll with zero padding words, so the chunk loop has
+// no tail.  fp32: products and a run of at most 32 chunks x 3 terms in fp32, then fp64 (Q19);
+// fp64: DFMA throughout.  Lanes are combined by a fixed xor butterfly: bitwise reproducible.
+constexpr int kUnroll = 4;
+constexpr int kGroupChunks = 32;
+
+struct SparseArgs {
+  int64_t n, n_rows, nw, npad;
+  const int64_t* row_ptr;
+  const uint32_t* mask;
+  const void* vals;
+  const void* Mst;
+};
+
+template <typename T, int B>
+__global__ void __launch_bounds__(256) demag_bitmap_kernel(SparseArgs a, EpiArgs e) {
+  const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (row >= a.n_rows) return;
+  const uint32_t lt = (1u << lane) - 1u;
+  const uint32_t* mrow[6];
+  const T* vrow[6];
+  int off[6];
+#pragma unroll
+  for (int p = 0; p < 6; ++p) {
+    const int64_t r = (int64_t)p * a.n_rows + row;
+    mrow[p] = a.mask + r * a.nw;
+    vrow[p] = (const T*)a.vals + a.row_ptr[r];
+    off[p] = 0;
+  }
+  const T* M = (const T*)a.Mst;
+  double acc[B][3];
+#pragma unroll
+  for (int b = 0; b < B; ++b) acc[b][0] = acc[b][1] = acc[b][2] = 0.0;
+  for (int64_t c0 = 0; c0 < a.nw; c0 += kGroupChunks) {
+    const int64_t cend = min(a.nw, c0 + (int64_t)kGroupChunks);
+    T run[B][3];
+#pragma unroll
+    for (int b = 0; b < B; ++b) run[b][0] = run[b][1] = run[b][2] = T(0);
+    for (int64_t c = c0; c < cend; c += kUnroll) {
+      uint32_t w[kUnroll][6];
+      T v[kUnroll][6];
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u)
+#pragma unroll
+        for (int p = 0; p < 6; ++p) w[u][p] = __ldg(mrow[p] + c + u);  // warp-uniform address
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u)
+#pragma unroll
+        for (int p = 0; p < 6; ++p) {
+          const uint32_t word = w[u][p];
+          v[u][p] = ((word >> lane) & 1u) ? __ldg(vrow[p] + off[p] + __popc(word & lt)) : T(0);
+          off[p] += __popc(word);
+        }
+#pragma unroll
+      for (int u = 0; u < kUnroll; ++u) {
+        const int64_t col = (c + u) * 32 + lane;  // < npad (npad is a multiple of 256 >= n)
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+          const T mx = M[((int64_t)b * 3 + 0) * a.npad + col];
+          const T my = M[((int64_t)b * 3 + 1) * a.npad + col];
+          const T mz = M[((int64_t)b * 3 + 2) * a.npad + col];
+          run[b][0] = fma(v[u][0], mx, fma(v[u][1], my, fma(v[u][2], mz, run[b][0])));
+          run[b][1] = fma(v[u][1], mx, fma(v[u][3], my, fma(v[u][4], mz, run[b][1])));
+          run[b][2] = fma(v[u][2], mx, fma(v[u][4], my, fma(v[u][5], mz, run[b][2])));
+        }
+      }
+    }
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+      acc[b][0] += (double)run[b][0];
+      acc[b][1] += (double)run[b][1];
+      acc[b][2] += (double)run[b][2];
+    }
+  }
+#pragma unroll
+  for (int b = 0; b < B; ++b)
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc)
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) acc[b][cc] += __shfl_xor_sync(0xffffffffu, acc[b][cc], o);
+  double s[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+  for (int b = 0; b < B; ++b)
+    if (lane == b) { s[0] = acc[b][0]; s[1] = acc[b][1]; s[2] = acc[b][2]; }
+  if (lane < B) {
+    const double hd[3] = {-s[0], -s[1], -s[2]};
+    row_epilogue(e, row, lane, hd);
+  }
+}
+
+template <typename T, int B>
+int launch_bitmap_B(mt_ctx* ctx, const SparseArgs& a, const EpiArgs& e) {
+  demag_bitmap_kernel<T, B><<<(unsigned)((a.n_rows + 7) / 8), 256, 0, ctx->stream>>>(a, e);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+template <typename T>
+int launch_bitmap(mt_ctx* ctx, const SparseArgs& a, const EpiArgs& e) {
+  switch (e.batch) {
+    case 1: return launch_bitmap_B<T, 1>(ctx, a, e);
+    case 2: return launch_bitmap_B<T, 2>(ctx, a, e);
+    case 3: return launch_bitmap_B<T, 3>(ctx, a, e);
+    case 4: return launch_bitmap_B<T, 4>(ctx, a, e);
+    case 5: return launch_bitmap_B<T, 5>(ctx, a, e);
+    case 6: return launch_bitmap_B<T, 6>(ctx, a, e);
+    case 7: return launch_bitmap_B<T, 7>(ctx, a, e);
+    case 8: return launch_bitmap_B<T, 8>(ctx, a, e);
+  }
+  return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
+}
+
+}  // namespace
+
+int mt_launch_select_hist(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                          unsigned long long prefix, int prefix_shift, int shift, int width,
+                          unsigned long long* hist) {
+  const unsigned grid = (unsigned)min((int64_t)ctx->num_sms * 4, 6 * n_rows);
+  if (dtype == MT_F32)
+    select_hist_kernel<float><<<grid, 512, 0, ctx->stream>>>((const float*)N, n, n_rows, ld, (uint32_t)prefix,
+                                                             prefix_shift, shift, width, hist);
+  else
+    select_hist_kernel<double><<<grid, 512, 0, ctx->stream>>>((const double*)N, n, n_rows, ld, prefix, prefix_shift,
+                                                              shift, width, hist);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+int mt_launch_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
+                           int64_t* row_ptr) {
+  const unsigned grid = (unsigned)((6 * n_rows + 7) / 8);
+  if (dtype == MT_F32)
+    sparse_count_kernel<float><<<grid, 256, 0, ctx->stream>>>((const float*)N, n, n_rows, ld, (float)tau, row_ptr);
+  else
+    sparse_count_kernel<double><<<grid, 256, 0, ctx->stream>>>((const double*)N, n, n_rows, ld, tau, row_ptr);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  scan_kernel<<<1, 1024, 0, ctx->stream>>>(row_ptr, 6 * n_rows);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+int mt_launch_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
+                          const int64_t* row_ptr, int64_t nw, uint32_t* mask, void* vals) {
+  const unsigned grid = (unsigned)((6 * n_rows + 7) / 8);
+  if (dtype == MT_F32)
+    sparse_fill_kernel<float><<<grid, 256, 0, ctx->stream>>>((const float*)N, n, n_rows, ld, (float)tau, row_ptr, nw,
+                                                             mask, (float*)vals);
+  else
+    sparse_fill_kernel<double><<<grid, 256, 0, ctx->stream>>>((const double*)N, n, n_rows, ld, tau, row_ptr, nw, mask,
+                                                              (double*)vals);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+int mt_launch_demag_sparse(mt_ctx* ctx, const mt_sparse_tensor* s, const void* Mst, int64_t npad, const EpiArgs& e) {
+  SparseArgs a;
+  a.n = s->n;
+  a.n_rows = s->n_rows;
+  a.nw = s->nw;
+  a.npad = npad;
+  a.row_ptr = s->row_ptr;
+  a.mask = s->mask;
+  a.vals = s->vals;
+  a.Mst = Mst;
+  const bool prof = ctx->prof_on && ctx->prof_ev && ctx->prof_count < MT_PROF_CAP;
+  if (prof) MT_CUDA_OK(ctx, cudaEventRecord(ctx->prof_ev[2 * ctx->prof_count], ctx->stream));
+  const int rc = s->dtype == MT_F32 ? launch_bitmap<float>(ctx, a, e) : launch_bitmap<double>(ctx, a, e);
+  if (prof) {
+    MT_CUDA_OK(ctx, cudaEventRecord(ctx->prof_ev[2 * ctx->prof_count + 1], ctx->stream));
+    ctx->prof_count++;
+  }
+  return rc;
+}

@@ -1,0 +1,157 @@
+"""-m gpu: F1 — thresholded tensor through the C-ABI against oracle/threshold.py.
+
+The dense input of the thresholding calls is the ORACLE's tensor (rounded to the stored dtype on the
+host and uploaded), so that threshold value, masks and packed values are integer/bit-exact
+comparisons; the field of the compressed tensor is compared with the oracle's field of the truncated
+tensor within north_star's H_d tolerances.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import threshold as OT
+from paper_2107_05364_b200 import binding as B
+from paper_2107_05364_b200 import workloads as W
+from tests import harness as H
+
+pytestmark = pytest.mark.gpu
+TOL_HD = {"f64": 1e-12, "f32": 1e-5}
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    c = B.mt_create(0)
+    yield c
+    c.close()
+
+
+def upload(N_ref, dtype):
+    """oracle tensor -> stored dtype on the host -> device planes [6][n][ld] (padding zero)."""
+    npdt = np.float32 if dtype == "f32" else np.float64
+    host = N_ref.astype(npdt)
+    n = host.shape[2]
+    ld = W.leading_dim(n, dtype)
+    dev = torch.zeros((6, host.shape[1], ld), dtype=B.torch_dtype(H.dtype_code(dtype)), device="cuda")
+    dev[:, :, :n] = torch.from_numpy(host).cuda()
+    return host, dev, ld
+
+
+def unpack(S, n):
+    """bitmap rows -> dense numpy planes (host-side decoding for the comparison only)."""
+    mask = S.mask.cpu().numpy().view(np.uint32)
+    vals = S.vals.cpu().numpy()
+    ptr = S.row_ptr.cpu().numpy()
+    out = np.zeros((6, S.n_rows, S.nw * 32), dtype=vals.dtype)
+    bits = ((mask[..., None] >> np.arange(32, dtype=np.uint32)) & 1).astype(bool).reshape(6, S.n_rows, -1)
+    for c in range(6):
+        for i in range(S.n_rows):
+            r = c * S.n_rows + i
+            out[c, i, bits[c, i]] = vals[ptr[r]:ptr[r + 1]]
+    assert not bits[:, :, n:].any()
+    return out[:, :, :n]
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+@pytest.mark.parametrize("grid", [(8, 8, 8), (13, 7, 3)])
+def test_threshold_value_and_bitmap_rows_are_exact(ctx, oracle, grid, dtype):
+    w = W.config5(*grid, batch=3)
+    n = w.n
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=True)
+    host, dev, ld = upload(N_ref, dtype)
+    code = H.dtype_code(dtype)
+    mult = np.array(OT.MULTIPLICITY).reshape(6, 1, 1)
+    for X in (0.0, 0.2, 0.4, 0.7, 0.93, 1.0):
+        tau_ref = OT.threshold_value(host, X)
+        tau, cnt = B.mt_threshold_value(ctx, dev, code, n, n, ld, X)
+        assert cnt == int((mult * (host != 0)).sum())
+        assert tau == tau_ref, (X, tau, tau_ref)
+        S = B.mt_sparse_build(ctx, dev, code, n, n, ld, tau)
+        torch.cuda.synchronize()
+        trunc = OT.truncate(host, tau_ref)
+        assert S.nnz == np.count_nonzero(trunc)
+        assert np.array_equal(unpack(S, n), trunc)
+        # field of the compressed tensor vs the oracle's field of the truncated tensor
+        m = torch.from_numpy(w.m).cuda()
+        Hd = torch.empty_like(m)
+        B.mt_demag_field_sparse(ctx, S, torch.from_numpy(w.Ms).cuda(), m, 3, Hd)
+        torch.cuda.synchronize()
+        ref = oracle.demag_field(trunc.astype(np.float64), w.Ms, w.m)
+        if S.nnz == 0:
+            assert not Hd.cpu().numpy().any()
+        else:
+            for b in range(3):
+                assert H.rel_l2(Hd[b].cpu().numpy(), ref[b]) <= TOL_HD[dtype]
+        Hd2 = torch.empty_like(m)
+        B.mt_demag_field_sparse(ctx, S, torch.from_numpy(w.Ms).cuda(), m, 3, Hd2)
+        assert torch.equal(Hd, Hd2)  # fixed reduction order
+
+
+@pytest.mark.parametrize("batch", [1, 5, 8])
+def test_sparse_field_batches_match_dense_path_on_truncated_tensor(ctx, oracle, batch):
+    """Dense kernels on the truncated tensor and the bitmap kernel on its compressed form agree."""
+    w = W.config5(20, 10, 2, batch=batch)
+    n = w.n
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=True)
+    host, dev, ld = upload(N_ref, "f32")
+    tau = OT.threshold_value(host, 0.5)
+    S = B.mt_sparse_build(ctx, dev, B.MT_F32, n, n, ld, tau)
+    trunc = OT.truncate(host, tau)
+    _, dev_t, _ = upload(trunc.astype(np.float64), "f32")
+    Ms = torch.from_numpy(w.Ms).cuda()
+    m = torch.from_numpy(w.m).cuda()
+    Hs, Hd = torch.empty_like(m), torch.empty_like(m)
+    B.mt_demag_field_sparse(ctx, S, Ms, m, batch, Hs)
+    B.mt_demag_field(ctx, dev_t, B.MT_F32, n, n, ld, Ms, m, batch, Hd)
+    torch.cuda.synchronize()
+    ref = oracle.demag_field(trunc.astype(np.float64), w.Ms, w.m)
+    for b in range(batch):
+        assert H.rel_l2(Hs[b].cpu().numpy(), ref[b]) <= 1e-5
+        assert H.rel_l2(Hs[b].cpu().numpy(), Hd[b].cpu().numpy()) <= 2e-6
+
+
+def test_thresholded_dynamics_follow_the_oracle_on_the_truncated_tensor(ctx, oracle):
+    """The experiment of PAPER.md:239 in small: config-2 physics (film, exchange, applied field) with a
+    40 % threshold; RK4 trajectory of the sparse path vs the oracle integrating the truncated tensor,
+    and the distance to the un-thresholded trajectory reported by the oracle itself."""
+    w = W.config2(24, 6, phase="dynamics")
+    n = w.n
+    tiles = H.dev_tiles(w)
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=True)
+    host, dev, ld = upload(N_ref, "f32")
+    tau, _ = B.mt_threshold_value(ctx, dev, B.MT_F32, n, n, ld, 0.4)
+    assert tau == OT.threshold_value(host, 0.4)
+    S = B.mt_sparse_build(ctx, dev, B.MT_F32, n, n, ld, tau)
+    prob = H.dev_problem(w, tiles, None, "f32", ld)
+    prob.N_sparse = S
+    dt, steps = 1e-13, 200
+    m = torch.from_numpy(w.m[:1].copy()).cuda()
+    samples = torch.zeros((16, 4), dtype=torch.float64, device="cuda")
+    _, res, _ = B.mt_integrate(ctx, prob, m, 1, 0.0, method=B.MT_RK4, dt=dt, t_end=steps * dt, sample_every=20,
+                               samples=samples)
+    trunc = OT.truncate(host, tau).astype(np.float64)
+    m_ref, s_ref, _ = oracle.integrate(H.oracle_problem(oracle, w, trunc), w.m[0], method=oracle.RK4, dt=dt,
+                                       t_end=steps * dt, sample_every=20, sample_cap=16, weights=w.vol)
+    assert res["n_samples"] == 10
+    s = samples[:10].cpu().numpy()
+    assert np.max(np.abs(s[:, 1:] - s_ref[:, 1:])) < 1e-4
+    assert np.max(np.abs(m[0].cpu().numpy() - m_ref)) < 1e-3
+    # energy through the sparse path too (F4 on F1)
+    E = torch.empty((1, 5), dtype=torch.float64, device="cuda")
+    B.mt_energy(ctx, prob, m, 1, E)
+    ref = oracle.energy_terms(H.oracle_problem(oracle, w, trunc), m[0].cpu().numpy(), vol=w.vol)
+    assert np.max(np.abs(E[0, :4].cpu().numpy() - ref)) <= 1e-5 * np.abs(ref).sum()
+
+
+def test_sparse_argument_checks(ctx):
+    Ms = torch.ones(4, dtype=torch.float64, device="cuda")
+    m = torch.zeros((1, 3, 4), dtype=torch.float64, device="cuda")
+    N = torch.zeros((6, 4, 4), dtype=torch.float32, device="cuda")
+    with pytest.raises(B.MtError):
+        B.mt_threshold_value(ctx, N, B.MT_F32, 4, 4, 4, 1.5)
+    tau, cnt = B.mt_threshold_value(ctx, N, B.MT_F32, 4, 4, 4, 0.3)   # all-zero tensor: nothing to rank
+    assert cnt == 0 and tau == float("inf")
+    S = B.mt_sparse_build(ctx, N, B.MT_F32, 4, 4, 4, 0.0)
+    assert S.nnz == 0
+    S.nw += 1
+    with pytest.raises(B.MtError):
+        B.mt_demag_field_sparse(ctx, S, Ms, m, 1, torch.empty_like(m))
