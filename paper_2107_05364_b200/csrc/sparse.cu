@@ -135,10 +135,8 @@ __global__ void __launch_bounds__(256) sparse_fill_kernel(const T* __restrict__ 
 }
 
 // ---- field kernel on bitmap rows (A4-A7 on the thresholded tensor) ---------------------------------
-// nw (mask words per row-plane) is a multiple of kUnroll with zero padding words, so the chunk loop has
-// no tail.  fp32: products and a run of at most 32 chunks x 3 terms in fp32, then fp64 (Q19);
+// fp32: products and a run of at most 32 chunks x 3 terms in fp32, then fp64 (Q19);
 // fp64: DFMA throughout.  Lanes are combined by a fixed xor butterfly: bitwise reproducible.
-constexpr int kUnroll = 4;
 constexpr int kGroupChunks = 32;
 
 struct SparseArgs {
@@ -149,6 +147,29 @@ struct SparseArgs {
   const void* Mst;
 };
 
+// One group = 32 chunks (1,024 columns): lane l loads the mask word of chunk c0 + l of every plane
+// (six coalesced 128-byte loads), a warp scan of the popcounts gives every chunk's offset into the
+// packed values, and a ballot gives the chunks that hold anything at all — the others are skipped,
+// which is where a thresholded tensor (near-field runs, "a more or less spherical region")
+// saves time as well as bytes.  Two non-empty chunks are processed per iteration so that their value
+// loads are in flight together.
+template <typename T, int B>
+__device__ __forceinline__ void bitmap_chunk(const uint32_t (&mw)[6], const uint32_t (&ex)[3], int c, bool valid, int lane,
+                                             uint32_t lt, const T* const (&vrow)[6], const int (&base)[6],
+                                             T (&v)[6]) {
+#pragma unroll
+  for (int q = 0; q < 3; ++q) {
+    const uint32_t e2 = __shfl_sync(0xffffffffu, ex[q], c);
+#pragma unroll
+    for (int h = 0; h < 2; ++h) {
+      const int p = 2 * q + h;
+      const uint32_t word = valid ? __shfl_sync(0xffffffffu, mw[p], c) : 0u;
+      const int st = (int)((e2 >> (16 * h)) & 0xffffu);
+      v[p] = ((word >> lane) & 1u) ? __ldg(vrow[p] + base[p] + st + __popc(word & lt)) : T(0);
+    }
+  }
+}
+
 template <typename T, int B>
 __global__ void __launch_bounds__(256) demag_bitmap_kernel(SparseArgs a, EpiArgs e) {
   const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -157,51 +178,71 @@ __global__ void __launch_bounds__(256) demag_bitmap_kernel(SparseArgs a, EpiArgs
   const uint32_t lt = (1u << lane) - 1u;
   const uint32_t* mrow[6];
   const T* vrow[6];
-  int off[6];
+  int base[6];
 #pragma unroll
   for (int p = 0; p < 6; ++p) {
     const int64_t r = (int64_t)p * a.n_rows + row;
     mrow[p] = a.mask + r * a.nw;
     vrow[p] = (const T*)a.vals + a.row_ptr[r];
-    off[p] = 0;
+    base[p] = 0;
   }
   const T* M = (const T*)a.Mst;
   double acc[B][3];
 #pragma unroll
   for (int b = 0; b < B; ++b) acc[b][0] = acc[b][1] = acc[b][2] = 0.0;
   for (int64_t c0 = 0; c0 < a.nw; c0 += kGroupChunks) {
-    const int64_t cend = min(a.nw, c0 + (int64_t)kGroupChunks);
+    uint32_t mw[6], ex[3], any = 0u;
+#pragma unroll
+    for (int p = 0; p < 6; ++p) {
+      mw[p] = (c0 + lane < a.nw) ? __ldg(mrow[p] + c0 + lane) : 0u;
+      any |= mw[p];
+    }
+    // inclusive scan of the popcounts, two planes per register (16-bit fields; a group holds <= 1,024)
+    uint32_t inc[3];
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+      const uint32_t own = (uint32_t)__popc(mw[2 * q]) | ((uint32_t)__popc(mw[2 * q + 1]) << 16);
+      uint32_t x = own;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t t = __shfl_up_sync(0xffffffffu, x, o);
+        if (lane >= o) x += t;
+      }
+      inc[q] = x;
+      ex[q] = x - own;
+    }
+    uint32_t nz = __ballot_sync(0xffffffffu, any != 0u);
     T run[B][3];
 #pragma unroll
     for (int b = 0; b < B; ++b) run[b][0] = run[b][1] = run[b][2] = T(0);
-    for (int64_t c = c0; c < cend; c += kUnroll) {
-      uint32_t w[kUnroll][6];
-      T v[kUnroll][6];
+    while (nz) {
+      const int ca = __ffs(nz) - 1;
+      nz &= nz - 1u;
+      const bool two = nz != 0u;
+      const int cb = two ? __ffs(nz) - 1 : ca;
+      nz &= nz - 1u;  // no-op when nz == 0
+      T va[6], vb[6];
+      bitmap_chunk<T, B>(mw, ex, ca, true, lane, lt, vrow, base, va);
+      bitmap_chunk<T, B>(mw, ex, cb, two, lane, lt, vrow, base, vb);
+      const int64_t cola = (c0 + ca) * 32 + lane, colb = (c0 + cb) * 32 + lane;  // < npad
 #pragma unroll
-      for (int u = 0; u < kUnroll; ++u)
-#pragma unroll
-        for (int p = 0; p < 6; ++p) w[u][p] = __ldg(mrow[p] + c + u);  // warp-uniform address
-#pragma unroll
-      for (int u = 0; u < kUnroll; ++u)
-#pragma unroll
-        for (int p = 0; p < 6; ++p) {
-          const uint32_t word = w[u][p];
-          v[u][p] = ((word >> lane) & 1u) ? __ldg(vrow[p] + off[p] + __popc(word & lt)) : T(0);
-          off[p] += __popc(word);
-        }
-#pragma unroll
-      for (int u = 0; u < kUnroll; ++u) {
-        const int64_t col = (c + u) * 32 + lane;  // < npad (npad is a multiple of 256 >= n)
-#pragma unroll
-        for (int b = 0; b < B; ++b) {
-          const T mx = M[((int64_t)b * 3 + 0) * a.npad + col];
-          const T my = M[((int64_t)b * 3 + 1) * a.npad + col];
-          const T mz = M[((int64_t)b * 3 + 2) * a.npad + col];
-          run[b][0] = fma(v[u][0], mx, fma(v[u][1], my, fma(v[u][2], mz, run[b][0])));
-          run[b][1] = fma(v[u][1], mx, fma(v[u][3], my, fma(v[u][4], mz, run[b][1])));
-          run[b][2] = fma(v[u][2], mx, fma(v[u][4], my, fma(v[u][5], mz, run[b][2])));
-        }
+      for (int b = 0; b < B; ++b) {
+        const T* Mb = M + (int64_t)b * 3 * a.npad;
+        const T ax = Mb[cola], ay = Mb[a.npad + cola], az = Mb[2 * a.npad + cola];
+        const T bx = Mb[colb], by = Mb[a.npad + colb], bz = Mb[2 * a.npad + colb];
+        run[b][0] = fma(va[0], ax, fma(va[1], ay, fma(va[2], az, run[b][0])));
+        run[b][1] = fma(va[1], ax, fma(va[3], ay, fma(va[4], az, run[b][1])));
+        run[b][2] = fma(va[2], ax, fma(va[4], ay, fma(va[5], az, run[b][2])));
+        run[b][0] = fma(vb[0], bx, fma(vb[1], by, fma(vb[2], bz, run[b][0])));
+        run[b][1] = fma(vb[1], bx, fma(vb[3], by, fma(vb[4], bz, run[b][1])));
+        run[b][2] = fma(vb[2], bx, fma(vb[4], by, fma(vb[5], bz, run[b][2])));
       }
+    }
+#pragma unroll
+    for (int q = 0; q < 3; ++q) {
+      const uint32_t tot = __shfl_sync(0xffffffffu, inc[q], 31);
+      base[2 * q] += (int)(tot & 0xffffu);
+      base[2 * q + 1] += (int)(tot >> 16);
     }
 #pragma unroll
     for (int b = 0; b < B; ++b) {
