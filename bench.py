@@ -29,8 +29,8 @@ UNIT = "evals/s"
 HBM_FALLBACK_GBS = 6650.0  # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); key = (config, tensor dtype, n_gpus)
-NCU_TRAFFIC_BYTES = {(5, "f32", 1): 103.082310e9 + 5.798656e6}
-NCU_TRAFFIC_SOURCE = "profiles/r01b_demag_tma_f32_b1_ncu_full.md"
+NCU_TRAFFIC_BYTES = {(5, "f32", 1): 103.082146e9 + 5.291520e6}
+NCU_TRAFFIC_SOURCE = "profiles/r02_ncu_full_summaries.md"
 
 
 def parse_args():
