@@ -155,6 +155,34 @@ int mt_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_r
 int mt_demag_field_sparse(mt_ctx* ctx, const mt_sparse_tensor* S, const double* Ms, const double* m,
                           int batch, double* Hd);
 
+/* ---- F3. Pair-symmetric half storage ("MagTense utilizes the fact that the tensor is
+ * symmetric ... reducing the scaling to ... almost N^2/2").  On a mesh of CONGRUENT axis-aligned
+ * cuboids N_ij = N_ji (the block depends on c_i - c_j only and is even in it), so only blocks with
+ * j >= i are kept, at tile granularity, and each serves two rows of the product: half the bytes per
+ * evaluation.  `data` is a DEVICE array of mt_sym_tensor_elems(n, dtype) elements in the tiled layout
+ * described in csrc/sym_layout.cuh (row blocks of 32, column tiles of 128 fp32 / 64 fp64, order of
+ * the kernel's loads), written by mt_assemble_tensor_sym only.                                     */
+typedef struct {
+  int64_t n;
+  int dtype;         /* MT_F32 | MT_F64 */
+  const void* data;
+} mt_sym_tensor;
+
+int64_t mt_sym_tensor_elems(int64_t n, int dtype);
+
+/* Assembles the kept half (every kept pair's closed form, fp64 arithmetic, rounded for MT_F32).
+ * status_flag (DEVICE int32, may be NULL) is OR-ed with 1 for a non-finite block and with 2 if any
+ * tile is not a cuboid (type 0) of the same size as tile 0 — the result must then not be used.
+ * Asynchronous.  Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA.                                          */
+int mt_assemble_tensor_sym(mt_ctx* ctx, const mt_tiles* tiles, int dtype, void* out,
+                           int32_t* status_flag);
+
+/* mt_demag_field from the half: Hd[b][a][i] for all n rows; same arithmetic rules (fp32 runs of at
+ * most 96 terms, then fp64), fixed reduction order.  States of a batch are evaluated one after the
+ * other (each streams the half once).                                                              */
+int mt_demag_field_sym(mt_ctx* ctx, const mt_sym_tensor* S, const double* Ms, const double* m,
+                       int batch, double* Hd);
+
 /* ---- A5 / A6. Effective field and Landau-Lifshitz right-hand side ------------------------------
  * H_eff = H_d + H_exch + H_anis + H_a                                   (Eq. 17)
  *   H_exch,i = c_ex,i * sum_{dir} (m_{i+} - 2 m_i + m_{i-}) * inv_d2[dir]   (Eq. 12 PAPER.md:94;
@@ -186,6 +214,8 @@ typedef struct {
   const double* vol;     /* [n] tile volumes: weights of <m> (A10); NULL = plain mean              */
   const mt_sparse_tensor* N_sparse; /* HOST pointer or NULL: when set, the demagnetising term uses this
                             thresholded tensor (F1) instead of N (N may then be NULL)  */
+  const mt_sym_tensor* N_sym; /* HOST pointer or NULL: demagnetising term from the pair-symmetric half
+                            (F3); takes precedence over N, after N_sparse                            */
 } mt_problem;
 
 /* dmdt[b][3][n] (required) and Heff[b][3][n] (optional, NULL to skip) for m[b][3][n].

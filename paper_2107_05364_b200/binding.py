@@ -26,7 +26,8 @@ COMPONENTS = ("xx", "xy", "xz", "yy", "yz", "zz")
 EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assemble_tensor",
            "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_energy",
            "mt_field_sweep", "mt_sparse_mask_words", "mt_threshold_value", "mt_sparse_count",
-           "mt_sparse_fill", "mt_demag_field_sparse", "mt_launch_count",
+           "mt_sparse_fill", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
+           "mt_demag_field_sym", "mt_launch_count",
            "mt_set_demag_variant", "mt_profile_begin", "mt_profile_end")
 
 
@@ -50,7 +51,12 @@ class _Problem(C.Structure):
         ("easy", C.c_void_p), ("easy_const", C.c_double * 3),
         ("H_a", C.c_void_p), ("H_a_const", C.c_double * 3),
         ("gamma", C.c_double), ("alpha_ll", C.c_double), ("vol", C.c_void_p), ("N_sparse", C.c_void_p),
+        ("N_sym", C.c_void_p),
     ]
+
+
+class _Sym(C.Structure):
+    _fields_ = [("n", C.c_int64), ("dtype", C.c_int), ("data", C.c_void_p)]
 
 
 class _Sparse(C.Structure):
@@ -111,6 +117,10 @@ def load() -> C.CDLL:
                                        C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.mt_demag_field_sparse.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p, C.c_void_p, C.c_int,
                                               C.c_void_p]
+        lib.mt_sym_tensor_elems.restype = C.c_int64
+        lib.mt_sym_tensor_elems.argtypes = [C.c_int64, C.c_int]
+        lib.mt_assemble_tensor_sym.argtypes = [C.c_void_p, C.POINTER(_Tiles), C.c_int, C.c_void_p, C.c_void_p]
+        lib.mt_demag_field_sym.argtypes = [C.c_void_p, C.POINTER(_Sym), C.c_void_p, C.c_void_p, C.c_int, C.c_void_p]
         lib.mt_energy.argtypes = [C.c_void_p, C.POINTER(_Problem), C.c_void_p, C.c_int, C.c_void_p]
         lib.mt_field_sweep.argtypes = [C.c_void_p, C.POINTER(_Problem), C.POINTER(_Opts), C.c_void_p, C.c_int64,
                                        C.c_void_p, C.c_int, C.c_void_p, C.POINTER(_Result)]
@@ -265,12 +275,16 @@ class Problem:
     alpha_ll: float = 0.0
     vol: torch.Tensor | None = None
     N_sparse: object = None  # SparseTensor (F1): used for the demagnetising term instead of N
+    N_sym: object = None     # SymTensor (F3): pair-symmetric half, congruent cuboid meshes only
 
     def _c(self) -> _Problem:
         s = _Problem()
         if self.N_sparse is not None:
             self._sparse_c = self.N_sparse._c()  # keep the struct alive while the call runs
             s.N_sparse = C.addressof(self._sparse_c)
+        if self.N_sym is not None:
+            self._sym_c = self.N_sym._c()
+            s.N_sym = C.addressof(self._sym_c)
         s.n = self.n
         s.N = _ptr(self.N, torch_dtype(self.dtype)) if self.N is not None else None
         s.dtype, s.ld = self.dtype, self.ld
@@ -390,3 +404,29 @@ def mt_demag_field_sparse(ctx: Context, S: SparseTensor, Ms: torch.Tensor, m: to
     s = S._c()
     ctx.check(ctx.lib.mt_demag_field_sparse(ctx.h, C.byref(s), _ptr(Ms, torch.float64), _ptr(m, torch.float64),
                                             batch, _ptr(Hd, torch.float64)))
+
+
+@dataclass
+class SymTensor:
+    """mt_sym_tensor (F3): the kept half in the tiled layout; `data` is a flat device tensor."""
+    n: int
+    dtype: int
+    data: torch.Tensor
+
+    def _c(self) -> _Sym:
+        return _Sym(self.n, self.dtype, _ptr(self.data, torch_dtype(self.dtype)))
+
+
+def mt_assemble_tensor_sym(ctx: Context, tiles: Tiles, dtype: int, status_flag: torch.Tensor | None = None) -> SymTensor:
+    """Allocates (torch) and assembles the pair-symmetric half; check status_flag & 2 == 0 afterwards."""
+    elems = int(ctx.lib.mt_sym_tensor_elems(tiles.n, dtype))
+    data = torch.empty(elems, dtype=torch_dtype(dtype), device=tiles.type.device)
+    t = tiles._c()
+    ctx.check(ctx.lib.mt_assemble_tensor_sym(ctx.h, C.byref(t), dtype, _ptr(data), _ptr(status_flag, torch.int32)))
+    return SymTensor(tiles.n, dtype, data)
+
+
+def mt_demag_field_sym(ctx: Context, S: SymTensor, Ms: torch.Tensor, m: torch.Tensor, batch: int, Hd: torch.Tensor):
+    s = S._c()
+    ctx.check(ctx.lib.mt_demag_field_sym(ctx.h, C.byref(s), _ptr(Ms, torch.float64), _ptr(m, torch.float64), batch,
+                                         _ptr(Hd, torch.float64)))

@@ -6,6 +6,7 @@
 #include <new>
 
 #include "mt_internal.cuh"
+#include "sym_layout.cuh"
 
 namespace {
 
@@ -38,8 +39,18 @@ int ensure_Mst(mt_ctx* ctx, int dtype, int batch, int64_t npad) {
   return MT_OK;
 }
 
-inline bool has_demag(const mt_problem* p) { return p->N != nullptr || p->N_sparse != nullptr; }
-inline int demag_dtype(const mt_problem* p) { return p->N_sparse ? p->N_sparse->dtype : p->dtype; }
+inline bool has_demag(const mt_problem* p) { return p->N != nullptr || p->N_sparse != nullptr || p->N_sym != nullptr; }
+inline int demag_dtype(const mt_problem* p) {
+  return p->N_sparse ? p->N_sparse->dtype : p->N_sym ? p->N_sym->dtype : p->dtype;
+}
+
+int check_sym(mt_ctx* ctx, const mt_sym_tensor* s) {
+  if (!s) return mt_fail(ctx, MT_ERR_INVALID_ARG, "symmetric tensor is NULL");
+  if (s->dtype != MT_F32 && s->dtype != MT_F64) return mt_fail(ctx, MT_ERR_INVALID_ARG, "unknown dtype %d", s->dtype);
+  if (s->n <= 0) return mt_fail(ctx, MT_ERR_INVALID_ARG, "n must be positive");
+  if (!s->data || ((uintptr_t)s->data & 15)) return mt_fail(ctx, MT_ERR_INVALID_ARG, "data null or not 16-byte aligned");
+  return MT_OK;
+}
 
 int check_sparse(mt_ctx* ctx, const mt_sparse_tensor* s) {
   if (!s) return mt_fail(ctx, MT_ERR_INVALID_ARG, "sparse tensor is NULL");
@@ -85,6 +96,12 @@ int check_problem(mt_ctx* ctx, const mt_problem* p, int batch) {
       return mt_fail(ctx, MT_ERR_INVALID_ARG, "sparse tensor must be n x n");
     return MT_OK;
   }
+  if (p->N_sym) {
+    int rc = check_sym(ctx, p->N_sym);
+    if (rc) return rc;
+    if (p->N_sym->n != p->n) return mt_fail(ctx, MT_ERR_INVALID_ARG, "symmetric tensor must have n tiles");
+    return MT_OK;
+  }
   if (p->N) return check_tensor_args(ctx, p->N, p->dtype, p->n, p->n, p->ld);
   return MT_OK;
 }
@@ -92,6 +109,7 @@ int check_problem(mt_ctx* ctx, const mt_problem* p, int batch) {
 // one evaluation of the fused right-hand side: field of the staged M (ctx->Mst[src]) + epilogue
 int eval_rhs(mt_ctx* ctx, const mt_problem* p, int64_t npad, int src, const EpiArgs& e) {
   if (p->N_sparse) return mt_launch_demag_sparse(ctx, p->N_sparse, ctx->Mst[src], npad, e);
+  if (p->N_sym) return mt_launch_demag_sym(ctx, p->N_sym, ctx->Mst[src], npad, e);
   if (p->N) return mt_launch_demag(ctx, p->N, p->dtype, p->n, p->n, p->ld, ctx->Mst[src], npad, e);
   return mt_launch_local_only(ctx, e);
 }
@@ -156,6 +174,7 @@ int mt_destroy(mt_ctx* c) {
   cudaFree(c->partial);
   cudaFree(c->rk);
   cudaFree(c->edens);
+  cudaFree(c->sym_ws);
   cudaFree(c->dscal);
   cudaFree(c->stage_io);
   cudaFreeHost(c->hscal);
@@ -284,6 +303,41 @@ int mt_llg_rhs(mt_ctx* ctx, const mt_problem* p, const double* m, int batch, dou
   e.k_out = dmdt;
   e.heff_out = Heff;
   return eval_rhs(ctx, p, npad, 0, e);
+}
+
+int64_t mt_sym_tensor_elems(int64_t n, int dtype) {
+  if (n <= 0 || (dtype != MT_F32 && dtype != MT_F64)) return 0;
+  const int tw = dtype == MT_F32 ? SymCfg<float>::TW : SymCfg<double>::TW;
+  return sym_total_tiles(n, tw) * (int64_t)6 * 32 * tw;
+}
+
+int mt_assemble_tensor_sym(mt_ctx* ctx, const mt_tiles* t, int dtype, void* out, int32_t* status_flag) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  if (!t || !t->type || !t->center || !t->size || t->n <= 0) return mt_fail(ctx, MT_ERR_INVALID_ARG, "tiles incomplete");
+  if (dtype != MT_F32 && dtype != MT_F64) return mt_fail(ctx, MT_ERR_INVALID_ARG, "unknown dtype %d", dtype);
+  if (!out || ((uintptr_t)out & 15)) return mt_fail(ctx, MT_ERR_INVALID_ARG, "out null or not 16-byte aligned");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  return mt_launch_assemble_sym(ctx, t, dtype, out, status_flag);
+}
+
+int mt_demag_field_sym(mt_ctx* ctx, const mt_sym_tensor* S, const double* Ms, const double* m, int batch, double* Hd) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_sym(ctx, S);
+  if (rc) return rc;
+  if (!Ms || !m || !Hd) return mt_fail(ctx, MT_ERR_INVALID_ARG, "Ms, m and Hd must be non-NULL");
+  if (batch < 1 || batch > MT_MAX_BATCH) return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  const int64_t npad = round_up(S->n, MT_COL_CHUNK);
+  if ((rc = ensure_Mst(ctx, S->dtype, batch, npad))) return rc;
+  if ((rc = mt_launch_stage_M(ctx, S->dtype, Ms, m, batch, S->n, npad, ctx->Mst[0]))) return rc;
+  EpiArgs e;
+  memset(&e, 0, sizeof(e));
+  e.mode = 0;
+  e.batch = batch;
+  e.n = S->n;
+  e.n_rows = S->n;
+  e.Hd = Hd;
+  return mt_launch_demag_sym(ctx, S, ctx->Mst[0], npad, e);
 }
 
 int64_t mt_sparse_mask_words(int64_t n) { return n <= 0 ? 0 : round_up((n + 31) / 32, 4); }

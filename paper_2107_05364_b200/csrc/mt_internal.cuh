@@ -25,6 +25,8 @@ struct mt_ctx {
   size_t partial_bytes;
   double* rk;  // integrator stages + scratch states
   size_t rk_bytes;
+  void* sym_ws;   // rowpart + colpart of the symmetric-half field kernel (F3)
+  size_t sym_ws_bytes;
   double* edens;  // [B][4][n] energy densities (mt_energy)
   size_t edens_bytes;
   unsigned long long* dscal;  // device scalars: [0] err bits, [1] torque bits
@@ -131,3 +133,6 @@ int mt_launch_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int
 int mt_launch_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
                           const int64_t* row_ptr, int64_t nw, uint32_t* mask, void* vals);
 int mt_launch_demag_sparse(mt_ctx* ctx, const mt_sparse_tensor* s, const void* Mst, int64_t npad, const EpiArgs& epi);
+// pair-symmetric half (assemble.cu, sym.cu)
+int mt_launch_assemble_sym(mt_ctx* ctx, const mt_tiles* t, int dtype, void* out, int32_t* status);
+int mt_launch_demag_sym(mt_ctx* ctx, const mt_sym_tensor* S, const void* Mst, int64_t npad, const EpiArgs& epi);

@@ -295,3 +295,21 @@ def test_uniformly_magnetised_cube_of_tiles(oracle):
         exp = cuboid6(oracle, (n1,) * 3, centers[i] - n1 / 2)
         assert np.max(np.abs(rowsum[:, i] - exp)) < 1e-14
     assert abs(rowsum[5].mean() - rowsum[0].mean()) < 1e-14
+
+
+# ---- F3: the pair symmetry the half storage relies on ------------------------------------
+def test_pair_symmetry_holds_on_congruent_grids_only(oracle):
+    """N_ij = N_ji for congruent axis-aligned cuboids (block even in c_i - c_j, P9); it fails for
+    cuboids of different sizes and for tetrahedra (Q2) — which is why F3 checks congruence."""
+    import numpy as np
+    c = np.array([[i + 0.5, j + 0.5, k + 0.5] for k in range(2) for j in range(3) for i in range(4)]) * [0.5, 0.7, 0.3]
+    n = len(c)
+    t = oracle.Tiles(type=np.zeros(n, np.int32), center=c, size=np.tile([0.5, 0.7, 0.3], (n, 1)),
+                     verts=np.zeros((n, 4, 3)), Ms=np.ones(n))
+    N = oracle.assemble_rows(t)
+    assert np.max(np.abs(N - N.transpose(0, 2, 1))) < 1e-16
+    size = np.tile([0.5, 0.7, 0.3], (n, 1))
+    size[3] = [0.25, 0.35, 0.15]
+    t2 = oracle.Tiles(type=np.zeros(n, np.int32), center=c, size=size, verts=np.zeros((n, 4, 3)), Ms=np.ones(n))
+    N2 = oracle.assemble_rows(t2)
+    assert np.max(np.abs(N2 - N2.transpose(0, 2, 1))) > 1e-3
