@@ -331,6 +331,48 @@ def main():
         out["batch8"] = {"state_evals_per_s": 8000.0 / ms_b8, "ms": ms_b8, "kernel_ms": kernel_ms["b8"],
                          "achieved_gbs": alg_b8 / (kernel_ms["b8"] * 1e-3) / 1e9,
                          "frac": alg_b8 / (kernel_ms["b8"] * 1e-3) / 1e9 / peak}
+        if world == 1 and w.grid is not None:
+            # ---- F3: the same field from the pair-symmetric half, congruent cuboid grid ----
+            st2 = torch.zeros(1, dtype=torch.int32, device=dev)
+            s0, s1 = ev(), ev()
+            s0.record()
+            S = B.mt_assemble_tensor_sym(ctx, tiles, code, st2)
+            s1.record()
+            torch.cuda.synchronize()
+            assert int(st2.item()) == 0
+            Hs = torch.empty_like(Hd1)
+
+            def step_sym():
+                B.mt_demag_field_sym(ctx, S, tiles.Ms, m1, 1, Hs)
+            ms_sym, _, _ = timed(step_sym, 3, max(5, K // 2), tag="sym")
+            step_field()
+            torch.cuda.synchronize()
+            sym_bytes = S.data.numel() * s
+            out["sym_half"] = {"evals_per_s": 1000.0 / ms_sym, "ms": ms_sym, "kernel_ms": kernel_ms["sym"],
+                               "resident_bytes": sym_bytes, "achieved_gbs": sym_bytes / (kernel_ms["sym"] * 1e-3) / 1e9,
+                               "frac": sym_bytes / (kernel_ms["sym"] * 1e-3) / 1e9 / peak,
+                               "assembly_ms": s0.elapsed_time(s1),
+                               "rel_l2_vs_full_tensor_field": float(((Hs - Hd1).norm() / Hd1.norm()).item()),
+                               "note": "NEXT row F3: half storage, every stored block used for two rows"}
+            del S
+            # ---- F1: thresholded tensor, fraction 0.9, bitmap rows ---------------------------
+            t0_, t1_, t2_ = ev(), ev(), ev()
+            t0_.record()
+            tau, _cnt = B.mt_threshold_value(ctx, N, code, n, rows, ld, 0.9)
+            t1_.record()
+            Sp = B.mt_sparse_build(ctx, N, code, n, rows, ld, tau)
+            t2_.record()
+            torch.cuda.synchronize()
+
+            def step_sparse():
+                B.mt_demag_field_sparse(ctx, Sp, tiles.Ms, m1, 1, Hs)
+            ms_sp, _, _ = timed(step_sparse, 3, max(5, K // 2))
+            out["threshold_0.9"] = {"evals_per_s": 1000.0 / ms_sp, "ms": ms_sp, "tau": tau, "kept_entries": Sp.nnz,
+                                    "resident_bytes": Sp.nbytes(), "select_ms": t0_.elapsed_time(t1_),
+                                    "compress_ms": t1_.elapsed_time(t2_),
+                                    "rel_l2_vs_full_tensor_field": float(((Hs - Hd1).norm() / Hd1.norm()).item()),
+                                    "note": "NEXT row F1: 90 % of the non-zero elements removed"}
+            del Sp
         if rank == 0 and world == 1:
             out["cpu_baseline"] = oracle_sample(w, band_rows=4096, calls=6)
     if rank == 0:

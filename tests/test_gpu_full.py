@@ -253,3 +253,37 @@ def test_config5_full_size(ctx, oracle):
     sub = np.arange(r0, r0 + 512, 16, dtype=np.int64)
     N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), rows=sub, long_double=True)
     check_tensor(Nb[:, ::16], N_ref, "f64", w.n)
+
+
+def test_config5_full_size_symmetric_half(ctx, oracle):
+    """F3 at BASELINE's full size, in the configuration bench.py times: the field from the 51.6 GB
+    pair-symmetric half on sampled rows against the oracle's rows of the full tensor; the uniform-m
+    property (sum_j N_ij = tensor of the whole block) on rows the sample does not contain."""
+    w = W.config5(batch=2)
+    tiles = H.dev_tiles(w)
+    status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    S = B.mt_assemble_tensor_sym(ctx, tiles, B.MT_F32, status)
+    torch.cuda.synchronize()
+    assert int(status.item()) == 0 and S.data.numel() * 4 < 0.502 * 6 * 65536 * 65536 * 4
+    rows = W.sample_rows(5, w.n, 96, extra=grid_corner_rows(w.grid) + [65535, 32768, 32767, 31, 32, 127, 128])
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), rows=rows, long_double=True)
+    Hd_ref = oracle.demag_field(N_ref, w.Ms, w.m)
+    m = torch.from_numpy(w.m).cuda()
+    Hd = torch.empty_like(m)
+    B.mt_demag_field_sym(ctx, S, tiles.Ms, m, 2, Hd)
+    torch.cuda.synchronize()
+    got = Hd.cpu().numpy()
+    for b in range(2):
+        assert H.rel_l2(got[b][:, rows], Hd_ref[b]) <= TOL_HD["f32"]
+    mu = torch.zeros((1, 3, w.n), dtype=torch.float64, device="cuda")
+    mu[0, 2] = 1.0
+    Hu = torch.empty_like(mu)
+    B.mt_demag_field_sym(ctx, S, tiles.Ms, mu, 1, Hu)
+    Hu = Hu.cpu().numpy()[0]
+    big = np.array([64.0, 64.0, 16.0])
+    for i in (0, 4097, 32768 + 2080, 65535):
+        blk = oracle.cuboid_block(0.5 * big, w.center[i] - 0.5 * big)
+        assert np.max(np.abs(Hu[:, i] + blk[[2, 4, 5]])) < 2e-5
+    Hd2 = torch.empty_like(m)
+    B.mt_demag_field_sym(ctx, S, tiles.Ms, m, 2, Hd2)
+    assert torch.equal(Hd, Hd2)
