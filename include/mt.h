@@ -93,6 +93,18 @@ typedef struct {
 int mt_assemble_tensor(mt_ctx* ctx, const mt_tiles* tiles, int dtype, int64_t row_begin,
                        int64_t row_end, void* out, int64_t ld, int32_t* status_flag);
 
+/* ---- F2. Far-field-stable assembly (the analytic form's "error at large distances
+ * being of the same magnitude as the elements of the tensor itself"; "different
+ * approximations for the demagnetization tensor depending on the distance").
+ * mode 0 (default): the closed form for every pair — the paper's method; its fp64 relative error per
+ *   block grows as ~5e-16 (r/edge)^3 (1e-10 at ~60 edges).
+ * mode 1: cuboid sources further than 16 of their longest edges from the target are evaluated as the
+ *   Gauss-Legendre quadrature (4^3 points, 3^3 beyond 48 edges) of the point-dipole kernel over the
+ *   source volume; per-block relative error <= 1e-11 at every distance.  Tetrahedron sources keep
+ *   the closed form.  Applies to the following mt_assemble_tensor calls of this ctx.
+ * Returns MT_OK or MT_ERR_INVALID_ARG.                                                              */
+int mt_set_assembly_mode(mt_ctx* ctx, int mode);
+
 /* ---- A4 / A7. Demagnetising field (Eq. 9 PAPER.md:78 with the sign and Ms reading DESIGN.md Q1;
  * "the most time consuming part" PAPER.md:17,122,138; moved to CUDA PAPER.md:145,223):
  *     Hd[b][a][i] = - sum_j sum_c N^{ac}_{ij} Ms[j] m[b][c][j],   i in [0, n_rows)

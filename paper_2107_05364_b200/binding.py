@@ -27,7 +27,7 @@ EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assembl
            "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_energy",
            "mt_field_sweep", "mt_sparse_mask_words", "mt_threshold_value", "mt_sparse_count",
            "mt_sparse_fill", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
-           "mt_demag_field_sym", "mt_launch_count",
+           "mt_demag_field_sym", "mt_set_assembly_mode", "mt_launch_count",
            "mt_set_demag_variant", "mt_profile_begin", "mt_profile_end")
 
 
@@ -97,6 +97,7 @@ def load() -> C.CDLL:
         lib.mt_create.argtypes = [C.POINTER(C.c_void_p), C.c_int, C.c_void_p]
         lib.mt_destroy.argtypes = [C.c_void_p]
         lib.mt_set_demag_variant.argtypes = [C.c_void_p, C.c_int]
+        lib.mt_set_assembly_mode.argtypes = [C.c_void_p, C.c_int]
         lib.mt_profile_begin.argtypes = [C.c_void_p]
         lib.mt_profile_end.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         lib.mt_assemble_tensor.argtypes = [C.c_void_p, C.POINTER(_Tiles), C.c_int, C.c_int64, C.c_int64,
@@ -430,3 +431,8 @@ def mt_demag_field_sym(ctx: Context, S: SymTensor, Ms: torch.Tensor, m: torch.Te
     s = S._c()
     ctx.check(ctx.lib.mt_demag_field_sym(ctx.h, C.byref(s), _ptr(Ms, torch.float64), _ptr(m, torch.float64), batch,
                                          _ptr(Hd, torch.float64)))
+
+
+def mt_set_assembly_mode(ctx: Context, mode: int):
+    """0: closed form everywhere (default, the paper's method); 1: far-field-stable (F2)."""
+    ctx.check(ctx.lib.mt_set_assembly_mode(ctx.h, mode))

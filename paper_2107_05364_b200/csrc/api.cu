@@ -227,6 +227,12 @@ int mt_set_demag_variant(mt_ctx* c, int variant) {
   return MT_OK;
 }
 
+int mt_set_assembly_mode(mt_ctx* c, int mode) {
+  if (!c || mode < 0 || mode > 1) return MT_ERR_INVALID_ARG;
+  c->assembly_mode = mode;
+  return MT_OK;
+}
+
 int mt_assemble_tensor(mt_ctx* ctx, const mt_tiles* t, int dtype, int64_t row_begin, int64_t row_end,
                        void* out, int64_t ld, int32_t* status_flag) {
   if (!ctx) return MT_ERR_INVALID_ARG;

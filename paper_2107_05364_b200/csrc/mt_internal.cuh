@@ -16,6 +16,7 @@ struct mt_ctx {
   cudaStream_t cap_stream;  // private stream for CUDA-graph capture
   int num_sms;
   int variant;  // 0 auto, 1 LDG, 2 TMA
+  int assembly_mode;  // 0 closed form everywhere (the paper's method), 1 far-field-stable (F2)
   int64_t launches;
   char err[512];
   // grow-only workspaces
