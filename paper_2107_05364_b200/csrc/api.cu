@@ -538,6 +538,10 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
     if (rc) return rc;
     rc = mt_launch_stage_M(ctx, demag_dtype(p), p->Ms, m, batch, n, npad, ctx->Mst[0]);
     if (rc) return rc;
+    // the second buffer is only ever written by the fused epilogue (rows < n): give its padding
+    // defined (zero) contents for this n as well, whatever an earlier problem left there
+    rc = mt_launch_stage_M(ctx, demag_dtype(p), p->Ms, m, batch, n, npad, ctx->Mst[1]);
+    if (rc) return rc;
   }
   unsigned long long* d_err = ctx->dscal;
   unsigned long long* d_tq = ctx->dscal + 1;
