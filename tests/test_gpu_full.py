@@ -287,3 +287,50 @@ def test_config5_full_size_symmetric_half(ctx, oracle):
     Hd2 = torch.empty_like(m)
     B.mt_demag_field_sym(ctx, S, tiles.Ms, m, 2, Hd2)
     assert torch.equal(Hd, Hd2)
+
+
+def test_config2_full_protocol_full_size_invariants_and_half_storage(ctx):
+    """The whole config-2 protocol at full size (160x40x1, 20,000 relax + 10,000 dynamics RK4 steps,
+    the work bench-class runs do) on the CUDA path: properties that hold at any size — |m| = 1, energy
+    non-increasing while relaxing (alpha > 0, constant field, uniform grid: PAPER.md:58) — and the two
+    storage formats of the same tensor (full six planes vs pair-symmetric half, F3) giving the same
+    <m>(t) within north_star's 1e-3."""
+    wr = W.config2(batch=1, phase="relax")
+    wd = W.config2(batch=1, phase="dynamics")
+    tiles = H.dev_tiles(wr)
+    N, ld, _ = H.assemble(ctx, tiles, "f32")
+    status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    S = B.mt_assemble_tensor_sym(ctx, tiles, B.MT_F32, status)
+    assert int(status.item()) == 0
+    dt = 1e-13
+    out = {}
+    for name in ("full", "half"):
+        pr = H.dev_problem(wr, tiles, N if name == "full" else None, "f32", ld)
+        pd = H.dev_problem(wd, tiles, N if name == "full" else None, "f32", ld)
+        if name == "half":
+            pr.N_sym = S
+            pd.N_sym = S
+        m = torch.from_numpy(wr.m[:1].copy()).cuda()
+        E = torch.empty((1, 5), dtype=torch.float64, device="cuda")
+        energies, t = [], 0.0
+        s1 = torch.zeros((200, 4), dtype=torch.float64, device="cuda")
+        for k in range(10):  # 10 x 2,000 relax steps, energy in between
+            B.mt_energy(ctx, pr, m, 1, E)
+            energies.append(float(E[0, 4].item()))
+            t, res, _ = B.mt_integrate(ctx, pr, m, 1, t, method=B.MT_RK4, dt=dt, t_end=t + 2000 * dt, sample_every=100,
+                                       samples=s1[20 * k:20 * (k + 1)])
+            assert res["accepted"] == 2000 and res["n_samples"] == 20
+        B.mt_energy(ctx, pr, m, 1, E)
+        energies.append(float(E[0, 4].item()))
+        # once relaxed the energy sits still to within the fp32 tensor's rounding of H_d (~1e-8 relative)
+        assert np.all(np.diff(energies) <= 1e-6 * abs(energies[-1])), energies
+        assert energies[-1] < 0.03 * energies[0]
+        s2 = torch.zeros((100, 4), dtype=torch.float64, device="cuda")
+        _, res, _ = B.mt_integrate(ctx, pd, m, 1, 0.0, method=B.MT_RK4, dt=dt, t_end=10000 * dt, sample_every=100, samples=s2)
+        assert res["accepted"] == 10000 and res["n_samples"] == 100
+        mm = m.cpu().numpy()[0]
+        assert np.max(np.abs(np.linalg.norm(mm, axis=0) - 1.0)) < 1e-14
+        out[name] = (s1.cpu().numpy(), s2.cpu().numpy())
+    assert np.max(np.abs(out["full"][0][:, 1:] - out["half"][0][:, 1:])) < 1e-3
+    assert np.max(np.abs(out["full"][1][:, 1:] - out["half"][1][:, 1:])) < 1e-3
+    assert np.max(np.abs(out["full"][1][-1, 1:] - out["full"][1][0, 1:])) > 0.05  # the field did move <m>
