@@ -30,6 +30,7 @@ HBM_FALLBACK_GBS = 6650.0  # B200_PROFILING.md fallback when MEASURED_PEAKS.json
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture (profiles/); key = (config, tensor dtype, n_gpus)
 NCU_TRAFFIC_BYTES = {(5, "f32", 1): 103.082146e9 + 5.291520e6}
+ASM_FP64_INST_PER_PAIR = 477.0  # DFMA + DADD + DMUL thread-instructions per cuboid pair (ncu, r02)
 NCU_TRAFFIC_SOURCE = "profiles/r02_ncu_full_summaries.md"
 
 
@@ -302,6 +303,17 @@ def main():
                                "the demag field kernel only (mt_profile_begin/end), averaged over the timed steps"}
     out["assembly"] = {"pairs_per_s": rows * n / (asm_ms * 1e-3) * world, "ms": asm_ms, "pairs": rows * n * world,
                        "launches": asm_launches, "dtype": dtype, "every_pair_evaluated": True}
+    # ALU roofline of the assembly kernel: FP64 pipe = 64 thread-instructions per
+    # clock per SM (ncu: sm__sass_thread_inst_executed_op_dfma_pred_on.peak_sustained); the kernel
+    # executes 477 DFMA + DADD + DMUL thread-instructions per cuboid pair (ncu r02 capture, static per pair)
+    sm_count = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    sm_hz = 1e6 * float((clocks or {}).get("sm_max_mhz") or 1965.0)
+    alu_peak = 64.0 * sm_count * sm_hz
+    asm_rate = ASM_FP64_INST_PER_PAIR * rows * n / (asm_ms * 1e-3)
+    out["assembly"]["roofline"] = {"bound": "alu", "achieved": asm_rate / 1e12, "peak": alu_peak / 1e12,
+                                   "unit": "T FP64 thread-inst/s", "frac": asm_rate / alu_peak,
+                                   "fp64_inst_per_pair": ASM_FP64_INST_PER_PAIR,
+                                   "source": "profiles/r02_ncu_full_summaries.md; peak at sm_max_mhz"}
 
     if not args.skip_extras:
         # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
