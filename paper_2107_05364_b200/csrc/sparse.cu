@@ -46,25 +46,33 @@ __global__ void __launch_bounds__(512) select_hist_kernel(const T* __restrict__ 
                                                           int prefix_shift, int shift, int width,
                                                           unsigned long long* __restrict__ hist) {
   typedef typename KeyOf<T>::type K;
-  __shared__ unsigned long long sh[kBins];
-  for (int k = threadIdx.x; k < kBins; k += blockDim.x) sh[k] = 0ull;
+  // 32-bit shared counters (a block sees far fewer than 2^31 elements: the launcher bounds the rows
+  // per block), flushed into the 64-bit global histogram.  Neighbouring columns hold values of similar
+  // magnitude, i.e. the same bin: lanes are aggregated with match.any so that a warp issues one shared
+  // atomic per distinct bin instead of up to 32 serialised ones.
+  __shared__ unsigned int sh[kBins];
+  for (int k = threadIdx.x; k < kBins; k += blockDim.x) sh[k] = 0u;
   __syncthreads();
   const int64_t rows_total = 6 * n_rows;
   const K dmask = (K)((1u << width) - 1u);
+  const int lane = threadIdx.x & 31;
+  const int64_t n_up = (n + 31) / 32 * 32;  // whole warps stay converged for the match
   for (int64_t r = blockIdx.x; r < rows_total; r += gridDim.x) {
     const int plane = (int)(r / n_rows);
-    const unsigned long long w = (plane == 1 || plane == 2 || plane == 4) ? 2ull : 1ull;
+    const unsigned int w = (plane == 1 || plane == 2 || plane == 4) ? 2u : 1u;
     const T* row = N + r * ld;
-    for (int64_t j = threadIdx.x; j < n; j += blockDim.x) {
-      const K key = KeyOf<T>::key(row[j]);
-      if (key == 0) continue;
-      if (prefix_shift < KeyOf<T>::bits && (key >> prefix_shift) != prefix) continue;
-      atomicAdd(&sh[(unsigned)((key >> shift) & dmask)], w);
+    for (int64_t j = threadIdx.x; j < n_up; j += blockDim.x) {
+      const K key = j < n ? KeyOf<T>::key(row[j]) : (K)0;
+      bool counted = key != 0;
+      if (counted && prefix_shift < KeyOf<T>::bits && (key >> prefix_shift) != prefix) counted = false;
+      const unsigned bin = counted ? (unsigned)((key >> shift) & dmask) : (unsigned)kBins;  // kBins = "none"
+      const unsigned peers = __match_any_sync(0xffffffffu, bin);
+      if (counted && lane == __ffs(peers) - 1) atomicAdd(&sh[bin], w * (unsigned)__popc(peers));
     }
   }
   __syncthreads();
   for (int k = threadIdx.x; k < kBins; k += blockDim.x)
-    if (sh[k]) atomicAdd(&hist[k], sh[k]);
+    if (sh[k]) atomicAdd(&hist[k], (unsigned long long)sh[k]);
 }
 
 template <typename T> __device__ __forceinline__ bool kept(T v, T tau) { return v != T(0) && !(fabs(v) < tau); }
@@ -295,7 +303,11 @@ int launch_bitmap(mt_ctx* ctx, const SparseArgs& a, const EpiArgs& e) {
 int mt_launch_select_hist(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
                           unsigned long long prefix, int prefix_shift, int shift, int width,
                           unsigned long long* hist) {
-  const unsigned grid = (unsigned)min((int64_t)ctx->num_sms * 4, 6 * n_rows);
+  // enough blocks that none sees 2^30 elements (32-bit shared counters with multiplicity 2)
+  int64_t blocks = (int64_t)ctx->num_sms * 4;
+  const int64_t need = (6 * n_rows * n + (1LL << 30) - 1) >> 30;
+  if (blocks < need) blocks = need;
+  const unsigned grid = (unsigned)min(blocks, 6 * n_rows);
   if (dtype == MT_F32)
     select_hist_kernel<float><<<grid, 512, 0, ctx->stream>>>((const float*)N, n, n_rows, ld, (uint32_t)prefix,
                                                              prefix_shift, shift, width, hist);
