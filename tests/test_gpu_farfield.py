@@ -79,3 +79,26 @@ def test_far_field_mode_field_matches_oracle(ctx, oracle):
         assert H.rel_l2(Hd[b].cpu().numpy(), ref[b]) <= 1e-12
     with pytest.raises(B.MtError):
         B.mt_set_assembly_mode(ctx, 7)
+
+
+def test_far_field_mode_applies_to_the_symmetric_half(ctx, oracle):
+    """mt_assemble_tensor_sym honours mt_set_assembly_mode: on a 160x3x1 bar (pairs out to 159 edges)
+    the field from the mode-1 half is closer to the oracle than from the mode-0 half, and both pass
+    the fp64 tolerance north_star sets for H_d."""
+    w = W.config5(160, 3, 1, batch=2)
+    tiles = H.dev_tiles(w)
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=True)
+    ref = oracle.demag_field(N_ref, w.Ms, w.m)
+    m = torch.from_numpy(w.m).cuda()
+    err = {}
+    for mode in (0, 1):
+        B.mt_set_assembly_mode(ctx, mode)
+        status = torch.zeros(1, dtype=torch.int32, device="cuda")
+        S = B.mt_assemble_tensor_sym(ctx, tiles, B.MT_F64, status)
+        Hd = torch.empty_like(m)
+        B.mt_demag_field_sym(ctx, S, tiles.Ms, m, 2, Hd)
+        torch.cuda.synchronize()
+        assert int(status.item()) == 0
+        err[mode] = max(H.rel_l2(Hd[b].cpu().numpy(), ref[b]) for b in range(2))
+        assert err[mode] <= 1e-12
+    assert err[1] <= err[0]

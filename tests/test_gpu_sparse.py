@@ -155,3 +155,26 @@ def test_sparse_argument_checks(ctx):
     S.nw += 1
     with pytest.raises(B.MtError):
         B.mt_demag_field_sparse(ctx, S, Ms, m, 1, torch.empty_like(m))
+
+
+def test_sparse_row_band(ctx, oracle):
+    """Thresholding a ROW BAND of the tensor (the multi-GPU shard unit of mt_assemble_tensor): the band's
+    own threshold, bitmap rows and field, against the oracle on the same rows."""
+    w = W.config5(12, 9, 3, batch=2)
+    n = w.n
+    rows = np.arange(70, 70 + 101, dtype=np.int64)
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), rows=rows, long_double=True)
+    host, dev, ld = upload(N_ref, "f32")
+    tau, _ = B.mt_threshold_value(ctx, dev, B.MT_F32, n, len(rows), ld, 0.6)
+    assert tau == OT.threshold_value(host, 0.6)
+    S = B.mt_sparse_build(ctx, dev, B.MT_F32, n, len(rows), ld, tau)
+    torch.cuda.synchronize()
+    trunc = OT.truncate(host, tau)
+    assert np.array_equal(unpack(S, n), trunc)
+    m = torch.from_numpy(w.m).cuda()
+    Hd = torch.empty((2, 3, len(rows)), dtype=torch.float64, device="cuda")
+    B.mt_demag_field_sparse(ctx, S, torch.from_numpy(w.Ms).cuda(), m, 2, Hd)
+    torch.cuda.synchronize()
+    ref = oracle.demag_field(trunc.astype(np.float64), w.Ms, w.m)
+    for b in range(2):
+        assert H.rel_l2(Hd[b].cpu().numpy(), ref[b]) <= 1e-5
