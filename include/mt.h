@@ -100,8 +100,9 @@ int mt_assemble_tensor(mt_ctx* ctx, const mt_tiles* tiles, int dtype, int64_t ro
  *   block grows as ~5e-16 (r/edge)^3 (1e-10 at ~60 edges).
  * mode 1: cuboid sources further than 16 of their longest edges from the target are evaluated as the
  *   Gauss-Legendre quadrature (4^3 points, 3^3 beyond 48 edges) of the point-dipole kernel over the
- *   source volume; per-block relative error <= 1e-11 at every distance.  Tetrahedron sources keep
- *   the closed form.  Applies to the following mt_assemble_tensor and mt_assemble_tensor_sym calls
+ *   source volume; per-block relative error <= 1e-11 at every distance.  Tetrahedron sources switch
+ *   at 8 of their longest edges to the same integral in collapsed coordinates (5^3 points, 4^3 beyond
+ *   24 edges).  Applies to the following mt_assemble_tensor and mt_assemble_tensor_sym calls
  *   of this ctx.
  * Returns MT_OK or MT_ERR_INVALID_ARG.                                                              */
 int mt_set_assembly_mode(mt_ctx* ctx, int mode);

@@ -102,3 +102,39 @@ def test_far_field_mode_applies_to_the_symmetric_half(ctx, oracle):
         err[mode] = max(H.rel_l2(Hd[b].cpu().numpy(), ref[b]) for b in range(2))
         assert err[mode] <= 1e-12
     assert err[1] <= err[0]
+
+
+def test_far_field_stable_assembly_tetrahedron_sources(ctx, oracle):
+    """F2 for tetrahedra: Delaunay tetrahedra of a small ball as sources, targets spread out to ~60
+    of their edges (config 4's range: ball of radius 1, slab at +3, edges ~0.1).  Mode 1 keeps every
+    block within 1e-10 of the long-double oracle; the fp64 polyhedron closed form (mode 0) is more
+    than 10x worse beyond 20 edges."""
+    w = W.config4(n_tets=400, n_cub=0, n_points=150, batch=1, body="tets")
+    n = w.n
+    edge = np.max(np.linalg.norm(w.verts[:, :, None, :] - w.verts[:, None, :, :], axis=3), axis=(1, 2))
+    # move every second tile's evaluation point far away along a seeded direction: the tensor only uses
+    # `center` of the TARGET and `verts` of the SOURCE, so this probes far-field blocks of real tetrahedra
+    rng = W.rng_for(4, 9)
+    far = np.arange(n) % 2 == 1
+    u = rng.standard_normal((n, 3))
+    u /= np.linalg.norm(u, axis=1, keepdims=True)
+    w.center = w.center.copy()
+    w.center[far] = u[far] * rng.uniform(3.0, 30.0, size=(far.sum(), 1))
+    tiles = H.dev_tiles(w)
+    rows = np.flatnonzero(far)[:40].astype(np.int64)
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), rows=rows, long_double=True)
+    src_cent = w.verts.mean(axis=1)
+    r = np.linalg.norm(w.center[rows][:, None, :] - src_cent[None, :, :], axis=2) / edge[None, :]
+    assert r.max() > 40
+    errs = {}
+    for mode in (0, 1):
+        B.mt_set_assembly_mode(ctx, mode)
+        N, ld, status = H.assemble(ctx, tiles, "f64")
+        assert status == 0
+        got = N[:, torch.from_numpy(rows).cuda(), :n].cpu().numpy()
+        errs[mode] = block_rel_err(got, N_ref)
+    assert errs[1].max() <= 1e-10, errs[1].max()
+    near = r < 7.9  # closed form in both modes (the two instantiations may contract FMAs differently)
+    assert errs[0][near].max() <= 1e-10 and errs[1][near].max() <= 1e-10
+    sel = r > 20
+    assert errs[0][sel].max() > 10 * errs[1][sel].max()
