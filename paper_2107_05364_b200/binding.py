@@ -26,7 +26,7 @@ COMPONENTS = ("xx", "xy", "xz", "yy", "yz", "zz")
 EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assemble_tensor",
            "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_energy",
            "mt_field_sweep", "mt_sparse_mask_words", "mt_threshold_value", "mt_sparse_count",
-           "mt_sparse_fill", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
+           "mt_sparse_fill", "mt_sparse_index", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
            "mt_demag_field_sym", "mt_set_assembly_mode", "mt_launch_count",
            "mt_set_demag_variant", "mt_profile_begin", "mt_profile_end")
 
@@ -61,7 +61,7 @@ class _Sym(C.Structure):
 
 class _Sparse(C.Structure):
     _fields_ = [("n", C.c_int64), ("n_rows", C.c_int64), ("dtype", C.c_int), ("nw", C.c_int64),
-                ("row_ptr", C.c_void_p), ("mask", C.c_void_p), ("vals", C.c_void_p)]
+                ("row_ptr", C.c_void_p), ("mask", C.c_void_p), ("vals", C.c_void_p), ("cols16", C.c_void_p)]
 
 
 class _Opts(C.Structure):
@@ -116,6 +116,7 @@ def load() -> C.CDLL:
                                         C.c_double, C.c_void_p, C.POINTER(C.c_int64)]
         lib.mt_sparse_fill.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64,
                                        C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.mt_sparse_index.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p]
         lib.mt_demag_field_sparse.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p, C.c_void_p, C.c_int,
                                               C.c_void_p]
         lib.mt_sym_tensor_elems.restype = C.c_int64
@@ -368,13 +369,18 @@ class SparseTensor:
     vals: torch.Tensor     # [nnz]
     nnz: int = 0
     tau: float = 0.0
+    cols16: object = None  # [nnz] uint16 index rows (mt_sparse_index) or None; the mask may be dropped then
 
     def _c(self) -> _Sparse:
         return _Sparse(self.n, self.n_rows, self.dtype, self.nw, _ptr(self.row_ptr, torch.int64),
-                       _ptr(self.mask, torch.int32), _ptr(self.vals, torch_dtype(self.dtype)))
+                       _ptr(self.mask, torch.int32) if self.mask is not None else None,
+                       _ptr(self.vals, torch_dtype(self.dtype)),
+                       _ptr(self.cols16, torch.uint16) if self.cols16 is not None else None)
 
     def nbytes(self) -> int:
-        return self.row_ptr.numel() * 8 + self.mask.numel() * 4 + self.vals.numel() * self.vals.element_size()
+        """Bytes one field evaluation streams: values + the index the kernel walks (16-bit columns if present)."""
+        idx = self.cols16.numel() * 2 if self.cols16 is not None else self.mask.numel() * 4
+        return self.row_ptr.numel() * 8 + idx + self.vals.numel() * self.vals.element_size()
 
 
 def mt_threshold_value(ctx: Context, N: torch.Tensor, dtype: int, n: int, n_rows: int, ld: int, fraction: float):
@@ -398,6 +404,18 @@ def mt_sparse_build(ctx: Context, N: torch.Tensor, dtype: int, n: int, n_rows: i
     ctx.check(ctx.lib.mt_sparse_fill(ctx.h, _ptr(N, torch_dtype(dtype)), dtype, n, n_rows, ld, float(tau),
                                      _ptr(row_ptr), _ptr(mask), _ptr(vals)))
     return SparseTensor(n, n_rows, dtype, nw, row_ptr, mask, vals, nnz=nnz.value, tau=float(tau))
+
+
+def mt_sparse_index(ctx: Context, S: SparseTensor, drop_mask: bool = False) -> SparseTensor:
+    """Adds the index rows (16-bit column of every packed value) to S; the field kernel then walks them."""
+    cols = torch.empty(max(1, S.nnz), dtype=torch.uint16, device=S.vals.device)
+    s = S._c()
+    ctx.check(ctx.lib.mt_sparse_index(ctx.h, C.byref(s), _ptr(cols, torch.uint16)))
+    S.cols16 = cols
+    if drop_mask:
+        ctx.stream.synchronize()  # the index kernel reads the mask
+        S.mask = None
+    return S
 
 
 def mt_demag_field_sparse(ctx: Context, S: SparseTensor, Ms: torch.Tensor, m: torch.Tensor, batch: int,

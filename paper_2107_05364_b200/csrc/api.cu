@@ -57,7 +57,9 @@ int check_sparse(mt_ctx* ctx, const mt_sparse_tensor* s) {
   if (s->dtype != MT_F32 && s->dtype != MT_F64) return mt_fail(ctx, MT_ERR_INVALID_ARG, "unknown dtype %d", s->dtype);
   if (s->n <= 0 || s->n_rows <= 0) return mt_fail(ctx, MT_ERR_INVALID_ARG, "n and n_rows must be positive");
   if (s->nw != mt_sparse_mask_words(s->n)) return mt_fail(ctx, MT_ERR_INVALID_ARG, "nw must be mt_sparse_mask_words(n)");
-  if (!s->row_ptr || !s->mask) return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and mask must be non-NULL");
+  if (!s->row_ptr || (!s->mask && !s->cols16))
+    return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and one of mask / cols16 must be non-NULL");
+  if (s->cols16 && s->n > 65536) return mt_fail(ctx, MT_ERR_INVALID_ARG, "cols16 given but n > 65536");
   return MT_OK;
 }
 
@@ -425,6 +427,16 @@ int mt_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_r
   if (!row_ptr || !mask) return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and mask must be non-NULL");
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
   return mt_launch_sparse_fill(ctx, N, dtype, n, n_rows, ld, tau, row_ptr, mt_sparse_mask_words(n), mask, vals);
+}
+
+int mt_sparse_index(mt_ctx* ctx, const mt_sparse_tensor* S, uint16_t* cols16) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_sparse(ctx, S);
+  if (rc) return rc;
+  if (S->n > 65536) return mt_fail(ctx, MT_ERR_INVALID_ARG, "index rows hold 16-bit columns: n must be <= 65536");
+  if (!cols16 || !S->mask) return mt_fail(ctx, MT_ERR_INVALID_ARG, "cols16 and S->mask must be non-NULL");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  return mt_launch_sparse_index(ctx, S, cols16);
 }
 
 int mt_demag_field_sparse(mt_ctx* ctx, const mt_sparse_tensor* S, const double* Ms, const double* m, int batch,

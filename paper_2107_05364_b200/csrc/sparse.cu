@@ -298,6 +298,145 @@ int launch_bitmap(mt_ctx* ctx, const SparseArgs& a, const EpiArgs& e) {
   return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
 }
 
+// ---- index rows: the second index of the thresholded tensor ----------------------------------------
+// cols[row_ptr[r] + k] = column of the k-th set bit of bitmap row r; one warp per (plane, row).
+__global__ void __launch_bounds__(256) sparse_index_kernel(const uint32_t* __restrict__ mask,
+                                                           const int64_t* __restrict__ row_ptr, int64_t n_rows,
+                                                           int64_t nw, uint16_t* __restrict__ cols) {
+  const int64_t r = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (r >= 6 * n_rows) return;
+  const uint32_t* mrow = mask + r * nw;
+  uint16_t* out = cols + row_ptr[r];
+  const uint32_t lt = (1u << lane) - 1u;
+  int64_t off = 0;
+  for (int64_t c0 = 0; c0 < nw; c0 += 32) {
+    const uint32_t mine = c0 + lane < nw ? __ldg(mrow + c0 + lane) : 0u;
+    uint32_t nz = __ballot_sync(0xffffffffu, mine != 0u);
+    while (nz) {
+      const int c = __ffs(nz) - 1;
+      nz &= nz - 1u;
+      const uint32_t word = __shfl_sync(0xffffffffu, mine, c);
+      if ((word >> lane) & 1u) out[off + __popc(word & lt)] = (uint16_t)((c0 + c) * 32 + lane);
+      off += __popc(word);
+    }
+  }
+}
+
+// Field kernel on index rows: one warp per target row walks the packed values of each of its six
+// plane rows in order (lane l takes entries l, l + 32, ...): one coalesced value load and one coalesced
+// 16-bit column load per 32 entries, M gathered at the columns (near-field runs are contiguous, so the
+// gathers fall in one or two 128-byte lines; M is L1/L2-resident), and only the products the plane
+// contributes: one for a diagonal plane, two for an off-diagonal one.  ~12 instructions per 32 kept
+// entries against ~150 per visited chunk of the bitmap decode.  fp32: a lane's run of kUnroll * kFlush
+// entries per plane is summed in fp32, then added to fp64 (Q19); fp64: DFMA throughout.
+// Fixed order (lane-strided walk, xor butterfly): bitwise reproducible.
+constexpr int kIdxUnroll = 8;
+constexpr int kIdxFlush = 8;
+
+template <int P> struct PlaneRC;  // plane -> (row component, column component) of the 3x3 block
+template <> struct PlaneRC<0> { static constexpr int r = 0, c = 0; };
+template <> struct PlaneRC<1> { static constexpr int r = 0, c = 1; };
+template <> struct PlaneRC<2> { static constexpr int r = 0, c = 2; };
+template <> struct PlaneRC<3> { static constexpr int r = 1, c = 1; };
+template <> struct PlaneRC<4> { static constexpr int r = 1, c = 2; };
+template <> struct PlaneRC<5> { static constexpr int r = 2, c = 2; };
+
+template <typename T, int B, int P>
+__device__ __forceinline__ void index_plane(const SparseArgs& a, const uint16_t* __restrict__ cols, int64_t row,
+                                            int lane, double (&acc)[B][3]) {
+  constexpr int R = PlaneRC<P>::r, Cc = PlaneRC<P>::c;
+  const int64_t r = (int64_t)P * a.n_rows + row;
+  const int64_t beg = __ldg(a.row_ptr + r), end = __ldg(a.row_ptr + r + 1);
+  const T* __restrict__ vals = (const T*)a.vals;
+  const T* __restrict__ M = (const T*)a.Mst;
+  for (int64_t k0 = beg + lane; k0 < end; k0 += 32 * kIdxUnroll * kIdxFlush) {
+    T runR[B], runC[B];
+#pragma unroll
+    for (int b = 0; b < B; ++b) runR[b] = runC[b] = T(0);
+    for (int f = 0; f < kIdxFlush; ++f) {
+      const int64_t k1 = k0 + (int64_t)f * 32 * kIdxUnroll;
+      if (k1 >= end) break;
+      T v[kIdxUnroll];
+      int col[kIdxUnroll];
+#pragma unroll
+      for (int u = 0; u < kIdxUnroll; ++u) {
+        const int64_t k = k1 + 32 * u;
+        const bool ok = k < end;
+        v[u] = ok ? __ldg(vals + k) : T(0);
+        col[u] = ok ? (int)__ldg(cols + k) : 0;
+      }
+#pragma unroll
+      for (int b = 0; b < B; ++b) {
+        const T* Mb = M + (int64_t)b * 3 * a.npad;
+#pragma unroll
+        for (int u = 0; u < kIdxUnroll; ++u) {
+          runR[b] = fma(v[u], __ldg(Mb + (int64_t)Cc * a.npad + col[u]), runR[b]);
+          if (R != Cc) runC[b] = fma(v[u], __ldg(Mb + (int64_t)R * a.npad + col[u]), runC[b]);
+        }
+      }
+    }
+#pragma unroll
+    for (int b = 0; b < B; ++b) {
+      acc[b][R] += (double)runR[b];
+      if (R != Cc) acc[b][Cc] += (double)runC[b];
+    }
+  }
+}
+
+template <typename T, int B>
+__global__ void __launch_bounds__(256) demag_index_kernel(SparseArgs a, const uint16_t* __restrict__ cols, EpiArgs e) {
+  const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
+  const int lane = threadIdx.x & 31;
+  if (row >= a.n_rows) return;
+  double acc[B][3];
+#pragma unroll
+  for (int b = 0; b < B; ++b) acc[b][0] = acc[b][1] = acc[b][2] = 0.0;
+  index_plane<T, B, 0>(a, cols, row, lane, acc);
+  index_plane<T, B, 1>(a, cols, row, lane, acc);
+  index_plane<T, B, 2>(a, cols, row, lane, acc);
+  index_plane<T, B, 3>(a, cols, row, lane, acc);
+  index_plane<T, B, 4>(a, cols, row, lane, acc);
+  index_plane<T, B, 5>(a, cols, row, lane, acc);
+#pragma unroll
+  for (int b = 0; b < B; ++b)
+#pragma unroll
+    for (int cc = 0; cc < 3; ++cc)
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) acc[b][cc] += __shfl_xor_sync(0xffffffffu, acc[b][cc], o);
+  double s[3] = {0.0, 0.0, 0.0};
+#pragma unroll
+  for (int b = 0; b < B; ++b)
+    if (lane == b) { s[0] = acc[b][0]; s[1] = acc[b][1]; s[2] = acc[b][2]; }
+  if (lane < B) {
+    const double hd[3] = {-s[0], -s[1], -s[2]};
+    row_epilogue(e, row, lane, hd);
+  }
+}
+
+template <typename T, int B>
+int launch_index_B(mt_ctx* ctx, const SparseArgs& a, const uint16_t* cols, const EpiArgs& e) {
+  demag_index_kernel<T, B><<<(unsigned)((a.n_rows + 7) / 8), 256, 0, ctx->stream>>>(a, cols, e);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+template <typename T>
+int launch_index(mt_ctx* ctx, const SparseArgs& a, const uint16_t* cols, const EpiArgs& e) {
+  switch (e.batch) {
+    case 1: return launch_index_B<T, 1>(ctx, a, cols, e);
+    case 2: return launch_index_B<T, 2>(ctx, a, cols, e);
+    case 3: return launch_index_B<T, 3>(ctx, a, cols, e);
+    case 4: return launch_index_B<T, 4>(ctx, a, cols, e);
+    case 5: return launch_index_B<T, 5>(ctx, a, cols, e);
+    case 6: return launch_index_B<T, 6>(ctx, a, cols, e);
+    case 7: return launch_index_B<T, 7>(ctx, a, cols, e);
+    case 8: return launch_index_B<T, 8>(ctx, a, cols, e);
+  }
+  return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
+}
+
 }  // namespace
 
 int mt_launch_select_hist(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
@@ -348,6 +487,14 @@ int mt_launch_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int6
   return MT_OK;
 }
 
+int mt_launch_sparse_index(mt_ctx* ctx, const mt_sparse_tensor* s, uint16_t* cols16) {
+  sparse_index_kernel<<<(unsigned)((6 * s->n_rows + 7) / 8), 256, 0, ctx->stream>>>(s->mask, s->row_ptr, s->n_rows,
+                                                                                  s->nw, cols16);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
 int mt_launch_demag_sparse(mt_ctx* ctx, const mt_sparse_tensor* s, const void* Mst, int64_t npad, const EpiArgs& e) {
   SparseArgs a;
   a.n = s->n;
@@ -360,7 +507,11 @@ int mt_launch_demag_sparse(mt_ctx* ctx, const mt_sparse_tensor* s, const void* M
   a.Mst = Mst;
   const bool prof = ctx->prof_on && ctx->prof_ev && ctx->prof_count < MT_PROF_CAP;
   if (prof) MT_CUDA_OK(ctx, cudaEventRecord(ctx->prof_ev[2 * ctx->prof_count], ctx->stream));
-  const int rc = s->dtype == MT_F32 ? launch_bitmap<float>(ctx, a, e) : launch_bitmap<double>(ctx, a, e);
+  int rc;
+  if (s->cols16)
+    rc = s->dtype == MT_F32 ? launch_index<float>(ctx, a, s->cols16, e) : launch_index<double>(ctx, a, s->cols16, e);
+  else
+    rc = s->dtype == MT_F32 ? launch_bitmap<float>(ctx, a, e) : launch_bitmap<double>(ctx, a, e);
   if (prof) {
     MT_CUDA_OK(ctx, cudaEventRecord(ctx->prof_ev[2 * ctx->prof_count + 1], ctx->stream));
     ctx->prof_count++;

@@ -84,6 +84,24 @@ def test_threshold_value_and_bitmap_rows_are_exact(ctx, oracle, grid, dtype):
         Hd2 = torch.empty_like(m)
         B.mt_demag_field_sparse(ctx, S, torch.from_numpy(w.Ms).cuda(), m, 3, Hd2)
         assert torch.equal(Hd, Hd2)  # fixed reduction order
+        # index rows: the 16-bit column of every packed value = the non-zero columns of the truncated
+        # tensor in (plane, row, column) order; the field kernel that walks them, with the mask dropped
+        B.mt_sparse_index(ctx, S, drop_mask=True)
+        assert S.mask is None
+        if S.nnz:
+            cols_ref = np.nonzero(trunc.reshape(6 * n, n))[1].astype(np.uint16)
+            assert np.array_equal(S.cols16.cpu().numpy(), cols_ref)
+        Hi = torch.empty_like(m)
+        B.mt_demag_field_sparse(ctx, S, torch.from_numpy(w.Ms).cuda(), m, 3, Hi)
+        torch.cuda.synchronize()
+        if S.nnz == 0:
+            assert not Hi.cpu().numpy().any()
+        else:
+            for b in range(3):
+                assert H.rel_l2(Hi[b].cpu().numpy(), ref[b]) <= TOL_HD[dtype]
+        Hi2 = torch.empty_like(m)
+        B.mt_demag_field_sparse(ctx, S, torch.from_numpy(w.Ms).cuda(), m, 3, Hi2)
+        assert torch.equal(Hi, Hi2)
 
 
 @pytest.mark.parametrize("batch", [1, 5, 8])
@@ -104,9 +122,15 @@ def test_sparse_field_batches_match_dense_path_on_truncated_tensor(ctx, oracle, 
     B.mt_demag_field(ctx, dev_t, B.MT_F32, n, n, ld, Ms, m, batch, Hd)
     torch.cuda.synchronize()
     ref = oracle.demag_field(trunc.astype(np.float64), w.Ms, w.m)
+    B.mt_sparse_index(ctx, S)
+    Hi = torch.empty_like(m)
+    B.mt_demag_field_sparse(ctx, S, Ms, m, batch, Hi)
+    torch.cuda.synchronize()
     for b in range(batch):
         assert H.rel_l2(Hs[b].cpu().numpy(), ref[b]) <= 1e-5
         assert H.rel_l2(Hs[b].cpu().numpy(), Hd[b].cpu().numpy()) <= 2e-6
+        assert H.rel_l2(Hi[b].cpu().numpy(), ref[b]) <= 1e-5
+        assert H.rel_l2(Hi[b].cpu().numpy(), Hd[b].cpu().numpy()) <= 2e-6
 
 
 def test_thresholded_dynamics_follow_the_oracle_on_the_truncated_tensor(ctx, oracle):
@@ -140,6 +164,19 @@ def test_thresholded_dynamics_follow_the_oracle_on_the_truncated_tensor(ctx, ora
     B.mt_energy(ctx, prob, m, 1, E)
     ref = oracle.energy_terms(H.oracle_problem(oracle, w, trunc), m[0].cpu().numpy(), vol=w.vol)
     assert np.max(np.abs(E[0, :4].cpu().numpy() - ref)) <= 1e-5 * np.abs(ref).sum()
+    # the same trajectory and energies with the field kernel on the index rows
+    B.mt_sparse_index(ctx, S, drop_mask=True)
+    prob.N_sparse = S
+    mi = torch.from_numpy(w.m[:1].copy()).cuda()
+    samples_i = torch.zeros((16, 4), dtype=torch.float64, device="cuda")
+    B.mt_integrate(ctx, prob, mi, 1, 0.0, method=B.MT_RK4, dt=dt, t_end=steps * dt, sample_every=20,
+                   samples=samples_i)
+    assert np.max(np.abs(samples_i[:10].cpu().numpy()[:, 1:] - s_ref[:, 1:])) < 1e-4
+    assert np.max(np.abs(mi[0].cpu().numpy() - m_ref)) < 1e-3
+    Ei = torch.empty((1, 5), dtype=torch.float64, device="cuda")
+    B.mt_energy(ctx, prob, mi, 1, Ei)
+    ref_i = oracle.energy_terms(H.oracle_problem(oracle, w, trunc), mi[0].cpu().numpy(), vol=w.vol)
+    assert np.max(np.abs(Ei[0, :4].cpu().numpy() - ref_i)) <= 1e-5 * np.abs(ref_i).sum()
 
 
 def test_sparse_argument_checks(ctx):
@@ -155,6 +192,11 @@ def test_sparse_argument_checks(ctx):
     S.nw += 1
     with pytest.raises(B.MtError):
         B.mt_demag_field_sparse(ctx, S, Ms, m, 1, torch.empty_like(m))
+    S.nw -= 1
+    S.n = 65537   # 16-bit columns cannot address it
+    S.nw = 2052
+    with pytest.raises(B.MtError):
+        B.mt_sparse_index(ctx, S)
 
 
 def test_sparse_row_band(ctx, oracle):
@@ -176,5 +218,11 @@ def test_sparse_row_band(ctx, oracle):
     B.mt_demag_field_sparse(ctx, S, torch.from_numpy(w.Ms).cuda(), m, 2, Hd)
     torch.cuda.synchronize()
     ref = oracle.demag_field(trunc.astype(np.float64), w.Ms, w.m)
+    B.mt_sparse_index(ctx, S)
+    assert np.array_equal(S.cols16.cpu().numpy(), np.nonzero(trunc.reshape(6 * len(rows), n))[1].astype(np.uint16))
+    Hi = torch.empty_like(Hd)
+    B.mt_demag_field_sparse(ctx, S, torch.from_numpy(w.Ms).cuda(), m, 2, Hi)
+    torch.cuda.synchronize()
     for b in range(2):
         assert H.rel_l2(Hd[b].cpu().numpy(), ref[b]) <= 1e-5
+        assert H.rel_l2(Hi[b].cpu().numpy(), ref[b]) <= 1e-5
