@@ -342,30 +342,59 @@ template <> struct PlaneRC<3> { static constexpr int r = 1, c = 1; };
 template <> struct PlaneRC<4> { static constexpr int r = 1, c = 2; };
 template <> struct PlaneRC<5> { static constexpr int r = 2, c = 2; };
 
+// The value and column streams are read once: they bypass L1 so that the gathered M stays there.
+__device__ __forceinline__ float ld_stream(const float* p) {
+  float v;
+  asm volatile("ld.global.nc.L1::no_allocate.f32 %0, [%1];" : "=f"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ double ld_stream(const double* p) {
+  double v;
+  asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
+  return v;
+}
+__device__ __forceinline__ int ld_stream(const uint16_t* p) {
+  unsigned short v;
+  asm volatile("ld.global.nc.L1::no_allocate.u16 %0, [%1];" : "=h"(v) : "l"(p));
+  return (int)v;
+}
+
+template <typename T>
+__device__ __forceinline__ void index_load(const T* __restrict__ vals, const uint16_t* __restrict__ cols, int64_t k,
+                                           int64_t end, T (&v)[kIdxUnroll], int (&col)[kIdxUnroll]) {
+#pragma unroll
+  for (int u = 0; u < kIdxUnroll; ++u) {
+    const int64_t ku = k + 32 * u;
+    const bool ok = ku < end;
+    v[u] = ok ? ld_stream(vals + ku) : T(0);
+    col[u] = ok ? ld_stream(cols + ku) : 0;
+  }
+}
+
+// beg/end: the plane row's range in vals/cols (read by the caller for all six planes up front).  The
+// next block's values and columns are requested before the current block's gathers are issued, so a
+// warp keeps two blocks of kIdxUnroll * 32 entries (2 x 1.5 KB) in flight towards HBM.
 template <typename T, int B, int P>
-__device__ __forceinline__ void index_plane(const SparseArgs& a, const uint16_t* __restrict__ cols, int64_t row,
-                                            int lane, double (&acc)[B][3]) {
+__device__ __forceinline__ void index_plane(const SparseArgs& a, const uint16_t* __restrict__ cols, int64_t beg,
+                                            int64_t end, int lane, double (&acc)[B][3]) {
   constexpr int R = PlaneRC<P>::r, Cc = PlaneRC<P>::c;
-  const int64_t r = (int64_t)P * a.n_rows + row;
-  const int64_t beg = __ldg(a.row_ptr + r), end = __ldg(a.row_ptr + r + 1);
   const T* __restrict__ vals = (const T*)a.vals;
   const T* __restrict__ M = (const T*)a.Mst;
-  for (int64_t k0 = beg + lane; k0 < end; k0 += 32 * kIdxUnroll * kIdxFlush) {
+  T vn[kIdxUnroll];
+  int cn[kIdxUnroll];
+  int64_t kb = beg;  // warp-uniform block start
+  index_load<T>(vals, cols, kb + lane, end, vn, cn);
+  while (kb < end) {
     T runR[B], runC[B];
 #pragma unroll
     for (int b = 0; b < B; ++b) runR[b] = runC[b] = T(0);
-    for (int f = 0; f < kIdxFlush; ++f) {
-      const int64_t k1 = k0 + (int64_t)f * 32 * kIdxUnroll;
-      if (k1 >= end) break;
+    for (int f = 0; f < kIdxFlush && kb < end; ++f) {
       T v[kIdxUnroll];
       int col[kIdxUnroll];
 #pragma unroll
-      for (int u = 0; u < kIdxUnroll; ++u) {
-        const int64_t k = k1 + 32 * u;
-        const bool ok = k < end;
-        v[u] = ok ? __ldg(vals + k) : T(0);
-        col[u] = ok ? (int)__ldg(cols + k) : 0;
-      }
+      for (int u = 0; u < kIdxUnroll; ++u) { v[u] = vn[u]; col[u] = cn[u]; }
+      kb += 32 * kIdxUnroll;
+      index_load<T>(vals, cols, kb + lane, end, vn, cn);
 #pragma unroll
       for (int b = 0; b < B; ++b) {
         const T* Mb = M + (int64_t)b * 3 * a.npad;
@@ -385,19 +414,31 @@ __device__ __forceinline__ void index_plane(const SparseArgs& a, const uint16_t*
 }
 
 template <typename T, int B>
-__global__ void __launch_bounds__(256) demag_index_kernel(SparseArgs a, const uint16_t* __restrict__ cols, EpiArgs e) {
+__global__ void __launch_bounds__(256, (B <= 2 ? 4 : 2)) demag_index_kernel(SparseArgs a, const uint16_t* __restrict__ cols, EpiArgs e) {
   const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
   if (row >= a.n_rows) return;
   double acc[B][3];
 #pragma unroll
   for (int b = 0; b < B; ++b) acc[b][0] = acc[b][1] = acc[b][2] = 0.0;
-  index_plane<T, B, 0>(a, cols, row, lane, acc);
-  index_plane<T, B, 1>(a, cols, row, lane, acc);
-  index_plane<T, B, 2>(a, cols, row, lane, acc);
-  index_plane<T, B, 3>(a, cols, row, lane, acc);
-  index_plane<T, B, 4>(a, cols, row, lane, acc);
-  index_plane<T, B, 5>(a, cols, row, lane, acc);
+  // the range of plane p + 1 is requested before plane p is walked
+  const int64_t* rp = a.row_ptr + row;
+  int64_t beg = __ldg(rp), end = __ldg(rp + 1), nbeg = 0, nend = 0;
+#define MT_INDEX_PLANE(P)                                      \
+  if (P < 5) {                                                 \
+    nbeg = __ldg(rp + (int64_t)(P + 1) * a.n_rows);            \
+    nend = __ldg(rp + (int64_t)(P + 1) * a.n_rows + 1);        \
+  }                                                            \
+  index_plane<T, B, P>(a, cols, beg, end, lane, acc);          \
+  beg = nbeg;                                                  \
+  end = nend;
+  MT_INDEX_PLANE(0)
+  MT_INDEX_PLANE(1)
+  MT_INDEX_PLANE(2)
+  MT_INDEX_PLANE(3)
+  MT_INDEX_PLANE(4)
+  MT_INDEX_PLANE(5)
+#undef MT_INDEX_PLANE
 #pragma unroll
   for (int b = 0; b < B; ++b)
 #pragma unroll
