@@ -176,7 +176,7 @@ int mt_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_r
 int mt_sparse_index(mt_ctx* ctx, const mt_sparse_tensor* S, uint16_t* cols16);
 
 /* mt_demag_field on the thresholded tensor: Hd[b][a][i] = - sum over kept entries; same arithmetic
- * rules (fp32 runs of at most 96 terms, then fp64), fixed reduction order.                          */
+ * rules (fp32 runs of at most 96 terms per lane, 64 on index rows, then fp64), fixed reduction order. */
 int mt_demag_field_sparse(mt_ctx* ctx, const mt_sparse_tensor* S, const double* Ms, const double* m,
                           int batch, double* Hd);
 
