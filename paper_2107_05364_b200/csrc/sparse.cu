@@ -38,6 +38,12 @@ template <> struct KeyOf<double> {
   }
 };
 
+template <typename T> struct Vec16;  // 16 bytes of the row: rows are 16-byte aligned (include/mt.h)
+template <> struct Vec16<float> { typedef float4 type; static constexpr int n = 4; };
+template <> struct Vec16<double> { typedef double2 type; static constexpr int n = 2; };
+__device__ __forceinline__ void unpack16(const float4& q, float (&x)[4]) { x[0] = q.x; x[1] = q.y; x[2] = q.z; x[3] = q.w; }
+__device__ __forceinline__ void unpack16(const double2& q, double (&x)[2]) { x[0] = q.x; x[1] = q.y; }
+
 // hist[d] += multiplicity of every non-zero element whose key has the given prefix above `shift+width`
 // and digit d at `shift`; planes xy, xz, yz (1, 2, 4) count twice (Q20).
 template <typename T>
@@ -46,28 +52,75 @@ __global__ void __launch_bounds__(512) select_hist_kernel(const T* __restrict__ 
                                                           int prefix_shift, int shift, int width,
                                                           unsigned long long* __restrict__ hist) {
   typedef typename KeyOf<T>::type K;
+  typedef typename Vec16<T>::type V;
+  constexpr int kV = Vec16<T>::n;
   // 32-bit shared counters (a block sees far fewer than 2^31 elements: the launcher bounds the rows
-  // per block), flushed into the 64-bit global histogram.  Neighbouring columns hold values of similar
-  // magnitude, i.e. the same bin: lanes are aggregated with match.any so that a warp issues one shared
-  // atomic per distinct bin instead of up to 32 serialised ones.
+  // per block), flushed into the 64-bit global histogram.  A lane reads 16 bytes (kV neighbouring
+  // columns), two such loads in flight.  Neighbouring columns hold values of similar magnitude, i.e.
+  // the same bin: per vector component a warp aggregates RUNS of equal bins over its lanes (one shuffle
+  // + one ballot) and issues one shared atomic per run instead of up to 32 serialised ones.  In the
+  // passes below the first almost no element carries the prefix: a warp whose elements are all
+  // uncounted skips the aggregation (one vote).
   __shared__ unsigned int sh[kBins];
   for (int k = threadIdx.x; k < kBins; k += blockDim.x) sh[k] = 0u;
   __syncthreads();
   const int64_t rows_total = 6 * n_rows;
   const K dmask = (K)((1u << width) - 1u);
   const int lane = threadIdx.x & 31;
-  const int64_t n_up = (n + 31) / 32 * 32;  // whole warps stay converged for the match
+  const uint32_t above = ~((2u << lane) - 1u);  // lanes above this one
+  // (key & pmask) == pval  <=>  the bits above prefix_shift equal the prefix (first pass: no bits)
+  const bool has_prefix = prefix_shift < KeyOf<T>::bits;
+  const K pmask = has_prefix ? ~(((K)1 << prefix_shift) - (K)1) : (K)0;
+  const K pval = has_prefix ? (K)(prefix << prefix_shift) : (K)0;
+  const int step = (int)blockDim.x * kV;
+  const int n_up = (int)((n + 32 * kV - 1) / (32 * kV)) * (32 * kV);  // whole warps stay converged
   for (int64_t r = blockIdx.x; r < rows_total; r += gridDim.x) {
     const int plane = (int)(r / n_rows);
     const unsigned int w = (plane == 1 || plane == 2 || plane == 4) ? 2u : 1u;
     const T* row = N + r * ld;
-    for (int64_t j = threadIdx.x; j < n_up; j += blockDim.x) {
-      const K key = j < n ? KeyOf<T>::key(row[j]) : (K)0;
-      bool counted = key != 0;
-      if (counted && prefix_shift < KeyOf<T>::bits && (key >> prefix_shift) != prefix) counted = false;
-      const unsigned bin = counted ? (unsigned)((key >> shift) & dmask) : (unsigned)kBins;  // kBins = "none"
-      const unsigned peers = __match_any_sync(0xffffffffu, bin);
-      if (counted && lane == __ffs(peers) - 1) atomicAdd(&sh[bin], w * (unsigned)__popc(peers));
+    for (int j0 = (int)threadIdx.x * kV; j0 < n_up; j0 += 2 * step) {
+      T x[2][kV];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int j = j0 + u * step;
+        if (j < ld) {
+          unpack16(__ldg(reinterpret_cast<const V*>(row + j)), x[u]);
+          if (j + kV > n) {  // the row's last vector: columns >= n are padding
+#pragma unroll
+            for (int c = 0; c < kV; ++c)
+              if (j + c >= n) x[u][c] = T(0);
+          }
+        } else {
+#pragma unroll
+          for (int c = 0; c < kV; ++c) x[u][c] = T(0);
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int j = j0 + u * step;
+        if (j - lane * kV >= n_up) break;  // warp-uniform
+        K key[kV];
+        bool counted[kV], any = false;
+#pragma unroll
+        for (int c = 0; c < kV; ++c) {
+          key[c] = KeyOf<T>::key(x[u][c]);
+          counted[c] = key[c] != 0 && (key[c] & pmask) == pval;
+          any |= counted[c];
+        }
+        if (!__any_sync(0xffffffffu, any)) continue;
+#pragma unroll
+        for (int c = 0; c < kV; ++c) {
+          const unsigned bin = counted[c] ? (unsigned)((key[c] >> shift) & dmask) : (unsigned)kBins;  // "none"
+          const unsigned prev = __shfl_up_sync(0xffffffffu, bin, 1);
+          const bool head = lane == 0 || bin != prev;
+          const uint32_t heads = __ballot_sync(0xffffffffu, head);
+          if (head && counted[c]) {
+            const uint32_t next = heads & above;
+            const int len = (next ? __ffs(next) - 1 : 32) - lane;
+            atomicAdd(&sh[bin], w * (unsigned)len);
+          }
+        }
+      }
     }
   }
   __syncthreads();
@@ -85,8 +138,15 @@ __global__ void __launch_bounds__(256) sparse_count_kernel(const T* __restrict__
   const int lane = threadIdx.x & 31;
   if (r >= 6 * n_rows) return;
   const T* row = N + r * ld;
+  typedef typename Vec16<T>::type V;
+  constexpr int kV = Vec16<T>::n;
   int c = 0;
-  for (int64_t j = lane; j < n; j += 32) c += kept(row[j], tau) ? 1 : 0;
+  for (int64_t j = (int64_t)lane * kV; j < n; j += 32 * kV) {  // 16-byte loads (rows are 16-byte aligned)
+    T x[kV];
+    unpack16(__ldg(reinterpret_cast<const V*>(row + j)), x);
+#pragma unroll
+    for (int q = 0; q < kV; ++q) c += (j + q < n && kept(x[q], tau)) ? 1 : 0;
+  }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) c += __shfl_xor_sync(0xffffffffu, c, off);
   if (lane == 0) counts[r] = c;
@@ -131,14 +191,21 @@ __global__ void __launch_bounds__(256) sparse_fill_kernel(const T* __restrict__ 
   uint32_t* mrow = mask + r * nw;
   T* out = vals + row_ptr[r];
   int64_t off = 0;
-  for (int64_t c = 0; c < nw; ++c) {
-    const int64_t j = c * 32 + lane;
-    const T v = j < n ? row[j] : T(0);
-    const bool k = kept(v, tau);
-    const uint32_t word = __ballot_sync(0xffffffffu, k);
-    if (k) out[off + __popc(word & ((1u << lane) - 1u))] = v;
-    if (lane == 0) mrow[c] = word;
-    off += __popc(word);
+  for (int64_t c0 = 0; c0 < nw; c0 += 4) {  // nw is a multiple of 4; four chunks loaded before any is packed
+    T v[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const int64_t j = (c0 + u) * 32 + lane;
+      v[u] = j < n ? __ldg(row + j) : T(0);
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const bool k = kept(v[u], tau);
+      const uint32_t word = __ballot_sync(0xffffffffu, k);
+      if (k) out[off + __popc(word & ((1u << lane) - 1u))] = v[u];
+      if (lane == 0) mrow[c0 + u] = word;
+      off += __popc(word);
+    }
   }
 }
 
