@@ -289,6 +289,82 @@ def test_config5_full_size_symmetric_half(ctx, oracle):
     assert torch.equal(Hd, Hd2)
 
 
+def test_config5_full_size_thresholded_index_rows(ctx, oracle):
+    """F1 at BASELINE's full size, in the configuration bench.py times (X = 0.9, index rows).
+    (1) the device's threshold value has the rank PAPER.md:239 defines, counted on the device tensor
+    with torch reductions (not this library's kernels); (2) on sampled target rows the bitmap, the
+    16-bit columns and the packed values equal the oracle's truncation of its own rows, with the cut
+    placed in a gap of the oracle's magnitudes next to the device's value (so that the last-bit
+    difference between the two assemblies cannot move an entry across it); (3) the field from the
+    index rows on those rows against the oracle's field of its truncated rows; the bitmap-row kernel
+    and the index-row kernel agree on every row."""
+    import math
+    from oracle import threshold as OT
+    w = W.config5(batch=2)
+    n = w.n
+    tiles = H.dev_tiles(w)
+    N, ld, status = H.assemble(ctx, tiles, "f32")
+    X = 0.9
+    tau_dev, cnt = B.mt_threshold_value(ctx, N, B.MT_F32, n, n, ld, X)
+    mult = (1, 2, 2, 1, 2, 1)
+    nonzero = below = ties = 0
+    for p in range(6):
+        for r0 in range(0, n, 8192):
+            a = N[p, r0:r0 + 8192, :n].abs()
+            nonzero += mult[p] * int(torch.count_nonzero(a))
+            below += mult[p] * int(((a < tau_dev) & (a != 0)).sum())
+            ties += mult[p] * int((a == tau_dev).sum())
+            del a
+    assert cnt == nonzero
+    k = math.floor(X * nonzero)
+    assert below <= k < below + ties, (below, k, ties)
+    # (2) sampled rows, cut in a gap of the oracle's magnitudes
+    rows = W.sample_rows(5, n, 64, extra=grid_corner_rows(w.grid) + [65535, 32768, 32767])
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), rows=rows, long_double=True)
+    host = N_ref.astype(np.float32)
+    mags = np.abs(host[(np.abs(host) > 0.5 * tau_dev) & (np.abs(host) < 2.0 * tau_dev)]).astype(np.float64)
+    mags = np.unique(mags)
+    gaps = np.nonzero(mags[1:] > mags[:-1] * 1.001)[0]
+    g = gaps[np.argmin(np.abs(np.log(mags[gaps] / tau_dev)))]
+    tau = float(np.float32(math.sqrt(mags[g] * mags[g + 1])))
+    assert mags[g] < tau < mags[g + 1] and 0.5 * tau_dev < tau < 2.0 * tau_dev
+    S = B.mt_sparse_build(ctx, N, B.MT_F32, n, n, ld, tau)
+    B.mt_sparse_index(ctx, S)
+    torch.cuda.synchronize()
+    assert 0.05 < S.nnz / (6.0 * n * n) < 0.2
+    trunc = OT.truncate(host, tau)
+    ridx = torch.from_numpy(rows).cuda()
+    for p in range(6):
+        ptr = S.row_ptr[p * n: (p + 1) * n + 1]
+        beg, end = ptr[:-1][ridx].cpu().numpy(), ptr[1:][ridx].cpu().numpy()
+        mask = S.mask[p].index_select(0, ridx).cpu().numpy().view(np.uint32)
+        bits = ((mask[..., None] >> np.arange(32, dtype=np.uint32)) & 1).astype(bool).reshape(len(rows), -1)
+        assert np.array_equal(bits[:, :n], trunc[p] != 0) and not bits[:, n:].any()
+        for q in range(len(rows)):
+            cols_ref = np.nonzero(trunc[p, q])[0]
+            assert end[q] - beg[q] == len(cols_ref)
+            assert np.array_equal(S.cols16[beg[q]:end[q]].cpu().numpy(), cols_ref.astype(np.uint16))
+            vals = S.vals[beg[q]:end[q]].cpu().numpy()
+            assert (H.f32_ulp_distance(vals, N_ref[p, q, cols_ref]) <= 1).all()
+    # (3) fields
+    m = torch.from_numpy(w.m).cuda()
+    Hb, Hi, Hi2 = torch.empty_like(m), torch.empty_like(m), torch.empty_like(m)
+    cols = S.cols16
+    S.cols16 = None
+    B.mt_demag_field_sparse(ctx, S, tiles.Ms, m, 2, Hb)      # bitmap-row kernel
+    S.cols16 = cols
+    B.mt_demag_field_sparse(ctx, S, tiles.Ms, m, 2, Hi)      # index-row kernel
+    B.mt_demag_field_sparse(ctx, S, tiles.Ms, m, 2, Hi2)
+    torch.cuda.synchronize()
+    assert torch.equal(Hi, Hi2)
+    ref = oracle.demag_field(trunc.astype(np.float64), w.Ms, w.m)
+    got_i, got_b = Hi.cpu().numpy(), Hb.cpu().numpy()
+    for b in range(2):
+        assert H.rel_l2(got_i[b][:, rows], ref[b]) <= TOL_HD["f32"]
+        assert H.rel_l2(got_b[b][:, rows], ref[b]) <= TOL_HD["f32"]
+        assert H.rel_l2(got_i[b], got_b[b]) <= 2e-6
+
+
 def test_config2_full_protocol_full_size_invariants_and_half_storage(ctx):
     """The whole config-2 protocol at full size (160x40x1, 20,000 relax + 10,000 dynamics RK4 steps,
     the work bench-class runs do) on the CUDA path: properties that hold at any size — |m| = 1, energy
