@@ -161,6 +161,41 @@ int64_t mt_sparse_mask_words(int64_t n);
 int mt_threshold_value(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
                        double fraction, double* tau_host, int64_t* count_host);
 
+/* The same selection fed BAND BY BAND, for a tensor that is never resident as a whole (the memory
+ * saving PAPER.md:237 is after: only one row band of the dense tensor and the compressed result are
+ * ever held).  One radix digit (11 bits) is fixed per pass; a pass = mt_select_accumulate on every
+ * row band of the tensor (any order, any band height: each band is assembled again per pass with
+ * mt_assemble_tensor), then one mt_select_advance.  Repeat until st->done; st->tau, st->count then
+ * equal what mt_threshold_value returns for the whole tensor (integer histograms: exact).
+ * hist: DEVICE array of 2048 unsigned 64-bit counters owned by the caller.  mt_select_begin and
+ * mt_select_accumulate are asynchronous; mt_select_advance synchronises the stream.                */
+typedef struct {
+  int dtype;
+  double fraction;
+  int hi;                          /* key bits [hi, 32|64) are fixed to prefix                     */
+  unsigned long long prefix, k, count;
+  int done;
+  double tau;                      /* valid once done (+inf: everything removed)                   */
+} mt_select_state;
+int mt_select_begin(mt_ctx* ctx, mt_select_state* st, int dtype, double fraction, unsigned long long* hist);
+int mt_select_accumulate(mt_ctx* ctx, const mt_select_state* st, const void* N, int64_t n, int64_t n_rows,
+                         int64_t ld, unsigned long long* hist);
+int mt_select_advance(mt_ctx* ctx, mt_select_state* st, unsigned long long* hist);
+
+/* Compression band by band into ONE n_total-row thresholded tensor: N holds rows [row0, row0+n_rows)
+ * of the dense tensor ([6][n_rows][ld]).  mt_sparse_count_band writes the band's kept-entry counts
+ * into counts[c*n_total + row0 + i] (DEVICE, [6*n_total + 1]; asynchronous); after every band,
+ * mt_sparse_scan turns the counts into row_ptr in place and returns the number of kept entries
+ * (synchronises); mt_sparse_fill_band writes the band's bitmap rows and packed values at their
+ * places in the whole tensor's mask / vals (asynchronous).  mt_sparse_count / mt_sparse_fill are the
+ * single-band case (row0 = 0, n_total = n_rows).                                                   */
+int mt_sparse_count_band(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                         double tau, int64_t row0, int64_t n_total, int64_t* counts);
+int mt_sparse_scan(mt_ctx* ctx, int64_t* row_ptr, int64_t n_total, int64_t* nnz_host);
+int mt_sparse_fill_band(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
+                        double tau, int64_t row0, int64_t n_total, const int64_t* row_ptr,
+                        uint32_t* mask, void* vals);
+
 /* Compression, two calls: mt_sparse_count fills row_ptr (DEVICE, [6*n_rows+1]) for threshold tau and
  * returns the number of kept entries in *nnz_host (synchronises); the caller allocates mask
  * ([6*n_rows*nw] uint32) and vals ([nnz] of dtype), then mt_sparse_fill writes them (asynchronous).

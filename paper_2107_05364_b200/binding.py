@@ -26,7 +26,8 @@ COMPONENTS = ("xx", "xy", "xz", "yy", "yz", "zz")
 EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assemble_tensor",
            "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_energy",
            "mt_field_sweep", "mt_sparse_mask_words", "mt_threshold_value", "mt_sparse_count",
-           "mt_sparse_fill", "mt_sparse_index", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
+           "mt_sparse_fill", "mt_sparse_index", "mt_select_begin", "mt_select_accumulate", "mt_select_advance",
+           "mt_sparse_count_band", "mt_sparse_scan", "mt_sparse_fill_band", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
            "mt_demag_field_sym", "mt_set_assembly_mode", "mt_launch_count",
            "mt_set_demag_variant", "mt_profile_begin", "mt_profile_end")
 
@@ -62,6 +63,11 @@ class _Sym(C.Structure):
 class _Sparse(C.Structure):
     _fields_ = [("n", C.c_int64), ("n_rows", C.c_int64), ("dtype", C.c_int), ("nw", C.c_int64),
                 ("row_ptr", C.c_void_p), ("mask", C.c_void_p), ("vals", C.c_void_p), ("cols16", C.c_void_p)]
+
+
+class _SelectState(C.Structure):
+    _fields_ = [("dtype", C.c_int), ("fraction", C.c_double), ("hi", C.c_int), ("prefix", C.c_ulonglong),
+                ("k", C.c_ulonglong), ("count", C.c_ulonglong), ("done", C.c_int), ("tau", C.c_double)]
 
 
 class _Opts(C.Structure):
@@ -116,6 +122,15 @@ def load() -> C.CDLL:
                                         C.c_double, C.c_void_p, C.POINTER(C.c_int64)]
         lib.mt_sparse_fill.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64,
                                        C.c_double, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.mt_select_begin.argtypes = [C.c_void_p, C.POINTER(_SelectState), C.c_int, C.c_double, C.c_void_p]
+        lib.mt_select_accumulate.argtypes = [C.c_void_p, C.POINTER(_SelectState), C.c_void_p, C.c_int64, C.c_int64,
+                                             C.c_int64, C.c_void_p]
+        lib.mt_select_advance.argtypes = [C.c_void_p, C.POINTER(_SelectState), C.c_void_p]
+        lib.mt_sparse_count_band.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64,
+                                             C.c_double, C.c_int64, C.c_int64, C.c_void_p]
+        lib.mt_sparse_scan.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
+        lib.mt_sparse_fill_band.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64,
+                                            C.c_double, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
         lib.mt_sparse_index.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p]
         lib.mt_demag_field_sparse.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p, C.c_void_p, C.c_int,
                                               C.c_void_p]
@@ -404,6 +419,54 @@ def mt_sparse_build(ctx: Context, N: torch.Tensor, dtype: int, n: int, n_rows: i
     ctx.check(ctx.lib.mt_sparse_fill(ctx.h, _ptr(N, torch_dtype(dtype)), dtype, n, n_rows, ld, float(tau),
                                      _ptr(row_ptr), _ptr(mask), _ptr(vals)))
     return SparseTensor(n, n_rows, dtype, nw, row_ptr, mask, vals, nnz=nnz.value, tau=float(tau))
+
+
+def mt_sparse_build_streamed(ctx: Context, tiles: Tiles, dtype: int, fraction: float, band_rows: int,
+                             status_flag: torch.Tensor | None = None, tau: float | None = None) -> SparseTensor:
+    """Thresholded tensor of `tiles` without ever holding the dense tensor: every pass (one per radix
+    digit of the selection, one for the counts, one for the fill) assembles the tensor again band by
+    band into one [6, band_rows, ld] buffer.  Sequence of C-ABI calls only: mt_assemble_tensor,
+    mt_select_*, mt_sparse_count_band / mt_sparse_scan / mt_sparse_fill_band.  `tau` given: the
+    selection passes are skipped."""
+    n = tiles.n
+    dev = tiles.type.device
+    tdt = torch_dtype(dtype)
+    vec = 4 if dtype == MT_F32 else 2
+    ld = (n + vec - 1) // vec * vec
+    band = torch.empty(6 * band_rows * ld, dtype=tdt, device=dev)
+    bands = [(r0, min(n, r0 + band_rows)) for r0 in range(0, n, band_rows)]
+
+    def assemble(r0, r1):
+        t = tiles._c()
+        ctx.check(ctx.lib.mt_assemble_tensor(ctx.h, C.byref(t), dtype, r0, r1, _ptr(band, tdt), ld,
+                                             _ptr(status_flag, torch.int32)))
+
+    if tau is None:
+        hist = torch.empty(2048, dtype=torch.int64, device=dev)
+        st = _SelectState()
+        ctx.check(ctx.lib.mt_select_begin(ctx.h, C.byref(st), dtype, float(fraction), _ptr(hist)))
+        while not st.done:
+            for r0, r1 in bands:
+                assemble(r0, r1)
+                ctx.check(ctx.lib.mt_select_accumulate(ctx.h, C.byref(st), _ptr(band, tdt), n, r1 - r0, ld, _ptr(hist)))
+            ctx.check(ctx.lib.mt_select_advance(ctx.h, C.byref(st), _ptr(hist)))
+        tau = st.tau
+    row_ptr = torch.empty(6 * n + 1, dtype=torch.int64, device=dev)
+    for r0, r1 in bands:
+        assemble(r0, r1)
+        ctx.check(ctx.lib.mt_sparse_count_band(ctx.h, _ptr(band, tdt), dtype, n, r1 - r0, ld, float(tau), r0, n,
+                                               _ptr(row_ptr)))
+    nnz = C.c_int64()
+    ctx.check(ctx.lib.mt_sparse_scan(ctx.h, _ptr(row_ptr), n, C.byref(nnz)))
+    nw = int(ctx.lib.mt_sparse_mask_words(n))
+    mask = torch.empty((6, n, nw), dtype=torch.int32, device=dev)
+    vals = torch.empty(max(1, nnz.value), dtype=tdt, device=dev)
+    for r0, r1 in bands:
+        assemble(r0, r1)
+        ctx.check(ctx.lib.mt_sparse_fill_band(ctx.h, _ptr(band, tdt), dtype, n, r1 - r0, ld, float(tau), r0, n,
+                                              _ptr(row_ptr), _ptr(mask), _ptr(vals)))
+    ctx.stream.synchronize()  # `band` is freed on return
+    return SparseTensor(n, n, dtype, nw, row_ptr, mask, vals, nnz=nnz.value, tau=float(tau))
 
 
 def mt_sparse_index(ctx: Context, S: SparseTensor, drop_mask: bool = False) -> SparseTensor:

@@ -350,6 +350,84 @@ int mt_demag_field_sym(mt_ctx* ctx, const mt_sym_tensor* S, const double* Ms, co
 
 int64_t mt_sparse_mask_words(int64_t n) { return n <= 0 ? 0 : round_up((n + 31) / 32, 4); }
 
+// ---- threshold selection, one radix digit per pass; the passes may be fed band by band ---------------
+namespace {
+constexpr int kSelDigit = 11, kSelBins = 1 << kSelDigit;
+inline int sel_bits(int dtype) { return dtype == MT_F32 ? 32 : 64; }
+}  // namespace
+
+int mt_select_begin(mt_ctx* ctx, mt_select_state* st, int dtype, double fraction, unsigned long long* hist) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  if (!st || !hist) return mt_fail(ctx, MT_ERR_INVALID_ARG, "state and hist must be non-NULL");
+  if (dtype != MT_F32 && dtype != MT_F64) return mt_fail(ctx, MT_ERR_INVALID_ARG, "unknown dtype %d", dtype);
+  if (!(fraction >= 0.0 && fraction <= 1.0)) return mt_fail(ctx, MT_ERR_INVALID_ARG, "fraction must be in [0, 1]");
+  memset(st, 0, sizeof(*st));
+  st->dtype = dtype;
+  st->fraction = fraction;
+  st->hi = sel_bits(dtype);
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  MT_CUDA_OK(ctx, cudaMemsetAsync(hist, 0, kSelBins * sizeof(unsigned long long), ctx->stream));
+  return MT_OK;
+}
+
+int mt_select_accumulate(mt_ctx* ctx, const mt_select_state* st, const void* N, int64_t n, int64_t n_rows, int64_t ld,
+                         unsigned long long* hist) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  if (!st || !hist) return mt_fail(ctx, MT_ERR_INVALID_ARG, "state and hist must be non-NULL");
+  if (st->done) return mt_fail(ctx, MT_ERR_INVALID_ARG, "selection already finished");
+  int rc = check_tensor_args(ctx, N, st->dtype, n, n_rows, ld);
+  if (rc) return rc;
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  const int width = st->hi >= kSelDigit ? kSelDigit : st->hi;
+  return mt_launch_select_hist(ctx, N, st->dtype, n, n_rows, ld, st->prefix, st->hi, st->hi - width, width, hist);
+}
+
+int mt_select_advance(mt_ctx* ctx, mt_select_state* st, unsigned long long* hist) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  if (!st || !hist) return mt_fail(ctx, MT_ERR_INVALID_ARG, "state and hist must be non-NULL");
+  if (st->done) return MT_OK;
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  unsigned long long* h = new (std::nothrow) unsigned long long[kSelBins];
+  if (!h) return mt_fail(ctx, MT_ERR_CUDA, "out of host memory");
+  cudaError_t ce = cudaMemcpyAsync(h, hist, kSelBins * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream);
+  if (ce == cudaSuccess) ce = cudaMemsetAsync(hist, 0, kSelBins * sizeof(unsigned long long), ctx->stream);
+  if (ce == cudaSuccess) ce = cudaStreamSynchronize(ctx->stream);
+  if (ce != cudaSuccess) {
+    delete[] h;
+    MT_CUDA_OK(ctx, ce);
+  }
+  const int bits = sel_bits(st->dtype);
+  const int width = st->hi >= kSelDigit ? kSelDigit : st->hi;
+  if (st->hi == bits) {  // first pass: total number of non-zero elements, and the rank to find
+    st->count = 0;
+    for (int b = 0; b < kSelBins; ++b) st->count += h[b];
+    st->k = (unsigned long long)floor(st->fraction * (double)st->count);
+    if (st->k >= st->count) {  // everything removed (also: nothing to rank)
+      st->done = 1;
+      st->tau = INFINITY;
+      delete[] h;
+      return MT_OK;
+    }
+  }
+  int b = 0;
+  while (b < (1 << width) - 1 && st->k >= h[b]) { st->k -= h[b]; ++b; }
+  delete[] h;
+  st->prefix = (st->prefix << width) | (unsigned long long)b;
+  st->hi -= width;
+  if (st->hi == 0) {
+    st->done = 1;
+    if (st->dtype == MT_F32) {
+      const uint32_t u = (uint32_t)st->prefix;
+      float f;
+      memcpy(&f, &u, 4);
+      st->tau = (double)f;
+    } else {
+      st->tau = bits_to_double(st->prefix);
+    }
+  }
+  return MT_OK;
+}
+
 int mt_threshold_value(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
                        double fraction, double* tau_host, int64_t* count_host) {
   if (!ctx) return MT_ERR_INVALID_ARG;
@@ -360,73 +438,69 @@ int mt_threshold_value(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
   // MSB-first radix select over the bit pattern of |v| (sign bit cleared: 31 / 63 significant bits),
   // 11-bit digits; each pass is one stream of the tensor and one 16 KB histogram read.
-  const int bits = dtype == MT_F32 ? 32 : 64;
-  const int kDigit = 11, kBins = 1 << kDigit;
   unsigned long long* d_hist = nullptr;
-  MT_CUDA_OK(ctx, cudaMalloc((void**)&d_hist, kBins * sizeof(unsigned long long)));
-  unsigned long long* h_hist = new (std::nothrow) unsigned long long[kBins];
-  if (!h_hist) { cudaFree(d_hist); return mt_fail(ctx, MT_ERR_CUDA, "out of host memory"); }
-  unsigned long long prefix = 0, k = 0, count = 0;
-  bool all_removed = false;
-  int hi = bits;  // bits [hi, bits) of the key are fixed to `prefix`
-  cudaError_t ce = cudaSuccess;
-  while (hi > 0 && !all_removed) {
-    const int width = hi >= kDigit ? kDigit : hi;
-    const int shift = hi - width;
-    if ((ce = cudaMemsetAsync(d_hist, 0, kBins * sizeof(unsigned long long), ctx->stream)) != cudaSuccess) break;
-    if ((rc = mt_launch_select_hist(ctx, N, dtype, n, n_rows, ld, prefix, hi, shift, width, d_hist))) break;
-    if ((ce = cudaMemcpyAsync(h_hist, d_hist, kBins * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream)) != cudaSuccess) break;
-    if ((ce = cudaStreamSynchronize(ctx->stream)) != cudaSuccess) break;
-    if (hi == bits) {  // first pass: total number of non-zero elements, and the rank to find
-      for (int b = 0; b < kBins; ++b) count += h_hist[b];
-      k = (unsigned long long)floor(fraction * (double)count);
-      if (k >= count) { all_removed = true; break; }
-    }
-    int b = 0;
-    while (b < (1 << width) - 1 && k >= h_hist[b]) { k -= h_hist[b]; ++b; }
-    prefix = (prefix << width) | (unsigned long long)b;
-    hi = shift;
+  MT_CUDA_OK(ctx, cudaMalloc((void**)&d_hist, kSelBins * sizeof(unsigned long long)));
+  mt_select_state st;
+  rc = mt_select_begin(ctx, &st, dtype, fraction, d_hist);
+  while (!rc && !st.done) {
+    if ((rc = mt_select_accumulate(ctx, &st, N, n, n_rows, ld, d_hist))) break;
+    rc = mt_select_advance(ctx, &st, d_hist);
   }
   cudaFree(d_hist);
-  delete[] h_hist;
   if (rc) return rc;
-  MT_CUDA_OK(ctx, ce);
-  if (count_host) *count_host = (int64_t)count;
-  if (all_removed) {
-    *tau_host = INFINITY;
-  } else if (dtype == MT_F32) {
-    const uint32_t u = (uint32_t)prefix;
-    float f;
-    memcpy(&f, &u, 4);
-    *tau_host = (double)f;
-  } else {
-    *tau_host = bits_to_double(prefix);
-  }
+  if (count_host) *count_host = (int64_t)st.count;
+  *tau_host = st.tau;
   return MT_OK;
 }
 
-int mt_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
-                    int64_t* row_ptr, int64_t* nnz_host) {
+int mt_sparse_count_band(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
+                         int64_t row0, int64_t n_total, int64_t* counts) {
   if (!ctx) return MT_ERR_INVALID_ARG;
   int rc = check_tensor_args(ctx, N, dtype, n, n_rows, ld);
   if (rc) return rc;
-  if (!row_ptr || !nnz_host) return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and nnz_host must be non-NULL");
+  if (!counts) return mt_fail(ctx, MT_ERR_INVALID_ARG, "counts must be non-NULL");
+  if (row0 < 0 || row0 + n_rows > n_total) return mt_fail(ctx, MT_ERR_INVALID_ARG, "band outside [0, n_total)");
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
-  if ((rc = mt_launch_sparse_count(ctx, N, dtype, n, n_rows, ld, tau, row_ptr))) return rc;
-  MT_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hscal, row_ptr + 6 * n_rows, 8, cudaMemcpyDeviceToHost, ctx->stream));
+  return mt_launch_sparse_count(ctx, N, dtype, n, n_rows, ld, tau, row0, n_total, counts);
+}
+
+int mt_sparse_scan(mt_ctx* ctx, int64_t* row_ptr, int64_t n_total, int64_t* nnz_host) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  if (!row_ptr || !nnz_host || n_total <= 0)
+    return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and nnz_host must be non-NULL, n_total positive");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  int rc = mt_launch_sparse_scan(ctx, row_ptr, n_total);
+  if (rc) return rc;
+  MT_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hscal, row_ptr + 6 * n_total, 8, cudaMemcpyDeviceToHost, ctx->stream));
   MT_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
   *nnz_host = (int64_t)ctx->hscal[0];
   return MT_OK;
 }
 
-int mt_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
-                   const int64_t* row_ptr, uint32_t* mask, void* vals) {
+int mt_sparse_fill_band(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
+                        int64_t row0, int64_t n_total, const int64_t* row_ptr, uint32_t* mask, void* vals) {
   if (!ctx) return MT_ERR_INVALID_ARG;
   int rc = check_tensor_args(ctx, N, dtype, n, n_rows, ld);
   if (rc) return rc;
   if (!row_ptr || !mask) return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and mask must be non-NULL");
+  if (row0 < 0 || row0 + n_rows > n_total) return mt_fail(ctx, MT_ERR_INVALID_ARG, "band outside [0, n_total)");
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
-  return mt_launch_sparse_fill(ctx, N, dtype, n, n_rows, ld, tau, row_ptr, mt_sparse_mask_words(n), mask, vals);
+  return mt_launch_sparse_fill(ctx, N, dtype, n, n_rows, ld, tau, row0, n_total, row_ptr, mt_sparse_mask_words(n), mask,
+                               vals);
+}
+
+int mt_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
+                    int64_t* row_ptr, int64_t* nnz_host) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  if (!row_ptr || !nnz_host) return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and nnz_host must be non-NULL");
+  int rc = mt_sparse_count_band(ctx, N, dtype, n, n_rows, ld, tau, 0, n_rows, row_ptr);
+  if (rc) return rc;
+  return mt_sparse_scan(ctx, row_ptr, n_rows, nnz_host);
+}
+
+int mt_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
+                   const int64_t* row_ptr, uint32_t* mask, void* vals) {
+  return mt_sparse_fill_band(ctx, N, dtype, n, n_rows, ld, tau, 0, n_rows, row_ptr, mask, vals);
 }
 
 int mt_sparse_index(mt_ctx* ctx, const mt_sparse_tensor* S, uint16_t* cols16) {

@@ -130,13 +130,17 @@ __global__ void __launch_bounds__(512) select_hist_kernel(const T* __restrict__ 
 
 template <typename T> __device__ __forceinline__ bool kept(T v, T tau) { return v != T(0) && !(fabs(v) < tau); }
 
-// counts[plane * n_rows + i] = kept entries of row i of the plane; one warp per (plane, row)
+// N holds rows [row0, row0 + n_rows) of a tensor of n_total rows (the whole tensor: row0 = 0, n_total =
+// n_rows): counts[plane * n_total + row0 + i] = kept entries of band row i of the plane; one warp per
+// (plane, band row)
 template <typename T>
 __global__ void __launch_bounds__(256) sparse_count_kernel(const T* __restrict__ N, int64_t n, int64_t n_rows,
-                                                           int64_t ld, T tau, int64_t* __restrict__ counts) {
+                                                           int64_t ld, T tau, int64_t row0, int64_t n_total,
+                                                           int64_t* __restrict__ counts) {
   const int64_t r = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
   if (r >= 6 * n_rows) return;
+  const int64_t R = (r / n_rows) * n_total + row0 + r % n_rows;
   const T* row = N + r * ld;
   typedef typename Vec16<T>::type V;
   constexpr int kV = Vec16<T>::n;
@@ -149,7 +153,7 @@ __global__ void __launch_bounds__(256) sparse_count_kernel(const T* __restrict__
   }
 #pragma unroll
   for (int off = 16; off > 0; off >>= 1) c += __shfl_xor_sync(0xffffffffu, c, off);
-  if (lane == 0) counts[r] = c;
+  if (lane == 0) counts[R] = c;
 }
 
 // in-place exclusive scan of len+1 int64 (slot len receives the total); one block, sequential chunks
@@ -181,15 +185,16 @@ __global__ void __launch_bounds__(1024) scan_kernel(int64_t* __restrict__ a, int
 // vals[row_ptr[plane * n_rows + i]] in column order.  One warp per (plane, row).
 template <typename T>
 __global__ void __launch_bounds__(256) sparse_fill_kernel(const T* __restrict__ N, int64_t n, int64_t n_rows,
-                                                          int64_t ld, T tau, const int64_t* __restrict__ row_ptr,
-                                                          int64_t nw, uint32_t* __restrict__ mask,
-                                                          T* __restrict__ vals) {
+                                                          int64_t ld, T tau, int64_t row0, int64_t n_total,
+                                                          const int64_t* __restrict__ row_ptr, int64_t nw,
+                                                          uint32_t* __restrict__ mask, T* __restrict__ vals) {
   const int64_t r = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
   if (r >= 6 * n_rows) return;
+  const int64_t R = (r / n_rows) * n_total + row0 + r % n_rows;  // row of the whole tensor (see count)
   const T* row = N + r * ld;
-  uint32_t* mrow = mask + r * nw;
-  T* out = vals + row_ptr[r];
+  uint32_t* mrow = mask + R * nw;
+  T* out = vals + row_ptr[R];
   int64_t off = 0;
   for (int64_t c0 = 0; c0 < nw; c0 += 4) {  // nw is a multiple of 4; four chunks loaded before any is packed
     T v[4];
@@ -567,29 +572,36 @@ int mt_launch_select_hist(mt_ctx* ctx, const void* N, int dtype, int64_t n, int6
 }
 
 int mt_launch_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
-                           int64_t* row_ptr) {
+                           int64_t row0, int64_t n_total, int64_t* counts) {
   const unsigned grid = (unsigned)((6 * n_rows + 7) / 8);
   if (dtype == MT_F32)
-    sparse_count_kernel<float><<<grid, 256, 0, ctx->stream>>>((const float*)N, n, n_rows, ld, (float)tau, row_ptr);
+    sparse_count_kernel<float><<<grid, 256, 0, ctx->stream>>>((const float*)N, n, n_rows, ld, (float)tau, row0,
+                                                              n_total, counts);
   else
-    sparse_count_kernel<double><<<grid, 256, 0, ctx->stream>>>((const double*)N, n, n_rows, ld, tau, row_ptr);
+    sparse_count_kernel<double><<<grid, 256, 0, ctx->stream>>>((const double*)N, n, n_rows, ld, tau, row0, n_total,
+                                                               counts);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
-  scan_kernel<<<1, 1024, 0, ctx->stream>>>(row_ptr, 6 * n_rows);
+  return MT_OK;
+}
+
+int mt_launch_sparse_scan(mt_ctx* ctx, int64_t* row_ptr, int64_t n_total) {
+  scan_kernel<<<1, 1024, 0, ctx->stream>>>(row_ptr, 6 * n_total);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   return MT_OK;
 }
 
 int mt_launch_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
-                          const int64_t* row_ptr, int64_t nw, uint32_t* mask, void* vals) {
+                          int64_t row0, int64_t n_total, const int64_t* row_ptr, int64_t nw, uint32_t* mask,
+                          void* vals) {
   const unsigned grid = (unsigned)((6 * n_rows + 7) / 8);
   if (dtype == MT_F32)
-    sparse_fill_kernel<float><<<grid, 256, 0, ctx->stream>>>((const float*)N, n, n_rows, ld, (float)tau, row_ptr, nw,
-                                                             mask, (float*)vals);
+    sparse_fill_kernel<float><<<grid, 256, 0, ctx->stream>>>((const float*)N, n, n_rows, ld, (float)tau, row0, n_total,
+                                                             row_ptr, nw, mask, (float*)vals);
   else
-    sparse_fill_kernel<double><<<grid, 256, 0, ctx->stream>>>((const double*)N, n, n_rows, ld, tau, row_ptr, nw, mask,
-                                                              (double*)vals);
+    sparse_fill_kernel<double><<<grid, 256, 0, ctx->stream>>>((const double*)N, n, n_rows, ld, tau, row0, n_total,
+                                                              row_ptr, nw, mask, (double*)vals);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   return MT_OK;

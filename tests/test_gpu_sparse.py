@@ -226,3 +226,50 @@ def test_sparse_row_band(ctx, oracle):
     for b in range(2):
         assert H.rel_l2(Hd[b].cpu().numpy(), ref[b]) <= 1e-5
         assert H.rel_l2(Hi[b].cpu().numpy(), ref[b]) <= 1e-5
+
+
+@pytest.mark.parametrize("dtype", ["f32", "f64"])
+def test_streamed_thresholding_equals_the_resident_path_and_the_oracle(ctx, oracle, dtype):
+    """PAPER.md:237 (memory): the thresholded tensor built band by band (mt_select_*, mt_sparse_*_band; the
+    dense tensor never resident) is bit-identical to the one built from the resident dense tensor — same
+    threshold, offsets, bitmaps, values — for band heights that do not divide n; and, with the cut placed
+    in a gap of the oracle's magnitudes, its bitmaps equal the oracle's truncation and its field the
+    oracle's field of the truncated tensor."""
+    w = W.config5(13, 7, 3, batch=2)
+    n = w.n
+    code = H.dtype_code(dtype)
+    tiles = H.dev_tiles(w)
+    N, ld, status = H.assemble(ctx, tiles, dtype)
+    assert status == 0
+    for X, band_rows in ((0.0, 64), (0.35, 37), (0.9, 100), (1.0, 273)):
+        tau, cnt = B.mt_threshold_value(ctx, N, code, n, n, ld, X)
+        S = B.mt_sparse_build(ctx, N, code, n, n, ld, tau)
+        T = B.mt_sparse_build_streamed(ctx, tiles, code, X, band_rows)
+        torch.cuda.synchronize()
+        assert T.tau == tau and T.nnz == S.nnz
+        assert torch.equal(T.row_ptr, S.row_ptr) and torch.equal(T.mask, S.mask)
+        if S.nnz:
+            assert torch.equal(T.vals, S.vals)
+    # against the oracle: cut in a gap of the oracle's magnitudes next to the device's 60 % value
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=True)
+    host = N_ref.astype(np.float32 if dtype == "f32" else np.float64)
+    tau_dev, _ = B.mt_threshold_value(ctx, N, code, n, n, ld, 0.6)
+    mags = np.unique(np.abs(host[np.abs(host) > 0]).astype(np.float64))
+    gaps = np.nonzero(mags[1:] > mags[:-1] * 1.001)[0]
+    g = gaps[np.argmin(np.abs(np.log(mags[gaps] / tau_dev)))]
+    tau = float(np.sqrt(mags[g] * mags[g + 1]))
+    if dtype == "f32":
+        tau = float(np.float32(tau))
+    assert mags[g] < tau < mags[g + 1]
+    T = B.mt_sparse_build_streamed(ctx, tiles, code, 0.6, 50, tau=tau)
+    B.mt_sparse_index(ctx, T)
+    torch.cuda.synchronize()
+    trunc = OT.truncate(host, tau)
+    assert np.array_equal(unpack(T, n) != 0, trunc != 0)
+    m = torch.from_numpy(w.m).cuda()
+    Hd = torch.empty_like(m)
+    B.mt_demag_field_sparse(ctx, T, tiles.Ms, m, 2, Hd)
+    torch.cuda.synchronize()
+    ref = oracle.demag_field(trunc.astype(np.float64), w.Ms, w.m)
+    for b in range(2):
+        assert H.rel_l2(Hd[b].cpu().numpy(), ref[b]) <= TOL_HD[dtype]
