@@ -346,6 +346,16 @@ def test_config5_full_size_thresholded_index_rows(ctx, oracle):
             assert np.array_equal(S.cols16[beg[q]:end[q]].cpu().numpy(), cols_ref.astype(np.uint16))
             vals = S.vals[beg[q]:end[q]].cpu().numpy()
             assert (H.f32_ulp_distance(vals, N_ref[p, q, cols_ref]) <= 1).all()
+    # (2b) the streamed build (dense tensor never resident: 4,096-row bands, 6.4 GB) gives the same
+    # threshold and, for the same cut, the same offsets, bitmaps and values (64-bit offsets throughout)
+    T = B.mt_sparse_build_streamed(ctx, tiles, B.MT_F32, X, 4096)
+    assert T.tau == tau_dev
+    del T
+    T = B.mt_sparse_build_streamed(ctx, tiles, B.MT_F32, X, 3000, tau=tau)
+    torch.cuda.synchronize()
+    assert T.nnz == S.nnz and torch.equal(T.row_ptr, S.row_ptr)
+    assert torch.equal(T.mask, S.mask) and torch.equal(T.vals, S.vals)
+    del T
     # (3) fields
     m = torch.from_numpy(w.m).cuda()
     Hb, Hi, Hi2 = torch.empty_like(m), torch.empty_like(m), torch.empty_like(m)
