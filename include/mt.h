@@ -133,8 +133,10 @@ int mt_demag_field_host(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_
  * (bit l of word w = column 32 w + l, 1 = kept) and the kept values are packed in column order from
  * vals[row_ptr[c*n_rows + i]].  nw = mt_sparse_mask_words(n) (a multiple of 4; padding words zero).
  * All arrays are DEVICE memory owned by the caller.
- * Optional second index ("index rows", n <= 65536): cols16[k] = source column of vals[k], written by
- * mt_sparse_index from the bitmap.  When cols16 is non-NULL the field kernel walks the packed values
+ * Optional second index ("index rows"): cols16[k] = source column of vals[k] modulo 65536, written by
+ * mt_sparse_index from the bitmap; for n > 65536 the columns fall in panels of 65,536 and
+ * panel_ptr[(c*n_rows + i)*(P-1) + q-1] (P = ceil(n/65536)) is the offset into vals at which panel
+ * q >= 1 of plane row (c, i) starts (a row's entries are in column order, so a panel is one run).  When cols16 is non-NULL the field kernel walks the packed values
  * (coalesced value + 16-bit column loads, gathered M) instead of decoding the bitmap column by column:
  * 6 bytes per kept fp32 entry instead of 4 + 1/8 per DENSE entry, i.e. smaller than the bitmap from
  * X ~ 0.94 and a far cheaper decode at any X.                                 */
@@ -145,7 +147,8 @@ typedef struct {
   const int64_t* row_ptr;  /* [6*n_rows + 1] offsets into vals (elements); last = number kept        */
   const uint32_t* mask;    /* [6][n_rows][nw]                                                        */
   const void* vals;        /* [row_ptr[6*n_rows]]                                                    */
-  const uint16_t* cols16;  /* NULL, or [row_ptr[6*n_rows]] column of every packed value (n <= 65536)  */
+  const uint16_t* cols16;  /* NULL, or [row_ptr[6*n_rows]] column (mod 65536) of every packed value  */
+  const int64_t* panel_ptr; /* n > 65536 with cols16: [6*n_rows][ceil(n/65536) - 1], else NULL         */
 } mt_sparse_tensor;
 
 int64_t mt_sparse_mask_words(int64_t n);
@@ -205,10 +208,11 @@ int mt_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_
 int mt_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
                    double tau, const int64_t* row_ptr, uint32_t* mask, void* vals);
 
-/* Index rows: cols16[row_ptr[c*n_rows+i] + k] = column of the k-th set bit of the bitmap row (c, i).
- * S->mask and S->row_ptr must be filled (mt_sparse_fill); S->cols16 is ignored; cols16 is a DEVICE
- * array of row_ptr[6*n_rows] uint16.  Asynchronous.  MT_ERR_INVALID_ARG when n > 65536.            */
-int mt_sparse_index(mt_ctx* ctx, const mt_sparse_tensor* S, uint16_t* cols16);
+/* Index rows: cols16[row_ptr[c*n_rows+i] + k] = column (mod 65536) of the k-th set bit of the bitmap
+ * row (c, i); panel_ptr as described above (may be NULL when n <= 65536).  S->mask and S->row_ptr
+ * must be filled (mt_sparse_fill); S->cols16 / S->panel_ptr are ignored; cols16 is a DEVICE array of
+ * row_ptr[6*n_rows] uint16, panel_ptr of 6*n_rows*(ceil(n/65536)-1) int64.  Asynchronous.          */
+int mt_sparse_index(mt_ctx* ctx, const mt_sparse_tensor* S, uint16_t* cols16, int64_t* panel_ptr);
 
 /* mt_demag_field on the thresholded tensor: Hd[b][a][i] = - sum over kept entries; same arithmetic
  * rules (fp32 runs of at most 96 terms per lane, 64 on index rows, then fp64), fixed reduction order. */

@@ -62,7 +62,7 @@ class _Sym(C.Structure):
 
 class _Sparse(C.Structure):
     _fields_ = [("n", C.c_int64), ("n_rows", C.c_int64), ("dtype", C.c_int), ("nw", C.c_int64),
-                ("row_ptr", C.c_void_p), ("mask", C.c_void_p), ("vals", C.c_void_p), ("cols16", C.c_void_p)]
+                ("row_ptr", C.c_void_p), ("mask", C.c_void_p), ("vals", C.c_void_p), ("cols16", C.c_void_p), ("panel_ptr", C.c_void_p)]
 
 
 class _SelectState(C.Structure):
@@ -131,7 +131,7 @@ def load() -> C.CDLL:
         lib.mt_sparse_scan.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
         lib.mt_sparse_fill_band.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64,
                                             C.c_double, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
-        lib.mt_sparse_index.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p]
+        lib.mt_sparse_index.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p, C.c_void_p]
         lib.mt_demag_field_sparse.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p, C.c_void_p, C.c_int,
                                               C.c_void_p]
         lib.mt_sym_tensor_elems.restype = C.c_int64
@@ -385,16 +385,20 @@ class SparseTensor:
     nnz: int = 0
     tau: float = 0.0
     cols16: object = None  # [nnz] uint16 index rows (mt_sparse_index) or None; the mask may be dropped then
+    panel_ptr: object = None  # n > 65536: [6*n_rows, ceil(n/65536)-1] int64 panel starts
 
     def _c(self) -> _Sparse:
         return _Sparse(self.n, self.n_rows, self.dtype, self.nw, _ptr(self.row_ptr, torch.int64),
                        _ptr(self.mask, torch.int32) if self.mask is not None else None,
                        _ptr(self.vals, torch_dtype(self.dtype)),
-                       _ptr(self.cols16, torch.uint16) if self.cols16 is not None else None)
+                       _ptr(self.cols16, torch.uint16) if self.cols16 is not None else None,
+                       _ptr(self.panel_ptr, torch.int64) if self.panel_ptr is not None else None)
 
     def nbytes(self) -> int:
         """Bytes one field evaluation streams: values + the index the kernel walks (16-bit columns if present)."""
         idx = self.cols16.numel() * 2 if self.cols16 is not None else self.mask.numel() * 4
+        if self.cols16 is not None and self.panel_ptr is not None:
+            idx += self.panel_ptr.numel() * 8
         return self.row_ptr.numel() * 8 + idx + self.vals.numel() * self.vals.element_size()
 
 
@@ -472,9 +476,12 @@ def mt_sparse_build_streamed(ctx: Context, tiles: Tiles, dtype: int, fraction: f
 def mt_sparse_index(ctx: Context, S: SparseTensor, drop_mask: bool = False) -> SparseTensor:
     """Adds the index rows (16-bit column of every packed value) to S; the field kernel then walks them."""
     cols = torch.empty(max(1, S.nnz), dtype=torch.uint16, device=S.vals.device)
+    panels = (S.n + 65535) // 65536
+    pp = (torch.empty((6 * S.n_rows, panels - 1), dtype=torch.int64, device=S.vals.device) if panels > 1 else None)
     s = S._c()
-    ctx.check(ctx.lib.mt_sparse_index(ctx.h, C.byref(s), _ptr(cols, torch.uint16)))
+    ctx.check(ctx.lib.mt_sparse_index(ctx.h, C.byref(s), _ptr(cols, torch.uint16), _ptr(pp, torch.int64)))
     S.cols16 = cols
+    S.panel_ptr = pp
     if drop_mask:
         ctx.stream.synchronize()  # the index kernel reads the mask
         S.mask = None

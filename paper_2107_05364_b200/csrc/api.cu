@@ -59,7 +59,8 @@ int check_sparse(mt_ctx* ctx, const mt_sparse_tensor* s) {
   if (s->nw != mt_sparse_mask_words(s->n)) return mt_fail(ctx, MT_ERR_INVALID_ARG, "nw must be mt_sparse_mask_words(n)");
   if (!s->row_ptr || (!s->mask && !s->cols16))
     return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and one of mask / cols16 must be non-NULL");
-  if (s->cols16 && s->n > 65536) return mt_fail(ctx, MT_ERR_INVALID_ARG, "cols16 given but n > 65536");
+  if (s->cols16 && s->n > 65536 && !s->panel_ptr)
+    return mt_fail(ctx, MT_ERR_INVALID_ARG, "cols16 with n > 65536 needs panel_ptr");
   return MT_OK;
 }
 
@@ -503,14 +504,19 @@ int mt_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_r
   return mt_sparse_fill_band(ctx, N, dtype, n, n_rows, ld, tau, 0, n_rows, row_ptr, mask, vals);
 }
 
-int mt_sparse_index(mt_ctx* ctx, const mt_sparse_tensor* S, uint16_t* cols16) {
+int mt_sparse_index(mt_ctx* ctx, const mt_sparse_tensor* S, uint16_t* cols16, int64_t* panel_ptr) {
   if (!ctx) return MT_ERR_INVALID_ARG;
-  int rc = check_sparse(ctx, S);
+  if (!S) return mt_fail(ctx, MT_ERR_INVALID_ARG, "sparse tensor is NULL");
+  mt_sparse_tensor t = *S;
+  t.cols16 = nullptr;  // ignored here (it may be the array being written)
+  t.panel_ptr = nullptr;
+  int rc = check_sparse(ctx, &t);
   if (rc) return rc;
-  if (S->n > 65536) return mt_fail(ctx, MT_ERR_INVALID_ARG, "index rows hold 16-bit columns: n must be <= 65536");
   if (!cols16 || !S->mask) return mt_fail(ctx, MT_ERR_INVALID_ARG, "cols16 and S->mask must be non-NULL");
+  if (S->n > 65536 && !panel_ptr)
+    return mt_fail(ctx, MT_ERR_INVALID_ARG, "n > 65536: panel_ptr ([6*n_rows][ceil(n/65536)-1]) must be non-NULL");
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
-  return mt_launch_sparse_index(ctx, S, cols16);
+  return mt_launch_sparse_index(ctx, S, cols16, panel_ptr);
 }
 
 int mt_demag_field_sparse(mt_ctx* ctx, const mt_sparse_tensor* S, const double* Ms, const double* m, int batch,

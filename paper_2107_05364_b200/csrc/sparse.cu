@@ -225,6 +225,8 @@ struct SparseArgs {
   const uint32_t* mask;
   const void* vals;
   const void* Mst;
+  const int64_t* panel_ptr;  // index rows with n > 65536: [6 * n_rows][npanels - 1] offsets into vals
+  int npanels;               // column panels of 65,536 (16-bit columns are relative to their panel)
 };
 
 // One group = 32 chunks (1,024 columns): lane l loads the mask word of chunk c0 + l of every plane
@@ -374,7 +376,8 @@ int launch_bitmap(mt_ctx* ctx, const SparseArgs& a, const EpiArgs& e) {
 // cols[row_ptr[r] + k] = column of the k-th set bit of bitmap row r; one warp per (plane, row).
 __global__ void __launch_bounds__(256) sparse_index_kernel(const uint32_t* __restrict__ mask,
                                                            const int64_t* __restrict__ row_ptr, int64_t n_rows,
-                                                           int64_t nw, uint16_t* __restrict__ cols) {
+                                                           int64_t nw, uint16_t* __restrict__ cols,
+                                                           int64_t* __restrict__ panel_ptr, int npanels) {
   const int64_t r = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
   if (r >= 6 * n_rows) return;
@@ -383,6 +386,8 @@ __global__ void __launch_bounds__(256) sparse_index_kernel(const uint32_t* __res
   const uint32_t lt = (1u << lane) - 1u;
   int64_t off = 0;
   for (int64_t c0 = 0; c0 < nw; c0 += 32) {
+    // a panel of 65,536 columns = 2,048 mask words: the packed offset at which panel q >= 1 starts
+    if (c0 && (c0 & 2047) == 0 && lane == 0) panel_ptr[r * (npanels - 1) + (c0 >> 11) - 1] = row_ptr[r] + off;
     const uint32_t mine = c0 + lane < nw ? __ldg(mrow + c0 + lane) : 0u;
     uint32_t nz = __ballot_sync(0xffffffffu, mine != 0u);
     while (nz) {
@@ -447,11 +452,11 @@ __device__ __forceinline__ void index_load(const T* __restrict__ vals, const uin
 // next block's values and columns are requested before the current block's gathers are issued, so a
 // warp keeps two blocks of kIdxUnroll * 32 entries (2 x 1.5 KB) in flight towards HBM.
 template <typename T, int B, int P>
-__device__ __forceinline__ void index_plane(const SparseArgs& a, const uint16_t* __restrict__ cols, int64_t beg,
-                                            int64_t end, int lane, double (&acc)[B][3]) {
+__device__ __forceinline__ void index_panel(const SparseArgs& a, const uint16_t* __restrict__ cols, int64_t beg,
+                                            int64_t end, int64_t col0, int lane, double (&acc)[B][3]) {
   constexpr int R = PlaneRC<P>::r, Cc = PlaneRC<P>::c;
   const T* __restrict__ vals = (const T*)a.vals;
-  const T* __restrict__ M = (const T*)a.Mst;
+  const T* __restrict__ M = (const T*)a.Mst + col0;
   T vn[kIdxUnroll];
   int cn[kIdxUnroll];
   int64_t kb = beg;  // warp-uniform block start
@@ -485,6 +490,19 @@ __device__ __forceinline__ void index_plane(const SparseArgs& a, const uint16_t*
   }
 }
 
+// A plane row = its column panels in turn (one panel when n <= 65,536: no extra loads).
+template <typename T, int B, int P>
+__device__ __forceinline__ void index_plane(const SparseArgs& a, const uint16_t* __restrict__ cols, int64_t row,
+                                            int64_t beg, int64_t end, int lane, double (&acc)[B][3]) {
+  const int64_t* pp = a.panel_ptr + ((int64_t)P * a.n_rows + row) * (a.npanels - 1);
+  int64_t b = beg;
+  for (int q = 0; q < a.npanels; ++q) {
+    const int64_t e = q + 1 < a.npanels ? __ldg(pp + q) : end;
+    index_panel<T, B, P>(a, cols, b, e, (int64_t)q << 16, lane, acc);
+    b = e;
+  }
+}
+
 template <typename T, int B>
 __global__ void __launch_bounds__(256, (B <= 2 ? 4 : 2)) demag_index_kernel(SparseArgs a, const uint16_t* __restrict__ cols, EpiArgs e) {
   const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
@@ -501,7 +519,7 @@ __global__ void __launch_bounds__(256, (B <= 2 ? 4 : 2)) demag_index_kernel(Spar
     nbeg = __ldg(rp + (int64_t)(P + 1) * a.n_rows);            \
     nend = __ldg(rp + (int64_t)(P + 1) * a.n_rows + 1);        \
   }                                                            \
-  index_plane<T, B, P>(a, cols, beg, end, lane, acc);          \
+  index_plane<T, B, P>(a, cols, row, beg, end, lane, acc);     \
   beg = nbeg;                                                  \
   end = nend;
   MT_INDEX_PLANE(0)
@@ -607,9 +625,9 @@ int mt_launch_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int6
   return MT_OK;
 }
 
-int mt_launch_sparse_index(mt_ctx* ctx, const mt_sparse_tensor* s, uint16_t* cols16) {
-  sparse_index_kernel<<<(unsigned)((6 * s->n_rows + 7) / 8), 256, 0, ctx->stream>>>(s->mask, s->row_ptr, s->n_rows,
-                                                                                  s->nw, cols16);
+int mt_launch_sparse_index(mt_ctx* ctx, const mt_sparse_tensor* s, uint16_t* cols16, int64_t* panel_ptr) {
+  sparse_index_kernel<<<(unsigned)((6 * s->n_rows + 7) / 8), 256, 0, ctx->stream>>>(
+      s->mask, s->row_ptr, s->n_rows, s->nw, cols16, panel_ptr, (int)((s->n + 65535) >> 16));
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   return MT_OK;
@@ -625,6 +643,8 @@ int mt_launch_demag_sparse(mt_ctx* ctx, const mt_sparse_tensor* s, const void* M
   a.mask = s->mask;
   a.vals = s->vals;
   a.Mst = Mst;
+  a.panel_ptr = s->panel_ptr;
+  a.npanels = (int)((s->n + 65535) >> 16);
   const bool prof = ctx->prof_on && ctx->prof_ev && ctx->prof_count < MT_PROF_CAP;
   if (prof) MT_CUDA_OK(ctx, cudaEventRecord(ctx->prof_ev[2 * ctx->prof_count], ctx->stream));
   int rc;

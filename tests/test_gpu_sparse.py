@@ -193,10 +193,10 @@ def test_sparse_argument_checks(ctx):
     with pytest.raises(B.MtError):
         B.mt_demag_field_sparse(ctx, S, Ms, m, 1, torch.empty_like(m))
     S.nw -= 1
-    S.n = 65537   # 16-bit columns cannot address it
-    S.nw = 2052
-    with pytest.raises(B.MtError):
-        B.mt_sparse_index(ctx, S)
+    import ctypes
+    S.n, S.nw = 65537, 2052   # more than one panel of 16-bit columns: panel_ptr is required
+    rc = ctx.lib.mt_sparse_index(ctx.h, ctypes.byref(S._c()), S.vals.data_ptr(), None)
+    assert rc != 0
 
 
 def test_sparse_row_band(ctx, oracle):
@@ -273,3 +273,41 @@ def test_streamed_thresholding_equals_the_resident_path_and_the_oracle(ctx, orac
     ref = oracle.demag_field(trunc.astype(np.float64), w.Ms, w.m)
     for b in range(2):
         assert H.rel_l2(Hd[b].cpu().numpy(), ref[b]) <= TOL_HD[dtype]
+
+
+def test_index_rows_beyond_65536_columns(ctx, oracle):
+    """n > 65,536: 16-bit columns are relative to panels of 65,536 columns and panel_ptr marks where a
+    plane row's second panel starts.  A 40-row band of a 66 x 50 x 20 mesh (n = 66,000), thresholded at
+    70 %: columns, panel offsets and field against the oracle's truncated rows."""
+    w = W.config5(66, 50, 20, batch=2)
+    n = w.n
+    assert n == 66000
+    rows = np.concatenate([np.arange(0, 20), np.arange(65530, 65545), np.arange(n - 5, n)]).astype(np.int64)
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), rows=rows, long_double=True)
+    host, dev, ld = upload(N_ref, "f32")
+    tau = OT.threshold_value(host, 0.7)
+    tau_dev, _ = B.mt_threshold_value(ctx, dev, B.MT_F32, n, len(rows), ld, 0.7)
+    assert tau_dev == tau
+    S = B.mt_sparse_build(ctx, dev, B.MT_F32, n, len(rows), ld, tau)
+    m = torch.from_numpy(w.m).cuda()
+    Ms = torch.from_numpy(w.Ms).cuda()
+    Hb = torch.empty((2, 3, len(rows)), dtype=torch.float64, device="cuda")
+    B.mt_demag_field_sparse(ctx, S, Ms, m, 2, Hb)
+    B.mt_sparse_index(ctx, S)
+    torch.cuda.synchronize()
+    trunc = OT.truncate(host, tau)
+    flat = trunc.reshape(6 * len(rows), n)
+    cols_ref = np.nonzero(flat)[1]
+    assert (cols_ref >= 65536).any()
+    assert np.array_equal(S.cols16.cpu().numpy(), (cols_ref & 0xFFFF).astype(np.uint16))
+    ptr = S.row_ptr.cpu().numpy()
+    first_panel = np.count_nonzero(flat[:, :65536], axis=1)
+    assert S.panel_ptr.shape == (6 * len(rows), 1)
+    assert np.array_equal(S.panel_ptr.cpu().numpy()[:, 0], ptr[:-1] + first_panel)
+    Hi = torch.empty_like(Hb)
+    B.mt_demag_field_sparse(ctx, S, Ms, m, 2, Hi)
+    torch.cuda.synchronize()
+    ref = oracle.demag_field(trunc.astype(np.float64), w.Ms, w.m)
+    for b in range(2):
+        assert H.rel_l2(Hb[b].cpu().numpy(), ref[b]) <= 1e-5
+        assert H.rel_l2(Hi[b].cpu().numpy(), ref[b]) <= 1e-5
