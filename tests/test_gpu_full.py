@@ -289,6 +289,40 @@ def test_config5_full_size_symmetric_half(ctx, oracle):
     assert torch.equal(Hd, Hd2)
 
 
+def gap_cut(host, tau_dev):
+    """A cut inside a > 1e-3 relative gap of the oracle's magnitudes, next to the device's threshold."""
+    import math
+    mags = np.abs(host[(np.abs(host) > 0.5 * tau_dev) & (np.abs(host) < 2.0 * tau_dev)]).astype(np.float64)
+    mags = np.unique(mags)
+    gaps = np.nonzero(mags[1:] > mags[:-1] * 1.001)[0]
+    g = gaps[np.argmin(np.abs(np.log(mags[gaps] / tau_dev)))]
+    tau = float(np.float32(math.sqrt(mags[g] * mags[g + 1])))
+    assert mags[g] < tau < mags[g + 1] and 0.5 * tau_dev < tau < 2.0 * tau_dev
+    return tau
+
+
+def check_sparse_rows(S, rows, N_ref, trunc, n):
+    """Bitmap rows, 16-bit columns (+ panel offsets) and packed values of the sampled target rows of a
+    whole-tensor SparseTensor against the oracle's truncated rows."""
+    ridx = torch.from_numpy(rows).cuda()
+    for p in range(6):
+        ptr = S.row_ptr[p * n: (p + 1) * n + 1]
+        beg, end = ptr[:-1][ridx].cpu().numpy(), ptr[1:][ridx].cpu().numpy()
+        mask = S.mask[p].index_select(0, ridx).cpu().numpy().view(np.uint32)
+        bits = ((mask[..., None] >> np.arange(32, dtype=np.uint32)) & 1).astype(bool).reshape(len(rows), -1)
+        assert np.array_equal(bits[:, :n], trunc[p] != 0) and not bits[:, n:].any()
+        pp = S.panel_ptr[p * n: (p + 1) * n].index_select(0, ridx).cpu().numpy() if S.panel_ptr is not None else None
+        for q in range(len(rows)):
+            cols_ref = np.nonzero(trunc[p, q])[0]
+            assert end[q] - beg[q] == len(cols_ref)
+            assert np.array_equal(S.cols16[beg[q]:end[q]].cpu().numpy(), (cols_ref & 0xFFFF).astype(np.uint16))
+            if pp is not None:
+                starts = [beg[q] + np.count_nonzero(cols_ref < 65536 * (k + 1)) for k in range(pp.shape[1])]
+                assert np.array_equal(pp[q], np.array(starts))
+            vals = S.vals[beg[q]:end[q]].cpu().numpy()
+            assert (H.f32_ulp_distance(vals, N_ref[p, q, cols_ref]) <= 1).all()
+
+
 def test_config5_full_size_thresholded_index_rows(ctx, oracle):
     """F1 at BASELINE's full size, in the configuration bench.py times (X = 0.9, index rows).
     (1) the device's threshold value has the rank PAPER.md:239 defines, counted on the device tensor
@@ -322,30 +356,13 @@ def test_config5_full_size_thresholded_index_rows(ctx, oracle):
     rows = W.sample_rows(5, n, 64, extra=grid_corner_rows(w.grid) + [65535, 32768, 32767])
     N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), rows=rows, long_double=True)
     host = N_ref.astype(np.float32)
-    mags = np.abs(host[(np.abs(host) > 0.5 * tau_dev) & (np.abs(host) < 2.0 * tau_dev)]).astype(np.float64)
-    mags = np.unique(mags)
-    gaps = np.nonzero(mags[1:] > mags[:-1] * 1.001)[0]
-    g = gaps[np.argmin(np.abs(np.log(mags[gaps] / tau_dev)))]
-    tau = float(np.float32(math.sqrt(mags[g] * mags[g + 1])))
-    assert mags[g] < tau < mags[g + 1] and 0.5 * tau_dev < tau < 2.0 * tau_dev
+    tau = gap_cut(host, tau_dev)
     S = B.mt_sparse_build(ctx, N, B.MT_F32, n, n, ld, tau)
     B.mt_sparse_index(ctx, S)
     torch.cuda.synchronize()
     assert 0.05 < S.nnz / (6.0 * n * n) < 0.2
     trunc = OT.truncate(host, tau)
-    ridx = torch.from_numpy(rows).cuda()
-    for p in range(6):
-        ptr = S.row_ptr[p * n: (p + 1) * n + 1]
-        beg, end = ptr[:-1][ridx].cpu().numpy(), ptr[1:][ridx].cpu().numpy()
-        mask = S.mask[p].index_select(0, ridx).cpu().numpy().view(np.uint32)
-        bits = ((mask[..., None] >> np.arange(32, dtype=np.uint32)) & 1).astype(bool).reshape(len(rows), -1)
-        assert np.array_equal(bits[:, :n], trunc[p] != 0) and not bits[:, n:].any()
-        for q in range(len(rows)):
-            cols_ref = np.nonzero(trunc[p, q])[0]
-            assert end[q] - beg[q] == len(cols_ref)
-            assert np.array_equal(S.cols16[beg[q]:end[q]].cpu().numpy(), cols_ref.astype(np.uint16))
-            vals = S.vals[beg[q]:end[q]].cpu().numpy()
-            assert (H.f32_ulp_distance(vals, N_ref[p, q, cols_ref]) <= 1).all()
+    check_sparse_rows(S, rows, N_ref, trunc, n)
     # (2b) the streamed build (dense tensor never resident: 4,096-row bands, 6.4 GB) gives the same
     # threshold and, for the same cut, the same offsets, bitmaps and values (64-bit offsets throughout)
     T = B.mt_sparse_build_streamed(ctx, tiles, B.MT_F32, X, 4096)
@@ -373,6 +390,43 @@ def test_config5_full_size_thresholded_index_rows(ctx, oracle):
         assert H.rel_l2(got_i[b][:, rows], ref[b]) <= TOL_HD["f32"]
         assert H.rel_l2(got_b[b][:, rows], ref[b]) <= TOL_HD["f32"]
         assert H.rel_l2(got_i[b], got_b[b]) <= 2e-6
+
+
+def test_beyond_hbm_size_thresholded_streamed(ctx, oracle):
+    """N = 131,072 tiles (128 x 64 x 16 unit cubes): the dense fp32 tensor is 412 GB and cannot exist on
+    one B200; thresholded at X = 0.95 and built band by band it is 34 GB.  Sampled
+    rows (bitmap, columns in two panels, values, field from both kernels) against the oracle."""
+    from oracle import threshold as OT
+    w = W.config5(128, 64, 16, batch=1)
+    n = w.n
+    assert n == 131072
+    tiles = H.dev_tiles(w)
+    status = torch.zeros(1, dtype=torch.int32, device="cuda")
+    T0 = B.mt_sparse_build_streamed(ctx, tiles, B.MT_F32, 0.95, 4096, status)
+    tau_dev = T0.tau
+    assert int(status.item()) == 0 and 0.04 < T0.nnz / (6.0 * n * n) < 0.06
+    del T0
+    rows = W.sample_rows(5, n, 32, extra=grid_corner_rows(w.grid) + [65535, 65536, n - 1])
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), rows=rows, long_double=True)
+    host = N_ref.astype(np.float32)
+    tau = gap_cut(host, tau_dev)
+    S = B.mt_sparse_build_streamed(ctx, tiles, B.MT_F32, 0.95, 4096, status, tau=tau)
+    B.mt_sparse_index(ctx, S)
+    torch.cuda.synchronize()
+    trunc = OT.truncate(host, tau)
+    check_sparse_rows(S, rows, N_ref, trunc, n)
+    m = torch.from_numpy(w.m).cuda()
+    Hb, Hi = torch.empty_like(m), torch.empty_like(m)
+    cols = S.cols16
+    S.cols16 = None
+    B.mt_demag_field_sparse(ctx, S, tiles.Ms, m, 1, Hb)
+    S.cols16 = cols
+    B.mt_demag_field_sparse(ctx, S, tiles.Ms, m, 1, Hi)
+    torch.cuda.synchronize()
+    ref = oracle.demag_field(trunc.astype(np.float64), w.Ms, w.m)
+    assert H.rel_l2(Hi.cpu().numpy()[0][:, rows], ref[0]) <= TOL_HD["f32"]
+    assert H.rel_l2(Hb.cpu().numpy()[0][:, rows], ref[0]) <= TOL_HD["f32"]
+    assert H.rel_l2(Hi.cpu().numpy()[0], Hb.cpu().numpy()[0]) <= 2e-6
 
 
 def test_config2_full_protocol_full_size_invariants_and_half_storage(ctx):
