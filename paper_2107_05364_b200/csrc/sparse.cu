@@ -490,10 +490,14 @@ __device__ __forceinline__ void index_panel(const SparseArgs& a, const uint16_t*
   }
 }
 
-// A plane row = its column panels in turn (one panel when n <= 65,536: no extra loads).
-template <typename T, int B, int P>
+// A plane row = its column panels in turn (PANELS = false, n <= 65,536: the one panel, nothing extra).
+template <typename T, int B, int P, bool PANELS>
 __device__ __forceinline__ void index_plane(const SparseArgs& a, const uint16_t* __restrict__ cols, int64_t row,
                                             int64_t beg, int64_t end, int lane, double (&acc)[B][3]) {
+  if (!PANELS) {
+    index_panel<T, B, P>(a, cols, beg, end, 0, lane, acc);
+    return;
+  }
   const int64_t* pp = a.panel_ptr + ((int64_t)P * a.n_rows + row) * (a.npanels - 1);
   int64_t b = beg;
   for (int q = 0; q < a.npanels; ++q) {
@@ -503,7 +507,7 @@ __device__ __forceinline__ void index_plane(const SparseArgs& a, const uint16_t*
   }
 }
 
-template <typename T, int B>
+template <typename T, int B, bool PANELS>
 __global__ void __launch_bounds__(256, (B <= 2 ? 4 : 2)) demag_index_kernel(SparseArgs a, const uint16_t* __restrict__ cols, EpiArgs e) {
   const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
@@ -519,7 +523,7 @@ __global__ void __launch_bounds__(256, (B <= 2 ? 4 : 2)) demag_index_kernel(Spar
     nbeg = __ldg(rp + (int64_t)(P + 1) * a.n_rows);            \
     nend = __ldg(rp + (int64_t)(P + 1) * a.n_rows + 1);        \
   }                                                            \
-  index_plane<T, B, P>(a, cols, row, beg, end, lane, acc);     \
+  index_plane<T, B, P, PANELS>(a, cols, row, beg, end, lane, acc); \
   beg = nbeg;                                                  \
   end = nend;
   MT_INDEX_PLANE(0)
@@ -547,7 +551,10 @@ __global__ void __launch_bounds__(256, (B <= 2 ? 4 : 2)) demag_index_kernel(Spar
 
 template <typename T, int B>
 int launch_index_B(mt_ctx* ctx, const SparseArgs& a, const uint16_t* cols, const EpiArgs& e) {
-  demag_index_kernel<T, B><<<(unsigned)((a.n_rows + 7) / 8), 256, 0, ctx->stream>>>(a, cols, e);
+  if (a.npanels > 1)
+    demag_index_kernel<T, B, true><<<(unsigned)((a.n_rows + 7) / 8), 256, 0, ctx->stream>>>(a, cols, e);
+  else
+    demag_index_kernel<T, B, false><<<(unsigned)((a.n_rows + 7) / 8), 256, 0, ctx->stream>>>(a, cols, e);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   return MT_OK;
