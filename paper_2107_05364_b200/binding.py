@@ -426,19 +426,28 @@ def mt_sparse_build(ctx: Context, N: torch.Tensor, dtype: int, n: int, n_rows: i
 
 
 def mt_sparse_build_streamed(ctx: Context, tiles: Tiles, dtype: int, fraction: float, band_rows: int,
-                             status_flag: torch.Tensor | None = None, tau: float | None = None) -> SparseTensor:
+                             status_flag: torch.Tensor | None = None, tau: float | None = None,
+                             row_begin: int = 0, row_end: int | None = None, allreduce=None) -> SparseTensor:
     """Thresholded tensor of `tiles` without ever holding the dense tensor: every pass (one per radix
     digit of the selection, one for the counts, one for the fill) assembles the tensor again band by
     band into one [6, band_rows, ld] buffer.  Sequence of C-ABI calls only: mt_assemble_tensor,
     mt_select_*, mt_sparse_count_band / mt_sparse_scan / mt_sparse_fill_band.  `tau` given: the
-    selection passes are skipped."""
+    selection passes are skipped.
+
+    Row-sharded (multi-GPU): `row_begin, row_end` = this rank's target rows; the
+    result then has n_rows = row_end - row_begin.  The threshold is a property of the WHOLE tensor: after
+    every selection pass `allreduce(hist)` must sum the 2,048-bin int64 device histogram over the ranks in
+    place (e.g. `lambda h: dist.all_reduce(h)`: 16 KB, the one exchange step of the build), so that every
+    rank fixes the same digit."""
     n = tiles.n
+    row_end = n if row_end is None else row_end
+    n_loc = row_end - row_begin
     dev = tiles.type.device
     tdt = torch_dtype(dtype)
     vec = 4 if dtype == MT_F32 else 2
     ld = (n + vec - 1) // vec * vec
     band = torch.empty(6 * band_rows * ld, dtype=tdt, device=dev)
-    bands = [(r0, min(n, r0 + band_rows)) for r0 in range(0, n, band_rows)]
+    bands = [(r0, min(row_end, r0 + band_rows)) for r0 in range(row_begin, row_end, band_rows)]
 
     def assemble(r0, r1):
         t = tiles._c()
@@ -453,24 +462,26 @@ def mt_sparse_build_streamed(ctx: Context, tiles: Tiles, dtype: int, fraction: f
             for r0, r1 in bands:
                 assemble(r0, r1)
                 ctx.check(ctx.lib.mt_select_accumulate(ctx.h, C.byref(st), _ptr(band, tdt), n, r1 - r0, ld, _ptr(hist)))
+            if allreduce is not None:
+                allreduce(hist)
             ctx.check(ctx.lib.mt_select_advance(ctx.h, C.byref(st), _ptr(hist)))
         tau = st.tau
-    row_ptr = torch.empty(6 * n + 1, dtype=torch.int64, device=dev)
+    row_ptr = torch.empty(6 * n_loc + 1, dtype=torch.int64, device=dev)
     for r0, r1 in bands:
         assemble(r0, r1)
-        ctx.check(ctx.lib.mt_sparse_count_band(ctx.h, _ptr(band, tdt), dtype, n, r1 - r0, ld, float(tau), r0, n,
-                                               _ptr(row_ptr)))
+        ctx.check(ctx.lib.mt_sparse_count_band(ctx.h, _ptr(band, tdt), dtype, n, r1 - r0, ld, float(tau),
+                                               r0 - row_begin, n_loc, _ptr(row_ptr)))
     nnz = C.c_int64()
-    ctx.check(ctx.lib.mt_sparse_scan(ctx.h, _ptr(row_ptr), n, C.byref(nnz)))
+    ctx.check(ctx.lib.mt_sparse_scan(ctx.h, _ptr(row_ptr), n_loc, C.byref(nnz)))
     nw = int(ctx.lib.mt_sparse_mask_words(n))
-    mask = torch.empty((6, n, nw), dtype=torch.int32, device=dev)
+    mask = torch.empty((6, n_loc, nw), dtype=torch.int32, device=dev)
     vals = torch.empty(max(1, nnz.value), dtype=tdt, device=dev)
     for r0, r1 in bands:
         assemble(r0, r1)
-        ctx.check(ctx.lib.mt_sparse_fill_band(ctx.h, _ptr(band, tdt), dtype, n, r1 - r0, ld, float(tau), r0, n,
-                                              _ptr(row_ptr), _ptr(mask), _ptr(vals)))
+        ctx.check(ctx.lib.mt_sparse_fill_band(ctx.h, _ptr(band, tdt), dtype, n, r1 - r0, ld, float(tau),
+                                              r0 - row_begin, n_loc, _ptr(row_ptr), _ptr(mask), _ptr(vals)))
     ctx.stream.synchronize()  # `band` is freed on return
-    return SparseTensor(n, n, dtype, nw, row_ptr, mask, vals, nnz=nnz.value, tau=float(tau))
+    return SparseTensor(n, n_loc, dtype, nw, row_ptr, mask, vals, nnz=nnz.value, tau=float(tau))
 
 
 def mt_sparse_index(ctx: Context, S: SparseTensor, drop_mask: bool = False) -> SparseTensor:

@@ -311,3 +311,67 @@ def test_index_rows_beyond_65536_columns(ctx, oracle):
     for b in range(2):
         assert H.rel_l2(Hb[b].cpu().numpy(), ref[b]) <= 1e-5
         assert H.rel_l2(Hi[b].cpu().numpy(), ref[b]) <= 1e-5
+
+
+def test_streamed_thresholding_row_sharded_with_histogram_allreduce(ctx, oracle):
+    """DESIGN.md section 9 on F1: two "ranks" (threads with their own mt_ctx and stream on this one GPU)
+    each build the thresholded rows of their half, exchanging only the selection histogram after every
+    pass (an in-place sum, what dist.all_reduce does).  Both fix the whole tensor's threshold, and their
+    bitmap rows / values / fields are the corresponding rows of the single-rank result."""
+    import threading
+    w = W.config5(13, 7, 3, batch=2)
+    n = w.n
+    tiles = H.dev_tiles(w)
+    whole = B.mt_sparse_build_streamed(ctx, tiles, B.MT_F32, 0.8, 64)
+    B.mt_sparse_index(ctx, whole)
+    m = torch.from_numpy(w.m).cuda()
+    Hw = torch.empty_like(m)
+    B.mt_demag_field_sparse(ctx, whole, tiles.Ms, m, 2, Hw)
+    torch.cuda.synchronize()
+    cut = 150
+    bounds = [(0, cut), (cut, n)]
+    barrier = threading.Barrier(2)
+    slots, parts, errors = [None, None], [None, None], []
+
+    def rank_main(rank):
+        try:
+            stream = torch.cuda.Stream()
+            with torch.cuda.stream(stream):
+                c = B.mt_create(0, stream)
+
+                def allreduce(hist):
+                    stream.synchronize()
+                    slots[rank] = hist.clone()
+                    barrier.wait()
+                    total = slots[0] + slots[1]
+                    barrier.wait()
+                    hist.copy_(total)
+
+                S = B.mt_sparse_build_streamed(c, tiles, B.MT_F32, 0.8, 40, row_begin=bounds[rank][0],
+                                               row_end=bounds[rank][1], allreduce=allreduce)
+                B.mt_sparse_index(c, S)
+                Hd = torch.empty((2, 3, S.n_rows), dtype=torch.float64, device="cuda")
+                B.mt_demag_field_sparse(c, S, tiles.Ms, m, 2, Hd)
+                stream.synchronize()
+                parts[rank] = (S, Hd)
+                c.close()
+        except Exception as exc:  # surfaced in the main thread
+            errors.append(exc)
+            barrier.abort()
+
+    threads = [threading.Thread(target=rank_main, args=(r,)) for r in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+    for rank, (r0, r1) in enumerate(bounds):
+        S, Hd = parts[rank]
+        assert S.tau == whole.tau and S.n_rows == r1 - r0
+        assert torch.equal(S.mask, whole.mask[:, r0:r1])
+        wp, sp = whole.row_ptr.cpu().numpy(), S.row_ptr.cpu().numpy()
+        for p in range(6):
+            a, b = wp[p * n + r0], wp[p * n + r1]
+            c0, c1 = sp[p * (r1 - r0)], sp[(p + 1) * (r1 - r0)]
+            assert b - a == c1 - c0 and torch.equal(whole.vals[a:b], S.vals[c0:c1])
+        assert torch.equal(Hd, Hw[:, :, r0:r1])   # same kernel, same rows, same order: bit-identical
