@@ -422,6 +422,25 @@ def main():
                     N = None
                     torch.cuda.synchronize()
                     torch.cuda.empty_cache()
+                    # the same config-5 thresholded tensor with the tiles listed along a Morton curve
+                    wm = W.reorder(w, W.morton_order(w))
+                    tm = H.dev_tiles(wm)
+                    Sm = B.mt_sparse_build_streamed(ctx, tm, code, 0.9, 4096)
+                    B.mt_sparse_index(ctx, Sm, drop_mask=True)
+                    mm = torch.from_numpy(wm.m[:1].copy()).to(dev)
+                    Hm = torch.empty_like(mm)
+
+                    def step_morton():
+                        B.mt_demag_field_sparse(ctx, Sm, tm.Ms, mm, 1, Hm)
+                    ms_mo, _, _ = timed(step_morton, 3, max(5, K // 2), tag="mo")
+                    perm_t = torch.from_numpy(wm.extra["perm"]).to(dev)
+                    out["threshold_0.9"]["morton_tile_order"] = {
+                        "ms": ms_mo, "kernel_ms": kernel_ms["mo"], "resident_bytes": Sm.nbytes(),
+                        "achieved_gbs": Sm.nbytes() / (kernel_ms["mo"] * 1e-3) / 1e9,
+                        "frac": Sm.nbytes() / (kernel_ms["mo"] * 1e-3) / 1e9 / peak,
+                        "rel_l2_vs_x_fastest_order": float(((Hm[0] - Hs[0][:, perm_t]).norm() / Hs.norm()).item()),
+                        "note": "same tiles, same threshold fraction, tiles listed along a Z-order curve (workloads.morton_order)"}
+                    del Sm
                     wb = W.config5(128, 64, 16, batch=1)
                     tb = H.dev_tiles(wb)
                     t7_, t8_ = ev(), ev()

@@ -11,6 +11,7 @@ ran them and stand in for them; no µmag solution da
 """
 from __future__ import annotations
 
+import dataclasses
 from dataclasses import dataclass, field
 
 import numpy as np
@@ -255,3 +256,48 @@ def leading_dim(n: int, dtype: str) -> int:
     """Row pitch in elements: rows 16-byte aligned (A3)."""
     v = 4 if dtype == "f32" else 2
     return (n + v - 1) // v * v
+
+
+def reorder(w: Workload, perm: np.ndarray) -> Workload:
+    """The same problem with tile k of the result = tile perm[k] of `w` (every per-tile array permuted,
+    neighbour indices renumbered).  Tile order is free in the method (`PAPER.md:124`: a list of tiles);
+    fields of the reordered problem are the permuted fields of the original."""
+    perm = np.asarray(perm, dtype=np.int64)
+    n = w.n
+    assert perm.shape == (n,) and np.array_equal(np.sort(perm), np.arange(n))
+    inv = np.empty(n, dtype=np.int64)
+    inv[perm] = np.arange(n)
+    nbr = None
+    if w.nbr is not None:
+        old = w.nbr[perm]
+        nbr = np.where(old >= 0, inv[np.maximum(old, 0)], -1).astype(w.nbr.dtype)
+    extra = dict(w.extra)
+    extra["perm"] = perm if "perm" not in w.extra else w.extra["perm"][perm]
+    return dataclasses.replace(
+        w, name=w.name + " (reordered)", type=np.ascontiguousarray(w.type[perm]),
+        center=np.ascontiguousarray(w.center[perm]), size=np.ascontiguousarray(w.size[perm]),
+        verts=np.ascontiguousarray(w.verts[perm]), Ms=np.ascontiguousarray(w.Ms[perm]),
+        vol=np.ascontiguousarray(w.vol[perm]), m=np.ascontiguousarray(w.m[:, :, perm]),
+        nbr=None if nbr is None else np.ascontiguousarray(nbr), grid=None, extra=extra)
+
+
+def morton_order(w: Workload, cell: float | None = None) -> np.ndarray:
+    """Permutation that sorts the tiles along a Z-order (Morton) curve through their centres (cell =
+    quantisation step, default the smallest tile edge).  Spatially close tiles get close indices, so the
+    kept entries of a thresholded tensor row (the near field, `PAPER.md:243`) form longer contiguous
+    column runs: the index-row kernel's gathers of M touch fewer lines."""
+    cell = float(w.size.min()) if cell is None else float(cell)
+    ijk = np.floor((w.center - w.center.min(axis=0)) / cell + 0.5).astype(np.uint64)
+    assert int(ijk.max()) < (1 << 21)
+
+    def spread(v):  # 21 bits -> every third bit
+        v = v & np.uint64(0x1FFFFF)
+        v = (v | (v << np.uint64(32))) & np.uint64(0x1F00000000FFFF)
+        v = (v | (v << np.uint64(16))) & np.uint64(0x1F0000FF0000FF)
+        v = (v | (v << np.uint64(8))) & np.uint64(0x100F00F00F00F00F)
+        v = (v | (v << np.uint64(4))) & np.uint64(0x10C30C30C30C30C3)
+        v = (v | (v << np.uint64(2))) & np.uint64(0x1249249249249249)
+        return v
+
+    code = spread(ijk[:, 0]) | (spread(ijk[:, 1]) << np.uint64(1)) | (spread(ijk[:, 2]) << np.uint64(2))
+    return np.argsort(code, kind="stable").astype(np.int64)

@@ -88,3 +88,39 @@ def test_sample_rows_and_leading_dim():
     assert r.dtype == np.int64 and len(r) >= 1024 and r[0] == 0 and r[-1] == 65535
     assert np.array_equal(r, W.sample_rows(5, 65536, 1024, extra=(0, 65535, 32768)))
     assert W.leading_dim(513, "f32") == 516 and W.leading_dim(513, "f64") == 514 and W.leading_dim(512, "f32") == 512
+
+
+def test_morton_order_and_reorder():
+    w = W.config3(4, batch=2)          # 4 x 4 x 4 cube with exchange neighbours
+    perm = W.morton_order(w)
+    assert np.array_equal(np.sort(perm), np.arange(w.n))
+    # the first eight tiles along the curve are the 2 x 2 x 2 block at the origin, x fastest, then y, then z
+    edge = w.size[0, 0]
+    first = np.rint((w.center[perm[:8]] - w.center.min(axis=0)) / edge).astype(int)
+    assert [tuple(c) for c in first] == [(0, 0, 0), (1, 0, 0), (0, 1, 0), (1, 1, 0), (0, 0, 1), (1, 0, 1), (0, 1, 1),
+                                         (1, 1, 1)]
+    r = W.reorder(w, perm)
+    assert r.grid is None and np.array_equal(r.center, w.center[perm]) and np.array_equal(r.m, w.m[:, :, perm])
+    # neighbour relation carried over: the neighbour of new tile k in direction d is the same physical tile
+    for k in range(w.n):
+        for d in range(6):
+            j_old = w.nbr[perm[k], d]
+            if j_old < 0:
+                assert r.nbr[k, d] == -1
+            else:
+                assert np.array_equal(r.center[r.nbr[k, d]], w.center[j_old])
+    # composing two reorderings records the composed permutation
+    rr = W.reorder(r, np.arange(w.n)[::-1].copy())
+    assert np.array_equal(rr.center, w.center[rr.extra["perm"]])
+
+
+def test_fields_of_a_reordered_problem_are_the_permuted_fields(oracle):
+    from tests import harness as H
+    w = W.config3(3, batch=2)
+    perm = W.morton_order(w)
+    r = W.reorder(w, perm)
+    N_w = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=True)
+    N_r = oracle.assemble_rows(H.oracle_tiles(oracle, r), long_double=True)
+    k_w, _ = oracle.llg_rhs(H.oracle_problem(oracle, w, N_w), w.m)
+    k_r, _ = oracle.llg_rhs(H.oracle_problem(oracle, r, N_r), r.m)
+    assert np.max(np.abs(k_r - k_w[:, :, perm])) <= 1e-13 * np.max(np.abs(k_w))
