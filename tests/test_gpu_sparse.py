@@ -375,3 +375,40 @@ def test_streamed_thresholding_row_sharded_with_histogram_allreduce(ctx, oracle)
             c0, c1 = sp[p * (r1 - r0)], sp[(p + 1) * (r1 - r0)]
             assert b - a == c1 - c0 and torch.equal(whole.vals[a:b], S.vals[c0:c1])
         assert torch.equal(Hd, Hw[:, :, r0:r1])   # same kernel, same rows, same order: bit-identical
+
+
+def test_morton_ordered_problem_through_the_device_path(ctx, oracle):
+    """Tiles listed along a Z-order curve (workloads.morton_order / reorder): the right-hand side with
+    exchange (renumbered neighbours), from the dense tensor and from index rows at a gap-placed 60 % cut,
+    against the oracle on the reordered problem."""
+    w0 = W.config3(6, batch=2)
+    w = W.reorder(w0, W.morton_order(w0))
+    n = w.n
+    tiles = H.dev_tiles(w)
+    N, ld, status = H.assemble(ctx, tiles, "f32")
+    assert status == 0
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=True)
+    prob = H.dev_problem(w, tiles, N, "f32", ld)
+    m = torch.from_numpy(w.m).cuda()
+    k = torch.empty_like(m)
+    B.mt_llg_rhs(ctx, prob, m, 2, k, None)
+    torch.cuda.synchronize()
+    k_ref, _ = oracle.llg_rhs(H.oracle_problem(oracle, w, N_ref), w.m)
+    for b in range(2):
+        assert H.rel_l2(k[b].cpu().numpy(), k_ref[b]) <= 1e-5
+    host = N_ref.astype(np.float32)
+    tau_dev, _ = B.mt_threshold_value(ctx, N, B.MT_F32, n, n, ld, 0.6)
+    mags = np.unique(np.abs(host[np.abs(host) > 0]).astype(np.float64))
+    gaps = np.nonzero(mags[1:] > mags[:-1] * 1.001)[0]
+    g = gaps[np.argmin(np.abs(np.log(mags[gaps] / tau_dev)))]
+    tau = float(np.float32(np.sqrt(mags[g] * mags[g + 1])))
+    S = B.mt_sparse_build_streamed(ctx, tiles, B.MT_F32, 0.6, 50, tau=tau)
+    B.mt_sparse_index(ctx, S, drop_mask=True)
+    prob.N = None
+    prob.N_sparse = S
+    B.mt_llg_rhs(ctx, prob, m, 2, k, None)
+    torch.cuda.synchronize()
+    trunc = OT.truncate(host, tau).astype(np.float64)
+    k_ref, _ = oracle.llg_rhs(H.oracle_problem(oracle, w, trunc), w.m)
+    for b in range(2):
+        assert H.rel_l2(k[b].cpu().numpy(), k_ref[b]) <= 1e-5
