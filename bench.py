@@ -425,8 +425,7 @@ def main():
                     # the same config-5 thresholded tensor with the tiles listed along a Morton curve
                     wm = W.reorder(w, W.morton_order(w))
                     tm = H.dev_tiles(wm)
-                    Sm = B.mt_sparse_build_streamed(ctx, tm, code, 0.9, 4096)
-                    B.mt_sparse_index(ctx, Sm, drop_mask=True)
+                    Sm = B.mt_sparse_build_streamed(ctx, tm, code, 0.9, 4096, index=True, keep_mask=False)
                     mm = torch.from_numpy(wm.m[:1].copy()).to(dev)
                     Hm = torch.empty_like(mm)
 
@@ -445,8 +444,8 @@ def main():
                     tb = H.dev_tiles(wb)
                     t7_, t8_ = ev(), ev()
                     t7_.record()
-                    Sb = B.mt_sparse_build_streamed(ctx, tb, code, 0.95, 4096)
-                    B.mt_sparse_index(ctx, Sb, drop_mask=True)
+                    torch.cuda.reset_peak_memory_stats()
+                    Sb = B.mt_sparse_build_streamed(ctx, tb, code, 0.95, 4096, index=True, keep_mask=False)
                     t8_.record()
                     mb = torch.from_numpy(wb.m[:1].copy()).to(dev)
                     Hb = torch.empty_like(mb)
@@ -460,6 +459,7 @@ def main():
                         "kept_entries": Sb.nnz, "tau": Sb.tau, "build_ms": t7_.elapsed_time(t8_),
                         "achieved_gbs": Sb.nbytes() / (kernel_ms["big"] * 1e-3) / 1e9,
                         "frac": Sb.nbytes() / (kernel_ms["big"] * 1e-3) / 1e9 / peak,
+                        "peak_allocated_bytes": int(torch.cuda.max_memory_allocated()),
                         "finite": bool(torch.isfinite(Hb).all().item()),
                         "note": "dense tensor (412 GB) cannot be resident; thresholded tensor built band by band"}
                     del Sb

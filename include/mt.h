@@ -199,6 +199,14 @@ int mt_sparse_fill_band(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_
                         double tau, int64_t row0, int64_t n_total, const int64_t* row_ptr,
                         uint32_t* mask, void* vals);
 
+/* mt_sparse_fill_band that also (cols16 non-NULL) writes the index rows in the same pass — cols16 and
+ * panel_ptr exactly as mt_sparse_index would derive them from the bitmap — and may then leave the
+ * bitmap out (mask NULL): the thresholded tensor is held as values + 16-bit columns only.            */
+int mt_sparse_fill_index_band(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows,
+                              int64_t ld, double tau, int64_t row0, int64_t n_total,
+                              const int64_t* row_ptr, uint32_t* mask, void* vals, uint16_t* cols16,
+                              int64_t* panel_ptr);
+
 /* Compression, two calls: mt_sparse_count fills row_ptr (DEVICE, [6*n_rows+1]) for threshold tau and
  * returns the number of kept entries in *nnz_host (synchronises); the caller allocates mask
  * ([6*n_rows*nw] uint32) and vals ([nnz] of dtype), then mt_sparse_fill writes them (asynchronous).

@@ -27,7 +27,7 @@ EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assembl
            "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_energy",
            "mt_field_sweep", "mt_sparse_mask_words", "mt_threshold_value", "mt_sparse_count",
            "mt_sparse_fill", "mt_sparse_index", "mt_select_begin", "mt_select_accumulate", "mt_select_advance",
-           "mt_sparse_count_band", "mt_sparse_scan", "mt_sparse_fill_band", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
+           "mt_sparse_count_band", "mt_sparse_scan", "mt_sparse_fill_band", "mt_sparse_fill_index_band", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
            "mt_demag_field_sym", "mt_set_assembly_mode", "mt_launch_count",
            "mt_set_demag_variant", "mt_profile_begin", "mt_profile_end")
 
@@ -131,6 +131,9 @@ def load() -> C.CDLL:
         lib.mt_sparse_scan.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
         lib.mt_sparse_fill_band.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64,
                                             C.c_double, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p]
+        lib.mt_sparse_fill_index_band.argtypes = [C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64, C.c_int64,
+                                                  C.c_double, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
+                                                  C.c_void_p, C.c_void_p, C.c_void_p]
         lib.mt_sparse_index.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p, C.c_void_p]
         lib.mt_demag_field_sparse.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p, C.c_void_p, C.c_int,
                                               C.c_void_p]
@@ -427,7 +430,8 @@ def mt_sparse_build(ctx: Context, N: torch.Tensor, dtype: int, n: int, n_rows: i
 
 def mt_sparse_build_streamed(ctx: Context, tiles: Tiles, dtype: int, fraction: float, band_rows: int,
                              status_flag: torch.Tensor | None = None, tau: float | None = None,
-                             row_begin: int = 0, row_end: int | None = None, allreduce=None) -> SparseTensor:
+                             row_begin: int = 0, row_end: int | None = None, allreduce=None,
+                             index: bool = False, keep_mask: bool = True) -> SparseTensor:
     """Thresholded tensor of `tiles` without ever holding the dense tensor: every pass (one per radix
     digit of the selection, one for the counts, one for the fill) assembles the tensor again band by
     band into one [6, band_rows, ld] buffer.  Sequence of C-ABI calls only: mt_assemble_tensor,
@@ -438,7 +442,12 @@ def mt_sparse_build_streamed(ctx: Context, tiles: Tiles, dtype: int, fraction: f
     result then has n_rows = row_end - row_begin.  The threshold is a property of the WHOLE tensor: after
     every selection pass `allreduce(hist)` must sum the 2,048-bin int64 device histogram over the ranks in
     place (e.g. `lambda h: dist.all_reduce(h)`: 16 KB, the one exchange step of the build), so that every
-    rank fixes the same digit."""
+    rank fixes the same digit.
+
+    `index=True`: the fill pass writes the index rows (16-bit columns, panel offsets) as well;
+    `keep_mask=False` then leaves the bitmap out altogether (values + columns only)."""
+    if not index and not keep_mask:
+        raise ValueError("keep_mask=False needs index=True")
     n = tiles.n
     row_end = n if row_end is None else row_end
     n_loc = row_end - row_begin
@@ -474,14 +483,19 @@ def mt_sparse_build_streamed(ctx: Context, tiles: Tiles, dtype: int, fraction: f
     nnz = C.c_int64()
     ctx.check(ctx.lib.mt_sparse_scan(ctx.h, _ptr(row_ptr), n_loc, C.byref(nnz)))
     nw = int(ctx.lib.mt_sparse_mask_words(n))
-    mask = torch.empty((6, n_loc, nw), dtype=torch.int32, device=dev)
+    mask = torch.empty((6, n_loc, nw), dtype=torch.int32, device=dev) if keep_mask else None
     vals = torch.empty(max(1, nnz.value), dtype=tdt, device=dev)
+    panels = (n + 65535) // 65536
+    cols = torch.empty(max(1, nnz.value), dtype=torch.uint16, device=dev) if index else None
+    pp = torch.empty((6 * n_loc, panels - 1), dtype=torch.int64, device=dev) if index and panels > 1 else None
     for r0, r1 in bands:
         assemble(r0, r1)
-        ctx.check(ctx.lib.mt_sparse_fill_band(ctx.h, _ptr(band, tdt), dtype, n, r1 - r0, ld, float(tau),
-                                              r0 - row_begin, n_loc, _ptr(row_ptr), _ptr(mask), _ptr(vals)))
+        ctx.check(ctx.lib.mt_sparse_fill_index_band(ctx.h, _ptr(band, tdt), dtype, n, r1 - r0, ld, float(tau),
+                                                    r0 - row_begin, n_loc, _ptr(row_ptr), _ptr(mask), _ptr(vals),
+                                                    _ptr(cols), _ptr(pp)))
     ctx.stream.synchronize()  # `band` is freed on return
-    return SparseTensor(n, n_loc, dtype, nw, row_ptr, mask, vals, nnz=nnz.value, tau=float(tau))
+    return SparseTensor(n, n_loc, dtype, nw, row_ptr, mask, vals, nnz=nnz.value, tau=float(tau), cols16=cols,
+                        panel_ptr=pp)
 
 
 def mt_sparse_index(ctx: Context, S: SparseTensor, drop_mask: bool = False) -> SparseTensor:

@@ -478,16 +478,26 @@ int mt_sparse_scan(mt_ctx* ctx, int64_t* row_ptr, int64_t n_total, int64_t* nnz_
   return MT_OK;
 }
 
-int mt_sparse_fill_band(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
-                        int64_t row0, int64_t n_total, const int64_t* row_ptr, uint32_t* mask, void* vals) {
+int mt_sparse_fill_index_band(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
+                              int64_t row0, int64_t n_total, const int64_t* row_ptr, uint32_t* mask, void* vals,
+                              uint16_t* cols16, int64_t* panel_ptr) {
   if (!ctx) return MT_ERR_INVALID_ARG;
   int rc = check_tensor_args(ctx, N, dtype, n, n_rows, ld);
   if (rc) return rc;
-  if (!row_ptr || !mask) return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and mask must be non-NULL");
+  if (!row_ptr || (!mask && !cols16)) return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and one of mask / cols16 must be non-NULL");
+  if (cols16 && n > 65536 && !panel_ptr)
+    return mt_fail(ctx, MT_ERR_INVALID_ARG, "n > 65536: panel_ptr must be non-NULL with cols16");
   if (row0 < 0 || row0 + n_rows > n_total) return mt_fail(ctx, MT_ERR_INVALID_ARG, "band outside [0, n_total)");
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
   return mt_launch_sparse_fill(ctx, N, dtype, n, n_rows, ld, tau, row0, n_total, row_ptr, mt_sparse_mask_words(n), mask,
-                               vals);
+                               vals, cols16, panel_ptr);
+}
+
+int mt_sparse_fill_band(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
+                        int64_t row0, int64_t n_total, const int64_t* row_ptr, uint32_t* mask, void* vals) {
+  if (ctx && !mask) return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr and mask must be non-NULL");
+  return mt_sparse_fill_index_band(ctx, N, dtype, n, n_rows, ld, tau, row0, n_total, row_ptr, mask, vals, nullptr,
+                                   nullptr);
 }
 
 int mt_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,

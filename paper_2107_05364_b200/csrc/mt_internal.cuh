@@ -134,7 +134,7 @@ int mt_launch_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int
 int mt_launch_sparse_scan(mt_ctx* ctx, int64_t* row_ptr, int64_t n_total);
 int mt_launch_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
                           int64_t row0, int64_t n_total, const int64_t* row_ptr, int64_t nw, uint32_t* mask,
-                          void* vals);
+                          void* vals, uint16_t* cols16, int64_t* panel_ptr);
 int mt_launch_sparse_index(mt_ctx* ctx, const mt_sparse_tensor* s, uint16_t* cols16, int64_t* panel_ptr);
 int mt_launch_demag_sparse(mt_ctx* ctx, const mt_sparse_tensor* s, const void* Mst, int64_t npad, const EpiArgs& epi);
 // pair-symmetric half (assemble.cu, sym.cu)

@@ -182,21 +182,29 @@ __global__ void __launch_bounds__(1024) scan_kernel(int64_t* __restrict__ a, int
 }
 
 // mask[(plane * n_rows + i) * nw + c] bit l = entry (i, 32 c + l) kept; kept values packed from
-// vals[row_ptr[plane * n_rows + i]] in column order.  One warp per (plane, row).
+// vals[row_ptr[plane * n_rows + i]] in column order.  One warp per (plane, row).  Optionally (cols
+// non-NULL) the index rows are written in the same pass — 16-bit column of every packed value and the
+// panel offsets, exactly what sparse_index_kernel derives from the bitmap — and the bitmap itself may
+// then be left out (mask NULL).
 template <typename T>
 __global__ void __launch_bounds__(256) sparse_fill_kernel(const T* __restrict__ N, int64_t n, int64_t n_rows,
                                                           int64_t ld, T tau, int64_t row0, int64_t n_total,
                                                           const int64_t* __restrict__ row_ptr, int64_t nw,
-                                                          uint32_t* __restrict__ mask, T* __restrict__ vals) {
+                                                          uint32_t* __restrict__ mask, T* __restrict__ vals,
+                                                          uint16_t* __restrict__ cols,
+                                                          int64_t* __restrict__ panel_ptr, int npanels) {
   const int64_t r = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
   if (r >= 6 * n_rows) return;
   const int64_t R = (r / n_rows) * n_total + row0 + r % n_rows;  // row of the whole tensor (see count)
   const T* row = N + r * ld;
-  uint32_t* mrow = mask + R * nw;
-  T* out = vals + row_ptr[R];
+  uint32_t* mrow = mask ? mask + R * nw : nullptr;
+  const int64_t base = row_ptr[R];
+  T* out = vals + base;
+  uint16_t* cout = cols ? cols + base : nullptr;
   int64_t off = 0;
   for (int64_t c0 = 0; c0 < nw; c0 += 4) {  // nw is a multiple of 4; four chunks loaded before any is packed
+    if (cout && c0 && (c0 & 2047) == 0 && lane == 0) panel_ptr[R * (npanels - 1) + (c0 >> 11) - 1] = base + off;
     T v[4];
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
@@ -207,8 +215,12 @@ __global__ void __launch_bounds__(256) sparse_fill_kernel(const T* __restrict__ 
     for (int u = 0; u < 4; ++u) {
       const bool k = kept(v[u], tau);
       const uint32_t word = __ballot_sync(0xffffffffu, k);
-      if (k) out[off + __popc(word & ((1u << lane) - 1u))] = v[u];
-      if (lane == 0) mrow[c0 + u] = word;
+      if (k) {
+        const int64_t at = off + __popc(word & ((1u << lane) - 1u));
+        out[at] = v[u];
+        if (cout) cout[at] = (uint16_t)((c0 + u) * 32 + lane);
+      }
+      if (mrow && lane == 0) mrow[c0 + u] = word;
       off += __popc(word);
     }
   }
@@ -619,14 +631,16 @@ int mt_launch_sparse_scan(mt_ctx* ctx, int64_t* row_ptr, int64_t n_total) {
 
 int mt_launch_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
                           int64_t row0, int64_t n_total, const int64_t* row_ptr, int64_t nw, uint32_t* mask,
-                          void* vals) {
+                          void* vals, uint16_t* cols16, int64_t* panel_ptr) {
   const unsigned grid = (unsigned)((6 * n_rows + 7) / 8);
+  const int npanels = (int)((n + 65535) >> 16);
   if (dtype == MT_F32)
     sparse_fill_kernel<float><<<grid, 256, 0, ctx->stream>>>((const float*)N, n, n_rows, ld, (float)tau, row0, n_total,
-                                                             row_ptr, nw, mask, (float*)vals);
+                                                             row_ptr, nw, mask, (float*)vals, cols16, panel_ptr, npanels);
   else
     sparse_fill_kernel<double><<<grid, 256, 0, ctx->stream>>>((const double*)N, n, n_rows, ld, tau, row0, n_total,
-                                                              row_ptr, nw, mask, (double*)vals);
+                                                              row_ptr, nw, mask, (double*)vals, cols16, panel_ptr,
+                                                              npanels);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   return MT_OK;

@@ -415,6 +415,11 @@ def test_beyond_hbm_size_thresholded_streamed(ctx, oracle):
     torch.cuda.synchronize()
     trunc = OT.truncate(host, tau)
     check_sparse_rows(S, rows, N_ref, trunc, n)
+    # index rows written by the fill pass itself (no bitmap held): the same columns, panel offsets, values
+    U = B.mt_sparse_build_streamed(ctx, tiles, B.MT_F32, 0.95, 4096, status, tau=tau, index=True, keep_mask=False)
+    assert U.mask is None and torch.equal(U.row_ptr, S.row_ptr) and torch.equal(U.vals, S.vals)
+    assert torch.equal(U.cols16, S.cols16) and torch.equal(U.panel_ptr, S.panel_ptr)
+    del U
     m = torch.from_numpy(w.m).cuda()
     Hb, Hi = torch.empty_like(m), torch.empty_like(m)
     cols = S.cols16

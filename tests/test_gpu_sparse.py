@@ -250,6 +250,13 @@ def test_streamed_thresholding_equals_the_resident_path_and_the_oracle(ctx, orac
         assert torch.equal(T.row_ptr, S.row_ptr) and torch.equal(T.mask, S.mask)
         if S.nnz:
             assert torch.equal(T.vals, S.vals)
+        # index rows written by the fill pass itself (bitmap left out) = those derived from the bitmap
+        B.mt_sparse_index(ctx, S)
+        U = B.mt_sparse_build_streamed(ctx, tiles, code, X, band_rows, index=True, keep_mask=False)
+        torch.cuda.synchronize()
+        assert U.mask is None and U.nnz == S.nnz and torch.equal(U.row_ptr, S.row_ptr)
+        if S.nnz:
+            assert torch.equal(U.vals, S.vals) and torch.equal(U.cols16, S.cols16)
     # against the oracle: cut in a gap of the oracle's magnitudes next to the device's 60 % value
     N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=True)
     host = N_ref.astype(np.float32 if dtype == "f32" else np.float64)
