@@ -136,8 +136,9 @@ int mt_demag_field_host(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_
  * Optional second index ("index rows"): cols16[k] = source column of vals[k] modulo 65536, written by
  * mt_sparse_index from the bitmap; for n > 65536 the columns fall in panels of 65,536 and
  * panel_ptr[(c*n_rows + i)*(P-1) + q-1] (P = ceil(n/65536)) is the offset into vals at which panel
- * q >= 1 of plane row (c, i) starts (a row's entries are in column order, so a panel is one run).  When cols16 is non-NULL the field kernel walks the packed values
- * (coalesced value + 16-bit column loads, gathered M) instead of decoding the bitmap column by column:
+ * q >= 1 of plane row (c, i) starts (a row's entries are in column order, so a panel is one run).
+ * When cols16 is non-NULL the field kernel walks the packed values (coalesced value + 16-bit column
+ * loads, gathered M) instead of decoding the bitmap column by column, and mask may be NULL:
  * 6 bytes per kept fp32 entry instead of 4 + 1/8 per DENSE entry, i.e. smaller than the bitmap from
  * X ~ 0.94 and a far cheaper decode at any X.                                 */
 typedef struct {
@@ -170,8 +171,10 @@ int mt_threshold_value(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t
  * row band of the tensor (any order, any band height: each band is assembled again per pass with
  * mt_assemble_tensor), then one mt_select_advance.  Repeat until st->done; st->tau, st->count then
  * equal what mt_threshold_value returns for the whole tensor (integer histograms: exact).
- * hist: DEVICE array of 2048 unsigned 64-bit counters owned by the caller.  mt_select_begin and
- * mt_select_accumulate are asynchronous; mt_select_advance synchronises the stream.                */
+ * hist: DEVICE array of 2048 unsigned 64-bit counters owned by the caller (row-sharded over several
+ * GPUs: sum it over the ranks before mt_select_advance).  mt_select_begin and mt_select_accumulate
+ * are asynchronous; mt_select_advance synchronises the stream.  Errors: MT_ERR_INVALID_ARG (NULL
+ * state / hist, fraction outside [0, 1], bad tensor arguments, accumulate after done), MT_ERR_CUDA. */
 typedef struct {
   int dtype;
   double fraction;
@@ -191,7 +194,8 @@ int mt_select_advance(mt_ctx* ctx, mt_select_state* st, unsigned long long* hist
  * mt_sparse_scan turns the counts into row_ptr in place and returns the number of kept entries
  * (synchronises); mt_sparse_fill_band writes the band's bitmap rows and packed values at their
  * places in the whole tensor's mask / vals (asynchronous).  mt_sparse_count / mt_sparse_fill are the
- * single-band case (row0 = 0, n_total = n_rows).                                                   */
+ * single-band case (row0 = 0, n_total = n_rows).  Errors: MT_ERR_INVALID_ARG (NULL pointers, band
+ * outside [0, n_total), bad tensor arguments), MT_ERR_CUDA.                                         */
 int mt_sparse_count_band(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
                          double tau, int64_t row0, int64_t n_total, int64_t* counts);
 int mt_sparse_scan(mt_ctx* ctx, int64_t* row_ptr, int64_t n_total, int64_t* nnz_host);
