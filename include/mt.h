@@ -316,15 +316,23 @@ typedef struct {
 
 typedef struct {
   int64_t accepted, rejected, rhs_calls, n_samples;
-  double t, dt_last, max_torque;
+  double t, dt_last;
+  double max_torque;     /* max_i |m_i x H_eff,i| of the last evaluation that measured it.  RK4 with
+                            torque_tol > 0: at the state the last examined step STARTED from (the
+                            stop test runs before a step is taken; the state returned at t_end has
+                            not been tested); RK4 with torque_tol <= 0: 0 (not measured).  DP45: at
+                            the stage-7 state of the last accepted step, before its renormalisation
+                            (Q10b)                                                        */
 } mt_integrator_result;
 
 /* Advance m_inout[batch][3][n] (DEVICE) from *t_inout (HOST) towards opts->t_end.  All states of
  * the batch share the step sequence.  samples (DEVICE, may be NULL) is [sample_cap][1+3*batch]:
  * t, then <m_x>,<m_y>,<m_z> per state.  host_out (HOST) receives the counters.  Synchronises the
  * stream before returning.  Resumable: (m, t, dt_last) is the whole state.
- * Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA, MT_ERR_STEP_UNDERFLOW, MT_ERR_MAX_STEPS (the state
- * reached so far is still written back).                                                          */
+ * Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA, MT_ERR_STEP_UNDERFLOW (DP45: the step fell below
+ * 16 eps max(|t|, |t_end|), or the error estimate is not finite — a NaN/inf in the state or in the
+ * tensor reaches it, Q11b), MT_ERR_MAX_STEPS (the state reached so far is still written
+ * back).  A tile with m_i = 0 stays at zero under renormalisation (Q10c).                */
 int mt_integrate(mt_ctx* ctx, const mt_problem* prob, const mt_integrator_opts* opts,
                  double* m_inout, int batch, double* t_inout, double* samples, int64_t sample_cap,
                  mt_integrator_result* host_out);

@@ -587,7 +587,7 @@ int mt_field_sweep(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o
   for (int64_t f = 0; f < n_fields; ++f) {
     for (int a = 0; a < 3; ++a) pk.H_a_const[a] = fields_host[3 * f + a];
     double t = 0.0;
-    mt_integrator_result r;
+    mt_integrator_result r = {};
     rc = mt_integrate(ctx, &pk, o, m, batch, &t, nullptr, 0, &r);
     total.accepted += r.accepted; total.rejected += r.rejected; total.rhs_calls += r.rhs_calls;
     total.t += r.t; total.dt_last = r.dt_last; total.max_torque = r.max_torque;
@@ -855,6 +855,12 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       res->rhs_calls += 6;
       const double err = bits_to_double(ctx->hscal[0]);
       const double tq7 = bits_to_double(ctx->hscal[1]);
+      if (!(err == err) || err > 1.79e308) {  // NaN/inf state or slope: no step size can repair it (Q11b)
+        res->rejected++;
+        status = MT_ERR_STEP_UNDERFLOW;
+        mt_fail(ctx, status, "non-finite error estimate at t = %g", t);
+        break;
+      }
       double fac = err > 0 ? 0.9 * pow(err, -0.2) : 5.0;
       fac = fmin(5.0, fmax(0.2, fac));
       if (err <= 1.0) {
@@ -875,7 +881,6 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       } else {
         res->rejected++;
         dt = h * fmin(1.0, fac);
-        if (!(err == err)) { status = MT_ERR_STEP_UNDERFLOW; mt_fail(ctx, status, "non-finite error estimate"); break; }
       }
     }
   }

@@ -30,6 +30,7 @@
 namespace {
 
 constexpr int kConsumerWarps = 8;
+constexpr int kMaxDevices = 64;  // device ordinals tracked by the per-device attribute flags (power of two)
 // shape of the packed-FMA batched kernel (see demag_tma_f32x2_kernel)
 #ifndef MT_B8_WARPS
 #define MT_B8_WARPS 8   /* measured at N = 32,768, B = 8 (r01): 8/128/3 4.55 ms; 12/64/4 5.04; 8/64/6 6.2 */
@@ -555,7 +556,7 @@ int make_map(mt_ctx* ctx, CUtensorMap* out, int dtype, const void* base, int ran
 
 // Cfg = tile geometry; kern = the kernel instantiated for it; m_rows = rows of the staged-M box (3 B)
 template <typename T, typename Cfg, typename Kern>
-int launch_tiles(mt_ctx* ctx, Kern kern, bool* attr_set, int m_rows, const void* N, int dtype, int64_t n,
+int launch_tiles(mt_ctx* ctx, Kern kern, unsigned char* attr_set, int m_rows, const void* N, int dtype, int64_t n,
                  int64_t n_rows, int64_t ld, const void* Mst, int64_t npad, const EpiArgs& e) {
   constexpr int RT = Cfg::RT;
   static_assert(Cfg::smem_bytes <= 227 * 1024, "ring does not fit shared memory");
@@ -583,9 +584,12 @@ int launch_tiles(mt_ctx* ctx, Kern kern, bool* attr_set, int m_rows, const void*
     const uint32_t box[2] = {(uint32_t)Cfg::CT, (uint32_t)m_rows};
     if ((rc = make_map(ctx, &tmM, dtype, Mst, 2, dims, strides, box))) return rc;
   }
-  if (!*attr_set) {
+  // the attribute is per DEVICE (a second mt_ctx on another device of the same process needs its own
+  // call): one flag per device ordinal and kernel instantiation
+  const int dev = ctx->device & (kMaxDevices - 1);
+  if (!attr_set[dev]) {
     MT_CUDA_OK(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::smem_bytes));
-    *attr_set = true;
+    attr_set[dev] = 1;
   }
   kern<<<(unsigned)P, Cfg::WARPS * 32, Cfg::smem_bytes, ctx->stream>>>(tmN, tmM, a, e);
   ctx->launches++;
@@ -600,8 +604,8 @@ int launch_tiles(mt_ctx* ctx, Kern kern, bool* attr_set, int m_rows, const void*
 template <typename T, int B, int RW, int CT, int STAGES>
 int launch_cfg(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
                int64_t npad, const EpiArgs& e) {
-  static bool attr_set = false;
-  return launch_tiles<T, TmaCfg<T, B, RW, CT, STAGES>>(ctx, demag_tma_kernel<T, B, RW, CT, STAGES>, &attr_set, 3 * B,
+  static unsigned char attr_set[kMaxDevices] = {};
+  return launch_tiles<T, TmaCfg<T, B, RW, CT, STAGES>>(ctx, demag_tma_kernel<T, B, RW, CT, STAGES>, attr_set, 3 * B,
                                                         N, dtype, n, n_rows, ld, Mst, npad, e);
 }
 
@@ -610,9 +614,9 @@ int launch_cfg(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows,
 template <int B, int WARPS, int CT, int STAGES>
 int launch_f32x2_shape(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
                        int64_t npad, const EpiArgs& e) {
-  static bool attr_set = false;
+  static unsigned char attr_set[kMaxDevices] = {};
   return launch_tiles<float, TmaCfg<float, B, kPackRW, CT, STAGES, WARPS>>(
-      ctx, demag_tma_f32x2_kernel<B, WARPS, CT, STAGES>, &attr_set, 3 * B, N, MT_F32, n, n_rows, ld, Mst, npad, e);
+      ctx, demag_tma_f32x2_kernel<B, WARPS, CT, STAGES>, attr_set, 3 * B, N, MT_F32, n, n_rows, ld, Mst, npad, e);
 }
 
 // fp32, 3 <= batch <= 8: packed-FMA kernels for 4 or 8 states (states beyond `batch` are computed on

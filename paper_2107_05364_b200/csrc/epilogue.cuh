@@ -6,7 +6,8 @@
 
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* p, double v) {
   // bit patterns of non-negative doubles order like unsigned integers; NaN (all-ones exponent with
-  // mantissa) compares above every finite value, so a NaN is never lost.
+  // mantissa, either sign) compares above every finite value, so a NaN handed to this function is
+  // never lost — callers must not launder it through fmax() first (fmax drops NaN operands).
   atomicMax(p, (unsigned long long)__double_as_longlong(v));
 }
 
@@ -32,9 +33,12 @@ __device__ __forceinline__ void stage_combine(const EpiArgs& e, int64_t i, int b
     yo[a] = e.base[sb + a * n + i] + e.h * s;
   }
   if (e.renorm) {
+    // a zero-length m_i (a non-magnetic tile) stays zero instead of becoming 0/0 (Q10c)
     const double r = sqrt(yo[0] * yo[0] + yo[1] * yo[1] + yo[2] * yo[2]);
+    if (r > 0.0) {
 #pragma unroll
-    for (int a = 0; a < 3; ++a) yo[a] /= r;
+      for (int a = 0; a < 3; ++a) yo[a] /= r;
+    }
   }
   double* yout = e.y_out + sb;
 #pragma unroll
@@ -143,7 +147,8 @@ __device__ __forceinline__ void row_epilogue(const EpiArgs& e, int64_t i, int b,
       }
       s *= e.h;
       const double sc = e.atol + e.rtol * fmax(fabs(e.ebase[sb + a * n + i]), fabs(mi[a]));
-      err = fmax(err, fabs(s) / sc);
+      const double q = fabs(s) / sc;
+      err = (q > err || q != q) ? q : err;  // a NaN must reach the controller (Q11b)
     }
     atomic_max_nonneg(e.err_bits, err);
   }

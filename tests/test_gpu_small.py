@@ -310,3 +310,23 @@ def test_batched_rk4_equals_individual_runs(ctx, oracle):
                                          sample_every=10, sample_cap=8)
         assert np.array_equal(m1[0], mb[b])
         assert np.array_equal(s1[:, 1:4], sb[:, 1 + 3 * b:4 + 3 * b])
+
+
+def test_dp45_nonfinite_state_is_an_error_and_zero_m_stays_zero(ctx):
+    """a NaN in m must reach the DP45 error estimate (no fmax laundering) and end the run
+    with MT_ERR_STEP_UNDERFLOW instead of MT_OK with a NaN state; m_i = 0 is a fixed point (Q10c, Q11b)."""
+    n = 3
+    Ms = torch.ones(n, dtype=torch.float64, device="cuda")
+    prob = B.Problem(n=n, Ms=Ms, H_a=(0.0, 0.0, 1.0), gamma=1.0, alpha_ll=0.5)
+    m0 = np.array([[[1.0, 0.0, 0.6], [0.0, 1.0, 0.0], [0.0, 0.0, 0.8]]])
+    bad = m0.copy()
+    bad[0, 1, 2] = np.nan
+    _, _, res, rc = run_gpu_integrate(ctx, prob, bad, 1, method=B.MT_DP45, dt=1e-2, t_end=1.0, max_steps=50,
+                                      allow=(B.MT_ERR_STEP_UNDERFLOW,))
+    assert rc == B.MT_ERR_STEP_UNDERFLOW and res["accepted"] == 0
+    zero = m0.copy()
+    zero[0, :, 1] = 0.0
+    for method in (B.MT_RK4, B.MT_DP45):
+        m, _, res, rc = run_gpu_integrate(ctx, prob, zero, 1, method=method, dt=1e-2, t_end=0.5)
+        assert rc == 0 and np.all(m[0][:, 1] == 0.0) and np.all(np.isfinite(m))
+        assert np.allclose(np.linalg.norm(m[0][:, [0, 2]], axis=0), 1.0, atol=1e-14)

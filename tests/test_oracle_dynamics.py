@@ -213,3 +213,23 @@ def test_torque_stop(oracle):
     assert res["max_torque"] <= 1e-5 and res["t"] < 100.0
     # |m x H| = sech(t): the stop time is acosh(1e5) up to one step
     assert abs(res["t"] - np.arccosh(1e5)) < 2.0
+
+
+# ---- readings Q10c / Q11b: behaviour at the edge of the domain --------------------------
+def test_dp45_nonfinite_state_ends_the_run_and_zero_m_stays_zero(oracle):
+    """A NaN in the state reaches the error estimate (it is not dropped by a max) and ends the run
+    with the step-underflow status instead of being 'accepted' with err = 0; a zero-length m_i is a
+    fixed point (no 0/0 on renormalisation)."""
+    n = 3
+    prob = oracle.Problem(n=n, Ms=np.ones(n), N=None, gamma=1.0, alpha_ll=0.5, H_a=(0.0, 0.0, 1.0))
+    m0 = np.array([[1.0, 0.0, 0.6], [0.0, 1.0, 0.0], [0.0, 0.0, 0.8]])
+    bad = m0.copy()
+    bad[1, 2] = np.nan
+    _, _, res = oracle.integrate(prob, bad, method=oracle.DP45, dt=1e-2, t_end=1.0, max_steps=50)
+    assert res["status"] == -4 and res["accepted"] == 0
+    zero = m0.copy()
+    zero[:, 1] = 0.0
+    for method in (oracle.RK4, oracle.DP45):
+        m, _, res = oracle.integrate(prob, zero, method=method, dt=1e-2, t_end=0.5)
+        assert res["status"] == 0 and np.all(m[:, 1] == 0.0) and np.all(np.isfinite(m))
+        assert np.allclose(np.linalg.norm(m[:, [0, 2]], axis=0), 1.0, atol=1e-14)
