@@ -379,8 +379,28 @@ int64_t mt_launch_count(const mt_ctx* ctx);
 int mt_profile_begin(mt_ctx* ctx);
 int mt_profile_end(mt_ctx* ctx, double* total_ms, int64_t* launches);
 
+/* Roofline denominators measured in place (bench.py; north_star: "assembly tile-pairs/s against
+ * FP64/FP32 pipe peak", "achieved HBM GB/s against B200 peak").  Runs a microbenchmark kernel on the
+ * ctx's stream four times (first = warm-up) and returns the best of the other three:
+ *   out_host[0] = rate, out_host[1] = the kernel's duration in ms (HOST array of 2 doubles).
+ *   MT_PEAK_DFMA      FP64 fused multiply-adds, thread-instructions per second, all SMs
+ *   MT_PEAK_FFMA      FP32 fused multiply-adds (three-register FFMA), thread-instructions per second
+ *   MT_PEAK_FFMA2     packed fma.rn.f32x2, thread-instructions per second (each = 2 FMAs)
+ *   MT_PEAK_MMA_TF32  warp-level mma.sync m16n8k8 tf32 (fp32 accumulate), multiply-adds per second
+ *   MT_PEAK_HBM_READ  read-only stream of buf[0..bytes) (DEVICE, 16-byte aligned, >= 32 KB per SM,
+ *                     should exceed the L2 several times) by 1-D bulk copies into shared memory,
+ *                     bytes per second; buf/bytes are ignored by the other kinds.
+ * Synchronous.  Not part of the compute path.  Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA.            */
+#define MT_PEAK_DFMA 0
+#define MT_PEAK_FFMA 1
+#define MT_PEAK_FFMA2 2
+#define MT_PEAK_MMA_TF32 3
+#define MT_PEAK_HBM_READ 4
+int mt_measure_peak(mt_ctx* ctx, int kind, const void* buf, int64_t bytes, double* out_host);
+
 /* Tuning / A-B testing hook: selects the demag kernel variant (0 = default choice by shape,
- * 1 = register-streaming LDG kernel, 2 = TMA bulk-tensor pipeline).  Returns MT_OK or
+ * 1 = register-streaming LDG kernel, 2 = TMA bulk-tensor pipeline, 3 = as 2 but batches of 5..8
+ * states on fp32 tensors use the packed-FFMA2 kernel instead of the tensor-core one).  Returns MT_OK or
  * MT_ERR_INVALID_ARG.  Results of all variants agree to rounding; each is deterministic.          */
 int mt_set_demag_variant(mt_ctx* ctx, int variant);
 

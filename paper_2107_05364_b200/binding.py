@@ -29,7 +29,7 @@ EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assembl
            "mt_sparse_fill", "mt_sparse_index", "mt_select_begin", "mt_select_accumulate", "mt_select_advance",
            "mt_sparse_count_band", "mt_sparse_scan", "mt_sparse_fill_band", "mt_sparse_fill_index_band", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
            "mt_demag_field_sym", "mt_set_assembly_mode", "mt_launch_count",
-           "mt_set_demag_variant", "mt_profile_begin", "mt_profile_end")
+           "mt_set_demag_variant", "mt_profile_begin", "mt_profile_end", "mt_measure_peak")
 
 
 class MtError(RuntimeError):
@@ -105,6 +105,7 @@ def load() -> C.CDLL:
         lib.mt_set_demag_variant.argtypes = [C.c_void_p, C.c_int]
         lib.mt_set_assembly_mode.argtypes = [C.c_void_p, C.c_int]
         lib.mt_profile_begin.argtypes = [C.c_void_p]
+        lib.mt_measure_peak.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64, C.POINTER(C.c_double)]
         lib.mt_profile_end.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
         lib.mt_assemble_tensor.argtypes = [C.c_void_p, C.POINTER(_Tiles), C.c_int, C.c_int64, C.c_int64,
                                            C.c_void_p, C.c_int64, C.c_void_p]
@@ -230,6 +231,17 @@ def mt_profile_end(ctx: Context):
     ms, cnt = C.c_double(0.0), C.c_int64(0)
     ctx.check(ctx.lib.mt_profile_end(ctx.h, C.byref(ms), C.byref(cnt)))
     return ms.value, cnt.value
+
+
+MT_PEAK_DFMA, MT_PEAK_FFMA, MT_PEAK_FFMA2, MT_PEAK_MMA_TF32, MT_PEAK_HBM_READ = 0, 1, 2, 3, 4
+
+
+def mt_measure_peak(ctx: Context, kind: int, buf: torch.Tensor | None = None):
+    """Returns (rate, ms) of one roofline-denominator microbenchmark (see mt.h)."""
+    out = (C.c_double * 2)()
+    nbytes = int(buf.numel() * buf.element_size()) if buf is not None else 0
+    ctx.check(ctx.lib.mt_measure_peak(ctx.h, kind, buf.data_ptr() if buf is not None else None, nbytes, out))
+    return out[0], out[1]
 
 
 @dataclass

@@ -16,7 +16,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(HERE, "libmagtile.so")
-SOURCES = ("api.cu", "demag.cu", "demag_tma.cu", "assemble.cu", "sparse.cu", "sym.cu")
+SOURCES = ("api.cu", "demag.cu", "demag_tma.cu", "assemble.cu", "sparse.cu", "sym.cu", "peaks.cu")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]
 
@@ -36,6 +36,9 @@ def _stale(target: str, deps) -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    # developer knob: extra nvcc flags (e.g. -DMT_MMA_FLUSH_TILES=1 for an A/B build); forces a rebuild
+    extra = os.environ.get("MT_NVCC_EXTRA", "").split()
+    force = force or bool(extra)
     headers = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))]
     headers.append(os.path.join(INCLUDE, "mt.h"))
     nvcc = _nvcc()
@@ -45,7 +48,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         o = os.path.join(CSRC, src[:-3] + ".o")
         objs.append(o)
         if force or _stale(o, [s] + headers):
-            cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o]
+            cmd = [nvcc] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-c", s, "-o", o]
             jobs.append(cmd)
 
     def run(cmd):

@@ -175,6 +175,7 @@ int mt_destroy(mt_ctx* c) {
   cudaFree(c->Mst[0]);
   cudaFree(c->Mst[1]);
   cudaFree(c->partial);
+  cudaFree(c->Mq);
   cudaFree(c->rk);
   cudaFree(c->edens);
   cudaFree(c->sym_ws);
@@ -225,7 +226,7 @@ int mt_profile_end(mt_ctx* c, double* total_ms, int64_t* launches) {
 }
 
 int mt_set_demag_variant(mt_ctx* c, int variant) {
-  if (!c || variant < 0 || variant > 2) return MT_ERR_INVALID_ARG;
+  if (!c || variant < 0 || variant > 3) return MT_ERR_INVALID_ARG;
   c->variant = variant;
   return MT_OK;
 }

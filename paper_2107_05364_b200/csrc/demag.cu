@@ -365,7 +365,7 @@ static int launch_demag_variant(mt_ctx* ctx, const void* N, int dtype, int64_t n
   if (ctx->variant != 1) {
     int rc = mt_launch_demag_tma(ctx, N, dtype, n, n_rows, ld, Mst, npad, epi);
     if (rc != MT_ERR_UNIMPLEMENTED) return rc;
-    if (ctx->variant == 2) return rc;
+    if (ctx->variant >= 2) return rc;
   }
   if (dtype == MT_F32) return launch_ldg<float>(ctx, N, n, n_rows, ld, Mst, npad, epi);
   return launch_ldg<double>(ctx, N, n, n_rows, ld, Mst, npad, epi);

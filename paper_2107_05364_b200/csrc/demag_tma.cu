@@ -492,6 +492,255 @@ __global__ void __launch_bounds__(WARPS * 32, 1)
   }
 }
 
+// ---- fp32 tensors, batches of 5..8 states: tensor-core consumer (error-compensated TF32) ------------
+// With 8 states a 24-byte tensor block carries 72 FMAs; at the HBM rate that is ~2/3 of the FP32 pipe
+// AND ~2/3 of the shared-memory bandwidth (every warp re-reads the eight states' M), which do not
+// overlap well at two warps per scheduler: the packed-FFMA2 kernel above stops at 0.76 of the HBM
+// peak (r02/r03 ncu).  Here the batched product is what it really is, a dense contraction
+//     H[(i,a), b] = sum_{(j,c)} N^{ac}_{ij} M[(j,c), b]           (3 n_rows x 3 n) x (3 n x 8),
+// and runs on the tensor cores (north_star allows them "if the batched form is a real dense
+// contraction that holds accuracy").  Accuracy: TF32 alone (10-bit mantissa) cannot hold the 1e-5
+// gate, so both operands are split, x = x_hi + x_lo with x_hi = RN_tf32(x) and x_lo = RN_tf32(x - x_hi)
+// (the subtraction is exact), and three products are accumulated: hi*hi + hi*lo + lo*hi; what is
+// dropped (lo*lo and the rounding of x_lo) is ~2^-22 relative per product, unbiased.  Products of
+// tf32 operands are exact in the tensor core; its fp32 accumulator is drained into per-lane fp64
+// sums every kMmaFlush tiles (<= 2 x 9 x 3 mma per accumulator in between).
+// Shape: RT = 64 rows x CT = 32 columns per stage; the tensor box lands in shared memory with the
+// 128-byte swizzle (a 32-float row = one swizzle span), so ldmatrix.x4 fetches a 16 x 8 fp32 A
+// fragment (four 8 x 16-byte matrices) without bank conflicts; warp w owns row block w & 3 (16 rows)
+// and part w >> 2 of the tile's four 8-column slabs (16 warps: one slab each; 8 warps: two).  M is re-laid out once per call
+// by mma_stage_kernel as [component][slab of 8 columns][state g][t][{hi(t), hi(t+4), lo(t), lo(t+4)}],
+// so that one LDS.128 per component is a lane's whole B fragment (k = t, t + 4; n = g) for hi and lo.
+// mma.sync m16n8k8: D (16 rows x 8 states) += A (16 x 8 columns) . B (8 columns x 8 states); the nine
+// plane-component products of a symmetric 3x3 block are nine such mma per split term (27 per slab).
+// No cross-lane reduction is needed: the mma sums over columns.  The warps that share a row block
+// add their fp64 sums through shared memory at the end of a row group (fixed order).
+// Measured at config 5 (r04): 18.4 ms against 20.5 ms for the packed-FFMA2 kernel, error 1.2e-7
+// against the fp64 tensor; the board sits at its 1 kW power cap in both (SM clock ~1.5 GHz) and the
+// time follows the energy per block: with the two correction products left out (accuracy lost) it is
+// 15.6 ms, 8 or 16 warps and early or late release of the stage make no difference.
+#ifndef MT_MMA_WARPS
+#define MT_MMA_WARPS 16
+#endif
+#ifndef MT_MMA_FLUSH_TILES
+#define MT_MMA_FLUSH_TILES 1  /* measured (N = 32,768, 8 states, vs the fp64 tensor): 1 -> 2.0e-7, 2 -> 4.3e-7, 8 -> 1.8e-6 */
+#endif
+constexpr int kMmaWarps = MT_MMA_WARPS, kMmaRT = 64, kMmaCT = 32, kMmaStages = 3;
+constexpr int kMmaKS = kMmaWarps / 4;           // warps that share a row block (column split of a tile)
+constexpr int kMmaSPW = (kMmaCT / 8) / kMmaKS;  // 8-column slabs per warp per tile
+constexpr int kMmaFlush = MT_MMA_FLUSH_TILES;
+static_assert(kMmaWarps == 8 || kMmaWarps == 16, "4 row blocks x 2 or 4 column slabs");
+struct MmaCfg {
+  static constexpr int WARPS = kMmaWarps, RT = kMmaRT, CT = kMmaCT;
+  static constexpr size_t tensor_bytes = (size_t)6 * kMmaRT * kMmaCT * 4;          // 49,152
+  static constexpr size_t m_bytes = (size_t)3 * (kMmaCT / 8) * 128 * 4;           // 6,144
+  static constexpr size_t stage_bytes = tensor_bytes + m_bytes;                  // 55,296 = 54 KB
+  static constexpr size_t exch_bytes = (size_t)(kMmaKS - 1) * 12 * 4 * 32 * sizeof(double);
+  static constexpr size_t smem_bytes = kMmaStages * stage_bytes + exch_bytes + 2 * kMmaStages * sizeof(uint64_t) + 1024;
+  static_assert(stage_bytes % 1024 == 0, "swizzled tiles must start on 1 KB boundaries");
+};
+
+__device__ __forceinline__ uint32_t tf32_rn(uint32_t x) { return (x + 0x1000u) & 0xffffe000u; }
+__device__ __forceinline__ void mma_tf32(float d[4], const uint32_t a[4], uint32_t b0, uint32_t b1) {
+  asm volatile(
+      "mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+      : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
+// plain staged M [MT_MAX_BATCH][3][npad] fp32 -> Mq[3][npad/8][8 states][4][4] (see above)
+__global__ void __launch_bounds__(256) mma_stage_kernel(const float* __restrict__ M, int64_t npad, float4* __restrict__ Mq) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // (comp, slab, g, t)
+  const int64_t slabs = npad / 8;
+  if (idx >= 3 * slabs * 32) return;
+  const int t = (int)(idx & 3), g = (int)((idx >> 2) & 7);
+  const int64_t slab = (idx >> 5) % slabs;
+  const int comp = (int)((idx >> 5) / slabs);
+  const float* src = M + ((int64_t)g * 3 + comp) * npad + slab * 8 + t;
+  const float v0 = src[0], v1 = src[4];
+  const uint32_t h0 = tf32_rn(__float_as_uint(v0)), h1 = tf32_rn(__float_as_uint(v1));
+  const float l0 = v0 - __uint_as_float(h0), l1 = v1 - __uint_as_float(h1);
+  Mq[idx] = make_float4(__uint_as_float(h0), __uint_as_float(h1), __uint_as_float(tf32_rn(__float_as_uint(l0))),
+                        __uint_as_float(tf32_rn(__float_as_uint(l1))));
+}
+
+__global__ void __launch_bounds__(kMmaWarps * 32, 1)
+    demag_tma_mma_kernel(const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmM, TmaArgs a,
+                         EpiArgs e) {
+  typedef MmaCfg Cfg;
+  constexpr int RT = kMmaRT, CT = kMmaCT, STAGES = kMmaStages, KS = kMmaKS, SPW = kMmaSPW;
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  double* exch = (double*)(smem + STAGES * Cfg::stage_bytes);
+  uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::stage_bytes + Cfg::exch_bytes);
+  const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int64_t P = gridDim.x, c = blockIdx.x;
+  const int64_t t0 = range_begin(a.tiles, P, c), t1 = range_begin(a.tiles, P, c + 1);
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < STAGES; ++s) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, kMmaWarps);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (t0 >= t1) return;
+
+  // producer (lane 0 of warp 0), as in demag_tma_kernel
+  uint64_t pol_stream = 0, pol_keep = 0;
+  int p_stage = 0;
+  uint32_t p_phase = 0;
+  int64_t p_t = t0, p_g = t0 / a.chunks, p_k = t0 % a.chunks;
+  const bool is_producer = (threadIdx.x == 0);
+  if (is_producer) {
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
+    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+  }
+  auto top_up = [&](int64_t must) {
+    while (p_t < t1) {
+      if (!mbar_test(empty0 + 8 * p_stage, p_phase ^ 1)) {
+        if (p_t > must) break;
+        mbar_wait(empty0 + 8 * p_stage, p_phase ^ 1);
+      }
+      const uint32_t dst = smem_u32(smem + (size_t)p_stage * Cfg::stage_bytes);
+      mbar_expect_tx(full0 + 8 * p_stage, (uint32_t)Cfg::stage_bytes);
+      tma_load_3d(dst, &tmN, (int)(p_k * CT), (int)(p_g * RT), 0, full0 + 8 * p_stage, pol_stream);
+      tma_load_3d(dst + (uint32_t)Cfg::tensor_bytes, &tmM, 0, (int)(p_k * (CT / 8)), 0, full0 + 8 * p_stage, pol_keep);
+      if (++p_stage == STAGES) { p_stage = 0; p_phase ^= 1; }
+      if (++p_k == a.chunks) { p_k = 0; ++p_g; }
+      ++p_t;
+    }
+  };
+
+  // consumer geometry: warp = (row block rb of 16 rows, column part ks of the tile)
+  const int rb = warp & 3, ks = warp >> 2;
+  const int g8 = lane >> 2, tig = lane & 3;
+  // ldmatrix: lane supplies the address of row (lane & 7) of matrix (lane >> 3); matrices = {rows 0-7,
+  // rows 8-15} x {columns 0-3, 4-7} of the slab, in the order of the A fragment registers a0..a3
+  const int lm_r = lane & 7, lm_j = lane >> 3;
+  const uint32_t lm_row_off = (uint32_t)(rb * 16 + lm_r + 8 * (lm_j & 1)) * 128u;
+  uint32_t lm_chunk[SPW];
+#pragma unroll
+  for (int q = 0; q < SPW; ++q) lm_chunk[q] = (uint32_t)(((2 * (SPW * ks + q) + (lm_j >> 1)) ^ lm_r) << 4);
+
+  float d[3][4];
+  double acc[3][4];
+#pragma unroll
+  for (int cc = 0; cc < 3; ++cc)
+#pragma unroll
+    for (int i = 0; i < 4; ++i) { d[cc][i] = 0.f; acc[cc][i] = 0.0; }
+  int since_flush = 0;
+  int stage = 0;
+  uint32_t phase = 0;
+  int64_t g = t0 / a.chunks, k = t0 % a.chunks;
+  const int64_t g_first = g;
+  bool head_in_range = (k == 0);
+  for (int64_t t = t0; t < t1; ++t) {
+    if (is_producer) top_up(t);
+    __syncwarp();
+    mbar_wait(full0 + 8 * stage, phase);
+    const uint32_t tile = smem_u32(smem + (size_t)stage * Cfg::stage_bytes);
+    const float4* mq = (const float4*)(smem + (size_t)stage * Cfg::stage_bytes + Cfg::tensor_bytes);
+    // all fragments of the warp's slabs go to registers first and the stage is handed back to the
+    // producer BEFORE the arithmetic: a stage is held for ~10 shared-memory loads instead of the
+    // whole tile's mma work
+    uint32_t raw[SPW][6][4];
+    float4 bq[SPW][3];
+#pragma unroll
+    for (int q = 0; q < SPW; ++q) {
+#pragma unroll
+      for (int p = 0; p < 6; ++p)
+        asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
+                     : "=r"(raw[q][p][0]), "=r"(raw[q][p][1]), "=r"(raw[q][p][2]), "=r"(raw[q][p][3])
+                     : "r"(tile + (uint32_t)p * (RT * 128u) + lm_row_off + lm_chunk[q]));
+#pragma unroll
+      for (int cc = 0; cc < 3; ++cc) bq[q][cc] = mq[(cc * (CT / 8) + SPW * ks + q) * 32 + lane];
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(empty0 + 8 * stage);
+#pragma unroll
+    for (int q = 0; q < SPW; ++q) {
+      // plane p multiplies component col(p) of M into row component row(p) and, off the diagonal,
+      // component row(p) into col(p): xx, xy, xz, yy, yz, zz
+#pragma unroll
+      for (int p = 0; p < 6; ++p) {
+        constexpr int prow[6] = {0, 0, 0, 1, 1, 2}, pcol[6] = {0, 1, 2, 1, 2, 2};
+        uint32_t hi[4], lo[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          hi[i] = tf32_rn(raw[q][p][i]);
+          lo[i] = __float_as_uint(__uint_as_float(raw[q][p][i]) - __uint_as_float(hi[i])) & 0xffffe000u;
+        }
+        const int ra = prow[p], ca = pcol[p];
+        const float4* b = bq[q];
+        // small terms first, the dominant hi*hi product last
+        mma_tf32(d[ra], lo, __float_as_uint(b[ca].x), __float_as_uint(b[ca].y));
+        mma_tf32(d[ra], hi, __float_as_uint(b[ca].z), __float_as_uint(b[ca].w));
+        mma_tf32(d[ra], hi, __float_as_uint(b[ca].x), __float_as_uint(b[ca].y));
+        if (ra != ca) {
+          mma_tf32(d[ca], lo, __float_as_uint(b[ra].x), __float_as_uint(b[ra].y));
+          mma_tf32(d[ca], hi, __float_as_uint(b[ra].z), __float_as_uint(b[ra].w));
+          mma_tf32(d[ca], hi, __float_as_uint(b[ra].x), __float_as_uint(b[ra].y));
+        }
+      }
+    }
+    if (++stage == STAGES) { stage = 0; phase ^= 1; }
+    const bool group_done = (k + 1 == a.chunks);
+    const bool emit = group_done || t + 1 == t1;
+    if (++since_flush == kMmaFlush || emit) {
+      since_flush = 0;
+#pragma unroll
+      for (int cc = 0; cc < 3; ++cc)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { acc[cc][i] += (double)d[cc][i]; d[cc][i] = 0.f; }
+    }
+    if (emit) {
+      // the KS warps of a row block (column parts of the tiles) add up through shared memory, in order
+      if (ks > 0) {
+#pragma unroll
+        for (int cc = 0; cc < 3; ++cc)
+#pragma unroll
+          for (int i = 0; i < 4; ++i) exch[(((ks - 1) * 3 + cc) * 4 + i) * 128 + rb * 32 + lane] = acc[cc][i];
+      }
+      __syncthreads();
+      if (ks == 0) {
+#pragma unroll 1
+        for (int i = 0; i < 4; ++i) {
+          const int rg = rb * 16 + g8 + 8 * (i >> 1), b = 2 * tig + (i & 1);
+          const int64_t row = g * RT + rg;
+          double s3[3];
+#pragma unroll
+          for (int cc = 0; cc < 3; ++cc) {
+            // (dynamic index i: pick without spilling acc to local memory)
+            double v = i == 0 ? acc[cc][0] : i == 1 ? acc[cc][1] : i == 2 ? acc[cc][2] : acc[cc][3];
+#pragma unroll
+            for (int w = 0; w < KS - 1; ++w) v += exch[((w * 3 + cc) * 4 + i) * 128 + rb * 32 + lane];
+            s3[cc] = v;
+          }
+          if (b < e.batch && row < a.n_rows) {
+            if (head_in_range && group_done) {
+              const double hd[3] = {-s3[0], -s3[1], -s3[2]};
+              row_epilogue(e, row, b, hd);
+            } else {
+              const int slot = (g == g_first) ? 0 : 1;
+              double* pp = a.partial + ((((int64_t)c * 2 + slot) * RT + rg) * e.batch + b) * 3;
+              pp[0] = s3[0]; pp[1] = s3[1]; pp[2] = s3[2];
+            }
+          }
+        }
+      }
+      __syncthreads();
+#pragma unroll
+      for (int cc = 0; cc < 3; ++cc)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) acc[cc][i] = 0.0;
+    }
+    if (group_done) { k = 0; ++g; head_in_range = true; } else { ++k; }
+  }
+}
+
 // second pass: groups that were split between CTAs — add the per-CTA partial sums in CTA order
 template <int RT>
 __global__ void __launch_bounds__(256) demag_tma_fixup_kernel(TmaArgs a, int64_t P, int B, EpiArgs e) {
@@ -542,13 +791,14 @@ EncodeTiledFn encode_fn() {
 }
 
 int make_map(mt_ctx* ctx, CUtensorMap* out, int dtype, const void* base, int rank, const uint64_t* dims,
-             const uint64_t* strides_bytes, const uint32_t* box) {
+             const uint64_t* strides_bytes, const uint32_t* box, bool swizzle128 = false) {
   EncodeTiledFn fn = encode_fn();
   if (!fn) return mt_fail(ctx, MT_ERR_CUDA, "cuTensorMapEncodeTiled is not available from the driver");
   const cuuint32_t ones[3] = {1, 1, 1};
   CUresult r = fn(out, dtype == MT_F32 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64,
                   (cuuint32_t)rank, const_cast<void*>(base), (const cuuint64_t*)dims, (const cuuint64_t*)strides_bytes,
-                  (const cuuint32_t*)box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                  (const cuuint32_t*)box, ones, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                  swizzle128 ? CU_TENSOR_MAP_SWIZZLE_128B : CU_TENSOR_MAP_SWIZZLE_NONE,
                   CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) return mt_fail(ctx, MT_ERR_CUDA, "cuTensorMapEncodeTiled failed (CUresult %d)", (int)r);
   return MT_OK;
@@ -619,11 +869,68 @@ int launch_f32x2_shape(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, in
       ctx, demag_tma_f32x2_kernel<B, WARPS, CT, STAGES>, attr_set, 3 * B, N, MT_F32, n, n_rows, ld, Mst, npad, e);
 }
 
+// fp32, 5 <= batch <= 8: tensor-core kernel (error-compensated TF32); states beyond `batch` are
+// computed on unused rows of M and dropped
+int launch_mma(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld, const void* Mst, int64_t npad,
+               const EpiArgs& e) {
+  typedef MmaCfg Cfg;
+  constexpr int RT = Cfg::RT;
+  static_assert(Cfg::smem_bytes <= 227 * 1024, "ring does not fit shared memory");
+  const int64_t P = ctx->num_sms;
+  TmaArgs a;
+  a.n_rows = n_rows;
+  a.groups = (n_rows + RT - 1) / RT;
+  a.chunks = (n + Cfg::CT - 1) / Cfg::CT;
+  a.tiles = a.groups * a.chunks;
+  int rc = mt_ensure_ws(ctx, (void**)&ctx->partial, &ctx->partial_bytes, (size_t)P * 2 * RT * e.batch * 3 * sizeof(double));
+  if (rc) return rc;
+  a.partial = ctx->partial;
+  // M re-laid out for the B fragments: hi/lo split, [3][npad/8][8 states][4][4] fp32
+  const size_t mq_bytes = (size_t)3 * (npad / 8) * 32 * sizeof(float4);
+  if ((rc = mt_ensure_ws(ctx, &ctx->Mq, &ctx->Mq_bytes, mq_bytes))) return rc;
+  {
+    const int64_t tot = 3 * (npad / 8) * 32;
+    mma_stage_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>((const float*)Mst, npad, (float4*)ctx->Mq);
+    ctx->launches++;
+    MT_CUDA_OK(ctx, cudaGetLastError());
+  }
+  alignas(64) CUtensorMap tmN, tmM;
+  {
+    const uint64_t dims[3] = {(uint64_t)n, (uint64_t)n_rows, 6};
+    const uint64_t strides[2] = {(uint64_t)ld * 4, (uint64_t)n_rows * (uint64_t)ld * 4};
+    const uint32_t box[3] = {(uint32_t)Cfg::CT, (uint32_t)RT, 6};
+    if ((rc = make_map(ctx, &tmN, MT_F32, N, 3, dims, strides, box, /*swizzle128=*/true))) return rc;
+  }
+  {
+    const uint64_t dims[3] = {128, (uint64_t)(npad / 8), 3};
+    const uint64_t strides[2] = {128 * 4, (uint64_t)(npad / 8) * 128 * 4};
+    const uint32_t box[3] = {128, (uint32_t)(Cfg::CT / 8), 3};
+    if ((rc = make_map(ctx, &tmM, MT_F32, ctx->Mq, 3, dims, strides, box))) return rc;
+  }
+  static unsigned char attr_set[kMaxDevices] = {};
+  const int dev = ctx->device & (kMaxDevices - 1);
+  if (!attr_set[dev]) {
+    MT_CUDA_OK(ctx, cudaFuncSetAttribute(demag_tma_mma_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)Cfg::smem_bytes));
+    attr_set[dev] = 1;
+  }
+  demag_tma_mma_kernel<<<(unsigned)P, Cfg::WARPS * 32, Cfg::smem_bytes, ctx->stream>>>(tmN, tmM, a, e);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  const int64_t tot = n_rows * e.batch;
+  demag_tma_fixup_kernel<RT><<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(a, P, e.batch, e);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
 // fp32, 3 <= batch <= 8: packed-FMA kernels for 4 or 8 states (states beyond `batch` are computed on
 // unused rows of M and dropped)
 int launch_f32x2(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld, const void* Mst, int64_t npad,
                  const EpiArgs& e) {
   if (e.batch <= 4) return launch_f32x2_shape<4, MT_B4_WARPS, MT_B4_CT, MT_B4_STAGES>(ctx, N, n, n_rows, ld, Mst, npad, e);
+  // variant 3 keeps the packed-FFMA2 kernel for A/B comparisons; the default is the tensor-core kernel
+  if (ctx->variant != 3) return launch_mma(ctx, N, n, n_rows, ld, Mst, npad, e);
   return launch_f32x2_shape<8, MT_B8_WARPS, MT_B8_CT, MT_B8_STAGES>(ctx, N, n, n_rows, ld, Mst, npad, e);
 }
 
@@ -656,7 +963,7 @@ int launch_T(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, i
 // (too few tiles to give every SM a share); the dispatcher then falls back to it.
 int mt_launch_demag_tma(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
                         const void* Mst, int64_t npad, const EpiArgs& e) {
-  if (ctx->variant != 2) {
+  if (ctx->variant != 2 && ctx->variant != 3) {
     const int64_t tiles = ((n_rows + 7) / 8) * ((n * (dtype == MT_F32 ? 4 : 8) + 1023) / 1024);
     if (tiles < 16LL * ctx->num_sms) return MT_ERR_UNIMPLEMENTED;
   }

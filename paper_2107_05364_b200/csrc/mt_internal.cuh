@@ -15,7 +15,7 @@ struct mt_ctx {
   cudaStream_t stream;
   cudaStream_t cap_stream;  // private stream for CUDA-graph capture
   int num_sms;
-  int variant;  // 0 auto, 1 LDG, 2 TMA
+  int variant;  // 0 auto, 1 LDG, 2 TMA, 3 TMA with the packed-FFMA2 kernel for batches of 5..8
   int assembly_mode;  // 0 closed form everywhere (the paper's method), 1 far-field-stable (F2)
   int64_t launches;
   char err[512];
@@ -24,6 +24,8 @@ struct mt_ctx {
   size_t Mst_bytes;
   double* partial;
   size_t partial_bytes;
+  void* Mq;  // staged M re-laid out for the tensor-core kernel's B fragments (demag_tma.cu)
+  size_t Mq_bytes;
   double* rk;  // integrator stages + scratch states
   size_t rk_bytes;
   void* sym_ws;   // rowpart + colpart of the symmetric-half field kernel (F3)
