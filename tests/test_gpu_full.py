@@ -148,6 +148,70 @@ def test_config3_sampled_rows(ctx, oracle, dtype):
     torch.cuda.empty_cache()
 
 
+def config3_dp45_segments(ctx, w, prob, t_end, seg, torque_tol):
+    """BASELINE config 3's own protocol (DP45, rtol/atol/dt0 of DESIGN.md Q11, stop test Q12) run in
+    segments of `seg` time units so that the energy can be read between them; mt_integrate is
+    resumable on (m, t, dt_last).  Returns sample rows [t, <m>], energies, counters."""
+    x = w.extra
+    m = torch.from_numpy(np.ascontiguousarray(w.m[:1])).cuda()
+    E = torch.zeros((1, 5), dtype=torch.float64, device="cuda")
+    row = torch.zeros((1, 4), dtype=torch.float64, device="cuda")
+    B.mt_energy(ctx, prob, m, 1, E)
+    energies, rows = [float(E[0, 4].item())], []
+    tot = dict(accepted=0, rejected=0, rhs_calls=0, max_torque=float("inf"))
+    t, dt = 0.0, x["dt0"]
+    while t < t_end and tot["max_torque"] > torque_tol:
+        t1 = min(t_end, t + seg)
+        t, res, _ = B.mt_integrate(ctx, prob, m, 1, t, method=B.MT_DP45, dt=dt, t_end=t1, rtol=x["rtol"],
+                                   atol=x["atol"], torque_tol=torque_tol, renormalize=True, sample_dt=t1 - t,
+                                   samples=row)
+        dt = res["dt_last"]
+        for k in ("accepted", "rejected", "rhs_calls"):
+            tot[k] += res[k]
+        tot["max_torque"] = res["max_torque"]
+        B.mt_energy(ctx, prob, m, 1, E)
+        energies.append(float(E[0, 4].item()))
+        rows.append(np.concatenate([[t], m[0].mean(dim=1).cpu().numpy()]))
+    return m.cpu().numpy(), np.array(rows), np.array(energies), tot, t
+
+
+def test_config3_full_size_dp45_fp32_vs_fp64(ctx):
+    """Config 3 as BASELINE.json states it, at its full size: "DP45 adaptive to equilibrium; both fp32
+    and fp64 tensor paths" (SP3 shape PAPER.md:185-187; RK(4,5) PAPER.md:143,181; stop test Eq. 2
+    PAPER.md:40).  The oracle cannot run 32^3 (parity of the same integrator is on the 8^3/16^3
+    replicas below and on sampled rows of the right-hand side above); here the two device paths are
+    held against each other and against what holds at any size: <m>(t) of the fp32- and the
+    fp64-tensor runs within 1e-3 at common times, |m| = 1, the free energy non-increasing (alpha > 0,
+    no applied field: PAPER.md:58), the torque falling towards the stop tolerance.  The driver's GPU
+    test step has a 20-minute limit, so the run stops at t = 8 (the first ~1,300 attempted steps: the
+    random start is smoothed, the step has reached the exchange stability limit); the whole protocol
+    (to |m x H| <= 1e-5 or t = 200) is what `bench.py --config 3 --protocol` runs and reports."""
+    T_END, SEG = 8.0, 1.0
+    out = {}
+    w = W.config3(32, batch=1)
+    tiles = H.dev_tiles(w)
+    for dtype in ("f32", "f64"):
+        N, ld, status = H.assemble(ctx, tiles, dtype)
+        assert status == 0
+        prob = H.dev_problem(w, tiles, N, dtype, ld)
+        out[dtype] = config3_dp45_segments(ctx, w, prob, T_END, SEG, w.extra["torque_tol"])
+        del N, prob
+        torch.cuda.empty_cache()
+    (m32, s32, e32, r32, t32), (m64, s64, e64, r64, t64) = out["f32"], out["f64"]
+    assert t32 == T_END and t64 == T_END and len(s32) == len(s64) == int(T_END / SEG)
+    assert np.array_equal(s32[:, 0], s64[:, 0])
+    assert np.max(np.abs(s32[:, 1:] - s64[:, 1:])) < 1e-3
+    assert np.max(np.abs(m32 - m64)) < 1e-3  # tile by tile as well: the fp32 tensor does not bend the path
+    for m, e, r in ((m32, e32, r32), (m64, e64, r64)):
+        assert np.max(np.abs(np.linalg.norm(m[0], axis=0) - 1.0)) < 1e-14
+        assert np.all(np.diff(e) <= 1e-12 * np.abs(e[0])), np.diff(e)
+        assert e[-1] < 0.5 * e[0]          # not vacuous: a random state has lost most of its exchange energy
+        assert r["rejected"] < r["accepted"] and r["rhs_calls"] >= 6 * r["accepted"]
+        assert np.isfinite(r["max_torque"]) and r["max_torque"] < 1.0
+    # the two runs take nearly the same step sequence (same controller, errors differ by ~1e-7 relative)
+    assert abs(r32["accepted"] - r64["accepted"]) <= 0.02 * r64["accepted"]
+
+
 def test_config3_trajectory_replicas(ctx, oracle):
     """DP45 trajectory parity on replicas both sides can run: 8^3 to equilibrium (torque stop) and a
     16^3 window; <m>(t) at common sample times within 1e-3."""
