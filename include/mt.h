@@ -259,6 +259,39 @@ int mt_assemble_tensor_sym(mt_ctx* ctx, const mt_tiles* tiles, int dtype, void* 
 int mt_demag_field_sym(mt_ctx* ctx, const mt_sym_tensor* S, const double* Ms, const double* m,
                        int batch, double* Hd);
 
+/* ---- 8(e). Row sharding over several GPUs (one process and one mt_ctx per GPU) --------------------
+ * The tensor shards by TARGET rows (every pair is independent): rank g of `world`
+ * assembles and keeps rows [g n / world, (g+1) n / world) (integer division) — the row band of
+ * mt_assemble_tensor — and evaluates the right-hand side of those rows.  Every evaluation needs the
+ * whole state on every rank ("RHS -> dense product -> LL"), so each Runge-Kutta
+ * stage ends with ONE exchange: the all-gather of the ranks' slices of the next stage state; DP45's
+ * error norm and the torque test add one max-reduction of two scalars per step.  The library does not
+ * link a communication layer: the caller supplies `exchange`, called on the host between kernels,
+ * which must ENQUEUE the collective on `cuda_stream` (the ctx's stream) and return 0, or non-zero on
+ * failure (-> MT_ERR_CUDA):
+ *   what == MT_XCHG_GATHER_STATE: all-gather `pack` IN PLACE over the ranks.  pack is
+ *     [world][batch][3][slice_pad] doubles; the fused epilogue has written rank `rank`'s block (its
+ *     rows' components of the next state, rows beyond the band's length unspecified); on completion
+ *     every rank holds every block (ncclAllGather / all_gather_into_tensor with the rank's block as
+ *     the send buffer).  The library then scatters the blocks into the full state and the staged M.
+ *   what == MT_XCHG_MAX_SCALARS: element-wise MAX over the ranks of the two 64-bit words of `scal`
+ *     (bit patterns of non-negative doubles or the canonical quiet NaN 0x7ff8000000000000: they order
+ *     like signed or unsigned 64-bit integers), result on every rank.
+ * All ranks must make the same calls with the same arguments (the host-side step controller then
+ * takes the same decisions everywhere).  pack, scal: DEVICE memory owned by the caller, at least
+ * world*batch*3*slice_pad doubles and 2 words; slice_pad >= the longest band, equal on all ranks.   */
+#define MT_XCHG_GATHER_STATE 0
+#define MT_XCHG_MAX_SCALARS 1
+typedef int (*mt_exchange_fn)(void* user, int what, void* cuda_stream);
+typedef struct {
+  int rank, world;
+  int64_t slice_pad;
+  double* pack;
+  unsigned long long* scal;
+  mt_exchange_fn exchange;
+  void* user;
+} mt_shard;
+
 /* ---- A5 / A6. Effective field and Landau-Lifshitz right-hand side ------------------------------
  * H_eff = H_d + H_exch + H_anis + H_a                                   (Eq. 17)
  *   H_exch,i = c_ex,i * sum_{dir} (m_{i+} - 2 m_i + m_{i-}) * inv_d2[dir]   (Eq. 12 PAPER.md:94;
@@ -269,7 +302,11 @@ int mt_demag_field_sym(mt_ctx* ctx, const mt_sym_tensor* S, const double* Ms, co
  * dm/dt = -gamma m x H_eff - alpha_ll m x (m x H_eff)                    (Eq. 1,  PAPER.md:33)
  * gamma and alpha_ll are the two prefactors exactly as written in Eq. 1 (Q5).
  * A NULL array pointer selects the scalar / constant beside it; nbr == NULL disables exchange;
- * N == NULL disables the demagnetising term.  The tensor must be square here (n rows).           */
+ * N == NULL disables the demagnetising term.  The tensor must be square here (n rows) unless
+ * `shard` is set: N (or N_sparse) then holds the rank's row band only, m and every per-tile array stay
+ * full-size on every rank, mt_llg_rhs writes the band's rows of dmdt / Heff (at their global
+ * positions; other rows untouched) and mt_integrate advances the whole state with one exchange per
+ * stage.  mt_energy, mt_field_sweep and N_sym do not take a sharded problem (MT_ERR_INVALID_ARG).  */
 typedef struct {
   int64_t n;
   const void* N;         /* [6][n][ld] or NULL                                                     */
@@ -292,6 +329,7 @@ typedef struct {
                             thresholded tensor (F1) instead of N (N may then be NULL)  */
   const mt_sym_tensor* N_sym; /* HOST pointer or NULL: demagnetising term from the pair-symmetric half
                             (F3); takes precedence over N, after N_sparse                            */
+  const mt_shard* shard; /* HOST pointer or NULL: row-sharded problem (section 8(e) above)           */
 } mt_problem;
 
 /* dmdt[b][3][n] (required) and Heff[b][3][n] (optional, NULL to skip) for m[b][3][n].

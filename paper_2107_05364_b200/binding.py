@@ -52,8 +52,17 @@ class _Problem(C.Structure):
         ("easy", C.c_void_p), ("easy_const", C.c_double * 3),
         ("H_a", C.c_void_p), ("H_a_const", C.c_double * 3),
         ("gamma", C.c_double), ("alpha_ll", C.c_double), ("vol", C.c_void_p), ("N_sparse", C.c_void_p),
-        ("N_sym", C.c_void_p),
+        ("N_sym", C.c_void_p), ("shard", C.c_void_p),
     ]
+
+
+MT_XCHG_GATHER_STATE, MT_XCHG_MAX_SCALARS = 0, 1
+EXCHANGE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int, C.c_void_p)
+
+
+class _Shard(C.Structure):
+    _fields_ = [("rank", C.c_int), ("world", C.c_int), ("slice_pad", C.c_int64), ("pack", C.c_void_p),
+                ("scal", C.c_void_p), ("exchange", EXCHANGE_FN), ("user", C.c_void_p)]
 
 
 class _Sym(C.Structure):
@@ -288,6 +297,39 @@ def mt_demag_field_host(ctx: Context, N: torch.Tensor, dtype: int, n: int, n_row
                                           _ptr(Hd_host, torch.float64)))
 
 
+class Shard:
+    """mt_shard (row sharding, mt.h section 8(e)): this rank's place in the partition, the all-gather
+    buffer `pack` [world, batch, 3, slice_pad] and the two reduction words `scal`, both preallocated
+    here once, and the exchange callback.  `exchange(what, pack, scal, cuda_stream)` must enqueue the
+    collective on `cuda_stream` (an int; 0 = legacy default stream): what == MT_XCHG_GATHER_STATE:
+    all-gather of pack[rank] into pack, in place; MT_XCHG_MAX_SCALARS: element-wise max of scal over
+    the ranks.  `sharding.dist_exchange` builds one from torch.distributed."""
+
+    def __init__(self, rank: int, world: int, n: int, batch: int, device, exchange):
+        if not (0 <= rank < world):
+            raise ValueError("need 0 <= rank < world")
+        self.rank, self.world, self.n, self.batch = rank, world, n, batch
+        self.slice_pad = (n + world - 1) // world
+        self.pack = torch.zeros((world, batch, 3, self.slice_pad), dtype=torch.float64, device=device)
+        self.scal = torch.zeros(2, dtype=torch.int64, device=device)
+        self.error = None
+
+        def _cb(_user, what, stream):
+            try:
+                exchange(int(what), self.pack, self.scal, int(stream or 0))
+                return 0
+            except Exception as exc:  # nothing may propagate through the C frames
+                self.error = exc
+                return 1
+
+        self._cb = EXCHANGE_FN(_cb)
+        self._c_struct = _Shard(rank, world, self.slice_pad, self.pack.data_ptr(), self.scal.data_ptr(), self._cb, None)
+
+    @property
+    def rows(self) -> tuple[int, int]:
+        return self.rank * self.n // self.world, (self.rank + 1) * self.n // self.world
+
+
 @dataclass
 class Problem:
     """mt_problem: tensor + local-term parameters.  Scalars or device tensors for c_ex, c_an;
@@ -308,6 +350,7 @@ class Problem:
     vol: torch.Tensor | None = None
     N_sparse: object = None  # SparseTensor (F1): used for the demagnetising term instead of N
     N_sym: object = None     # SymTensor (F3): pair-symmetric half, congruent cuboid meshes only
+    shard: object = None     # Shard: N (or N_sparse) holds this rank's row band only
 
     def _c(self) -> _Problem:
         s = _Problem()
@@ -317,6 +360,8 @@ class Problem:
         if self.N_sym is not None:
             self._sym_c = self.N_sym._c()
             s.N_sym = C.addressof(self._sym_c)
+        if self.shard is not None:
+            s.shard = C.addressof(self.shard._c_struct)
         s.n = self.n
         s.N = _ptr(self.N, torch_dtype(self.dtype)) if self.N is not None else None
         s.dtype, s.ld = self.dtype, self.ld

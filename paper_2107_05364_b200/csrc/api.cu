@@ -64,12 +64,22 @@ int check_sparse(mt_ctx* ctx, const mt_sparse_tensor* s) {
   return MT_OK;
 }
 
+// rows [r0, r1) of the right-hand side this rank evaluates: all of them, or the rank's band of a
+// row-sharded problem (mt.h section 8(e): begin(g) = g n / world)
+inline int64_t band_begin(const mt_problem* p) {
+  return p->shard ? (int64_t)(((unsigned __int128)p->shard->rank * (unsigned __int128)p->n) / (unsigned)p->shard->world) : 0;
+}
+inline int64_t band_end(const mt_problem* p) {
+  return p->shard ? (int64_t)(((unsigned __int128)(p->shard->rank + 1) * (unsigned __int128)p->n) / (unsigned)p->shard->world) : p->n;
+}
+
 void fill_problem(EpiArgs& e, const mt_problem* p, int batch) {
   memset(&e, 0, sizeof(e));
   e.mode = 1;
   e.batch = batch;
   e.n = p->n;
-  e.n_rows = p->n;
+  e.n_rows = band_end(p) - band_begin(p);
+  e.row0 = band_begin(p);
   e.Ms = p->Ms;
   e.nbr = p->nbr;
   for (int a = 0; a < 3; ++a) {
@@ -92,11 +102,22 @@ int check_problem(mt_ctx* ctx, const mt_problem* p, int batch) {
   if (!p) return mt_fail(ctx, MT_ERR_INVALID_ARG, "problem is NULL");
   if (p->n <= 0 || !p->Ms) return mt_fail(ctx, MT_ERR_INVALID_ARG, "problem needs n > 0 and Ms");
   if (batch < 1 || batch > MT_MAX_BATCH) return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
+  if (const mt_shard* sh = p->shard) {
+    if (sh->world < 1 || sh->rank < 0 || sh->rank >= sh->world)
+      return mt_fail(ctx, MT_ERR_INVALID_ARG, "shard: need 0 <= rank < world");
+    if (sh->world > p->n) return mt_fail(ctx, MT_ERR_INVALID_ARG, "shard: more ranks than tiles");
+    if (!sh->pack || !sh->scal || !sh->exchange)
+      return mt_fail(ctx, MT_ERR_INVALID_ARG, "shard: pack, scal and exchange must be non-NULL");
+    if (sh->slice_pad < (p->n + sh->world - 1) / sh->world)
+      return mt_fail(ctx, MT_ERR_INVALID_ARG, "shard: slice_pad is shorter than the longest band");
+    if (p->N_sym) return mt_fail(ctx, MT_ERR_INVALID_ARG, "the pair-symmetric half cannot be row-sharded");
+  }
+  const int64_t rows = band_end(p) - band_begin(p);
   if (p->N_sparse) {
     int rc = check_sparse(ctx, p->N_sparse);
     if (rc) return rc;
-    if (p->N_sparse->n != p->n || p->N_sparse->n_rows != p->n)
-      return mt_fail(ctx, MT_ERR_INVALID_ARG, "sparse tensor must be n x n");
+    if (p->N_sparse->n != p->n || p->N_sparse->n_rows != rows)
+      return mt_fail(ctx, MT_ERR_INVALID_ARG, "sparse tensor must be n x n (sharded: the rank's band x n)");
     return MT_OK;
   }
   if (p->N_sym) {
@@ -105,7 +126,7 @@ int check_problem(mt_ctx* ctx, const mt_problem* p, int batch) {
     if (p->N_sym->n != p->n) return mt_fail(ctx, MT_ERR_INVALID_ARG, "symmetric tensor must have n tiles");
     return MT_OK;
   }
-  if (p->N) return check_tensor_args(ctx, p->N, p->dtype, p->n, p->n, p->ld);
+  if (p->N) return check_tensor_args(ctx, p->N, p->dtype, p->n, rows, p->ld);
   return MT_OK;
 }
 
@@ -113,7 +134,7 @@ int check_problem(mt_ctx* ctx, const mt_problem* p, int batch) {
 int eval_rhs(mt_ctx* ctx, const mt_problem* p, int64_t npad, int src, const EpiArgs& e) {
   if (p->N_sparse) return mt_launch_demag_sparse(ctx, p->N_sparse, ctx->Mst[src], npad, e);
   if (p->N_sym) return mt_launch_demag_sym(ctx, p->N_sym, ctx->Mst[src], npad, e);
-  if (p->N) return mt_launch_demag(ctx, p->N, p->dtype, p->n, p->n, p->ld, ctx->Mst[src], npad, e);
+  if (p->N) return mt_launch_demag(ctx, p->N, p->dtype, p->n, e.n_rows, p->ld, ctx->Mst[src], npad, e);
   return mt_launch_local_only(ctx, e);
 }
 
@@ -556,6 +577,7 @@ int mt_energy(mt_ctx* ctx, const mt_problem* p, const double* m, int batch, doub
   int rc = check_problem(ctx, p, batch);
   if (rc) return rc;
   if (!m || !E_out) return mt_fail(ctx, MT_ERR_INVALID_ARG, "m and E_out must be non-NULL");
+  if (p->shard) return mt_fail(ctx, MT_ERR_INVALID_ARG, "mt_energy does not take a row-sharded problem");
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
   const int64_t npad = round_up(p->n, MT_COL_CHUNK);
   rc = mt_ensure_ws(ctx, (void**)&ctx->edens, &ctx->edens_bytes, (size_t)batch * 4 * p->n * sizeof(double));
@@ -581,6 +603,7 @@ int mt_field_sweep(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o
   if (!o || !fields_host || n_fields < 0 || !m || !rows)
     return mt_fail(ctx, MT_ERR_INVALID_ARG, "opts, fields, m and rows must be non-NULL");
   if (p->H_a) return mt_fail(ctx, MT_ERR_INVALID_ARG, "mt_field_sweep sets the uniform applied field: H_a must be NULL");
+  if (p->shard) return mt_fail(ctx, MT_ERR_INVALID_ARG, "mt_field_sweep does not take a row-sharded problem");
   const int64_t stride = 8 * (int64_t)batch;
   mt_problem pk = *p;
   mt_integrator_result total;
@@ -646,8 +669,37 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
     rc = mt_launch_stage_M(ctx, demag_dtype(p), p->Ms, m, batch, n, npad, ctx->Mst[1]);
     if (rc) return rc;
   }
-  unsigned long long* d_err = ctx->dscal;
-  unsigned long long* d_tq = ctx->dscal + 1;
+  // Row-sharded problem (mt.h section 8(e)): every stage's combine writes this rank's rows into its
+  // block of the all-gather buffer; `finish` then gathers the blocks and scatters them into the full
+  // stage state (and the staged M).  The error / torque maxima live in the caller's `scal` and are
+  // max-reduced over the ranks before the host reads them.
+  const mt_shard* sh = p->shard;
+  unsigned long long* d_err = sh ? sh->scal : ctx->dscal;
+  unsigned long long* d_tq = d_err + 1;
+  auto xchg = [&](int what) -> int {
+    if (sh->exchange(sh->user, what, (void*)st) != 0)
+      return mt_fail(ctx, MT_ERR_CUDA, "shard exchange callback failed (what = %d)", what);
+    return MT_OK;
+  };
+  auto route = [&](EpiArgs& e, double* y_dst, void* M_dst) {
+    if (!sh) { e.y_out = y_dst; e.M_out = M_dst; return; }
+    e.y_out = sh->pack + (int64_t)sh->rank * batch * 3 * sh->slice_pad;
+    e.y_ld = sh->slice_pad;
+    e.y_row0 = band_begin(p);
+    e.M_out = nullptr;
+  };
+  auto finish = [&](double* y_dst, void* M_dst) -> int {
+    if (!sh) return MT_OK;
+    int r = xchg(MT_XCHG_GATHER_STATE);
+    if (r) return r;
+    return mt_launch_unpack(ctx, sh->pack, sh->world, sh->slice_pad, batch, n, npad, p->Ms, y_dst, M_dst, demag_dtype(p));
+  };
+  auto read_scalars = [&](int count) -> int {  // d_err[0 .. count) -> ctx->hscal, after the ranks' maxima are combined
+    if (sh) { int r = xchg(MT_XCHG_MAX_SCALARS); if (r) return r; }
+    MT_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hscal, d_err + (2 - count), 8 * count, cudaMemcpyDeviceToHost, st));
+    MT_CUDA_OK(ctx, cudaStreamSynchronize(st));
+    return MT_OK;
+  };
   double t = *t_inout;
   const double t0 = t;
   int status = MT_OK;
@@ -667,30 +719,35 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
     auto stage1 = [&]() -> int {  // k1 = f(m); ya = m + dt/2 k1
       EpiArgs e = base;
       e.y = m; e.k_out = k[0]; e.torque_bits = want_tq ? d_tq : nullptr;
-      e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[0]; e.coef[0] = 1.0; e.base = m; e.h = 0.5 * dt; e.y_out = ya;
-      e.M_out = has_demag(p) ? ctx->Mst[1] : nullptr;
-      return eval_rhs(ctx, p, npad, 0, e);
+      e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[0]; e.coef[0] = 1.0; e.base = m; e.h = 0.5 * dt;
+      void* Md = has_demag(p) ? ctx->Mst[1] : nullptr;
+      route(e, ya, Md);
+      int r = eval_rhs(ctx, p, npad, 0, e);
+      return r ? r : finish(ya, Md);
     };
     auto stages234 = [&]() -> int {
       int r;
       EpiArgs e = base;  // stage 2: k2 = f(ya); yb = m + dt/2 k2
       e.y = ya; e.k_out = k[1];
-      e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[1]; e.coef[0] = 1.0; e.base = m; e.h = 0.5 * dt; e.y_out = yb;
-      e.M_out = has_demag(p) ? ctx->Mst[0] : nullptr;
-      if ((r = eval_rhs(ctx, p, npad, 1, e))) return r;
+      e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[1]; e.coef[0] = 1.0; e.base = m; e.h = 0.5 * dt;
+      void* M0 = has_demag(p) ? ctx->Mst[0] : nullptr;
+      void* M1 = has_demag(p) ? ctx->Mst[1] : nullptr;
+      route(e, yb, M0);
+      if ((r = eval_rhs(ctx, p, npad, 1, e)) || (r = finish(yb, M0))) return r;
       e = base;  // stage 3: k3 = f(yb); ya = m + dt k3
       e.y = yb; e.k_out = k[2];
-      e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[2]; e.coef[0] = 1.0; e.base = m; e.h = dt; e.y_out = ya;
-      e.M_out = has_demag(p) ? ctx->Mst[1] : nullptr;
-      if ((r = eval_rhs(ctx, p, npad, 0, e))) return r;
+      e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[2]; e.coef[0] = 1.0; e.base = m; e.h = dt;
+      route(e, ya, M1);
+      if ((r = eval_rhs(ctx, p, npad, 0, e)) || (r = finish(ya, M1))) return r;
       e = base;  // stage 4: k4 = f(ya); m <- m + dt/6 (k1 + 2 k2 + 2 k3 + k4), renormalised, restaged
       e.y = ya; e.k_out = k[3];
       e.do_comb = 1; e.ncomb = 4;
       for (int s = 0; s < 4; ++s) e.kptr[s] = k[s];
       e.coef[0] = 1.0; e.coef[1] = 2.0; e.coef[2] = 2.0; e.coef[3] = 1.0;
-      e.base = m; e.h = dt / 6.0; e.y_out = m; e.renorm = o->renormalize;
-      e.M_out = has_demag(p) ? ctx->Mst[0] : nullptr;
-      return eval_rhs(ctx, p, npad, 1, e);
+      e.base = m; e.h = dt / 6.0; e.renorm = o->renormalize;
+      route(e, m, M0);
+      if ((r = eval_rhs(ctx, p, npad, 1, e))) return r;
+      return finish(m, M0);
     };
     auto sample_if_due = [&](int64_t done) -> int {
       if (o->sample_every > 0 && done % o->sample_every == 0 && samples && res->n_samples < sample_cap) {
@@ -705,10 +762,9 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       // the stop test (Eq. 2) needs the torque of every step's first stage: one host
       // read per step; a satisfied test leaves m untouched
       while (done < nsteps) {
-        MT_CUDA_OK(ctx, cudaMemsetAsync(d_tq, 0, 8, st));
+        MT_CUDA_OK(ctx, cudaMemsetAsync(d_err, 0, 16, st));
         if ((rc = stage1())) return rc;
-        MT_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hscal, d_tq, 8, cudaMemcpyDeviceToHost, st));
-        MT_CUDA_OK(ctx, cudaStreamSynchronize(st));
+        if ((rc = read_scalars(1))) return rc;
         res->max_torque = bits_to_double(ctx->hscal[0]);
         if (res->max_torque <= o->torque_tol) break;
         if ((rc = stages234())) return rc;
@@ -726,7 +782,7 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       cudaGraphExec_t exec = nullptr;
       int64_t graph_launches = 0;
       while (done < nsteps && !rc) {
-        if (done >= chunk && done % chunk == 0 && nsteps - done >= chunk) {
+        if (!sh && done >= chunk && done % chunk == 0 && nsteps - done >= chunk) {  // (exchange callbacks are host calls)
           if (!exec) {
             // capture on a private stream (the caller's may be the legacy default stream, which cannot
             // be captured); the instantiated graph is then launched on the caller's stream
@@ -777,12 +833,11 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
     int64_t next_sample = 1;
     // k1 = f(m)
     {
-      MT_CUDA_OK(ctx, cudaMemsetAsync(d_tq, 0, 8, st));
+      MT_CUDA_OK(ctx, cudaMemsetAsync(d_err, 0, 16, st));
       EpiArgs e = base;
       e.y = m; e.k_out = k[0]; e.torque_bits = d_tq;
       if ((rc = eval_rhs(ctx, p, npad, 0, e))) return rc;
-      MT_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hscal, d_tq, 8, cudaMemcpyDeviceToHost, st));
-      MT_CUDA_OK(ctx, cudaStreamSynchronize(st));
+      if ((rc = read_scalars(1))) return rc;
       res->max_torque = bits_to_double(ctx->hscal[0]);
       res->rhs_calls = 1;
     }
@@ -820,9 +875,10 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       int src = 0;
       {
         EpiArgs e = base;
-        e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[0]; e.coef[0] = DP_A[1][0]; e.base = m; e.h = h; e.y_out = ya;
-        e.M_out = has_demag(p) ? ctx->Mst[src ^ 1] : nullptr;
-        if ((rc = mt_launch_combine(ctx, e))) return rc;
+        e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[0]; e.coef[0] = DP_A[1][0]; e.base = m; e.h = h;
+        void* Md = has_demag(p) ? ctx->Mst[src ^ 1] : nullptr;
+        route(e, ya, Md);
+        if ((rc = mt_launch_combine(ctx, e)) || (rc = finish(ya, Md))) return rc;
         src ^= 1;
       }
       double* yin = ya;
@@ -832,9 +888,10 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
         e.y = yin; e.k_out = k[s];
         e.do_comb = 1; e.ncomb = s + 1;
         for (int j = 0; j <= s; ++j) { e.kptr[j] = k[j]; e.coef[j] = DP_A[s + 1][j]; }
-        e.base = m; e.h = h; e.y_out = yout;
-        e.M_out = has_demag(p) ? ctx->Mst[src ^ 1] : nullptr;
-        if ((rc = eval_rhs(ctx, p, npad, src, e))) return rc;
+        e.base = m; e.h = h;
+        void* Md = has_demag(p) ? ctx->Mst[src ^ 1] : nullptr;
+        route(e, yout, Md);
+        if ((rc = eval_rhs(ctx, p, npad, src, e)) || (rc = finish(yout, Md))) return rc;
         src ^= 1;
         double* tmp = yin; yin = yout; yout = tmp;
       }
@@ -847,12 +904,11 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
         e.nerr = 7;
         for (int j = 0; j < 7; ++j) { e.eptr[j] = k[j]; e.ecoef[j] = DP_E[j]; }
         e.ebase = m; e.atol = o->atol; e.rtol = o->rtol; e.err_bits = d_err; e.h = h;
-        e.do_comb = 1; e.ncomb = 0; e.base = yin; e.y_out = mc; e.renorm = o->renormalize;
-        e.M_out = nullptr;
+        e.do_comb = 1; e.ncomb = 0; e.base = yin; e.renorm = o->renormalize;
+        route(e, mc, nullptr);  // sharded: the candidate's rows wait in the gather buffer for the verdict
         if ((rc = eval_rhs(ctx, p, npad, src, e))) return rc;
       }
-      MT_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hscal, d_err, 16, cudaMemcpyDeviceToHost, st));
-      MT_CUDA_OK(ctx, cudaStreamSynchronize(st));
+      if ((rc = read_scalars(2))) return rc;
       res->rhs_calls += 6;
       const double err = bits_to_double(ctx->hscal[0]);
       const double tq7 = bits_to_double(ctx->hscal[1]);
@@ -866,7 +922,8 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       fac = fmin(5.0, fmax(0.2, fac));
       if (err <= 1.0) {
         t = clipped ? t_target : t + h;
-        MT_CUDA_OK(ctx, cudaMemcpyAsync(m, mc, (size_t)sv * sizeof(double), cudaMemcpyDeviceToDevice, st));
+        if (sh) { if ((rc = finish(m, nullptr))) return rc; }
+        else MT_CUDA_OK(ctx, cudaMemcpyAsync(m, mc, (size_t)sv * sizeof(double), cudaMemcpyDeviceToDevice, st));
         double* tmp = k[0]; k[0] = k[6]; k[6] = tmp;  // FSAL
         res->max_torque = tq7;
         res->accepted++;

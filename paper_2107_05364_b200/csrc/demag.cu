@@ -208,17 +208,43 @@ __global__ void __launch_bounds__(256) demag_reduce_kernel(const double* partial
   row_epilogue(e, row, b, hd);
 }
 
+// both walk the launch's rows (all n, or a rank's band [row0, row0 + n_rows) of a sharded problem)
 __global__ void __launch_bounds__(256) local_only_kernel(EpiArgs e) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= e.n * e.batch) return;
+  if (idx >= e.n_rows * e.batch) return;
   const double hd[3] = {0.0, 0.0, 0.0};
-  row_epilogue(e, idx % e.n, (int)(idx / e.n), hd);
+  row_epilogue(e, idx % e.n_rows, (int)(idx / e.n_rows), hd);
 }
 
 __global__ void __launch_bounds__(256) combine_kernel(EpiArgs e) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= e.n * e.batch) return;
-  stage_combine(e, idx % e.n, (int)(idx / e.n), nullptr);
+  if (idx >= e.n_rows * e.batch) return;
+  stage_combine(e, e.row0 + idx % e.n_rows, (int)(idx / e.n_rows), nullptr);
+}
+
+// Row-sharded problems (mt.h section 8(e)): after the all-gather, block g of `pack` holds rows
+// [g n / world, (g+1) n / world) of the next stage state as [B][3][pad]; scatter into y[B][3][n] and
+// stage M = Ms*y in the tensor's dtype (padding j in [n, npad) zeroed as stage_M_kernel does).
+template <typename T>
+__global__ void __launch_bounds__(256) unpack_kernel(const double* __restrict__ pack, int world, int64_t pad,
+                                                     int64_t n, int64_t npad, int rows /* B*3 */,
+                                                     const double* __restrict__ Ms, double* __restrict__ y,
+                                                     T* __restrict__ M) {
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int r = blockIdx.y;
+  if (j >= npad || r >= rows) return;
+  if (j >= n) {
+    if (M) M[(int64_t)r * npad + j] = T(0);
+    return;
+  }
+  // owner of row j under the band rule begin(g) = g n / world: the largest g with begin(g) <= j
+  int g = (int)(((unsigned __int128)(j + 1) * (unsigned __int128)world - 1) / (unsigned __int128)n);
+  while (g + 1 < world && (int64_t)(((unsigned __int128)(g + 1) * (unsigned __int128)n) / (unsigned)world) <= j) ++g;
+  while (g > 0 && (int64_t)(((unsigned __int128)g * (unsigned __int128)n) / (unsigned)world) > j) --g;
+  const int64_t b0 = (int64_t)(((unsigned __int128)g * (unsigned __int128)n) / (unsigned)world);
+  const double v = pack[((int64_t)g * rows + r) * pad + (j - b0)];
+  y[(int64_t)r * n + j] = v;
+  if (M) M[(int64_t)r * npad + j] = (T)(Ms[j] * v);
 }
 
 // M[b][c][j] = T(Ms[j] * m[b][c][j]), zero in the padding j in [n, npad)
@@ -383,8 +409,20 @@ int mt_launch_demag(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_
   return rc;
 }
 
+int mt_launch_unpack(mt_ctx* ctx, const double* pack, int world, int64_t pad, int batch, int64_t n, int64_t npad,
+                     const double* Ms, double* y, void* M_out, int M_dtype) {
+  dim3 grid((unsigned)((npad + 255) / 256), (unsigned)(batch * 3));
+  if (M_dtype == MT_F32)
+    unpack_kernel<float><<<grid, 256, 0, ctx->stream>>>(pack, world, pad, n, npad, batch * 3, Ms, y, (float*)M_out);
+  else
+    unpack_kernel<double><<<grid, 256, 0, ctx->stream>>>(pack, world, pad, n, npad, batch * 3, Ms, y, (double*)M_out);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
 int mt_launch_local_only(mt_ctx* ctx, const EpiArgs& epi) {
-  const int64_t tot = epi.n * epi.batch;
+  const int64_t tot = epi.n_rows * epi.batch;
   local_only_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(epi);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
@@ -392,7 +430,7 @@ int mt_launch_local_only(mt_ctx* ctx, const EpiArgs& epi) {
 }
 
 int mt_launch_combine(mt_ctx* ctx, const EpiArgs& epi) {
-  const int64_t tot = epi.n * epi.batch;
+  const int64_t tot = epi.n_rows * epi.batch;
   combine_kernel<<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(epi);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());

@@ -6,9 +6,11 @@
 
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long* p, double v) {
   // bit patterns of non-negative doubles order like unsigned integers; NaN (all-ones exponent with
-  // mantissa, either sign) compares above every finite value, so a NaN handed to this function is
-  // never lost — callers must not launder it through fmax() first (fmax drops NaN operands).
-  atomicMax(p, (unsigned long long)__double_as_longlong(v));
+  // mantissa) compares above every finite value, so a NaN handed to this function is never lost —
+  // callers must not launder it through fmax() first (fmax drops NaN operands).  A NaN is stored as the
+  // canonical positive quiet NaN so that the word also orders correctly as a SIGNED integer (the
+  // max-reduction over ranks of a row-sharded problem may be done on int64, mt.h section 8(e)).
+  atomicMax(p, v != v ? 0x7ff8000000000000ull : (unsigned long long)__double_as_longlong(v));
 }
 
 __device__ __forceinline__ void cross3(const double a[3], const double b[3], double o[3]) {
@@ -40,9 +42,10 @@ __device__ __forceinline__ void stage_combine(const EpiArgs& e, int64_t i, int b
       for (int a = 0; a < 3; ++a) yo[a] /= r;
     }
   }
-  double* yout = e.y_out + sb;
+  const int64_t yld = e.y_ld ? e.y_ld : n;
+  double* yout = e.y_out + (int64_t)b * 3 * yld + (i - e.y_row0);
 #pragma unroll
-  for (int a = 0; a < 3; ++a) yout[a * n + i] = yo[a];
+  for (int a = 0; a < 3; ++a) yout[a * yld] = yo[a];
   if (e.M_out) {
     const double ms = e.Ms[i];
     const int64_t sm = (int64_t)b * 3 * e.npad;
@@ -58,7 +61,7 @@ __device__ __forceinline__ void stage_combine(const EpiArgs& e, int64_t i, int b
   }
 }
 
-// hd = H_d,i for state b (already carrying the minus sign of H = -N.M).
+// hd = H_d,i for state b (already carrying the minus sign of H = -N.M); i = row of the launch.
 __device__ __forceinline__ void row_epilogue(const EpiArgs& e, int64_t i, int b, const double hd[3]) {
   if (e.mode == 0) {
     double* o = e.Hd + (int64_t)b * 3 * e.n_rows;
@@ -67,6 +70,7 @@ __device__ __forceinline__ void row_epilogue(const EpiArgs& e, int64_t i, int b,
     o[2 * e.n_rows + i] = hd[2];
     return;
   }
+  i += e.row0;  // per-tile arrays and state vectors are full-size: global tile index from here on
   const int64_t n = e.n;
   const int64_t sb = (int64_t)b * 3 * n;
   const double* y = e.y + sb;

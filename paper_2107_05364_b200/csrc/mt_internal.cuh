@@ -65,7 +65,8 @@ struct EpiArgs {
   int mode;        // 0: store H_d only; 1: effective field + LL right-hand side (+ optional stages)
   int batch;
   int64_t n;       // tiles per state (stride of SoA vectors)
-  int64_t n_rows;  // rows of the launch (== n for mode 1)
+  int64_t n_rows;  // rows of the launch (== n for mode 1 unless the problem is row-sharded)
+  int64_t row0;    // mode 1: global index of the launch's first row (row-sharded problems; else 0)
   double* Hd;      // mode 0 output [B][3][n_rows]
   // mode 1 inputs
   const double* y;  // state the right-hand side is evaluated at [B][3][n]
@@ -95,6 +96,8 @@ struct EpiArgs {
   const double* base;
   double h;
   double* y_out;
+  int64_t y_ld;    // y_out is [B][3][y_ld] holding rows y_row0 .. (0, 0: [B][3][n] from row 0): a rank's
+  int64_t y_row0;  // block of the all-gather buffer when the problem is row-sharded
   int renorm;
   void* M_out;
   int M_dtype;
@@ -115,6 +118,10 @@ int mt_launch_demag(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_
                     const void* Mst, int64_t npad, const EpiArgs& epi);
 int mt_launch_local_only(mt_ctx* ctx, const EpiArgs& epi);  // N == NULL: H_d = 0
 int mt_launch_combine(mt_ctx* ctx, const EpiArgs& epi);     // stage combine without a field evaluation
+// row-sharded problems: blocks [world][B][3][pad] of the gathered stage state -> full state y[B][3][n]
+// and (M_out non-NULL) the staged Ms*y in the tensor's dtype
+int mt_launch_unpack(mt_ctx* ctx, const double* pack, int world, int64_t pad, int batch, int64_t n, int64_t npad,
+                     const double* Ms, double* y, void* M_out, int M_dtype);
 int mt_launch_mean(mt_ctx* ctx, const double* m, const double* vol, int batch, int64_t n, double t,
                    double* sample_row);
 int mt_ensure_ws(mt_ctx* ctx, void** p, size_t* cur, size_t need);

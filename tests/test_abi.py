@@ -42,7 +42,8 @@ def test_binding_struct_layouts_match_header_sizes():
     assert ctypes.sizeof(binding._Tiles) == 8 + 5 * 8
     assert ctypes.sizeof(binding._Opts) == 80
     assert ctypes.sizeof(binding._Result) == 56
-    assert ctypes.sizeof(binding._Problem) == 8 + 8 + 8 + 8 + 8 + 8 + 24 + 16 + 16 + 8 + 24 + 8 + 24 + 16 + 8 + 8 + 8
+    assert ctypes.sizeof(binding._Problem) == 8 + 8 + 8 + 8 + 8 + 8 + 24 + 16 + 16 + 8 + 24 + 8 + 24 + 16 + 8 + 8 + 8 + 8
+    assert ctypes.sizeof(binding._Shard) == 4 + 4 + 8 + 8 + 8 + 8 + 8  # rank, world, slice_pad, pack, scal, exchange, user
     assert ctypes.sizeof(binding._Sym) == 24
     assert ctypes.sizeof(binding._SelectState) == 64  # int, double, int, 3 x u64, int, double (8-byte aligned)
     assert ctypes.sizeof(binding._Sparse) == 8 + 8 + 8 + 8 + 5 * 8  # int dtype padded to 8; + cols16, panel_ptr

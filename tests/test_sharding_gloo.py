@@ -1,7 +1,10 @@
-"""World-size-2 (and 3) `gloo` test of the N > 1 host logic: band bounds,
-the all-gather of the per-rank field slices and their reassembly.  No GPU here, so the per-band field a
-rank's kernels would produce is stood in for by the oracle evaluated on that band of rows; what is under
-test is `paper_2107_05364_b200.sharding`, the code `bench.py --gpus N` runs over NCCL.
+"""World-size-2 (and 3) `gloo` tests of the N > 1 host logic: band bounds,
+the all-gather of the per-rank slices through the preallocated padded blocks, their reassembly, and a
+row-sharded RK4 trajectory driven through `binding.Shard`'s exchange callback.  No GPU here, so what a
+rank's kernels would compute for its rows is stood in for by the oracle evaluated on that band of rows;
+what is under test is `paper_2107_05364_b200.sharding` and the callback plumbing of `binding.Shard`, the
+code `bench.py --gpus N` runs over NCCL (the library side of the same protocol is covered on one GPU by
+tests/test_gpu_sharded.py).
 """
 import os
 import socket
@@ -78,3 +81,75 @@ def test_sharded_field_reassembles_to_the_full_field(oracle, world, grid):
     N = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=False)
     want = oracle.demag_field(N, w.Ms, w.m)
     np.testing.assert_array_equal(got, want)
+
+
+def _rk4_worker(rank: int, world: int, port: int, grid, steps: int, dt: float, q):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    try:
+        from oracle import mt_oracle as O
+        from paper_2107_05364_b200 import binding as B
+        w = W.config3(grid)          # exchange + anisotropy + demag: neighbours cross the band boundary
+        n = w.n
+        r0, r1 = S.row_band(rank, world, n)
+        rows = np.arange(r0, r1, dtype=np.int64)
+        N_band = O.assemble_rows(H.oracle_tiles(O, w), rows=rows, long_double=False, nthreads=1)
+        prob = H.oracle_problem(O, w, N_band, rows=rows)
+        shard = B.Shard(rank, world, n, 1, "cpu", S.dist_exchange(dist, rank))
+        assert shard.rows == (r0, r1)
+
+        def f(y):  # this rank's rows of the right-hand side at the full state y [1, 3, n]
+            k, _ = O.llg_rhs(prob, y, nthreads=1)
+            return k[0]
+
+        def stage(y_rows):  # what the library does per stage: own block -> gather -> full state
+            shard.pack[rank, 0, :, : r1 - r0] = torch.from_numpy(y_rows)
+            assert shard._cb(None, S.GATHER_STATE, None) == 0, shard.error
+            return S.unpack(shard.pack, n).numpy()
+
+        m = w.m[:1].copy()
+        for _ in range(steps):
+            mr = m[0][:, r0:r1]
+            k1 = f(m)
+            k2 = f(stage(mr + 0.5 * dt * k1))
+            k3 = f(stage(mr + 0.5 * dt * k2))
+            k4 = f(stage(mr + dt * k3))
+            new = mr + (dt / 6.0) * (k1 + 2.0 * k2 + 2.0 * k3 + k4)
+            new = new / np.linalg.norm(new, axis=0, keepdims=True)
+            m = stage(new)
+        # the two reduction words: every rank ends with the maximum
+        shard.scal[0], shard.scal[1] = 10 + rank, 100 - rank
+        assert shard._cb(None, S.MAX_SCALARS, None) == 0, shard.error
+        assert shard.scal.tolist() == [10 + world - 1, 100]
+        chk = torch.from_numpy(m.copy())
+        dist.broadcast(chk, src=0)
+        assert torch.equal(chk, torch.from_numpy(m))  # every rank holds the same state, bit for bit
+        if rank == 0:
+            q.put(m)
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world", [2, 3])
+def test_row_sharded_rk4_trajectory_matches_the_oracle(oracle, world):
+    """RK4 with every stage's state exchanged through the Shard callback (blocks [world, 1, 3, pad], in-place
+    all-gather, index reassembly; 125 rows over 2 and 3 ranks: uneven bands) against the oracle's own
+    unsharded RK4."""
+    grid, steps, dt = 5, 6, 2e-3
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_rk4_worker, args=(r, world, port, grid, steps, dt, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    got = q.get(timeout=180)
+    for p in procs:
+        p.join(timeout=120)
+        assert p.exitcode == 0
+    w = W.config3(grid)
+    N = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=False)
+    want, _, res = oracle.integrate(H.oracle_problem(oracle, w, N), w.m[0], method=oracle.RK4, dt=dt, t_end=steps * dt)
+    assert res["accepted"] == steps
+    assert np.max(np.abs(got[0] - want)) < 1e-13
+    assert np.max(np.abs(want - w.m[0])) > 1e-3  # the state moved
