@@ -1,14 +1,17 @@
 #!/usr/bin/env python
 """bench.py — headline measurement of the MagTense hot path on B200 (contract: see DESIGN.md §8).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 5]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 1..5] [--protocol]
 
 One "step" = one evaluation of the demagnetising field H_d = -N.(Ms m) (mt_demag_field, batch 1)
 over the whole resident tensor of BASELINE.json config 5 (64x64x16 = 65,536 unit cubes, 103.08 GB
 fp32 six-component tensor in HBM).  Around the timed steps the same run also reports: full-tensor
-assembly (tile-pairs/s), the fused Landau-Lifshitz right-hand side, the batch-8 variant, the
-end-to-end path with host buffers, the oracle timed on the host cores, clocks, and the roofline
-of the dominant kernel.  Prints ONE JSON line on rank 0.
+assembly (tile-pairs/s against the measured DFMA rate), the fused Landau-Lifshitz right-hand side, the
+batch-8 variant, the end-to-end path with host buffers, the microbenchmarked pipe / read-stream peaks,
+the other four configs (`all_configs`), the oracle timed on the host cores (all cores and one thread),
+clocks, and the roofline of the dominant kernel.  `--config k` puts another BASELINE config in the
+headline position; `--protocol` additionally runs that config's own workload as BASELINE.json states
+it (e.g. config 3: DP45 to equilibrium on the fp32 and the fp64 tensor).  Prints ONE JSON line on rank 0.
 """
 from __future__ import annotations
 
@@ -27,11 +30,22 @@ if ROOT not in sys.path:
 METRIC = "demag_Hd_evals_per_s"
 UNIT = "evals/s"
 HBM_FALLBACK_GBS = 6650.0  # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture (profiles/); key = (config, tensor dtype, n_gpus)
-NCU_TRAFFIC_BYTES = {(5, "f32", 1): 103.082146e9 + 5.291520e6}
-ASM_FP64_INST_PER_PAIR = 477.0  # DFMA + DADD + DMUL thread-instructions per cuboid pair (ncu, r02)
-NCU_TRAFFIC_SOURCE = "profiles/r02_ncu_full_summaries.md"
+# Counters read from committed `ncu --set full` captures (profiles/); every entry names the capture it
+# comes from and the commit whose kernels were captured, so that a stale entry can be seen as such.
+NCU_CAPTURES = {
+    # dram__bytes_read.sum + dram__bytes_write.sum per launch of the batch-1 field kernel;
+    # key = (config, tensor dtype, n_gpus)
+    "traffic_bytes": {
+        (5, "f32", 1): {"value": 103.082146e9 + 5.291520e6, "source": "profiles/r02_ncu_full_summaries.md",
+                        "kernel_commit": "45b85d2 (demag_tma_kernel unchanged since)"},
+    },
+    # DFMA + DADD + DMUL thread-instructions per tile pair of the assembly kernels
+    "asm_fp64_inst_per_pair": {
+        "cuboid": {"value": 386.4, "source": "profiles/r05_assembly_ncu_full.md", "kernel_commit": "6521e8f"},
+        "tet": {"value": 502.6, "source": "profiles/r05_assembly_ncu_full.md", "kernel_commit": "6521e8f"},
+    },
+}
+FLOORS_NOTE = "floor = tensor bytes / measured HBM peak (MEASURED_PEAKS.json hbm_gbs)"
 
 
 def parse_args():
@@ -40,31 +54,47 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=5, choices=[2, 3, 5])
+    ap.add_argument("--config", type=int, default=5, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--dtype", default="", choices=["", "f32", "f64"], help="tensor dtype (default: the config's)")
+    ap.add_argument("--protocol", action="store_true", help="also run the config's own workload as BASELINE.json states it")
+    ap.add_argument("--protocol-t-end", type=float, default=0.0, help="config 3 protocol: stop time (default 200)")
     ap.add_argument("--grid", type=str, default="", help="override nx,ny,nz (debug only; marks the line invalid)")
     ap.add_argument("--variant", type=int, default=0, help="demag kernel variant (0 auto, 1 LDG, 2 TMA)")
     ap.add_argument("--skip-extras", action="store_true", help="only the headline metric (used under ncu)")
     return ap.parse_args()
 
 
+def config_workload(cfg: int, dtype: str = "", batch: int = 8):
+    """(workload, description, tensor dtype) of BASELINE.json config `cfg`."""
+    from paper_2107_05364_b200 import workloads as W
+    if cfg == 1:
+        return W.config1(batch=min(batch, 4)), "config1: 8x8x8 unit cubes, N=512 tiles, fp64 tensor 12.6 MB (L2-resident)", dtype or "f64"
+    if cfg == 2:
+        return W.config2(batch=batch), "config2: 160x40x1 film, N=6400 tiles, fp32 tensor 0.98 GB", dtype or "f32"
+    if cfg == 3:
+        d = dtype or "f32"
+        return (W.config3(32, batch=batch, dtype=d),
+                f"config3: 32x32x32 cubes, N=32768 tiles, {d} tensor {'25.77' if d == 'f32' else '51.54'} GB", d)
+    if cfg == 4:
+        d = dtype or "f32"
+        return (W.config4(batch=batch),
+                f"config4: 20000 tetrahedra + 16384 octree cuboids, N=36384 tiles, {d} tensor {'31.77' if d == 'f32' else '63.54'} GB", d)
+    return W.config5(batch=batch), "config5: 64x64x16 unit cubes, N=65536 tiles, fp32 tensor 103.08 GB resident in HBM", dtype or "f32"
+
+
 def make_workload(args):
     from paper_2107_05364_b200 import workloads as W
     if args.grid:
         nx, ny, nz = (int(x) for x in args.grid.split(","))
-        w = W.config5(nx, ny, nz, batch=8)
-        return w, f"DEBUG grid {nx}x{ny}x{nz} (not a BASELINE config)", "f32"
-    if args.config == 5:
-        return W.config5(batch=8), "config5: 64x64x16 unit cubes, N=65536 tiles, fp32 tensor 103.08 GB resident in HBM", "f32"
-    if args.config == 3:
-        return W.config3(32, batch=8), "config3: 32x32x32 cubes, N=32768 tiles, fp32 tensor 25.77 GB", "f32"
-    return W.config2(batch=8), "config2: 160x40x1 film, N=6400 tiles, fp32 tensor 0.98 GB", "f32"
+        return W.config5(nx, ny, nz, batch=8), f"DEBUG grid {nx}x{ny}x{nz} (not a BASELINE config)", "f32"
+    return config_workload(args.config, args.dtype)
 
 
 def peak_hbm():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         try:
-            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs: read+write copy)"
         except Exception:
             pass
     return HBM_FALLBACK_GBS, "fallback (B200_PROFILING.md)"
@@ -116,145 +146,135 @@ class ClockSampler:
         return out
 
 
-def oracle_sample(w, band_rows: int, calls: int):
-    """The oracle as it stands, on a bounded sample: a `band_rows`-row band of the full-size tensor
-    (fp64 closed forms), then `calls` evaluations of H_d on that band; evals/s is extrapolated
-    linearly to all n rows.  Returns dict for cpu_baseline."""
+# ---- the oracle on the host cores ------------------------------------------------------------------------
+ORACLE_BAND_ROWS = 4096  # both oracle legs (cpu_baseline and --impl reference) time H_d on the same band
+
+
+def oracle_band(w, band_rows: int, threads: int):
+    """Rows 0, s, 2s, ... of the full-size tensor (fp64 closed forms, the oracle as it stands), assembled
+    with `threads` OpenMP threads.  Returns (O, N_band, rows, assembly seconds)."""
     import numpy as np
     from oracle import mt_oracle as O
     from tests import harness as H
-    threads = O.max_threads()
-    rows = np.arange(0, w.n, max(1, w.n // band_rows), dtype=np.int64)[:band_rows]
+    stride = max(1, w.n // band_rows)
+    rows = np.arange(0, w.n, stride, dtype=np.int64)[:band_rows]
     t0 = time.perf_counter()
     N = O.assemble_rows(H.oracle_tiles(O, w), rows=rows, long_double=False, nthreads=threads)
-    t_asm = time.perf_counter() - t0
+    return O, N, rows, time.perf_counter() - t0
+
+
+def oracle_time_field(O, N, w, calls: int, threads: int, warmup: int = 1) -> float:
+    for _ in range(warmup):
+        O.demag_field(N, w.Ms, w.m[:1], nthreads=threads)
     t0 = time.perf_counter()
     for _ in range(calls):
         O.demag_field(N, w.Ms, w.m[:1], nthreads=threads)
-    t_gemv = (time.perf_counter() - t0) / calls
-    evals_per_s = 1.0 / (t_gemv * w.n / len(rows))
-    return {
-        "value": evals_per_s, "unit": UNIT, "cores": threads, "kind": "oracle",
-        "sample": f"{len(rows)} of {w.n} target rows (stride {max(1, w.n // band_rows)}), {calls} H_d calls on the "
-                  f"stored fp64 band, extrapolated x{w.n / len(rows):.0f} to all rows",
+    return (time.perf_counter() - t0) / calls
+
+
+def oracle_sample(w):
+    """cpu_baseline: the oracle on a bounded sample of the same workload — a band of ORACLE_BAND_ROWS rows
+    of the stored fp64 tensor on all cores, and a 256-row band on ONE thread (both are
+    asked for); evals/s extrapolated linearly to all n rows and labelled as such."""
+    from oracle import mt_oracle as O0
+    threads = O0.max_threads()
+    t_all0 = time.perf_counter()
+    O, N, rows, t_asm = oracle_band(w, ORACLE_BAND_ROWS, threads)
+    t_gemv = oracle_time_field(O, N, w, calls=6, threads=threads)
+    scale = w.n / len(rows)
+    out = {
+        "value": 1.0 / (t_gemv * scale), "unit": UNIT, "cores": threads, "kind": "oracle",
+        "sample": f"{len(rows)} of {w.n} target rows (stride {max(1, w.n // ORACLE_BAND_ROWS)}), 6 H_d calls on the "
+                  f"stored fp64 band, extrapolated x{scale:.0f} to all rows",
+        "band_ms_per_call": t_gemv * 1e3,
         "assembly_pairs_per_s": len(rows) * w.n / t_asm,
         "assembly_sample": f"{len(rows) * w.n} pairs, fp64 closed forms, OpenMP over rows",
-        "seconds": t_asm + t_gemv * calls,
     }
+    del N
+    O, N1, rows1, t_asm1 = oracle_band(w, 256, 1)
+    t_gemv1 = oracle_time_field(O, N1, w, calls=3, threads=1)
+    out["single_thread"] = {
+        "value": 1.0 / (t_gemv1 * w.n / len(rows1)), "unit": UNIT, "cores": 1,
+        "sample": f"{len(rows1)} of {w.n} target rows, 3 H_d calls, extrapolated x{w.n / len(rows1):.0f}",
+        "band_ms_per_call": t_gemv1 * 1e3,
+        "assembly_pairs_per_s": len(rows1) * w.n / t_asm1,
+    }
+    out["seconds"] = time.perf_counter() - t_all0
+    return out
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle on the host cores, same metric/config; rank 0 only."""
+    """--impl reference: the CPU oracle on the host cores, same metric/config; rank 0 only.  A step is
+    one H_d evaluation on the ORACLE_BAND_ROWS-row band of the stored fp64 tensor (the same sample the
+    main line's cpu_baseline uses); `ms_per_step` is the MEASURED time of that step, `value` the
+    extrapolation to all rows, labelled."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
     w, wname, dtype = make_workload(args)
-    band = 64
+    from oracle import mt_oracle as O0
+    threads = O0.max_threads()
     steps = max(1, args.steps)
-    import numpy as np
-    from oracle import mt_oracle as O
-    from tests import harness as H
-    threads = O.max_threads()
-    rows = np.arange(0, w.n, max(1, w.n // band), dtype=np.int64)[:band]
-    N = O.assemble_rows(H.oracle_tiles(O, w), rows=rows, long_double=False, nthreads=threads)
-    for _ in range(max(1, min(args.warmup, 3))):
-        O.demag_field(N, w.Ms, w.m[:1], nthreads=threads)
-    t0 = time.perf_counter()
-    for _ in range(steps):
-        O.demag_field(N, w.Ms, w.m[:1], nthreads=threads)
-    dt = (time.perf_counter() - t0) / steps
-    ms_full = dt * (w.n / len(rows)) * 1e3
-    val = 1000.0 / ms_full
-    sample = (f"each step = H_d on {len(rows)} of {w.n} rows of the stored fp64 tensor band (oracle, OpenMP), "
-              f"extrapolated x{w.n / len(rows):.0f}")
+    O, N, rows, t_asm = oracle_band(w, ORACLE_BAND_ROWS, threads)
+    dt = oracle_time_field(O, N, w, calls=steps, threads=threads, warmup=max(1, min(args.warmup, 3)))
+    scale = w.n / len(rows)
+    val = 1.0 / (dt * scale)
+    sample = (f"each step = H_d on {len(rows)} of {w.n} rows of the stored fp64 tensor band (oracle, OpenMP, "
+              f"{threads} threads); ms_per_step is that band's measured time; value extrapolates x{scale:.0f} to all rows")
     line = {
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": steps,
-        "warmup": args.warmup, "ms_per_step": ms_full, "higher_is_better": True, "scaling": "strong",
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "strong",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": {"workload": wname},
-        "cpu_baseline": {"value": val, "unit": UNIT, "kind": "oracle", "cores": threads, "sample": sample},
+        "cpu_baseline": {"value": val, "unit": UNIT, "kind": "oracle", "cores": threads, "sample": sample,
+                         "assembly_pairs_per_s": len(rows) * w.n / t_asm,
+                         "full_evaluation_ms_extrapolated": dt * scale * 1e3},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line))
 
 
-def main():
-    args = parse_args()
-    if args.impl == "reference":
-        return run_reference(args)
+# ---- the device side -------------------------------------------------------------------------------------
+class Runner:
+    """One rank's context, timing helpers and per-kernel event timing (mt_profile_*)."""
 
-    import numpy as np
-    import torch
-    from paper_2107_05364_b200 import binding as B
-    from paper_2107_05364_b200 import sharding as S
-    from paper_2107_05364_b200 import workloads as W
-    from tests import harness as H
+    def __init__(self, args):
+        import torch
+        from paper_2107_05364_b200 import binding as B
+        self.torch, self.B, self.args = torch, B, args
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+        self.dist = None
+        if self.world > 1:
+            import torch.distributed as dist
+            dist.init_process_group("nccl", device_id=torch.device(f"cuda:{self.local_rank}"))
+            self.dist = dist
+        torch.cuda.set_device(self.local_rank)
+        self.dev = f"cuda:{self.local_rank}"
+        self.ctx = B.mt_create(self.local_rank)
+        if args.variant:
+            B.mt_set_demag_variant(self.ctx, args.variant)
+        self.kernel_ms = {}
+        self.peak, self.peak_src = peak_hbm()
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local_rank}"))
-    torch.cuda.set_device(local_rank)
-    dev = f"cuda:{local_rank}"
+    def ev(self):
+        return self.torch.cuda.Event(enable_timing=True)
 
-    w, wname, dtype = make_workload(args)
-    n = w.n
-    code = H.dtype_code(dtype)
-    ctx = B.mt_create(local_rank)
-    if args.variant:
-        B.mt_set_demag_variant(ctx, args.variant)
-    tiles = H.dev_tiles(w, dev)
-    # rows of this rank (§8e: the tensor is sharded by target rows; no collective in assembly)
-    r0, r1 = S.row_band(rank, world, n)
-    rows = r1 - r0
-    ld = W.leading_dim(n, dtype)
-    N = torch.empty((6, rows, ld), dtype=B.torch_dtype(code), device=dev)
-    status = torch.zeros(1, dtype=torch.int32, device=dev)
+    def barrier(self):
+        if self.dist is not None:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
 
-    def ev():
-        return torch.cuda.Event(enable_timing=True)
-
-    def barrier():
-        if dist is not None:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    # ---- assembly (A1-A3): every pair's closed form, timed once ---------------------------------
-    barrier()
-    a0, a1 = ev(), ev()
-    l0 = ctx.launches
-    a0.record()
-    B.mt_assemble_tensor(ctx, tiles, code, r0, r1, N, ld, status)
-    a1.record()
-    torch.cuda.synchronize()
-    asm_ms = a0.elapsed_time(a1)
-    asm_launches = ctx.launches - l0
-    assert int(status.item()) == 0, "singular geometry flagged"
-
-    m_all = torch.from_numpy(w.m).to(dev)              # [8, 3, n]
-    m1 = m_all[:1].contiguous()
-    Hd1 = torch.empty((1, 3, rows), dtype=torch.float64, device=dev)
-    gather_scratch = (torch.empty((world, 1, 3, S.max_band_rows(world, n)), dtype=torch.float64, device=dev)
-                      if world > 1 else None)
-
-    def step_field():
-        B.mt_demag_field(ctx, N, code, n, rows, ld, tiles.Ms, m1, 1, Hd1)
-        if dist is not None:  # the one real exchange step: every rank needs the whole field / next m
-            S.all_gather_field(dist, Hd1, n, rank, world, scratch=gather_scratch)
-
-    kernel_ms = {}
-
-    def timed(fn, warmup, steps, clocks=False, tag=None):
+    def timed(self, fn, warmup, steps, clocks=False, tag=None):
         """CUDA-event time per step (max over ranks).  With `tag`, the library also brackets every
         launch of the demag field kernel with its own events on the launching stream
         (mt_profile_begin/end): kernel_ms[tag] = that kernel's average device time per launch."""
+        B, ctx = self.B, self.ctx
         for _ in range(warmup):
             fn()
-        barrier()
-        sampler = ClockSampler(local_rank) if (clocks and rank == 0) else None
-        e0, e1 = ev(), ev()
+        self.barrier()
+        sampler = ClockSampler(self.local_rank) if (clocks and self.rank == 0) else None
+        e0, e1 = self.ev(), self.ev()
         l0 = ctx.launches
         if tag:
             B.mt_profile_begin(ctx)
@@ -262,211 +282,566 @@ def main():
         for _ in range(steps):
             fn()
         e1.record()
-        barrier()
+        self.barrier()
         if tag:
             tot, cnt = B.mt_profile_end(ctx)
-            kernel_ms[tag] = tot / max(1, cnt)
+            self.kernel_ms[tag] = tot / max(1, cnt)
         ms = e0.elapsed_time(e1) / steps
-        if dist is not None:
-            t = torch.tensor([ms, kernel_ms.get(tag, 0.0)], device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        if self.dist is not None:
+            t = self.torch.tensor([ms, self.kernel_ms.get(tag, 0.0)], device=self.dev)
+            self.dist.all_reduce(t, op=self.dist.ReduceOp.MAX)
             ms = float(t[0].item())
             if tag:
-                kernel_ms[tag] = float(t[1].item())
+                self.kernel_ms[tag] = float(t[1].item())
         return ms, (ctx.launches - l0), (sampler.stop() if sampler else None)
 
+    def assemble(self, tiles, code, r0, r1, ld):
+        """Every pair's closed form, timed once with CUDA events.  Returns (N, ms, launches)."""
+        torch, B = self.torch, self.B
+        N = torch.empty((6, r1 - r0, ld), dtype=B.torch_dtype(code), device=self.dev)
+        status = torch.zeros(1, dtype=torch.int32, device=self.dev)
+        self.barrier()
+        a0, a1 = self.ev(), self.ev()
+        l0 = self.ctx.launches
+        a0.record()
+        B.mt_assemble_tensor(self.ctx, tiles, code, r0, r1, N, ld, status)
+        a1.record()
+        torch.cuda.synchronize()
+        assert int(status.item()) == 0, "singular geometry flagged"
+        return N, a0.elapsed_time(a1), self.ctx.launches - l0
+
+    def measured_peaks(self, buf):
+        """Pipe and read-stream ceilings measured in this process on this device (mt_measure_peak)."""
+        B = self.B
+        out = {}
+        for name, kind in (("dfma_thread_inst_per_s", B.MT_PEAK_DFMA), ("ffma_thread_inst_per_s", B.MT_PEAK_FFMA),
+                           ("ffma2_thread_inst_per_s", B.MT_PEAK_FFMA2), ("mma_tf32_fma_per_s", B.MT_PEAK_MMA_TF32)):
+            out[name] = B.mt_measure_peak(self.ctx, kind)[0]
+        nbytes = min(buf.numel() * buf.element_size(), 16 << 30)
+        out["hbm_read_gbs"] = B.mt_measure_peak(self.ctx, B.MT_PEAK_HBM_READ, buf.view(-1)[: nbytes // buf.element_size()])[0] / 1e9
+        out["note"] = ("microbenchmarks of csrc/peaks.cu run on the bench's own stream: best of three after a warm-up; "
+                       "hbm_read = read-only stream by bulk copies into shared memory over "
+                       f"{nbytes / 2**30:.1f} GiB of the resident tensor")
+        return out
+
+
+def tensor_bytes(rows, n, s, batch=1):
+    """Algorithmic bytes of one field evaluation: tensor once, staged M, field out."""
+    return 6.0 * rows * n * s + batch * 3.0 * n * s + batch * 24.0 * rows
+
+
+def assembly_roofline(w, rows, asm_ms, dfma_peak):
+    """ALU roofline of the assembly: FP64 arithmetic thread-instructions (DFMA + DADD + DMUL, counted by
+    ncu per pair and kernel) per second against the measured DFMA issue rate."""
+    c = NCU_CAPTURES["asm_fp64_inst_per_pair"]
+    n_tet = int((w.type == 1).sum())
+    n_cub = w.n - n_tet
+    inst = rows * (n_cub * c["cuboid"]["value"] + n_tet * c["tet"]["value"])
+    rate = inst / (asm_ms * 1e-3)
+    return {"bound": "alu", "achieved": rate / 1e12, "peak": dfma_peak / 1e12 if dfma_peak else None,
+            "unit": "T FP64 thread-inst/s", "frac": rate / dfma_peak if dfma_peak else None,
+            "fp64_inst_per_pair": {"cuboid": c["cuboid"]["value"], "tet": c["tet"]["value"]},
+            "source": c["cuboid"]["source"], "kernel_commit": c["cuboid"]["kernel_commit"],
+            "peak_source": "measured in this run: mt_measure_peak(MT_PEAK_DFMA)"}
+
+
+def measure_config(R, cfg: int, dtype: str, steps: int):
+    """One BASELINE config end to end at its full size: assembly, mt_demag_field, mt_llg_rhs (batch 1)."""
+    import torch
+    from paper_2107_05364_b200 import workloads as W
+    from tests import harness as H
+    B = R.B
+    w, name, dtype = config_workload(cfg, dtype, batch=1)
+    n, code, s = w.n, H.dtype_code(dtype), (4 if dtype == "f32" else 8)
+    tiles = H.dev_tiles(w, R.dev)
+    ld = W.leading_dim(n, dtype)
+    N, asm_ms, _ = R.assemble(tiles, code, 0, n, ld)
+    m1 = torch.from_numpy(w.m[:1].copy()).to(R.dev)
+    Hd = torch.empty((1, 3, n), dtype=torch.float64, device=R.dev)
+    k1 = torch.empty_like(m1)
+    prob = H.dev_problem(w, tiles, N, dtype, ld)
+    tag = f"c{cfg}{dtype}"
+    ms_f, _, _ = R.timed(lambda: B.mt_demag_field(R.ctx, N, code, n, n, ld, tiles.Ms, m1, 1, Hd), 3, steps, tag=tag)
+    ms_r, _, _ = R.timed(lambda: B.mt_llg_rhs(R.ctx, prob, m1, 1, k1, None), 3, steps)
+    nbytes = tensor_bytes(n, n, s)
+    kms = R.kernel_ms[tag]
+    out = {"workload": name, "n": n, "dtype": dtype, "tensor_bytes": 6.0 * n * n * s,
+           "assembly_ms": asm_ms, "assembly_pairs_per_s": n * n / (asm_ms * 1e-3),
+           "assembly_roofline_frac": assembly_roofline(w, n, asm_ms, R.dfma_peak)["frac"],
+           "field_ms": ms_f, "field_kernel_ms": kms, "evals_per_s": 1000.0 / ms_f,
+           "achieved_gbs": nbytes / (kms * 1e-3) / 1e9, "frac": nbytes / (kms * 1e-3) / 1e9 / R.peak,
+           "floor_ms": nbytes / R.peak / 1e6, "rhs_ms": ms_r, "finite": bool(torch.isfinite(Hd).all().item())}
+    if 6.0 * n * n * s < 126e6:
+        out["note"] = "tensor is L2-resident (126 MB L2): the HBM roofline does not apply; the call is launch-bound"
+    del N, prob
+    torch.cuda.empty_cache()
+    return out
+
+
+def integrate_timed(R, prob, m, batch, **kw):
+    """mt_integrate bracketed by CUDA events; returns (t, counters, ms, launches)."""
+    e0, e1 = R.ev(), R.ev()
+    l0 = R.ctx.launches
+    e0.record()
+    t, res, rc = R.B.mt_integrate(R.ctx, prob, m, batch, kw.pop("t0", 0.0), allow=(R.B.MT_ERR_MAX_STEPS,), **kw)
+    e1.record()
+    R.torch.cuda.synchronize()
+    return t, res, e0.elapsed_time(e1), R.ctx.launches - l0
+
+
+def run_protocol(R, args, w, tiles, N, ld, dtype):
+    """The config's own workload as BASELINE.json words it, on the resident tensor of the headline run."""
+    import numpy as np
+    import torch
+    from paper_2107_05364_b200 import workloads as W
+    from tests import harness as H
+    B, ctx, dev = R.B, R.ctx, R.dev
+    n, code, s = w.n, H.dtype_code(dtype), (4 if dtype == "f32" else 8)
+    floor_ms = tensor_bytes(n, n, s) / R.peak / 1e6
+    m1 = torch.from_numpy(w.m[:1].copy()).to(dev)
+    out = {"config": args.config, "floor_ms_per_rhs": floor_ms, "floor_note": FLOORS_NOTE}
+
+    def block(fn, count):  # `count` back-to-back calls as one timed block
+        fn()
+        torch.cuda.synchronize()
+        e0, e1 = R.ev(), R.ev()
+        e0.record()
+        for _ in range(count):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        return e0.elapsed_time(e1)
+
+    if args.config in (1, 4, 5):
+        count = {1: 100, 4: 1000, 5: 200}[args.config]
+        Hd = torch.empty((1, 3, n), dtype=torch.float64, device=dev)
+        k1 = torch.empty_like(m1)
+        prob = H.dev_problem(w, tiles, N, dtype, ld)
+        ms = block(lambda: B.mt_demag_field(ctx, N, code, n, n, ld, tiles.Ms, m1, 1, Hd), count)
+        out["field"] = {"calls": count, "total_ms": ms, "ms_per_call": ms / count}
+        if args.config != 5:
+            ms = block(lambda: B.mt_llg_rhs(ctx, prob, m1, 1, k1, None), count)
+            out["llg_rhs"] = {"calls": count, "total_ms": ms, "ms_per_call": ms / count}
+        else:
+            m8 = torch.from_numpy(w.m).to(dev)
+            Hd8 = torch.empty((8, 3, n), dtype=torch.float64, device=dev)
+            ms = block(lambda: B.mt_demag_field(ctx, N, code, n, n, ld, tiles.Ms, m8, 8, Hd8), count)
+            out["field_batch8"] = {"calls": count, "total_ms": ms, "ms_per_call": ms / count,
+                                   "state_evals_per_s": 8 * count / (ms * 1e-3)}
+    elif args.config == 2:
+        # relax 2 ns with alpha = 1 and no applied field, then 1 ns under 25 mT at 170 degrees (DESIGN.md Q12/Q13)
+        x = w.extra
+        m = m1.clone()
+        for phase, steps in (("relax", x["relax_steps"]), ("dynamics", x["dynamics_steps"])):
+            wp = W.config2(batch=1, phase=phase)
+            prob = H.dev_problem(wp, tiles, N, dtype, ld)
+            samples = torch.zeros((steps // 100 + 1, 4), dtype=torch.float64, device=dev)
+            t, res, ms, launches = integrate_timed(R, prob, m, 1, method=B.MT_RK4, dt=x["dt"], t_end=steps * x["dt"],
+                                                   sample_every=100, samples=samples)
+            out[phase] = {"rk4_steps": res["accepted"], "rhs_calls": res["rhs_calls"], "total_ms": ms,
+                          "us_per_rhs": 1e3 * ms / max(1, res["rhs_calls"]), "launches": launches,
+                          "mean_m_end": samples[res["n_samples"] - 1, 1:].tolist()}
+        out["norm_error"] = float((m[0].norm(dim=0) - 1.0).abs().max().item())
+    else:
+        # config 3: DP45 to equilibrium (|m x H_eff| <= 1e-5 or t = 200), fp32 and fp64 tensors (Q11/Q12)
+        x = w.extra
+        t_end = args.protocol_t_end or x["t_end"]
+        runs = {}
+        for dt_name in ("f32", "f64"):
+            if dt_name == dtype:
+                Nn, ldn = N, ld
+            else:
+                ldn = W.leading_dim(n, dt_name)
+                Nn, _, _ = R.assemble(tiles, H.dtype_code(dt_name), 0, n, ldn)
+            prob = H.dev_problem(w, tiles, Nn, dt_name, ldn)
+            m = m1.clone()
+            E = torch.zeros((1, 5), dtype=torch.float64, device=dev)
+            B.mt_energy(ctx, prob, m, 1, E)
+            e_start = float(E[0, 4].item())
+            cap = int(t_end) + 2
+            samples = torch.zeros((cap, 4), dtype=torch.float64, device=dev)
+            t, res, ms, launches = integrate_timed(R, prob, m, 1, method=B.MT_DP45, dt=x["dt0"], t_end=t_end,
+                                                   rtol=x["rtol"], atol=x["atol"], torque_tol=x["torque_tol"],
+                                                   sample_dt=1.0, samples=samples)
+            B.mt_energy(ctx, prob, m, 1, E)
+            fl = tensor_bytes(n, n, 4 if dt_name == "f32" else 8) / R.peak / 1e6
+            runs[dt_name] = {"accepted": res["accepted"], "rejected": res["rejected"], "rhs_calls": res["rhs_calls"],
+                             "t_reached": t, "max_torque": res["max_torque"], "dt_last": res["dt_last"],
+                             "stopped_by": "torque" if res["max_torque"] <= x["torque_tol"] else "t_end",
+                             "total_s": ms * 1e-3, "ms_per_rhs": ms / max(1, res["rhs_calls"]), "floor_ms_per_rhs": fl,
+                             "frac_of_floor": fl / (ms / max(1, res["rhs_calls"])), "launches": launches,
+                             "energy_start": e_start, "energy_end": float(E[0, 4].item()),
+                             "mean_m_end": m[0].mean(dim=1).tolist(),
+                             "norm_error": float((m[0].norm(dim=0) - 1.0).abs().max().item())}
+            runs[dt_name]["_samples"] = samples[: res["n_samples"]].cpu().numpy()
+            if Nn is not N:
+                del Nn
+            del prob
+            torch.cuda.empty_cache()
+        a, b = runs["f32"].pop("_samples"), runs["f64"].pop("_samples")
+        k = min(len(a), len(b))
+        out.update(runs)
+        out["t_end"] = t_end
+        out["common_samples"] = k
+        out["max_abs_mean_m_f32_vs_f64"] = float(np.max(np.abs(a[:k, 1:] - b[:k, 1:]))) if k else None
+    return out
+
+def run_extras(R, args, out, w, tiles, N, ld, dtype, m_all, m1, Hd1, step_field, K):
+    """Everything around the headline: end-to-end path, fused right-hand side, batch 8, the NEXT rows'
+    formats (F1/F3), the other configs, small-N integrator costs, the oracle on the host cores."""
+    import torch
+    from paper_2107_05364_b200 import sharding as S
+    from paper_2107_05364_b200 import workloads as W
+    from tests import harness as H
+    B, ctx, dev, world, rank, dist, peak, kernel_ms = R.B, R.ctx, R.dev, R.world, R.rank, R.dist, R.peak, R.kernel_ms
+    n, code, s = w.n, H.dtype_code(dtype), (4 if dtype == "f32" else 8)
+    r0, r1 = S.row_band(rank, world, n)
+    rows = r1 - r0
+    nb = m_all.shape[0]
+    # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
+    m_host = torch.from_numpy(w.m[:1].copy()).pin_memory()
+    Hd_host = torch.empty((1, 3, rows), dtype=torch.float64).pin_memory()
+    ms_e2e, _, _ = R.timed(lambda: B.mt_demag_field_host(ctx, N, code, n, rows, ld, tiles.Ms, m_host, 1, Hd_host),
+                           3, max(5, K // 2))
+    out["e2e"] = {"value": 1000.0 / ms_e2e, "unit": UNIT, "ms_per_step": ms_e2e,
+                  "h2d_bytes_per_step": 3 * n * 8, "d2h_bytes_per_step": 3 * rows * 8}
+    # ---- fused right-hand side (A4-A6) and the batched variant (A7) ---------------------------------
+    prob = H.dev_problem(w, tiles, N, dtype, ld)
+    shard = None
+    if world > 1:
+        shard = B.Shard(rank, world, n, 1, dev, S.dist_exchange(dist, rank))
+        prob.shard = shard
+    k1 = torch.empty_like(m1)
+    ms_rhs, _, _ = R.timed(lambda: B.mt_llg_rhs(ctx, prob, m1, 1, k1, None), 3, max(5, K // 2))
+    out["llg_rhs"] = {"evals_per_s": 1000.0 / ms_rhs, "ms": ms_rhs}
+    if world > 1:
+        # the simulation loop, row-sharded (mt.h section 8(e)): RK4 steps of mt_integrate, one in-place
+        # all-gather of the next stage state per right-hand side
+        mi = m1.clone()
+        steps_rk = 8
+        dt_rk = float(w.extra.get("dt", 1e-3)) if isinstance(w.extra, dict) else 1e-3
+        integrate_timed(R, prob, mi, 1, method=B.MT_RK4, dt=dt_rk, t_end=2 * dt_rk)
+        R.barrier()
+        t, res, ms, launches = integrate_timed(R, prob, mi, 1, method=B.MT_RK4, dt=dt_rk, t_end=steps_rk * dt_rk)
+        tt = torch.tensor([ms], device=dev)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        out["sharded_rk4"] = {"rhs_calls": res["rhs_calls"], "ms_per_rhs": float(tt.item()) / res["rhs_calls"],
+                              "rhs_evals_per_s": 1000.0 * res["rhs_calls"] / float(tt.item()),
+                              "exchange": "one all_gather_into_tensor (NCCL) of the next stage state per right-hand side",
+                              "finite": bool(torch.isfinite(mi).all().item())}
+    if nb >= 8:
+        Hd8 = torch.empty((8, 3, rows), dtype=torch.float64, device=dev)
+        ms_b8, _, _ = R.timed(lambda: B.mt_demag_field(ctx, N, code, n, rows, ld, tiles.Ms, m_all, 8, Hd8),
+                              3, max(5, K // 4), tag="b8")
+        alg_b8 = tensor_bytes(rows, n, s, batch=8)
+        out["batch8"] = {"state_evals_per_s": 8000.0 / ms_b8, "ms": ms_b8, "kernel_ms": kernel_ms["b8"],
+                         "achieved_gbs": alg_b8 / (kernel_ms["b8"] * 1e-3) / 1e9,
+                         "frac": alg_b8 / (kernel_ms["b8"] * 1e-3) / 1e9 / peak,
+                         "kernel": "demag_tma_mma_kernel (3xTF32 mma.sync, fp64 drain)" if dtype == "f32" else "demag_tma_kernel<double, 8>"}
+        del Hd8
+    if world == 1 and w.grid is not None and n >= 4096:
+        extras_formats(R, args, out, w, tiles, N, ld, dtype, m1, Hd1, step_field, K)
+    if world == 1 and args.config == 5 and not args.grid:
+        try:
+            out["all_configs"] = [measure_config(R, c, d, 10) for c, d in ((1, "f64"), (2, "f32"), (3, "f32"), (3, "f64"), (4, "f32"))]
+            out["all_configs"].append({"workload": out["config"]["workload"], "n": n, "dtype": dtype,
+                                       "tensor_bytes": 6.0 * n * n * s, "assembly_ms": out["assembly"]["ms"],
+                                       "assembly_pairs_per_s": out["assembly"]["pairs_per_s"],
+                                       "assembly_roofline_frac": out["assembly"]["roofline"]["frac"],
+                                       "field_ms": out["ms_per_step"], "field_kernel_ms": kernel_ms["b1"],
+                                       "evals_per_s": out["value"], "achieved_gbs": out["roofline"]["achieved"],
+                                       "frac": out["roofline"]["frac"], "rhs_ms": ms_rhs})
+            out["threshold_curve_config2"] = threshold_curve(R, 2, K)
+            out["integrators_small_n"] = integrators_small_n(R)
+        except Exception as exc:  # an extra must never cost the headline line
+            out["all_configs_error"] = repr(exc)[:300]
+    if rank == 0 and world == 1:
+        out["cpu_baseline"] = oracle_sample(w)
+
+def extras_formats(R, args, out, w, tiles, N, ld, dtype, m1, Hd1, step_field, K):
+    """NEXT rows on the headline tensor: F3 pair-symmetric half, F1 thresholded tensor (X = 0.9)."""
+    import torch
+    from paper_2107_05364_b200 import workloads as W
+    from tests import harness as H
+    B, ctx, dev, peak, kernel_ms = R.B, R.ctx, R.dev, R.peak, R.kernel_ms
+    n, code, s = w.n, H.dtype_code(dtype), (4 if dtype == "f32" else 8)
+    rows = n
+    ev = R.ev
+    # ---- F3: the same field from the pair-symmetric half (PAPER.md:153), congruent cuboid grid ----
+    st2 = torch.zeros(1, dtype=torch.int32, device=dev)
+    s0, s1 = ev(), ev()
+    s0.record()
+    Sy = B.mt_assemble_tensor_sym(ctx, tiles, code, st2)
+    s1.record()
+    torch.cuda.synchronize()
+    assert int(st2.item()) == 0
+    Hs = torch.empty_like(Hd1)
+    ms_sym, _, _ = R.timed(lambda: B.mt_demag_field_sym(ctx, Sy, tiles.Ms, m1, 1, Hs), 3, max(5, K // 2), tag="sym")
+    step_field()
+    torch.cuda.synchronize()
+    sym_bytes = Sy.data.numel() * s
+    out["sym_half"] = {"evals_per_s": 1000.0 / ms_sym, "ms": ms_sym, "kernel_ms": kernel_ms["sym"],
+                       "resident_bytes": sym_bytes, "achieved_gbs": sym_bytes / (kernel_ms["sym"] * 1e-3) / 1e9,
+                       "frac": sym_bytes / (kernel_ms["sym"] * 1e-3) / 1e9 / peak,
+                       "assembly_ms": s0.elapsed_time(s1),
+                       "rel_l2_vs_full_tensor_field": float(((Hs - Hd1).norm() / Hd1.norm()).item()),
+                       "note": "NEXT row F3: half storage, every stored block used for two rows"}
+    del Sy
+    torch.cuda.empty_cache()
+    # ---- F1: thresholded tensor (PAPER.md:239), fraction 0.9 ------------------------------------------
+    t0_, t1_, t2_ = ev(), ev(), ev()
+    t0_.record()
+    tau, _cnt = B.mt_threshold_value(ctx, N, code, n, rows, ld, 0.9)
+    t1_.record()
+    Sp = B.mt_sparse_build(ctx, N, code, n, rows, ld, tau)
+    t2_.record()
+    torch.cuda.synchronize()
+
+    def step_sparse():
+        B.mt_demag_field_sparse(ctx, Sp, tiles.Ms, m1, 1, Hs)
+    ms_sp, _, _ = R.timed(step_sparse, 3, max(5, K // 2), tag="sp")
+    bm_bytes = Sp.nbytes()
+    err_bm = float(((Hs - Hd1).norm() / Hd1.norm()).item())
+    # index rows (16-bit column per packed value): the field kernel walks the packed values
+    t3_, t4_ = ev(), ev()
+    t3_.record()
+    B.mt_sparse_index(ctx, Sp, drop_mask=True)
+    t4_.record()
+    ms_ix, _, _ = R.timed(step_sparse, 3, max(5, K // 2), tag="ix")
+    ix_bytes = Sp.nbytes()
+    th = {"evals_per_s": 1000.0 / ms_ix, "ms": ms_ix, "kernel_ms": kernel_ms["ix"],
+          "layout": "index rows (fp32 value + 16-bit column per kept entry)",
+          "tau": tau, "kept_entries": Sp.nnz, "resident_bytes": ix_bytes,
+          "achieved_gbs": ix_bytes / (kernel_ms["ix"] * 1e-3) / 1e9,
+          "frac": ix_bytes / (kernel_ms["ix"] * 1e-3) / 1e9 / peak,
+          "select_ms": t0_.elapsed_time(t1_), "compress_ms": t1_.elapsed_time(t2_),
+          "index_ms": t3_.elapsed_time(t4_),
+          "rel_l2_vs_full_tensor_field": float(((Hs - Hd1).norm() / Hd1.norm()).item()),
+          "bitmap_rows": {"ms": ms_sp, "kernel_ms": kernel_ms["sp"], "resident_bytes": bm_bytes,
+                          "achieved_gbs": bm_bytes / (kernel_ms["sp"] * 1e-3) / 1e9,
+                          "rel_l2_vs_full_tensor_field": err_bm},
+          "note": "NEXT row F1: 90 % of the non-zero elements removed"}
+    out["threshold_0.9"] = th
+    kept = Sp.nnz
+    del Sp
+    torch.cuda.empty_cache()
+    # streamed build: the same thresholded tensor from 4,096-row bands, dense tensor not needed
+    t5_, t6_ = ev(), ev()
+    t5_.record()
+    St = B.mt_sparse_build_streamed(ctx, tiles, code, 0.9, 4096)
+    t6_.record()
+    torch.cuda.synchronize()
+    th["streamed_build"] = {
+        "ms": t5_.elapsed_time(t6_), "band_rows": 4096, "band_bytes": 6 * 4096 * ld * s,
+        "same_tau_as_resident": bool(St.tau == tau), "same_kept_entries": bool(St.nnz == kept),
+        "peak_bytes_without_dense_tensor": 6 * 4096 * ld * s + St.nbytes() + St.nnz * 2,
+        "note": "5 assemblies of every band (3 selection passes, count, fill); dense tensor never resident"}
+    del St
+    torch.cuda.empty_cache()
+    if args.config != 5 or args.grid:
+        return
+    # ---- extras beyond the headline workload (guarded: a failure here cannot cost the headline line) ----
+    try:
+        # the same config-5 thresholded tensor with the tiles listed along a Morton curve
+        wm = W.reorder(w, W.morton_order(w))
+        tm = H.dev_tiles(wm, dev)
+        Sm = B.mt_sparse_build_streamed(ctx, tm, code, 0.9, 4096, index=True, keep_mask=False)
+        mm = torch.from_numpy(wm.m[:1].copy()).to(dev)
+        Hm = torch.empty_like(mm)
+        ms_mo, _, _ = R.timed(lambda: B.mt_demag_field_sparse(ctx, Sm, tm.Ms, mm, 1, Hm), 3, max(5, K // 2), tag="mo")
+        perm_t = torch.from_numpy(wm.extra["perm"]).to(dev)
+        th["morton_tile_order"] = {
+            "ms": ms_mo, "kernel_ms": kernel_ms["mo"], "resident_bytes": Sm.nbytes(),
+            "achieved_gbs": Sm.nbytes() / (kernel_ms["mo"] * 1e-3) / 1e9,
+            "frac": Sm.nbytes() / (kernel_ms["mo"] * 1e-3) / 1e9 / peak,
+            "rel_l2_vs_x_fastest_order": float(((Hm[0] - Hs[0][:, perm_t]).norm() / Hs.norm()).item()),
+            "note": "same tiles, same threshold fraction, tiles listed along a Z-order curve (workloads.morton_order)"}
+        del Sm
+        torch.cuda.empty_cache()
+        # beyond the dense tensor's size: N = 131,072 (dense fp32 412 GB), X = 0.95, streamed build
+        wb = W.config5(128, 64, 16, batch=1)
+        tb = H.dev_tiles(wb, dev)
+        t7_, t8_ = ev(), ev()
+        t7_.record()
+        base_alloc = int(torch.cuda.memory_allocated())
+        torch.cuda.reset_peak_memory_stats()
+        Sb = B.mt_sparse_build_streamed(ctx, tb, code, 0.95, 4096, index=True, keep_mask=False)
+        t8_.record()
+        mb = torch.from_numpy(wb.m[:1].copy()).to(dev)
+        Hb = torch.empty_like(mb)
+        ms_big, _, _ = R.timed(lambda: B.mt_demag_field_sparse(ctx, Sb, tb.Ms, mb, 1, Hb), 3, max(5, K // 2), tag="big")
+        out["beyond_dense_n131072_x0.95"] = {
+            "evals_per_s": 1000.0 / ms_big, "ms": ms_big, "kernel_ms": kernel_ms["big"],
+            "n": wb.n, "dense_bytes": 6 * wb.n * wb.n * s, "resident_bytes": Sb.nbytes(),
+            "kept_entries": Sb.nnz, "tau": Sb.tau, "build_ms": t7_.elapsed_time(t8_),
+            "achieved_gbs": Sb.nbytes() / (kernel_ms["big"] * 1e-3) / 1e9,
+            "frac": Sb.nbytes() / (kernel_ms["big"] * 1e-3) / 1e9 / peak,
+            "peak_allocated_bytes_of_the_build": int(torch.cuda.max_memory_allocated()) - base_alloc,
+            "finite": bool(torch.isfinite(Hb).all().item()),
+            "note": "dense tensor (412 GB) cannot be resident; thresholded tensor built band by band "
+                    "(beside the 103 GB tensor of the headline run, which stays resident)"}
+        del Sb
+        torch.cuda.empty_cache()
+    except Exception as exc:
+        out["beyond_dense_n131072_x0.95"] = {"error": repr(exc)[:300]}
+
+def threshold_curve(R, cfg: int, K: int):
+    """Time and memory of one field evaluation against the threshold fraction X on config `cfg`, the dense
+    tensor beside it: the shape of the paper's Fig. 7a, on both thresholded layouts."""
+    import torch
+    from paper_2107_05364_b200 import workloads as W
+    from tests import harness as H
+    B, ctx, dev = R.B, R.ctx, R.dev
+    w, name, dtype = config_workload(cfg, batch=1)
+    n, code = w.n, H.dtype_code(dtype)
+    tiles = H.dev_tiles(w, dev)
+    ld = W.leading_dim(n, dtype)
+    N, _, _ = R.assemble(tiles, code, 0, n, ld)
+    m1 = torch.from_numpy(w.m[:1].copy()).to(dev)
+    Hd = torch.empty((1, 3, n), dtype=torch.float64, device=dev)
+    Hs = torch.empty_like(Hd)
+    reps = max(20, K)
+    ms_dense, _, _ = R.timed(lambda: B.mt_demag_field(ctx, N, code, n, n, ld, tiles.Ms, m1, 1, Hd), 5, reps)
+    pts = []
+    for X in (0.0, 0.1, 0.2, 0.4, 0.6, 0.8, 0.9, 0.95):
+        tau, _ = B.mt_threshold_value(ctx, N, code, n, n, ld, X)
+        Sp = B.mt_sparse_build(ctx, N, code, n, n, ld, tau)
+        ms_bm, _, _ = R.timed(lambda: B.mt_demag_field_sparse(ctx, Sp, tiles.Ms, m1, 1, Hs), 5, reps)
+        bm_bytes = Sp.nbytes()
+        B.mt_sparse_index(ctx, Sp, drop_mask=True)
+        ms_ix, _, _ = R.timed(lambda: B.mt_demag_field_sparse(ctx, Sp, tiles.Ms, m1, 1, Hs), 5, reps)
+        pts.append({"X": X, "index_rows_ms": ms_ix, "bitmap_rows_ms": ms_bm, "index_rows_bytes": Sp.nbytes(),
+                    "bitmap_rows_bytes": bm_bytes, "kept_entries": Sp.nnz,
+                    "rel_l2_vs_dense_field": float(((Hs - Hd).norm() / Hd.norm()).item())})
+        del Sp
+    dense_bytes = 6.0 * n * ld * (4 if dtype == "f32" else 8)
+    del N
+    torch.cuda.empty_cache()
+    return {"workload": name, "dense_ms": ms_dense, "dense_bytes": dense_bytes, "points": pts,
+            "note": "Fig. 7a's axes (time per field evaluation vs threshold fraction); index rows cost 6 B per kept "
+                    "fp32 entry, so at small X they are larger and slower than the dense tensor — the slowdown the "
+                    "paper reports for its sparse matrix at small thresholds — and win from X ~ 0.45"}
+
+
+def integrators_small_n(R):
+    """Per-right-hand-side cost INSIDE mt_integrate where the step is launch-bound (configs 1 and 2):
+    RK4 (CUDA-graph replay) and DP45 (host controller, one 16-byte read per attempted step)."""
+    import torch
+    from paper_2107_05364_b200 import workloads as W
+    from tests import harness as H
+    B, ctx, dev = R.B, R.ctx, R.dev
+    res_all = {}
+    for cfg in (1, 2):
+        w, name, dtype = config_workload(cfg, batch=1)
+        n, code = w.n, H.dtype_code(dtype)
+        tiles = H.dev_tiles(w, dev)
+        ld = W.leading_dim(n, dtype)
+        N, _, _ = R.assemble(tiles, code, 0, n, ld)
+        prob = H.dev_problem(w, tiles, N, dtype, ld)
+        dt = float(w.extra["dt"]) if cfg == 2 else 1e-2
+        m = torch.from_numpy(w.m[:1].copy()).to(dev)
+        integrate_timed(R, prob, m, 1, method=B.MT_RK4, dt=dt, t_end=130 * dt)   # warm-up incl. graph capture
+        t, r, ms, _ = integrate_timed(R, prob, m, 1, method=B.MT_RK4, dt=dt, t_end=2048 * dt)
+        entry = {"n": n, "rk4": {"steps": r["accepted"], "us_per_rhs": 1e3 * ms / r["rhs_calls"]}}
+        m = torch.from_numpy(w.m[:1].copy()).to(dev)
+        t_end = 400 * dt
+        integrate_timed(R, prob, m, 1, method=B.MT_DP45, dt=dt, t_end=20 * dt, rtol=1e-6, atol=1e-8)
+        t, r, ms, _ = integrate_timed(R, prob, m, 1, method=B.MT_DP45, dt=dt, t_end=t_end, rtol=1e-6, atol=1e-8, t0=20 * dt)
+        entry["dp45"] = {"accepted": r["accepted"], "rejected": r["rejected"], "us_per_rhs": 1e3 * ms / max(1, r["rhs_calls"])}
+        res_all[f"config{cfg}"] = entry
+        del N, prob
+        torch.cuda.empty_cache()
+    return res_all
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2107_05364_b200 import sharding as S
+    from paper_2107_05364_b200 import workloads as W
+    from tests import harness as H
+
+    R = Runner(args)
+    B, ctx, dev, world, rank, dist = R.B, R.ctx, R.dev, R.world, R.rank, R.dist
+    peak = R.peak
+
+    w, wname, dtype = make_workload(args)
+    n = w.n
+    code = H.dtype_code(dtype)
+    s = 4 if dtype == "f32" else 8
+    tiles = H.dev_tiles(w, dev)
+    # rows of this rank (§8e: the tensor is sharded by target rows; no collective in assembly)
+    r0, r1 = S.row_band(rank, world, n)
+    rows = r1 - r0
+    ld = W.leading_dim(n, dtype)
+    # ---- assembly (A1-A3): every pair's closed form, timed once ---------------------------------
+    N, asm_ms, asm_launches = R.assemble(tiles, code, r0, r1, ld)
+
+    m_all = torch.from_numpy(w.m).to(dev)              # [B, 3, n]
+    nb = m_all.shape[0]
+    m1 = m_all[:1].contiguous()
+    Hd1 = torch.empty((1, 3, rows), dtype=torch.float64, device=dev)
+    # the one real exchange step of the sharded field: all-gather of the ranks' slices through
+    # preallocated, equally padded blocks (nothing allocated or reassembled inside the timed step)
+    gather = S.FieldGather(dist, rank, world, n, 1, dev) if world > 1 else None
+
+    def step_field():
+        B.mt_demag_field(ctx, N, code, n, rows, ld, tiles.Ms, m1, 1, Hd1)
+        if gather is not None:
+            gather.gather(Hd1)
+
     K, Wm = max(1, args.steps), max(3, args.warmup)
-    ms_step, launches, clocks = timed(step_field, Wm, K, clocks=True, tag="b1")
+    ms_step, launches, clocks = R.timed(step_field, Wm, K, clocks=True, tag="b1")
+    kernel_ms = R.kernel_ms
     value = 1000.0 / ms_step
+    l2_resident = 6.0 * rows * n * s < 126e6
 
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
         "dtype": dtype, "data": "synthetic",
         "config": {"workload": wname, "parallelism": f"row-sharded x{world}" if world > 1 else "single GPU",
-                   "l2": "tensor streamed per step is far larger than the 126 MB L2: no flush needed",
+                   "l2": ("tensor (12.6 MB) is L2-resident by design of this config: no flush, the HBM roofline does not apply"
+                          if l2_resident else
+                          "tensor streamed per step is far larger than the 126 MB L2: no flush needed"),
                    "batch": 1, "demag_variant": args.variant},
         "gpu_launches": launches, "clocks": clocks,
     }
     # ---- roofline of the dominant kernel (demag GEMV): algorithmic bytes 6 n^2 s + 3 n s + 24 n ---
-    s = 4 if dtype == "f32" else 8
-    alg_bytes = 6.0 * rows * n * s + 3.0 * n * s + 24.0 * rows
-    peak, peak_src = peak_hbm()
+    alg_bytes = tensor_bytes(rows, n, s)
     achieved = alg_bytes / (kernel_ms["b1"] * 1e-3) / 1e9
+    cap = NCU_CAPTURES["traffic_bytes"].get((args.config, dtype, world)) if not args.grid else None
     out["roofline"] = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                       "traffic": NCU_TRAFFIC_BYTES.get((args.config, dtype, world)) if not args.grid else None,
-                       "traffic_source": NCU_TRAFFIC_SOURCE,
-                       "peak_source": peak_src, "kernel": "demag field kernel (per rank), batch 1",
+                       "traffic": cap["value"] if cap else None,
+                       "traffic_source": (f"{cap['source']}, kernel as of {cap['kernel_commit']}" if cap else None),
+                       "peak_source": R.peak_src, "kernel": "demag field kernel (per rank), batch 1",
                        "kernel_ms": kernel_ms["b1"], "kernel_share_of_step": kernel_ms["b1"] / ms_step,
                        "algorithmic_bytes_per_launch": alg_bytes,
                        "note": "duration = CUDA events recorded by the library on the launching stream around "
-                               "the demag field kernel only (mt_profile_begin/end), averaged over the timed steps"}
+                               "the demag field kernel only (mt_profile_begin/end), averaged over the timed steps; "
+                               "the peak is a read+write copy, this kernel is a pure read stream: see "
+                               "measured_peaks.hbm_read_gbs and roofline.frac_of_read_peak"}
+    # measured ceilings (DFMA / FFMA / FFMA2 / mma.sync tf32 issue rates, read-only HBM stream)
+    R.dfma_peak = None
+    if rows * ld * 6 * s >= (1 << 30):
+        out["measured_peaks"] = R.measured_peaks(N)
+    else:
+        scratch = torch.empty(4 << 30, dtype=torch.uint8, device=dev)
+        scratch.zero_()
+        out["measured_peaks"] = R.measured_peaks(scratch)
+        del scratch
+    R.dfma_peak = out["measured_peaks"]["dfma_thread_inst_per_s"]
+    out["roofline"]["frac_of_read_peak"] = achieved / out["measured_peaks"]["hbm_read_gbs"]
     out["assembly"] = {"pairs_per_s": rows * n / (asm_ms * 1e-3) * world, "ms": asm_ms, "pairs": rows * n * world,
-                       "launches": asm_launches, "dtype": dtype, "every_pair_evaluated": True}
-    # ALU roofline of the assembly kernel: FP64 pipe = 64 thread-instructions per
-    # clock per SM (ncu: sm__sass_thread_inst_executed_op_dfma_pred_on.peak_sustained); the kernel
-    # executes 477 DFMA + DADD + DMUL thread-instructions per cuboid pair (ncu r02 capture, static per pair)
-    sm_count = torch.cuda.get_device_properties(local_rank).multi_processor_count
-    sm_hz = 1e6 * float((clocks or {}).get("sm_max_mhz") or 1965.0)
-    alu_peak = 64.0 * sm_count * sm_hz
-    asm_rate = ASM_FP64_INST_PER_PAIR * rows * n / (asm_ms * 1e-3)
-    out["assembly"]["roofline"] = {"bound": "alu", "achieved": asm_rate / 1e12, "peak": alu_peak / 1e12,
-                                   "unit": "T FP64 thread-inst/s", "frac": asm_rate / alu_peak,
-                                   "fp64_inst_per_pair": ASM_FP64_INST_PER_PAIR,
-                                   "source": "profiles/r02_ncu_full_summaries.md; peak at sm_max_mhz"}
-
+                       "launches": asm_launches, "dtype": dtype, "every_pair_evaluated": True,
+                       "roofline": assembly_roofline(w, rows, asm_ms, R.dfma_peak)}
     if not args.skip_extras:
-        # ---- end to end through the C-ABI with HOST buffers (pinned), copies inside the timed region
-        m_host = torch.from_numpy(w.m[:1].copy()).pin_memory()
-        Hd_host = torch.empty((1, 3, rows), dtype=torch.float64).pin_memory()
-
-        def step_e2e():
-            B.mt_demag_field_host(ctx, N, code, n, rows, ld, tiles.Ms, m_host, 1, Hd_host)
-        ms_e2e, _, _ = timed(step_e2e, 3, max(5, K // 2))
-        out["e2e"] = {"value": 1000.0 / ms_e2e, "unit": UNIT, "ms_per_step": ms_e2e,
-                      "h2d_bytes_per_step": 3 * n * 8, "d2h_bytes_per_step": 3 * rows * 8}
-        # ---- fused right-hand side (A4-A6) and batch 8 (A7) ----------------------------------------
-        prob = H.dev_problem(w, tiles, N, dtype, ld) if world == 1 else None
-        if prob is not None:
-            k1 = torch.empty_like(m1)
-
-            def step_rhs():
-                B.mt_llg_rhs(ctx, prob, m1, 1, k1, None)
-            ms_rhs, _, _ = timed(step_rhs, 3, max(5, K // 2))
-            out["llg_rhs"] = {"evals_per_s": 1000.0 / ms_rhs, "ms": ms_rhs}
-        Hd8 = torch.empty((8, 3, rows), dtype=torch.float64, device=dev)
-
-        def step_b8():
-            B.mt_demag_field(ctx, N, code, n, rows, ld, tiles.Ms, m_all, 8, Hd8)
-        ms_b8, _, _ = timed(step_b8, 3, max(5, K // 4), tag="b8")
-        alg_b8 = 6.0 * rows * n * s + 8 * 3.0 * n * s + 8 * 24.0 * rows
-        out["batch8"] = {"state_evals_per_s": 8000.0 / ms_b8, "ms": ms_b8, "kernel_ms": kernel_ms["b8"],
-                         "achieved_gbs": alg_b8 / (kernel_ms["b8"] * 1e-3) / 1e9,
-                         "frac": alg_b8 / (kernel_ms["b8"] * 1e-3) / 1e9 / peak}
-        if world == 1 and w.grid is not None:
-            # ---- F3: the same field from the pair-symmetric half, congruent cuboid grid ----
-            st2 = torch.zeros(1, dtype=torch.int32, device=dev)
-            s0, s1 = ev(), ev()
-            s0.record()
-            S = B.mt_assemble_tensor_sym(ctx, tiles, code, st2)
-            s1.record()
-            torch.cuda.synchronize()
-            assert int(st2.item()) == 0
-            Hs = torch.empty_like(Hd1)
-
-            def step_sym():
-                B.mt_demag_field_sym(ctx, S, tiles.Ms, m1, 1, Hs)
-            ms_sym, _, _ = timed(step_sym, 3, max(5, K // 2), tag="sym")
-            step_field()
-            torch.cuda.synchronize()
-            sym_bytes = S.data.numel() * s
-            out["sym_half"] = {"evals_per_s": 1000.0 / ms_sym, "ms": ms_sym, "kernel_ms": kernel_ms["sym"],
-                               "resident_bytes": sym_bytes, "achieved_gbs": sym_bytes / (kernel_ms["sym"] * 1e-3) / 1e9,
-                               "frac": sym_bytes / (kernel_ms["sym"] * 1e-3) / 1e9 / peak,
-                               "assembly_ms": s0.elapsed_time(s1),
-                               "rel_l2_vs_full_tensor_field": float(((Hs - Hd1).norm() / Hd1.norm()).item()),
-                               "note": "NEXT row F3: half storage, every stored block used for two rows"}
-            del S
-            # ---- F1: thresholded tensor, fraction 0.9, bitmap rows ---------------------------
-            t0_, t1_, t2_ = ev(), ev(), ev()
-            t0_.record()
-            tau, _cnt = B.mt_threshold_value(ctx, N, code, n, rows, ld, 0.9)
-            t1_.record()
-            Sp = B.mt_sparse_build(ctx, N, code, n, rows, ld, tau)
-            t2_.record()
-            torch.cuda.synchronize()
-
-            def step_sparse():
-                B.mt_demag_field_sparse(ctx, Sp, tiles.Ms, m1, 1, Hs)
-            ms_sp, _, _ = timed(step_sparse, 3, max(5, K // 2), tag="sp")
-            bm_bytes = Sp.nbytes()
-            err_bm = float(((Hs - Hd1).norm() / Hd1.norm()).item())
-            # index rows (16-bit column per packed value): the field kernel walks the packed values
-            t3_, t4_ = ev(), ev()
-            t3_.record()
-            B.mt_sparse_index(ctx, Sp, drop_mask=True)
-            t4_.record()
-            ms_ix, _, _ = timed(step_sparse, 3, max(5, K // 2), tag="ix")
-            ix_bytes = Sp.nbytes()
-            out["threshold_0.9"] = {"evals_per_s": 1000.0 / ms_ix, "ms": ms_ix, "kernel_ms": kernel_ms["ix"],
-                                    "layout": "index rows (fp32 value + 16-bit column per kept entry)",
-                                    "tau": tau, "kept_entries": Sp.nnz, "resident_bytes": ix_bytes,
-                                    "achieved_gbs": ix_bytes / (kernel_ms["ix"] * 1e-3) / 1e9,
-                                    "frac": ix_bytes / (kernel_ms["ix"] * 1e-3) / 1e9 / peak,
-                                    "select_ms": t0_.elapsed_time(t1_), "compress_ms": t1_.elapsed_time(t2_),
-                                    "index_ms": t3_.elapsed_time(t4_),
-                                    "rel_l2_vs_full_tensor_field": float(((Hs - Hd1).norm() / Hd1.norm()).item()),
-                                    "bitmap_rows": {"ms": ms_sp, "kernel_ms": kernel_ms["sp"], "resident_bytes": bm_bytes,
-                                                    "achieved_gbs": bm_bytes / (kernel_ms["sp"] * 1e-3) / 1e9,
-                                                    "rel_l2_vs_full_tensor_field": err_bm},
-                                    "note": "NEXT row F1: 90 % of the non-zero elements removed"}
-            del Sp
-            # streamed build: the same thresholded tensor from 4,096-row bands, dense tensor not needed
-            torch.cuda.synchronize()
-            t5_, t6_ = ev(), ev()
-            t5_.record()
-            St = B.mt_sparse_build_streamed(ctx, tiles, code, 0.9, 4096)
-            t6_.record()
-            torch.cuda.synchronize()
-            out["threshold_0.9"]["streamed_build"] = {
-                "ms": t5_.elapsed_time(t6_), "band_rows": 4096, "band_bytes": 6 * 4096 * ld * s,
-                "same_tau_as_resident": bool(St.tau == tau), "same_kept_entries": bool(St.nnz == out["threshold_0.9"]["kept_entries"]),
-                "peak_bytes_without_dense_tensor": 6 * 4096 * ld * s + St.nbytes() + St.nnz * 2,
-                "note": "5 assemblies of every band (3 selection passes, count, fill); dense tensor never resident"}
-            del St
-            # ---- beyond the dense tensor's size: N = 131,072 (dense fp32 412 GB), X = 0.95, streamed build.
-            # Not the headline workload: an extra, after the 103 GB tensor has been released.
-            if args.config == 5 and not args.grid:
-                try:
-                    prob.N = None
-                    N = None
-                    torch.cuda.synchronize()
-                    torch.cuda.empty_cache()
-                    # the same config-5 thresholded tensor with the tiles listed along a Morton curve
-                    wm = W.reorder(w, W.morton_order(w))
-                    tm = H.dev_tiles(wm)
-                    Sm = B.mt_sparse_build_streamed(ctx, tm, code, 0.9, 4096, index=True, keep_mask=False)
-                    mm = torch.from_numpy(wm.m[:1].copy()).to(dev)
-                    Hm = torch.empty_like(mm)
-
-                    def step_morton():
-                        B.mt_demag_field_sparse(ctx, Sm, tm.Ms, mm, 1, Hm)
-                    ms_mo, _, _ = timed(step_morton, 3, max(5, K // 2), tag="mo")
-                    perm_t = torch.from_numpy(wm.extra["perm"]).to(dev)
-                    out["threshold_0.9"]["morton_tile_order"] = {
-                        "ms": ms_mo, "kernel_ms": kernel_ms["mo"], "resident_bytes": Sm.nbytes(),
-                        "achieved_gbs": Sm.nbytes() / (kernel_ms["mo"] * 1e-3) / 1e9,
-                        "frac": Sm.nbytes() / (kernel_ms["mo"] * 1e-3) / 1e9 / peak,
-                        "rel_l2_vs_x_fastest_order": float(((Hm[0] - Hs[0][:, perm_t]).norm() / Hs.norm()).item()),
-                        "note": "same tiles, same threshold fraction, tiles listed along a Z-order curve (workloads.morton_order)"}
-                    del Sm
-                    wb = W.config5(128, 64, 16, batch=1)
-                    tb = H.dev_tiles(wb)
-                    t7_, t8_ = ev(), ev()
-                    t7_.record()
-                    torch.cuda.reset_peak_memory_stats()
-                    Sb = B.mt_sparse_build_streamed(ctx, tb, code, 0.95, 4096, index=True, keep_mask=False)
-                    t8_.record()
-                    mb = torch.from_numpy(wb.m[:1].copy()).to(dev)
-                    Hb = torch.empty_like(mb)
-
-                    def step_big():
-                        B.mt_demag_field_sparse(ctx, Sb, tb.Ms, mb, 1, Hb)
-                    ms_big, _, _ = timed(step_big, 3, max(5, K // 2), tag="big")
-                    out["beyond_dense_n131072_x0.95"] = {
-                        "evals_per_s": 1000.0 / ms_big, "ms": ms_big, "kernel_ms": kernel_ms["big"],
-                        "n": wb.n, "dense_bytes": 6 * wb.n * wb.n * s, "resident_bytes": Sb.nbytes(),
-                        "kept_entries": Sb.nnz, "tau": Sb.tau, "build_ms": t7_.elapsed_time(t8_),
-                        "achieved_gbs": Sb.nbytes() / (kernel_ms["big"] * 1e-3) / 1e9,
-                        "frac": Sb.nbytes() / (kernel_ms["big"] * 1e-3) / 1e9 / peak,
-                        "peak_allocated_bytes": int(torch.cuda.max_memory_allocated()),
-                        "finite": bool(torch.isfinite(Hb).all().item()),
-                        "note": "dense tensor (412 GB) cannot be resident; thresholded tensor built band by band"}
-                    del Sb
-                except Exception as exc:  # an extra must never cost the headline line
-                    out["beyond_dense_n131072_x0.95"] = {"error": repr(exc)[:300]}
-        if rank == 0 and world == 1:
-            out["cpu_baseline"] = oracle_sample(w, band_rows=4096, calls=6)
+        run_extras(R, args, out, w, tiles, N, ld, dtype, m_all, m1, Hd1, step_field, K)
+    if args.protocol and world == 1:
+        out["protocol"] = run_protocol(R, args, w, tiles, N, ld, dtype)
     if rank == 0:
         print(json.dumps(out))
     ctx.close()

@@ -671,7 +671,11 @@ __global__ void __launch_bounds__(kMmaWarps * 32, 1)
 #pragma unroll
         for (int i = 0; i < 4; ++i) {
           hi[i] = tf32_rn(raw[q][p][i]);
+#ifdef MT_MMA_LO_NOMASK
+          lo[i] = __float_as_uint(__uint_as_float(raw[q][p][i]) - __uint_as_float(hi[i]));  // the mma reads 19 bits
+#else
           lo[i] = __float_as_uint(__uint_as_float(raw[q][p][i]) - __uint_as_float(hi[i])) & 0xffffe000u;
+#endif
         }
         const int ra = prow[p], ca = pcol[p];
         const float4* b = bq[q];

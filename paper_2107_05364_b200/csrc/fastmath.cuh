@@ -55,3 +55,45 @@ __device__ __forceinline__ double log_ratio_fast(double a, double b) {
   if (fabs(d) <= 0.125 * s) return 2.0 * atanh_small(quot_pos(d, s));
   return log(a / b);
 }
+
+// sqrt(x) for positive normal x without the library's special-case branch (whose convergence barriers
+// keep the compiler from interleaving the eight independent square roots of a pair): 64-bit MUFU seed
+// of 1/sqrt(x) (20 bits), two coupled Goldschmidt steps (g -> sqrt(x), h -> 1/(2 sqrt(x))), one residual
+// correction: <= 1 ulp.  x = 0 gives NaN (inf * 0): a target on a source corner is singular anyway.
+__device__ __forceinline__ double sqrt_pos(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double g = x * y, h = 0.5 * y;
+  double e = fma(-h, g, 0.5);
+  g = fma(g, e, g);
+  h = fma(h, e, h);
+  e = fma(-h, g, 0.5);
+  g = fma(g, e, g);
+  h = fma(h, e, h);
+  return fma(fma(-g, g, x), h, g);
+}
+
+// Several small-argument evaluations at once: r[k] = atan(n[k]/d[k]) for k < NA, atanh(n[k]/d[k]) for
+// NA <= k < NA + NH (atan's series is atanh's at -t^2, so all share the coefficients and run as
+// independent chains the compiler can interleave).  Requires |n[k]| <= d[k]/8, d[k] > 0.
+// A cuboid pair has NA = 3 angles + NH = 3 logs, a tetrahedron pair 4 solid angles + 6 edge logs.
+template <int NA, int NH>
+__device__ __forceinline__ void many_small(const double* n, const double* d, double* r) {
+  constexpr int K = NA + NH;
+  double t[K], u[K], p[K];
+#pragma unroll
+  for (int k = 0; k < K; ++k) t[k] = quot_pos(n[k], d[k]);
+#pragma unroll
+  for (int k = 0; k < K; ++k) {
+    u[k] = t[k] * t[k];
+    if (k < NA) u[k] = -u[k];
+    p[k] = 1.0 / 17.0;
+  }
+  constexpr double c[7] = {1.0 / 15.0, 1.0 / 13.0, 1.0 / 11.0, 1.0 / 9.0, 1.0 / 7.0, 1.0 / 5.0, 1.0 / 3.0};
+#pragma unroll
+  for (int j = 0; j < 7; ++j)
+#pragma unroll
+    for (int k = 0; k < K; ++k) p[k] = fma(p[k], u[k], c[j]);
+#pragma unroll
+  for (int k = 0; k < K; ++k) r[k] = fma(t[k], p[k] * u[k], t[k]);
+}

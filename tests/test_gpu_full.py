@@ -142,7 +142,7 @@ def test_config3_sampled_rows(ctx, oracle, dtype):
     tiles = H.dev_tiles(w)
     N, ld, status = H.assemble(ctx, tiles, dtype)   # 25.8 GB / 51.5 GB
     assert status == 0
-    rows = W.sample_rows(3, w.n, 256, extra=grid_corner_rows(w.grid))
+    rows = W.sample_rows(3, w.n, 1024, extra=grid_corner_rows(w.grid))
     sampled_row_checks(ctx, oracle, w, tiles, N, ld, dtype, rows, w.m, 3)
     del N
     torch.cuda.empty_cache()
@@ -245,21 +245,42 @@ def test_config3_trajectory_replicas(ctx, oracle):
 
 
 # ---- config 4: 20,000 tetrahedra + 16,384 octree cuboids -----------------------------------------------
-def degenerate_pairs(w, limit=64):
-    """Targets whose centre lies exactly in a face plane of some cuboid source (guard rule A.3):
-    enumerate on the host, return target rows."""
+def degenerate_alignments(w, per_kind=8, chunk=1024):
+    """Guard rules of SURVEY A.3 (Q8): every (cuboid target, cuboid source) pair of the mesh
+    whose target centre lies exactly in the plane of a source face (one coordinate of d equals +-h:
+    "face" alignment) or on the line of a source edge (two coordinates: "edge" alignment), outside the
+    source.  ALL such pairs are enumerated on the host (16,384^2 pairs, exact comparisons); they are
+    classified by kind = (aligned axes, signs) and `per_kind` target rows are returned for every kind
+    that occurs, so that each branch of the guard rules is exercised.  (Checking every aligned pair's row
+    against the long-double oracle is out of reach: two thirds of the octree's leaves have at least one —
+    ~11,000 rows x 36,384 sources = 4e8 long-double pairs, minutes of host time.)
+    Returns (rows, {kind: number of pairs})."""
     cub = np.where(w.type == 0)[0]
-    c, h = w.center[cub], 0.5 * w.size[cub]
-    rows = []
-    big = cub[w.size[cub][:, 0] > w.size[cub][:, 0].min()]
-    for i in big[: 4 * limit]:
-        d = w.center[i] - c
-        on_plane = (np.abs(np.abs(d) - h) == 0.0).any(axis=1) & (np.abs(d) > h).any(axis=1)
-        if on_plane.any():
-            rows.append(int(i))
-        if len(rows) >= limit:
-            break
-    return rows
+    dev = "cuda" if torch.cuda.is_available() else "cpu"   # 2.7e8 pairs: exact comparisons, done with torch
+    c = torch.from_numpy(w.center[cub]).to(dev)
+    h = torch.from_numpy(0.5 * w.size[cub]).to(dev)
+    counts = np.zeros(27, dtype=np.int64)           # kind code: sum over axes of (1 + [d_ax > 0]) * 3^ax
+    targets = [set() for _ in range(27)]
+    pw = torch.tensor([1, 3, 9], dtype=torch.int64, device=dev)
+    for a0 in range(0, len(cub), chunk):
+        d = c[a0:a0 + chunk, None, :] - c[None, :, :]                 # [targets, sources, 3]
+        on = d.abs() == h[None, :, :]
+        outside = (d.abs() > h[None, :, :]).any(dim=2)
+        code = ((on.to(torch.int64) * (1 + (d > 0).to(torch.int64))) * pw).sum(dim=2)
+        code[~outside] = 0
+        counts += torch.bincount(code.reshape(-1), minlength=27).cpu().numpy()
+        for kc in torch.unique(code).tolist():
+            if kc:
+                targets[kc].update((a0 + torch.nonzero((code == kc).any(dim=1))[:, 0]).tolist())
+    kinds, rows = {}, set()
+    for kc in range(1, 27):
+        if counts[kc]:
+            kind = tuple((ax, 1 if (kc // 3**ax) % 3 == 2 else -1) for ax in range(3) if (kc // 3**ax) % 3)
+            kinds[kind] = int(counts[kc])
+            t = np.array(sorted(targets[kc]))
+            rng = W.rng_for(4, 100 + kc)
+            rows.update(int(cub[i]) for i in rng.choice(t, size=min(per_kind, len(t)), replace=False))
+    return sorted(rows), kinds
 
 
 def test_config4_full_size_sampled_rows(ctx, oracle):
@@ -268,10 +289,14 @@ def test_config4_full_size_sampled_rows(ctx, oracle):
     tiles = H.dev_tiles(w)
     N, ld, status = H.assemble(ctx, tiles, "f32")   # 31.8 GB
     assert status == 0
-    deg = degenerate_pairs(w)
-    assert len(deg) > 0  # the 2:1 octree does produce aligned pairs
+    deg, kinds = degenerate_alignments(w)
+    # the 2:1 octree does produce aligned pairs: face-plane alignments along every axis and both sides,
+    # and edge-line alignments (two coordinates at once)
+    assert all(((ax, sg),) in kinds for ax in range(3) for sg in (-1, 1)), sorted(kinds)
+    assert any(len(k) == 2 for k in kinds) and not any(len(k) == 3 for k in kinds), sorted(kinds)
+    assert len(deg) >= 32 and sum(kinds.values()) > 100000
     rng = W.rng_for(4, 9)
-    rows = np.array(sorted(set(rng.choice(20000, 128, replace=False)) | set(20000 + rng.choice(16384, 128, replace=False))
+    rows = np.array(sorted(set(rng.choice(20000, 512, replace=False)) | set(20000 + rng.choice(16384, 512, replace=False))
                            | set(deg)), dtype=np.int64)
     sampled_row_checks(ctx, oracle, w, tiles, N, ld, "f32", rows, w.m, 4)
     del N
@@ -292,7 +317,7 @@ def test_config5_full_size(ctx, oracle):
     tiles = H.dev_tiles(w)
     N, ld, status = H.assemble(ctx, tiles, "f32")   # 103.08 GB: plane has 2^32 elements (64-bit indexing)
     assert status == 0 and N.numel() == 6 * 65536 * 65536
-    rows = W.sample_rows(5, w.n, 192, extra=grid_corner_rows(w.grid) + [65535, 32768, 32767])
+    rows = W.sample_rows(5, w.n, 1024, extra=grid_corner_rows(w.grid) + [65535, 32768, 32767])
     Hd = sampled_row_checks(ctx, oracle, w, tiles, N, ld, "f32", rows, w.m, 5)
     # properties that hold at any size: uniform m -> H_d,i = -(sum_j N_ij) m, and sum_j N_ij is the
     # tensor of the whole 64x64x16 block at centre i (superposition): check rows of the GPU field
