@@ -39,7 +39,7 @@ extern "C" {
 #define MT_OK 0
 #define MT_ERR_INVALID_ARG (-1)       /* null / misaligned pointer, ld < n, n <= 0, bad dtype, batch < 1 */
 #define MT_ERR_CUDA (-2)              /* launch / allocation failure; text in mt_last_error            */
-#define MT_ERR_SINGULAR_GEOMETRY (-3) /* reserved for callers that read *status_flag (see assembly)    */
+#define MT_ERR_SINGULAR_GEOMETRY (-3) /* mt_check_status: an assembled block was non-finite (see assembly) */
 #define MT_ERR_STEP_UNDERFLOW (-4)    /* DP45 step size fell below 16 ulp of t                          */
 #define MT_ERR_MAX_STEPS (-5)         /* integrator hit max_steps before t_end                          */
 #define MT_ERR_UNIMPLEMENTED (-6)
@@ -92,6 +92,13 @@ typedef struct {
  * Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA.                                                        */
 int mt_assemble_tensor(mt_ctx* ctx, const mt_tiles* tiles, int dtype, int64_t row_begin,
                        int64_t row_end, void* out, int64_t ld, int32_t* status_flag);
+
+/* Reads a status flag written by the assembly calls (they are asynchronous and only OR bits into it):
+ * synchronises the stream and returns MT_OK when *status_flag (DEVICE int32) is 0,
+ * MT_ERR_SINGULAR_GEOMETRY when bit 0 is set (a target centre on a source face or edge: the tensor
+ * holds non-finite blocks and must not be used), MT_ERR_INVALID_ARG when only bit 1 is set
+ * (mt_assemble_tensor_sym on a mesh that is not one of congruent cuboids).                          */
+int mt_check_status(mt_ctx* ctx, const int32_t* status_flag);
 
 /* ---- F2. Far-field-stable assembly (the analytic form's "error at large distances
  * being of the same magnitude as the elements of the tensor itself"; "different
@@ -170,15 +177,18 @@ int mt_threshold_value(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t
  * ever held).  One radix digit (11 bits) is fixed per pass; a pass = mt_select_accumulate on every
  * row band of the tensor (any order, any band height: each band is assembled again per pass with
  * mt_assemble_tensor), then one mt_select_advance.  Repeat until st->done; st->tau, st->count then
- * equal what mt_threshold_value returns for the whole tensor (integer histograms: exact).
- * hist: DEVICE array of 2048 unsigned 64-bit counters owned by the caller (row-sharded over several
- * GPUs: sum it over the ranks before mt_select_advance).  mt_select_begin and mt_select_accumulate
+ * equal what mt_threshold_value returns for the whole tensor (integer histograms: exact).  The first pass
+ * fixes 11 bits (every element binned), each later pass up to 20 bits (only the elements carrying the
+ * prefix are binned): 2 passes for MT_F32, 4 for MT_F64.
+ * hist: DEVICE array of MT_SELECT_HIST_WORDS unsigned 64-bit counters owned by the caller (row-sharded
+ * over several GPUs: sum it over the ranks before mt_select_advance).  mt_select_begin and mt_select_accumulate
  * are asynchronous; mt_select_advance synchronises the stream.  Errors: MT_ERR_INVALID_ARG (NULL
  * state / hist, fraction outside [0, 1], bad tensor arguments, accumulate after done), MT_ERR_CUDA. */
+#define MT_SELECT_HIST_WORDS (1 << 20)
 typedef struct {
   int dtype;
   double fraction;
-  int hi;                          /* key bits [hi, 32|64) are fixed to prefix                     */
+  int hi;                          /* key bits [hi, 31|63) are fixed to prefix                     */
   unsigned long long prefix, k, count;
   int done;
   double tau;                      /* valid once done (+inf: everything removed)                   */
@@ -210,6 +220,31 @@ int mt_sparse_fill_index_band(mt_ctx* ctx, const void* N, int dtype, int64_t n, 
                               int64_t ld, double tau, int64_t row0, int64_t n_total,
                               const int64_t* row_ptr, uint32_t* mask, void* vals, uint16_t* cols16,
                               int64_t* panel_ptr);
+
+/* The streamed build as two library calls (the band loop and the passes run inside the library; only
+ * the allocation of the result, whose size the first call returns, stays with the caller).  Rows
+ * [row_begin, row_end) of the tensor of `tiles` (the whole tensor, or a rank's band) are assembled band by
+ * band into `band` (DEVICE, [6][band_rows][ld], ld as for mt_assemble_tensor) once per pass.
+ *  mt_sparse_stream_count: fraction in [0, 1]: runs the selection passes (one assembly of every band per
+ *    radix digit) and writes the threshold to *tau_host; fraction < 0: *tau_host is taken as given.  Then
+ *    one more pass counts the kept entries: row_ptr (DEVICE, [6*(row_end-row_begin) + 1]) and *nnz_host.
+ *    Row-sharded: the threshold is a property of the WHOLE tensor, so `allreduce` (may be NULL on a
+ *    single rank) is called once per selection pass and must sum `hist` (DEVICE, MT_SELECT_HIST_WORDS
+ *    64-bit counters, caller-owned; may be NULL when allreduce is NULL) over the ranks in place, enqueued
+ *    on cuda_stream.
+ *  mt_sparse_stream_fill: one more pass writes mask (may be NULL with cols16), vals, and, when cols16 is
+ *    non-NULL, the index rows (cols16, panel_ptr) at their places, as mt_sparse_fill_index_band does.
+ * status_flag as in mt_assemble_tensor.  Both synchronise the stream before returning.
+ * Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA (also: a non-zero return of allreduce).                    */
+typedef int (*mt_allreduce_fn)(void* user, unsigned long long* hist, void* cuda_stream);
+int mt_sparse_stream_count(mt_ctx* ctx, const mt_tiles* tiles, int dtype, double fraction, int64_t row_begin,
+                           int64_t row_end, void* band, int64_t band_rows, int64_t ld, int64_t* row_ptr,
+                           unsigned long long* hist, mt_allreduce_fn allreduce, void* user,
+                           int32_t* status_flag, double* tau_host, int64_t* nnz_host);
+int mt_sparse_stream_fill(mt_ctx* ctx, const mt_tiles* tiles, int dtype, double tau, int64_t row_begin,
+                          int64_t row_end, void* band, int64_t band_rows, int64_t ld, const int64_t* row_ptr,
+                          uint32_t* mask, void* vals, uint16_t* cols16, int64_t* panel_ptr,
+                          int32_t* status_flag);
 
 /* Compression, two calls: mt_sparse_count fills row_ptr (DEVICE, [6*n_rows+1]) for threshold tau and
  * returns the number of kept entries in *nnz_host (synchronises); the caller allocates mask
@@ -435,6 +470,18 @@ int mt_profile_end(mt_ctx* ctx, double* total_ms, int64_t* launches);
 #define MT_PEAK_MMA_TF32 3
 #define MT_PEAK_HBM_READ 4
 int mt_measure_peak(mt_ctx* ctx, int kind, const void* buf, int64_t bytes, double* out_host);
+
+/* Where the DP45 step controller runs (A9).  0 (default): on the device for problems of at most 8,192
+ * tiles that are not row-sharded — an attempted step is then a fixed launch sequence replayed from a CUDA
+ * graph, the accept / reject decision, the next step size, the clipping to sample times and the stop
+ * tests are taken by a one-thread kernel, and the host reads the controller state every 8 or 16 attempts
+ * (attempts replayed after the end of the run do nothing) — and on the host otherwise (one 16-byte read
+ * per attempted step: invisible once a step takes milliseconds).  1: always on the host.  2: always on
+ * the device (not for row-sharded problems, which stay on the host).  Both follow the same rules
+ * (Q11/Q11b); the device evaluates err^(-1/5) with CUDA's pow, the host with the C library's,
+ * so the two step sequences can differ in the last bit of dt.
+ * Returns MT_OK or MT_ERR_INVALID_ARG.                                                              */
+int mt_set_step_control(mt_ctx* ctx, int mode);
 
 /* Tuning / A-B testing hook: selects the demag kernel variant (0 = default choice by shape,
  * 1 = register-streaming LDG kernel, 2 = TMA bulk-tensor pipeline, 3 = as 2 but batches of 5..8

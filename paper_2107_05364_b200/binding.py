@@ -22,14 +22,16 @@ MT_ERR_INVALID_ARG, MT_ERR_CUDA, MT_ERR_SINGULAR_GEOMETRY = -1, -2, -3
 MT_ERR_STEP_UNDERFLOW, MT_ERR_MAX_STEPS, MT_ERR_UNIMPLEMENTED = -4, -5, -6
 MT_F32, MT_F64 = 0, 1
 MT_RK4, MT_DP45 = 0, 1
+MT_SELECT_HIST_WORDS = 1 << 20
 COMPONENTS = ("xx", "xy", "xz", "yy", "yz", "zz")
 EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assemble_tensor",
-           "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_energy",
+           "mt_check_status", "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_energy",
            "mt_field_sweep", "mt_sparse_mask_words", "mt_threshold_value", "mt_sparse_count",
            "mt_sparse_fill", "mt_sparse_index", "mt_select_begin", "mt_select_accumulate", "mt_select_advance",
-           "mt_sparse_count_band", "mt_sparse_scan", "mt_sparse_fill_band", "mt_sparse_fill_index_band", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
+           "mt_sparse_count_band", "mt_sparse_scan", "mt_sparse_fill_band", "mt_sparse_fill_index_band",
+           "mt_sparse_stream_count", "mt_sparse_stream_fill", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
            "mt_demag_field_sym", "mt_set_assembly_mode", "mt_launch_count",
-           "mt_set_demag_variant", "mt_profile_begin", "mt_profile_end", "mt_measure_peak")
+           "mt_set_demag_variant", "mt_set_step_control", "mt_profile_begin", "mt_profile_end", "mt_measure_peak")
 
 
 class MtError(RuntimeError):
@@ -58,6 +60,7 @@ class _Problem(C.Structure):
 
 MT_XCHG_GATHER_STATE, MT_XCHG_MAX_SCALARS = 0, 1
 EXCHANGE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_int, C.c_void_p)
+ALLREDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_void_p)
 
 
 class _Shard(C.Structure):
@@ -113,6 +116,8 @@ def load() -> C.CDLL:
         lib.mt_destroy.argtypes = [C.c_void_p]
         lib.mt_set_demag_variant.argtypes = [C.c_void_p, C.c_int]
         lib.mt_set_assembly_mode.argtypes = [C.c_void_p, C.c_int]
+        lib.mt_set_step_control.argtypes = [C.c_void_p, C.c_int]
+        lib.mt_check_status.argtypes = [C.c_void_p, C.c_void_p]
         lib.mt_profile_begin.argtypes = [C.c_void_p]
         lib.mt_measure_peak.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64, C.POINTER(C.c_double)]
         lib.mt_profile_end.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
@@ -145,6 +150,12 @@ def load() -> C.CDLL:
                                                   C.c_double, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p,
                                                   C.c_void_p, C.c_void_p, C.c_void_p]
         lib.mt_sparse_index.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p, C.c_void_p]
+        lib.mt_sparse_stream_count.argtypes = [C.c_void_p, C.POINTER(_Tiles), C.c_int, C.c_double, C.c_int64, C.c_int64,
+                                               C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, ALLREDUCE_FN,
+                                               C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
+        lib.mt_sparse_stream_fill.argtypes = [C.c_void_p, C.POINTER(_Tiles), C.c_int, C.c_double, C.c_int64, C.c_int64,
+                                              C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
+                                              C.c_void_p, C.c_void_p, C.c_void_p]
         lib.mt_demag_field_sparse.argtypes = [C.c_void_p, C.POINTER(_Sparse), C.c_void_p, C.c_void_p, C.c_int,
                                               C.c_void_p]
         lib.mt_sym_tensor_elems.restype = C.c_int64
@@ -231,6 +242,11 @@ def mt_set_demag_variant(ctx: Context, variant: int):
     ctx.check(ctx.lib.mt_set_demag_variant(ctx.h, variant))
 
 
+def mt_set_step_control(ctx: Context, mode: int):
+    """DP45 controller: 0 auto (device for small unsharded problems), 1 host, 2 device."""
+    ctx.check(ctx.lib.mt_set_step_control(ctx.h, mode))
+
+
 def mt_profile_begin(ctx: Context):
     ctx.check(ctx.lib.mt_profile_begin(ctx.h))
 
@@ -278,6 +294,11 @@ def mt_assemble_tensor(ctx: Context, tiles: Tiles, dtype: int, row_begin: int, r
     t = tiles._c()
     ctx.check(ctx.lib.mt_assemble_tensor(ctx.h, C.byref(t), dtype, row_begin, row_end,
                                          _ptr(out, torch_dtype(dtype)), ld, _ptr(status_flag, torch.int32)))
+
+
+def mt_check_status(ctx: Context, status_flag: torch.Tensor, allow=()):
+    """Synchronises and raises MtError(MT_ERR_SINGULAR_GEOMETRY / MT_ERR_INVALID_ARG) when the assembly flagged."""
+    return ctx.check(ctx.lib.mt_check_status(ctx.h, _ptr(status_flag, torch.int32)), allow=allow)
 
 
 def mt_demag_field(ctx: Context, N: torch.Tensor, dtype: int, n: int, n_rows: int, ld: int,
@@ -491,9 +512,9 @@ def mt_sparse_build_streamed(ctx: Context, tiles: Tiles, dtype: int, fraction: f
                              index: bool = False, keep_mask: bool = True) -> SparseTensor:
     """Thresholded tensor of `tiles` without ever holding the dense tensor: every pass (one per radix
     digit of the selection, one for the counts, one for the fill) assembles the tensor again band by
-    band into one [6, band_rows, ld] buffer.  Sequence of C-ABI calls only: mt_assemble_tensor,
-    mt_select_*, mt_sparse_count_band / mt_sparse_scan / mt_sparse_fill_band.  `tau` given: the
-    selection passes are skipped.
+    band into one [6, band_rows, ld] buffer.  Two library calls, mt_sparse_stream_count and
+    mt_sparse_stream_fill (the band loop and the passes run inside the library); this function only
+    allocates.  `tau` given: the selection passes are skipped.
 
     Row-sharded (multi-GPU): `row_begin, row_end` = this rank's target rows; the
     result then has n_rows = row_end - row_begin.  The threshold is a property of the WHOLE tensor: after
@@ -513,44 +534,38 @@ def mt_sparse_build_streamed(ctx: Context, tiles: Tiles, dtype: int, fraction: f
     vec = 4 if dtype == MT_F32 else 2
     ld = (n + vec - 1) // vec * vec
     band = torch.empty(6 * band_rows * ld, dtype=tdt, device=dev)
-    bands = [(r0, min(row_end, r0 + band_rows)) for r0 in range(row_begin, row_end, band_rows)]
-
-    def assemble(r0, r1):
-        t = tiles._c()
-        ctx.check(ctx.lib.mt_assemble_tensor(ctx.h, C.byref(t), dtype, r0, r1, _ptr(band, tdt), ld,
-                                             _ptr(status_flag, torch.int32)))
-
-    if tau is None:
-        hist = torch.empty(2048, dtype=torch.int64, device=dev)
-        st = _SelectState()
-        ctx.check(ctx.lib.mt_select_begin(ctx.h, C.byref(st), dtype, float(fraction), _ptr(hist)))
-        while not st.done:
-            for r0, r1 in bands:
-                assemble(r0, r1)
-                ctx.check(ctx.lib.mt_select_accumulate(ctx.h, C.byref(st), _ptr(band, tdt), n, r1 - r0, ld, _ptr(hist)))
-            if allreduce is not None:
-                allreduce(hist)
-            ctx.check(ctx.lib.mt_select_advance(ctx.h, C.byref(st), _ptr(hist)))
-        tau = st.tau
     row_ptr = torch.empty(6 * n_loc + 1, dtype=torch.int64, device=dev)
-    for r0, r1 in bands:
-        assemble(r0, r1)
-        ctx.check(ctx.lib.mt_sparse_count_band(ctx.h, _ptr(band, tdt), dtype, n, r1 - r0, ld, float(tau),
-                                               r0 - row_begin, n_loc, _ptr(row_ptr)))
+    hist = torch.empty(MT_SELECT_HIST_WORDS, dtype=torch.int64, device=dev) if allreduce is not None else None
+    err = []
+
+    def _cb(_user, _hist, _stream):
+        try:
+            allreduce(hist)
+            return 0
+        except Exception as exc:  # nothing may propagate through the C frames
+            err.append(exc)
+            return 1
+
+    cb = ALLREDUCE_FN(_cb) if allreduce is not None else ALLREDUCE_FN()
+    t = tiles._c()
+    tau_c = C.c_double(float(tau) if tau is not None else 0.0)
     nnz = C.c_int64()
-    ctx.check(ctx.lib.mt_sparse_scan(ctx.h, _ptr(row_ptr), n_loc, C.byref(nnz)))
+    rc = ctx.lib.mt_sparse_stream_count(ctx.h, C.byref(t), dtype, float(fraction) if tau is None else -1.0, row_begin,
+                                        row_end, _ptr(band, tdt), band_rows, ld, _ptr(row_ptr), _ptr(hist), cb, None,
+                                        _ptr(status_flag, torch.int32), C.byref(tau_c), C.byref(nnz))
+    if err:
+        raise err[0]
+    ctx.check(rc)
+    tau = tau_c.value
     nw = int(ctx.lib.mt_sparse_mask_words(n))
     mask = torch.empty((6, n_loc, nw), dtype=torch.int32, device=dev) if keep_mask else None
     vals = torch.empty(max(1, nnz.value), dtype=tdt, device=dev)
     panels = (n + 65535) // 65536
     cols = torch.empty(max(1, nnz.value), dtype=torch.uint16, device=dev) if index else None
     pp = torch.empty((6 * n_loc, panels - 1), dtype=torch.int64, device=dev) if index and panels > 1 else None
-    for r0, r1 in bands:
-        assemble(r0, r1)
-        ctx.check(ctx.lib.mt_sparse_fill_index_band(ctx.h, _ptr(band, tdt), dtype, n, r1 - r0, ld, float(tau),
-                                                    r0 - row_begin, n_loc, _ptr(row_ptr), _ptr(mask), _ptr(vals),
-                                                    _ptr(cols), _ptr(pp)))
-    ctx.stream.synchronize()  # `band` is freed on return
+    ctx.check(ctx.lib.mt_sparse_stream_fill(ctx.h, C.byref(t), dtype, float(tau), row_begin, row_end, _ptr(band, tdt),
+                                            band_rows, ld, _ptr(row_ptr), _ptr(mask), _ptr(vals), _ptr(cols), _ptr(pp),
+                                            _ptr(status_flag, torch.int32)))
     return SparseTensor(n, n_loc, dtype, nw, row_ptr, mask, vals, nnz=nnz.value, tau=float(tau), cols16=cols,
                         panel_ptr=pp)
 

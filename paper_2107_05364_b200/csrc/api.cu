@@ -180,8 +180,12 @@ int mt_create(mt_ctx** out, int device, void* cuda_stream) {
     return MT_ERR_CUDA;
   }
   c->num_sms = prop.multiProcessorCount;
-  if (cudaMalloc((void**)&c->dscal, 8 * sizeof(unsigned long long)) != cudaSuccess ||
-      cudaMallocHost((void**)&c->hscal, 8 * sizeof(unsigned long long)) != cudaSuccess) {
+  // device scalars: [0] err bits, [1] torque bits, [2..5] the selection's bin search, [8 + 2048 ..] 256
+  // per-step torque words of an RK4 chunk; the pinned mirror holds
+  // the two words, the search result or the chunk's torques
+  if (cudaMalloc((void**)&c->dscal, (8 + 2048 + 256) * sizeof(unsigned long long)) != cudaSuccess ||
+      cudaMallocHost((void**)&c->hscal, 2048 * sizeof(unsigned long long)) != cudaSuccess) {
+    cudaFree(c->dscal);
     delete c;
     return MT_ERR_CUDA;
   }
@@ -202,6 +206,9 @@ int mt_destroy(mt_ctx* c) {
   cudaFree(c->sym_ws);
   cudaFree(c->dscal);
   cudaFree(c->stage_io);
+  cudaFree(c->dp_dev);
+  cudaFree(c->sel_hist);
+  cudaFreeHost(c->dp_host);
   cudaFreeHost(c->hscal);
   cudaFreeHost(c->pinned_io);
   if (c->cap_stream) cudaStreamDestroy(c->cap_stream);
@@ -252,6 +259,12 @@ int mt_set_demag_variant(mt_ctx* c, int variant) {
   return MT_OK;
 }
 
+int mt_set_step_control(mt_ctx* c, int mode) {
+  if (!c || mode < 0 || mode > 2) return MT_ERR_INVALID_ARG;
+  c->step_control = mode;
+  return MT_OK;
+}
+
 int mt_set_assembly_mode(mt_ctx* c, int mode) {
   if (!c || mode < 0 || mode > 1) return MT_ERR_INVALID_ARG;
   c->assembly_mode = mode;
@@ -270,6 +283,18 @@ int mt_assemble_tensor(mt_ctx* ctx, const mt_tiles* t, int dtype, int64_t row_be
   if (rc) return rc;
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
   return mt_launch_assemble(ctx, t, dtype, row_begin, row_end, out, ld, status_flag);
+}
+
+int mt_check_status(mt_ctx* ctx, const int32_t* status_flag) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  if (!status_flag) return mt_fail(ctx, MT_ERR_INVALID_ARG, "status_flag must be non-NULL");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  MT_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hscal, status_flag, sizeof(int32_t), cudaMemcpyDeviceToHost, ctx->stream));
+  MT_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  const int32_t f = *(const int32_t*)ctx->hscal;
+  if (f & 1) return mt_fail(ctx, MT_ERR_SINGULAR_GEOMETRY, "assembly produced a non-finite block: a target centre lies on a source face or edge");
+  if (f & 2) return mt_fail(ctx, MT_ERR_INVALID_ARG, "the pair-symmetric half needs a mesh of congruent axis-aligned cuboids");
+  return MT_OK;
 }
 
 int mt_demag_field(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
@@ -374,9 +399,24 @@ int mt_demag_field_sym(mt_ctx* ctx, const mt_sym_tensor* S, const double* Ms, co
 int64_t mt_sparse_mask_words(int64_t n) { return n <= 0 ? 0 : round_up((n + 31) / 32, 4); }
 
 // ---- threshold selection, one radix digit per pass; the passes may be fed band by band ---------------
+// Digits: the first pass fixes the top 11 bits of the 31 / 63-bit key (every element is binned: shared-
+// memory histogram with warp-aggregated runs), every later pass up to 20 bits (only the few elements that
+// carry the prefix are binned, straight into the global histogram): 2 passes for fp32, 4 for fp64
+// (r03: 3 and 6 passes of 11 bits).
 namespace {
-constexpr int kSelDigit = 11, kSelBins = 1 << kSelDigit;
-inline int sel_bits(int dtype) { return dtype == MT_F32 ? 32 : 64; }
+constexpr int kSelFirst = 11, kSelWide = 20;
+constexpr int64_t kSelHistWords = MT_SELECT_HIST_WORDS;
+static_assert(kSelHistWords == (1 << kSelWide), "histogram size = widest digit");
+inline int sel_bits(int dtype) { return dtype == MT_F32 ? 31 : 63; }  // the sign bit is cleared
+inline int sel_width(const mt_select_state* st) {
+  const int w = st->hi == sel_bits(st->dtype) ? kSelFirst : kSelWide;
+  return st->hi >= w ? w : st->hi;
+}
+int ensure_sel_hist(mt_ctx* ctx) {
+  if (ctx->sel_hist) return MT_OK;
+  MT_CUDA_OK(ctx, cudaMalloc((void**)&ctx->sel_hist, (size_t)kSelHistWords * sizeof(unsigned long long)));
+  return MT_OK;
+}
 }  // namespace
 
 int mt_select_begin(mt_ctx* ctx, mt_select_state* st, int dtype, double fraction, unsigned long long* hist) {
@@ -389,7 +429,7 @@ int mt_select_begin(mt_ctx* ctx, mt_select_state* st, int dtype, double fraction
   st->fraction = fraction;
   st->hi = sel_bits(dtype);
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
-  MT_CUDA_OK(ctx, cudaMemsetAsync(hist, 0, kSelBins * sizeof(unsigned long long), ctx->stream));
+  MT_CUDA_OK(ctx, cudaMemsetAsync(hist, 0, (size_t)kSelHistWords * sizeof(unsigned long long), ctx->stream));
   return MT_OK;
 }
 
@@ -401,7 +441,9 @@ int mt_select_accumulate(mt_ctx* ctx, const mt_select_state* st, const void* N, 
   int rc = check_tensor_args(ctx, N, st->dtype, n, n_rows, ld);
   if (rc) return rc;
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
-  const int width = st->hi >= kSelDigit ? kSelDigit : st->hi;
+  const int width = sel_width(st);
+  // the kernels test (key & ~((1 << hi) - 1)) == prefix << hi: in the first pass hi = 31 / 63 and the
+  // prefix is empty (the cleared sign bit)
   return mt_launch_select_hist(ctx, N, st->dtype, n, n_rows, ld, st->prefix, st->hi, st->hi - width, width, hist);
 }
 
@@ -410,32 +452,28 @@ int mt_select_advance(mt_ctx* ctx, mt_select_state* st, unsigned long long* hist
   if (!st || !hist) return mt_fail(ctx, MT_ERR_INVALID_ARG, "state and hist must be non-NULL");
   if (st->done) return MT_OK;
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
-  unsigned long long* h = new (std::nothrow) unsigned long long[kSelBins];
-  if (!h) return mt_fail(ctx, MT_ERR_CUDA, "out of host memory");
-  cudaError_t ce = cudaMemcpyAsync(h, hist, kSelBins * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream);
-  if (ce == cudaSuccess) ce = cudaMemsetAsync(hist, 0, kSelBins * sizeof(unsigned long long), ctx->stream);
-  if (ce == cudaSuccess) ce = cudaStreamSynchronize(ctx->stream);
-  if (ce != cudaSuccess) {
-    delete[] h;
-    MT_CUDA_OK(ctx, ce);
-  }
   const int bits = sel_bits(st->dtype);
-  const int width = st->hi >= kSelDigit ? kSelDigit : st->hi;
-  if (st->hi == bits) {  // first pass: total number of non-zero elements, and the rank to find
-    st->count = 0;
-    for (int b = 0; b < kSelBins; ++b) st->count += h[b];
-    st->k = (unsigned long long)floor(st->fraction * (double)st->count);
+  const int width = sel_width(st);
+  const bool first = st->hi == bits;
+  // the bin that holds rank k is found on the device (one block over the histogram): 32 bytes come back
+  unsigned long long* d_out = ctx->dscal + 2;
+  int rc = mt_launch_select_find(ctx, hist, 1 << width, st->k, first ? 1 : 0, st->fraction, d_out);
+  if (rc) return rc;
+  MT_CUDA_OK(ctx, cudaMemcpyAsync(ctx->hscal, d_out, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, ctx->stream));
+  MT_CUDA_OK(ctx, cudaMemsetAsync(hist, 0, (size_t)kSelHistWords * sizeof(unsigned long long), ctx->stream));
+  MT_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  const unsigned long long total = ctx->hscal[0], bin = ctx->hscal[1], rem = ctx->hscal[2];
+  if (first) {  // total number of non-zero elements, and the rank to find
+    st->count = total;
+    st->k = ctx->hscal[3];
     if (st->k >= st->count) {  // everything removed (also: nothing to rank)
       st->done = 1;
       st->tau = INFINITY;
-      delete[] h;
       return MT_OK;
     }
   }
-  int b = 0;
-  while (b < (1 << width) - 1 && st->k >= h[b]) { st->k -= h[b]; ++b; }
-  delete[] h;
-  st->prefix = (st->prefix << width) | (unsigned long long)b;
+  st->k = rem;
+  st->prefix = (st->prefix << width) | bin;
   st->hi -= width;
   if (st->hi == 0) {
     st->done = 1;
@@ -459,17 +497,16 @@ int mt_threshold_value(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t
   if (!tau_host || !(fraction >= 0.0 && fraction <= 1.0))
     return mt_fail(ctx, MT_ERR_INVALID_ARG, "fraction must be in [0, 1] and tau_host non-NULL");
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
-  // MSB-first radix select over the bit pattern of |v| (sign bit cleared: 31 / 63 significant bits),
-  // 11-bit digits; each pass is one stream of the tensor and one 16 KB histogram read.
-  unsigned long long* d_hist = nullptr;
-  MT_CUDA_OK(ctx, cudaMalloc((void**)&d_hist, kSelBins * sizeof(unsigned long long)));
+  // MSB-first radix select over the bit pattern of |v| (31 / 63 significant bits); each pass is one
+  // stream of the tensor; the histogram is ctx-owned (no allocation per call after the first)
+  if ((rc = ensure_sel_hist(ctx))) return rc;
+  unsigned long long* d_hist = ctx->sel_hist;
   mt_select_state st;
   rc = mt_select_begin(ctx, &st, dtype, fraction, d_hist);
   while (!rc && !st.done) {
     if ((rc = mt_select_accumulate(ctx, &st, N, n, n_rows, ld, d_hist))) break;
     rc = mt_select_advance(ctx, &st, d_hist);
   }
-  cudaFree(d_hist);
   if (rc) return rc;
   if (count_host) *count_host = (int64_t)st.count;
   *tau_host = st.tau;
@@ -534,6 +571,78 @@ int mt_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_
 int mt_sparse_fill(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
                    const int64_t* row_ptr, uint32_t* mask, void* vals) {
   return mt_sparse_fill_band(ctx, N, dtype, n, n_rows, ld, tau, 0, n_rows, row_ptr, mask, vals);
+}
+
+namespace {
+int check_stream_args(mt_ctx* ctx, const mt_tiles* t, int dtype, int64_t row_begin, int64_t row_end, const void* band,
+                      int64_t band_rows, int64_t ld) {
+  if (!t || !t->type || !t->center || !t->size || t->n <= 0) return mt_fail(ctx, MT_ERR_INVALID_ARG, "tiles incomplete");
+  if (row_begin < 0 || row_end <= row_begin || row_end > t->n)
+    return mt_fail(ctx, MT_ERR_INVALID_ARG, "row band [%lld, %lld) outside [0, %lld)", (long long)row_begin,
+                   (long long)row_end, (long long)t->n);
+  if (band_rows <= 0) return mt_fail(ctx, MT_ERR_INVALID_ARG, "band_rows must be positive");
+  return check_tensor_args(ctx, band, dtype, t->n, band_rows, ld);
+}
+}  // namespace
+
+int mt_sparse_stream_count(mt_ctx* ctx, const mt_tiles* t, int dtype, double fraction, int64_t row_begin,
+                           int64_t row_end, void* band, int64_t band_rows, int64_t ld, int64_t* row_ptr,
+                           unsigned long long* hist, mt_allreduce_fn allreduce, void* user, int32_t* status_flag,
+                           double* tau_host, int64_t* nnz_host) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_stream_args(ctx, t, dtype, row_begin, row_end, band, band_rows, ld);
+  if (rc) return rc;
+  if (!row_ptr || !tau_host || !nnz_host) return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr, tau_host and nnz_host must be non-NULL");
+  if (fraction > 1.0) return mt_fail(ctx, MT_ERR_INVALID_ARG, "fraction must be in [0, 1] (or negative: tau given)");
+  if (allreduce && !hist) return mt_fail(ctx, MT_ERR_INVALID_ARG, "allreduce needs a caller-owned hist");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  const int64_t n_loc = row_end - row_begin;
+  if (fraction >= 0.0) {
+    if (!hist && (rc = ensure_sel_hist(ctx))) return rc;
+    unsigned long long* h = hist ? hist : ctx->sel_hist;
+    mt_select_state st;
+    if ((rc = mt_select_begin(ctx, &st, dtype, fraction, h))) return rc;
+    while (!st.done) {
+      for (int64_t r0 = row_begin; r0 < row_end; r0 += band_rows) {
+        const int64_t r1 = r0 + band_rows < row_end ? r0 + band_rows : row_end;
+        if ((rc = mt_launch_assemble(ctx, t, dtype, r0, r1, band, ld, status_flag))) return rc;
+        if ((rc = mt_select_accumulate(ctx, &st, band, t->n, r1 - r0, ld, h))) return rc;
+      }
+      if (allreduce && allreduce(user, h, (void*)ctx->stream) != 0)
+        return mt_fail(ctx, MT_ERR_CUDA, "histogram all-reduce callback failed");
+      if ((rc = mt_select_advance(ctx, &st, h))) return rc;
+    }
+    *tau_host = st.tau;
+  }
+  for (int64_t r0 = row_begin; r0 < row_end; r0 += band_rows) {
+    const int64_t r1 = r0 + band_rows < row_end ? r0 + band_rows : row_end;
+    if ((rc = mt_launch_assemble(ctx, t, dtype, r0, r1, band, ld, status_flag))) return rc;
+    if ((rc = mt_launch_sparse_count(ctx, band, dtype, t->n, r1 - r0, ld, *tau_host, r0 - row_begin, n_loc, row_ptr))) return rc;
+  }
+  return mt_sparse_scan(ctx, row_ptr, n_loc, nnz_host);
+}
+
+int mt_sparse_stream_fill(mt_ctx* ctx, const mt_tiles* t, int dtype, double tau, int64_t row_begin, int64_t row_end,
+                          void* band, int64_t band_rows, int64_t ld, const int64_t* row_ptr, uint32_t* mask, void* vals,
+                          uint16_t* cols16, int64_t* panel_ptr, int32_t* status_flag) {
+  if (!ctx) return MT_ERR_INVALID_ARG;
+  int rc = check_stream_args(ctx, t, dtype, row_begin, row_end, band, band_rows, ld);
+  if (rc) return rc;
+  if (!row_ptr || !vals || (!mask && !cols16))
+    return mt_fail(ctx, MT_ERR_INVALID_ARG, "row_ptr, vals and one of mask / cols16 must be non-NULL");
+  if (cols16 && t->n > 65536 && !panel_ptr)
+    return mt_fail(ctx, MT_ERR_INVALID_ARG, "n > 65536: panel_ptr must be non-NULL with cols16");
+  MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  const int64_t n_loc = row_end - row_begin;
+  for (int64_t r0 = row_begin; r0 < row_end; r0 += band_rows) {
+    const int64_t r1 = r0 + band_rows < row_end ? r0 + band_rows : row_end;
+    if ((rc = mt_launch_assemble(ctx, t, dtype, r0, r1, band, ld, status_flag))) return rc;
+    if ((rc = mt_launch_sparse_fill(ctx, band, dtype, t->n, r1 - r0, ld, tau, r0 - row_begin, n_loc, row_ptr,
+                                    mt_sparse_mask_words(t->n), mask, vals, cols16, panel_ptr)))
+      return rc;
+  }
+  MT_CUDA_OK(ctx, cudaStreamSynchronize(ctx->stream));
+  return MT_OK;
 }
 
 int mt_sparse_index(mt_ctx* ctx, const mt_sparse_tensor* S, uint16_t* cols16, int64_t* panel_ptr) {
@@ -651,14 +760,15 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
   const int64_t npad = round_up(n, MT_COL_CHUNK);
   const int64_t stride = 1 + 3 * (int64_t)batch;
   memset(res, 0, sizeof(*res));
-  // workspace: k1..k7, two scratch states, candidate state
-  rc = mt_ensure_ws(ctx, (void**)&ctx->rk, &ctx->rk_bytes, (size_t)(7 + 3) * sv * sizeof(double));
+  // workspace: k1..k7, two scratch states, candidate state, chunk-start backup (RK4 stop test)
+  rc = mt_ensure_ws(ctx, (void**)&ctx->rk, &ctx->rk_bytes, (size_t)(7 + 4) * sv * sizeof(double));
   if (rc) return rc;
   double* k[7];
   for (int s = 0; s < 7; ++s) k[s] = ctx->rk + (int64_t)s * sv;
   double* ya = ctx->rk + 7 * sv;
   double* yb = ctx->rk + 8 * sv;
   double* mc = ctx->rk + 9 * sv;
+  double* mb = ctx->rk + 10 * sv;
   if (has_demag(p)) {
     rc = ensure_Mst(ctx, demag_dtype(p), batch, npad);
     if (rc) return rc;
@@ -716,9 +826,9 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
     bool hit_max = false;
     if (o->max_steps > 0 && nsteps > o->max_steps) { nsteps = o->max_steps; hit_max = true; }
     const bool want_tq = o->torque_tol > 0;
-    auto stage1 = [&]() -> int {  // k1 = f(m); ya = m + dt/2 k1
+    auto stage1 = [&](unsigned long long* tq) -> int {  // k1 = f(m); ya = m + dt/2 k1
       EpiArgs e = base;
-      e.y = m; e.k_out = k[0]; e.torque_bits = want_tq ? d_tq : nullptr;
+      e.y = m; e.k_out = k[0]; e.torque_bits = tq;
       e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[0]; e.coef[0] = 1.0; e.base = m; e.h = 0.5 * dt;
       void* Md = has_demag(p) ? ctx->Mst[1] : nullptr;
       route(e, ya, Md);
@@ -758,12 +868,12 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       return MT_OK;
     };
     int64_t done = 0;
-    if (want_tq) {
-      // the stop test (Eq. 2) needs the torque of every step's first stage: one host
-      // read per step; a satisfied test leaves m untouched
+    if (want_tq && sh) {
+      // row-sharded: the stop test (Eq. 2) needs the ranks' maxima combined, one exchange
+      // and one host read per step; a satisfied test leaves m untouched
       while (done < nsteps) {
         MT_CUDA_OK(ctx, cudaMemsetAsync(d_err, 0, 16, st));
-        if ((rc = stage1())) return rc;
+        if ((rc = stage1(d_tq))) return rc;
         if ((rc = read_scalars(1))) return rc;
         res->max_torque = bits_to_double(ctx->hscal[0]);
         if (res->max_torque <= o->torque_tol) break;
@@ -772,17 +882,38 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
         if ((rc = sample_if_due(done))) return rc;
       }
     } else {
-      // `chunk` steps are captured once into a CUDA graph and replayed (every buffer is back in its
-      // role after a step).  The first chunk runs eagerly: it sizes the workspaces, which must not be
-      // allocated under capture.
+      // Steps run in chunks; a whole chunk is captured once into a CUDA graph and replayed (every buffer
+      // is back in its role after a step).  The first chunk runs eagerly: it sizes the workspaces, which
+      // must not be allocated under capture.  With the stop test (Eq. 2) every step of a chunk
+      // leaves the torque of the state it started from in its own device word; the host reads the chunk's
+      // words once (one synchronisation per chunk instead of per step) and, when a step's test was
+      // satisfied, goes back to the chunk's first state and repeats the steps before it: the state
+      // returned is the one the per-step test would have stopped at, bit for bit.
       int64_t chunk = o->sample_every > 0 ? o->sample_every : 64;
       if (chunk > 256) chunk = 256;
       while (o->sample_every > 0 && o->sample_every % chunk) chunk--;  // chunk divides sample_every
+      unsigned long long* slots = ctx->dscal + 8 + 2048;
       cudaGraph_t graph = nullptr;
       cudaGraphExec_t exec = nullptr;
       int64_t graph_launches = 0;
-      while (done < nsteps && !rc) {
-        if (!sh && done >= chunk && done % chunk == 0 && nsteps - done >= chunk) {  // (exchange callbacks are host calls)
+      bool stopped = false;
+      auto run_steps = [&](int64_t count, bool with_tq) -> int {
+        int r = MT_OK;
+        for (int64_t s = 0; s < count && !r; ++s) {
+          r = stage1(with_tq ? slots + s : nullptr);
+          if (!r) r = stages234();
+        }
+        return r;
+      };
+      while (done < nsteps && !rc && !stopped) {
+        const bool use_graph = !sh && done >= chunk && done % chunk == 0 && nsteps - done >= chunk;  // (exchange callbacks are host calls)
+        int64_t kk = chunk - done % chunk;
+        if (kk > nsteps - done) kk = nsteps - done;
+        if (want_tq) {
+          MT_CUDA_OK(ctx, cudaMemcpyAsync(mb, m, (size_t)sv * sizeof(double), cudaMemcpyDeviceToDevice, st));
+          MT_CUDA_OK(ctx, cudaMemsetAsync(slots, 0, 8 * (size_t)kk, st));
+        }
+        if (use_graph) {
           if (!exec) {
             // capture on a private stream (the caller's may be the legacy default stream, which cannot
             // be captured); the instantiated graph is then launched on the caller's stream
@@ -792,11 +923,7 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
             ctx->stream = ctx->cap_stream;
             const int prof_saved = ctx->prof_on;
             ctx->prof_on = 0;  // timing events must not become graph nodes
-            int r = MT_OK;
-            for (int64_t s = 0; s < chunk && !r; ++s) {
-              r = stage1();
-              if (!r) r = stages234();
-            }
+            const int r = run_steps(chunk, want_tq);
             ctx->stream = st;
             ctx->prof_on = prof_saved;
             cudaError_t ce = cudaStreamEndCapture(ctx->cap_stream, &graph);
@@ -809,13 +936,33 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
           cudaError_t ce = cudaGraphLaunch(exec, st);
           if (ce != cudaSuccess) { rc = mt_fail(ctx, MT_ERR_CUDA, "cudaGraphLaunch: %s", cudaGetErrorString(ce)); break; }
           ctx->launches += graph_launches;
-          done += chunk;
-        } else {
-          if ((rc = stage1())) break;
-          if ((rc = stages234())) break;
-          done++;
+        } else if ((rc = run_steps(kk, want_tq))) {
+          break;
         }
-        rc = sample_if_due(done);
+        if (want_tq) {
+          cudaError_t ce = cudaMemcpyAsync(ctx->hscal, slots, 8 * (size_t)kk, cudaMemcpyDeviceToHost, st);
+          if (ce == cudaSuccess) ce = cudaStreamSynchronize(st);
+          if (ce != cudaSuccess) { rc = mt_fail(ctx, MT_ERR_CUDA, "reading the chunk's torques: %s", cudaGetErrorString(ce)); break; }
+          int64_t hit = -1;
+          for (int64_t s = 0; s < kk && hit < 0; ++s)
+            if (bits_to_double(ctx->hscal[s]) <= o->torque_tol) hit = s;
+          if (hit < 0) {
+            res->max_torque = bits_to_double(ctx->hscal[kk - 1]);
+            done += kk;
+          } else {
+            // step `hit` of the chunk would not have been taken: rebuild the state it started from
+            cudaError_t c2 = cudaMemcpyAsync(m, mb, (size_t)sv * sizeof(double), cudaMemcpyDeviceToDevice, st);
+            if (c2 != cudaSuccess) { rc = mt_fail(ctx, MT_ERR_CUDA, "restoring the chunk's first state: %s", cudaGetErrorString(c2)); break; }
+            if (has_demag(p) && (rc = mt_launch_stage_M(ctx, demag_dtype(p), p->Ms, m, batch, n, npad, ctx->Mst[0]))) break;
+            if ((rc = run_steps(hit, false))) break;
+            res->max_torque = bits_to_double(ctx->hscal[hit]);
+            done += hit;
+            stopped = true;
+          }
+        } else {
+          done += kk;
+        }
+        if (!stopped) rc = sample_if_due(done);
       }
       if (exec) cudaGraphExecDestroy(exec);
       if (graph) cudaGraphDestroy(graph);
@@ -841,7 +988,125 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       res->max_torque = bits_to_double(ctx->hscal[0]);
       res->rhs_calls = 1;
     }
-    while (t < o->t_end) {
+    // Small problems: an attempted step costs tens of microseconds, of which the host round trip of the
+    // controller (16-byte read + synchronisation + relaunch) is a large part.  The controller then runs on
+    // the device (DpState, demag.cu): one attempted step is a fixed sequence of launches replayed from a
+    // CUDA graph, and the host looks at the state every kLook attempts.  Attempts replayed after the run
+    // has ended do nothing (their kernels see active == 0), but still stream the tensor: hence small n only.
+    const bool use_dev = !sh && (ctx->step_control == 2 || (ctx->step_control == 0 && n <= 8192));
+    if (use_dev) {
+      if (!ctx->dp_dev) {
+        MT_CUDA_OK(ctx, cudaMalloc((void**)&ctx->dp_dev, sizeof(DpState)));
+        MT_CUDA_OK(ctx, cudaMallocHost((void**)&ctx->dp_host, sizeof(DpState)));
+      }
+      DpState* S = ctx->dp_dev;
+      DpState* Hs = ctx->dp_host;
+      memset(Hs, 0, sizeof(*Hs));
+      Hs->t = t; Hs->dt = dt; Hs->t_end = o->t_end; Hs->t0 = t0; Hs->sample_dt = o->sample_dt;
+      Hs->rtol = o->rtol; Hs->atol = o->atol; Hs->torque_tol = o->torque_tol; Hs->max_torque = res->max_torque;
+      Hs->max_steps = o->max_steps; Hs->sample_cap = sample_cap; Hs->has_samples = samples != nullptr;
+      Hs->next_sample = 1; Hs->rhs_calls = 1; Hs->status = MT_DP_RUN;
+      MT_CUDA_OK(ctx, cudaMemcpyAsync(S, Hs, sizeof(DpState), cudaMemcpyHostToDevice, st));
+      auto attempt = [&]() -> int {
+        int r;
+        if ((r = mt_launch_dp_begin(ctx, S))) return r;
+        EpiArgs e = base;  // y2 = m + h a21 k1
+        e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[0]; e.coef[0] = DP_A[1][0]; e.base = m;
+        e.h_dev = &S->h; e.active_dev = &S->active; e.y_out = ya;
+        e.M_out = has_demag(p) ? ctx->Mst[1] : nullptr;
+        if ((r = mt_launch_combine(ctx, e))) return r;
+        int src = 1;
+        double* yin = ya;
+        double* yout = yb;
+        for (int sg = 1; sg <= 5; ++sg) {
+          e = base;
+          e.y = yin; e.k_out = k[sg];
+          e.do_comb = 1; e.ncomb = sg + 1;
+          for (int j = 0; j <= sg; ++j) { e.kptr[j] = k[j]; e.coef[j] = DP_A[sg + 1][j]; }
+          e.base = m; e.h_dev = &S->h; e.active_dev = &S->active; e.y_out = yout;
+          e.M_out = has_demag(p) ? ctx->Mst[src ^ 1] : nullptr;
+          if ((r = eval_rhs(ctx, p, npad, src, e))) return r;
+          src ^= 1;
+          double* tmp = yin; yin = yout; yout = tmp;
+        }
+        e = base;  // k7 = f(y7), error estimate, torque, (renormalised) candidate
+        e.y = yin; e.k_out = k[6]; e.torque_bits = &S->tq_bits;
+        e.nerr = 7;
+        for (int j = 0; j < 7; ++j) { e.eptr[j] = k[j]; e.ecoef[j] = DP_E[j]; }
+        e.ebase = m; e.atol = o->atol; e.rtol = o->rtol; e.err_bits = &S->err_bits;
+        e.h_dev = &S->h; e.active_dev = &S->active;
+        e.do_comb = 1; e.ncomb = 0; e.base = yin; e.y_out = mc; e.renorm = o->renormalize;
+        if ((r = eval_rhs(ctx, p, npad, src, e))) return r;
+        if ((r = mt_launch_dp_decide(ctx, S))) return r;
+        if ((r = mt_launch_dp_commit(ctx, S, m, mc, k[0], k[6], sv))) return r;
+        if (samples && (r = mt_launch_mean_cond(ctx, S, m, p->vol, batch, n, samples, stride))) return r;
+        return MT_OK;
+      };
+      auto look = [&]() -> int {  // mirror the state; true stop tests of the loop head evaluated here as well
+        MT_CUDA_OK(ctx, cudaMemcpyAsync(Hs, S, sizeof(DpState), cudaMemcpyDeviceToHost, st));
+        MT_CUDA_OK(ctx, cudaStreamSynchronize(st));
+        return MT_OK;
+      };
+      auto finished = [&]() -> bool {
+        if (Hs->status != MT_DP_RUN) return true;
+        if (!(Hs->t < Hs->t_end)) return true;
+        if (o->torque_tol > 0 && Hs->max_torque <= o->torque_tol) return true;
+        if (o->max_steps > 0 && Hs->accepted + Hs->rejected >= o->max_steps) { Hs->status = MT_DP_MAX_STEPS; return true; }
+        return false;
+      };
+      const int kLook = n <= 2048 ? 16 : 8;
+      cudaGraph_t graph = nullptr;
+      cudaGraphExec_t exec = nullptr;
+      int64_t graph_launches = 0;
+      bool first = true;
+      while (!rc && !finished()) {
+        if (first) {  // eagerly: sizes the workspaces, which must not be allocated under capture
+          first = false;
+          if ((rc = attempt())) break;
+        } else {
+          if (!exec) {
+            if (!ctx->cap_stream) MT_CUDA_OK(ctx, cudaStreamCreateWithFlags(&ctx->cap_stream, cudaStreamNonBlocking));
+            const int64_t l0 = ctx->launches;
+            MT_CUDA_OK(ctx, cudaStreamBeginCapture(ctx->cap_stream, cudaStreamCaptureModeThreadLocal));
+            ctx->stream = ctx->cap_stream;
+            const int prof_saved = ctx->prof_on;
+            ctx->prof_on = 0;
+            const int r = attempt();
+            ctx->stream = st;
+            ctx->prof_on = prof_saved;
+            cudaError_t ce = cudaStreamEndCapture(ctx->cap_stream, &graph);
+            graph_launches = ctx->launches - l0;
+            ctx->launches = l0;
+            if (r) { if (graph) cudaGraphDestroy(graph); return r; }
+            MT_CUDA_OK(ctx, ce);
+            MT_CUDA_OK(ctx, cudaGraphInstantiate(&exec, graph, 0));
+          }
+          // near t_end look sooner: replays past the end of the run are wasted launches
+          int q_max = kLook;
+          const double rem = (Hs->t_end - Hs->t) / Hs->dt;
+          if (rem < (double)q_max) q_max = rem > 1.0 ? (int)ceil(rem) : 1;
+          for (int q = 0; q < q_max && !rc; ++q) {
+            cudaError_t ce = cudaGraphLaunch(exec, st);
+            if (ce != cudaSuccess) rc = mt_fail(ctx, MT_ERR_CUDA, "cudaGraphLaunch: %s", cudaGetErrorString(ce));
+            ctx->launches += graph_launches;
+          }
+        }
+        if (!rc) rc = look();
+      }
+      if (exec) cudaGraphExecDestroy(exec);
+      if (graph) cudaGraphDestroy(graph);
+      if (rc) return rc;
+      t = Hs->t;
+      res->accepted = Hs->accepted; res->rejected = Hs->rejected; res->rhs_calls = Hs->rhs_calls;
+      res->n_samples = Hs->n_samples; res->max_torque = Hs->max_torque; res->dt_last = Hs->dt_last;
+      if (Hs->status == MT_DP_MAX_STEPS) status = MT_ERR_MAX_STEPS;
+      if (Hs->status == MT_DP_UNDERFLOW) status = MT_ERR_STEP_UNDERFLOW;
+      if (Hs->status == MT_DP_NONFINITE) {
+        status = MT_ERR_STEP_UNDERFLOW;
+        mt_fail(ctx, status, "non-finite error estimate at t = %g", t);
+      }
+    }
+    while (!use_dev && t < o->t_end) {
       if (o->torque_tol > 0 && res->max_torque <= o->torque_tol) break;
       if (o->max_steps > 0 && res->accepted + res->rejected >= o->max_steps) { status = MT_ERR_MAX_STEPS; break; }
       double t_target = o->t_end;

@@ -101,6 +101,7 @@ __global__ void __launch_bounds__(kWarps * 32) demag_ldg_kernel(DemagArgs<T> a, 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t row = (int64_t)blockIdx.x * kWarps + warp;
   if (row >= a.n_rows) return;
+  if (e.active_dev && !*e.active_dev) return;  // replayed attempt of a finished device-controlled DP45 run
   const int split = blockIdx.y;
   const int64_t nvec = a.n / W;
   const int64_t v0 = (int64_t)split * a.vec_per_split;
@@ -219,7 +220,95 @@ __global__ void __launch_bounds__(256) local_only_kernel(EpiArgs e) {
 __global__ void __launch_bounds__(256) combine_kernel(EpiArgs e) {
   const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= e.n_rows * e.batch) return;
+  if (e.active_dev && !*e.active_dev) return;
   stage_combine(e, e.row0 + idx % e.n_rows, (int)(idx / e.n_rows), nullptr);
+}
+
+// ---- device-resident DP45 controller (A9): the host loop of mt_integrate, one thread ------------------
+// Same rules as the host controller (Q11/Q11b): dp_begin is the top of the loop (stop tests,
+// clipping to the next sample time / t_end, h_min), dp_decide its bottom (accept / reject, next dt).
+__device__ __forceinline__ double dp_bits(unsigned long long b) { return __longlong_as_double((long long)b); }
+
+__device__ __forceinline__ void dp_take_sample(DpState* s) {
+  if (s->has_samples && s->n_samples < s->sample_cap) {
+    s->sample_flag = 1;
+    s->sample_row = s->n_samples++;
+    s->sample_t = s->t;
+  }
+  s->next_sample++;
+}
+
+__global__ void dp_begin_kernel(DpState* s) {
+  s->active = 0;
+  s->accept = 0;
+  s->sample_flag = 0;
+  if (s->status != MT_DP_RUN) return;
+  if (!(s->t < s->t_end)) { s->status = MT_DP_T_END; return; }
+  if (s->torque_tol > 0 && s->max_torque <= s->torque_tol) { s->status = MT_DP_TORQUE; return; }
+  if (s->max_steps > 0 && s->accepted + s->rejected >= s->max_steps) { s->status = MT_DP_MAX_STEPS; return; }
+  double t_target = s->t_end;
+  int hit_sample = 0;
+  if (s->sample_dt > 0) {
+    const double ts = s->t0 + (double)s->next_sample * s->sample_dt;
+    if (ts <= t_target) { t_target = ts; hit_sample = 1; }
+  }
+  double h = s->dt;
+  int clipped = 0;
+  if (s->t + h >= t_target) { h = t_target - s->t; clipped = 1; }
+  const double h_min = 16.0 * 2.220446049250313e-16 * fmax(fabs(s->t), fabs(s->t_end));
+  if (h <= h_min) {
+    if (clipped) {  // land on the target without a step
+      s->t = t_target;
+      if (hit_sample) dp_take_sample(s);
+      return;
+    }
+    s->status = MT_DP_UNDERFLOW;
+    return;
+  }
+  s->h = h;
+  s->t_target = t_target;
+  s->clipped = clipped;
+  s->hit_sample = hit_sample;
+  s->err_bits = 0ull;
+  s->tq_bits = 0ull;
+  s->active = 1;
+}
+
+__global__ void dp_decide_kernel(DpState* s) {
+  if (!s->active) return;
+  s->rhs_calls += 6;
+  const double err = dp_bits(s->err_bits), tq7 = dp_bits(s->tq_bits);
+  if (!(err == err) || err > 1.79e308) {  // NaN/inf state or slope: no step size can repair it (Q11b)
+    s->rejected++;
+    s->status = MT_DP_NONFINITE;
+    return;
+  }
+  double fac = err > 0 ? 0.9 * pow(err, -0.2) : 5.0;
+  fac = fmin(5.0, fmax(0.2, fac));
+  const double h = s->h;
+  if (err <= 1.0) {
+    s->t = s->clipped ? s->t_target : s->t + h;
+    s->accept = 1;
+    s->max_torque = tq7;
+    s->accepted++;
+    s->dt_last = h;
+    if (s->clipped && s->hit_sample) dp_take_sample(s);
+    s->dt = s->clipped ? fmax(s->dt, h * fac) : h * fac;
+  } else {
+    s->rejected++;
+    s->dt = h * fmin(1.0, fac);
+  }
+}
+
+// accepted: m <- candidate, k1 <- k7 (FSAL; the host controller swaps pointers, a replayed graph cannot)
+__global__ void __launch_bounds__(256) dp_commit_kernel(const DpState* s, double* __restrict__ m,
+                                                        const double* __restrict__ mc, double* __restrict__ k1,
+                                                        const double* __restrict__ k7, int64_t count) {
+  if (!s->accept) return;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= count) return;
+  m[i] = mc[i];
+  k1[i] = k7[i];
 }
 
 // Row-sharded problems (mt.h section 8(e)): after the all-gather, block g of `pack` holds rows
@@ -282,6 +371,37 @@ __global__ void __launch_bounds__(1024) mean_kernel(const double* __restrict__ m
   if (threadIdx.x == 0) {
     out[1 + b * 3 + c] = sh[0] / shw[0];
     if (c == 0 && b == 0) out[0] = t;
+  }
+}
+
+// the same observable, written only when the device-resident DP45 controller flagged a sample
+__global__ void __launch_bounds__(1024) mean_cond_kernel(const DpState* st, const double* __restrict__ m,
+                                                         const double* __restrict__ vol, int64_t n, int batch,
+                                                         double* __restrict__ samples, int64_t stride) {
+  if (!st->sample_flag) return;
+  __shared__ double sh[1024], shw[1024];
+  const int c = blockIdx.x, b = blockIdx.y;
+  const double* v = m + ((int64_t)b * 3 + c) * n;
+  double s = 0.0, w = 0.0;
+  for (int64_t i = threadIdx.x; i < n; i += 1024) {
+    const double wi = vol ? vol[i] : 1.0;
+    s += wi * v[i];
+    w += wi;
+  }
+  sh[threadIdx.x] = s;
+  shw[threadIdx.x] = w;
+  __syncthreads();
+  for (int off = 512; off > 0; off >>= 1) {
+    if ((int)threadIdx.x < off) {
+      sh[threadIdx.x] += sh[threadIdx.x + off];
+      shw[threadIdx.x] += shw[threadIdx.x + off];
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) {
+    double* out = samples + st->sample_row * stride;
+    out[1 + b * 3 + c] = sh[0] / shw[0];
+    if (c == 0 && b == 0) out[0] = st->sample_t;
   }
 }
 
@@ -440,6 +560,36 @@ int mt_launch_combine(mt_ctx* ctx, const EpiArgs& epi) {
 int mt_launch_mean(mt_ctx* ctx, const double* m, const double* vol, int batch, int64_t n, double t,
                    double* sample_row) {
   mean_kernel<<<dim3(3, (unsigned)batch), 1024, 0, ctx->stream>>>(m, vol, n, batch, t, sample_row);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+int mt_launch_dp_begin(mt_ctx* ctx, DpState* st) {
+  dp_begin_kernel<<<1, 1, 0, ctx->stream>>>(st);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+int mt_launch_dp_decide(mt_ctx* ctx, DpState* st) {
+  dp_decide_kernel<<<1, 1, 0, ctx->stream>>>(st);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+int mt_launch_dp_commit(mt_ctx* ctx, const DpState* st, double* m, const double* mc, double* k1, const double* k7,
+                        int64_t count) {
+  dp_commit_kernel<<<(unsigned)((count + 255) / 256), 256, 0, ctx->stream>>>(st, m, mc, k1, k7, count);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+int mt_launch_mean_cond(mt_ctx* ctx, const DpState* st, const double* m, const double* vol, int batch, int64_t n,
+                        double* samples, int64_t stride) {
+  mean_cond_kernel<<<dim3(3, (unsigned)batch), 1024, 0, ctx->stream>>>(st, m, vol, n, batch, samples, stride);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   return MT_OK;

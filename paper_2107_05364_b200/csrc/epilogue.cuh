@@ -24,6 +24,7 @@ __device__ __forceinline__ void cross3(const double a[3], const double b[3], dou
 __device__ __forceinline__ void stage_combine(const EpiArgs& e, int64_t i, int b, const double* kcur) {
   const int64_t n = e.n;
   const int64_t sb = (int64_t)b * 3 * n;
+  const double h = e.h_dev ? *e.h_dev : e.h;
   double yo[3];
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
@@ -32,7 +33,7 @@ __device__ __forceinline__ void stage_combine(const EpiArgs& e, int64_t i, int b
       const double kj = (kcur && e.kptr[j] == e.k_out) ? kcur[a] : e.kptr[j][sb + a * n + i];
       s += e.coef[j] * kj;
     }
-    yo[a] = e.base[sb + a * n + i] + e.h * s;
+    yo[a] = e.base[sb + a * n + i] + h * s;
   }
   if (e.renorm) {
     // a zero-length m_i (a non-magnetic tile) stays zero instead of becoming 0/0 (Q10c)
@@ -70,6 +71,7 @@ __device__ __forceinline__ void row_epilogue(const EpiArgs& e, int64_t i, int b,
     o[2 * e.n_rows + i] = hd[2];
     return;
   }
+  if (e.active_dev && !*e.active_dev) return;  // device-resident controller: this attempt does not integrate
   i += e.row0;  // per-tile arrays and state vectors are full-size: global tile index from here on
   const int64_t n = e.n;
   const int64_t sb = (int64_t)b * 3 * n;
@@ -149,7 +151,7 @@ __device__ __forceinline__ void row_epilogue(const EpiArgs& e, int64_t i, int b,
         const double kj = (e.eptr[j] == e.k_out) ? k[a] : e.eptr[j][sb + a * n + i];
         s += e.ecoef[j] * kj;
       }
-      s *= e.h;
+      s *= e.h_dev ? *e.h_dev : e.h;
       const double sc = e.atol + e.rtol * fmax(fabs(e.ebase[sb + a * n + i]), fabs(mi[a]));
       const double q = fabs(s) / sc;
       err = (q > err || q != q) ? q : err;  // a NaN must reach the controller (Q11b)

@@ -10,11 +10,15 @@
 #define MT_MAX_STAGES 7
 #define MT_COL_CHUNK 256 /* staged-M padding granule (elements) */
 
+struct DpState;
 struct mt_ctx {
   int device;
   cudaStream_t stream;
   cudaStream_t cap_stream;  // private stream for CUDA-graph capture
   int num_sms;
+  int step_control;  // DP45 controller: 0 auto (device for small problems), 1 host, 2 device
+  DpState* dp_dev;   // device copy of the controller state (lazily allocated)
+  DpState* dp_host;  // pinned mirror
   int variant;  // 0 auto, 1 LDG, 2 TMA, 3 TMA with the packed-FFMA2 kernel for batches of 5..8
   int assembly_mode;  // 0 closed form everywhere (the paper's method), 1 far-field-stable (F2)
   int64_t launches;
@@ -28,6 +32,7 @@ struct mt_ctx {
   size_t Mq_bytes;
   double* rk;  // integrator stages + scratch states
   size_t rk_bytes;
+  unsigned long long* sel_hist;  // MT_SELECT_HIST_WORDS counters of mt_threshold_value / mt_sparse_stream_count (lazy)
   void* sym_ws;   // rowpart + colpart of the symmetric-half field kernel (F3)
   size_t sym_ws_bytes;
   double* edens;  // [B][4][n] energy densities (mt_energy)
@@ -38,12 +43,16 @@ struct mt_ctx {
   size_t stage_io_bytes;
   double* pinned_io;
   size_t pinned_io_bytes;
-  // TMA descriptor cache (variant 2)
-  const void* tm_base;
-  int tm_dtype;
-  int64_t tm_n, tm_rows, tm_ld;
-  alignas(64) unsigned char tm_desc[128];
-  int tm_valid;
+  // TMA descriptor cache (demag_tma.cu): a tensor map depends only on the base address and the
+  // geometry, so it is encoded once per (tensor, box shape) and ctx instead of once per launch
+  struct TmEntry {
+    const void* base;
+    int dtype, rank, swizzle, valid;
+    uint64_t dims[3], strides[2];
+    uint32_t box[3];
+    alignas(64) unsigned char map[128];
+  } tm_cache[8];
+  int tm_next;
   // per-kernel timing of the demag field kernel (mt_profile_begin / mt_profile_end)
   int prof_on;
   int prof_count;
@@ -95,6 +104,8 @@ struct EpiArgs {
   double coef[MT_MAX_STAGES];
   const double* base;
   double h;
+  const double* h_dev;    // non-NULL: the step h is read from the device (device-resident DP45 controller)
+  const int* active_dev;  // non-NULL and *active_dev == 0: the launch's epilogue / combine does nothing
   double* y_out;
   int64_t y_ld;    // y_out is [B][3][y_ld] holding rows y_row0 .. (0, 0: [B][3][n] from row 0): a rank's
   int64_t y_row0;  // block of the all-gather buffer when the problem is row-sharded
@@ -110,6 +121,34 @@ struct EpiArgs {
   double atol, rtol;
   unsigned long long* err_bits;
 };
+
+// ---- device-resident DP45 step controller (api.cu, demag.cu) --------------------------------------
+// The state of the controller of A9 when it runs on the device: one attempted step is then a fixed
+// sequence of launches (replayed from a CUDA graph) with no host round trip; the host reads this
+// struct every few attempted steps.  Same rules as the host controller (Q11/Q11b).
+struct DpState {
+  double t, dt, h, t_target, t_end, t0, sample_dt, sample_t;
+  double rtol, atol, torque_tol, max_torque, dt_last;
+  unsigned long long err_bits, tq_bits;
+  long long accepted, rejected, rhs_calls, n_samples, sample_cap, next_sample, max_steps, sample_row;
+  int status;       // MT_DP_* below
+  int active;       // this attempt integrates (stage kernels do their work)
+  int accept;       // this attempt was accepted (commit copies the candidate and k7)
+  int sample_flag;  // a sample row is due at the end of this attempt
+  int clipped, hit_sample, has_samples, pad_;
+};
+#define MT_DP_RUN 0
+#define MT_DP_T_END 1
+#define MT_DP_TORQUE 2
+#define MT_DP_UNDERFLOW 3
+#define MT_DP_NONFINITE 4
+#define MT_DP_MAX_STEPS 5
+int mt_launch_dp_begin(mt_ctx* ctx, DpState* st);
+int mt_launch_dp_decide(mt_ctx* ctx, DpState* st);
+int mt_launch_dp_commit(mt_ctx* ctx, const DpState* st, double* m, const double* mc, double* k1, const double* k7,
+                        int64_t count);
+int mt_launch_mean_cond(mt_ctx* ctx, const DpState* st, const double* m, const double* vol, int batch, int64_t n,
+                        double* samples, int64_t stride);
 
 // launchers (demag.cu)
 int mt_launch_stage_M(mt_ctx* ctx, int dtype, const double* Ms, const double* m, int batch, int64_t n,
@@ -138,6 +177,8 @@ int mt_launch_demag_tma(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_
 int mt_launch_select_hist(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
                           unsigned long long prefix, int prefix_shift, int shift, int width,
                           unsigned long long* hist);
+int mt_launch_select_find(mt_ctx* ctx, const unsigned long long* hist, int nbins, unsigned long long k, int first_pass,
+                          double fraction, unsigned long long* out4);
 int mt_launch_sparse_count(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, double tau,
                            int64_t row0, int64_t n_total, int64_t* counts);
 int mt_launch_sparse_scan(mt_ctx* ctx, int64_t* row_ptr, int64_t n_total);

@@ -128,6 +128,87 @@ __global__ void __launch_bounds__(512) select_hist_kernel(const T* __restrict__ 
     if (sh[k]) atomicAdd(&hist[k], (unsigned long long)sh[k]);
 }
 
+// Wide digit (up to 20 bits) for the passes after the first: only the elements that carry the prefix
+// fixed so far are counted — a few percent of the tensor after the first 11 bits, almost none later —
+// so their bins are added straight to the global histogram (64-bit atomics in L2, spread over up to 2^20
+// bins: no contention to speak of).  One pass of this kind replaces two 11-bit passes.
+template <typename T>
+__global__ void __launch_bounds__(512) select_hist_wide_kernel(const T* __restrict__ N, int64_t n, int64_t n_rows,
+                                                               int64_t ld, typename KeyOf<T>::type prefix,
+                                                               int prefix_shift, int shift, int width,
+                                                               unsigned long long* __restrict__ hist) {
+  typedef typename KeyOf<T>::type K;
+  typedef typename Vec16<T>::type V;
+  constexpr int kV = Vec16<T>::n;
+  const int64_t rows_total = 6 * n_rows;
+  const K dmask = (K)(((K)1 << width) - (K)1);
+  const K pmask = ~(((K)1 << prefix_shift) - (K)1);
+  const K pval = (K)(prefix << prefix_shift);
+  const int step = (int)blockDim.x * kV;
+  for (int64_t r = blockIdx.x; r < rows_total; r += gridDim.x) {
+    const int plane = (int)(r / n_rows);
+    const unsigned long long w = (plane == 1 || plane == 2 || plane == 4) ? 2ull : 1ull;
+    const T* row = N + r * ld;
+    for (int j0 = (int)threadIdx.x * kV; j0 < n; j0 += 2 * step) {
+      T x[2][kV];
+#pragma unroll
+      for (int u = 0; u < 2; ++u) {
+        const int j = j0 + u * step;
+#pragma unroll
+        for (int c = 0; c < kV; ++c) x[u][c] = T(0);
+        if (j < n) {
+          unpack16(__ldg(reinterpret_cast<const V*>(row + j)), x[u]);
+#pragma unroll
+          for (int c = 0; c < kV; ++c)
+            if (j + c >= n) x[u][c] = T(0);  // padding of the row's last vector
+        }
+      }
+#pragma unroll
+      for (int u = 0; u < 2; ++u)
+#pragma unroll
+        for (int c = 0; c < kV; ++c) {
+          const K key = KeyOf<T>::key(x[u][c]);
+          if (key != 0 && (key & pmask) == pval) atomicAdd(&hist[(size_t)((key >> shift) & dmask)], w);
+        }
+    }
+  }
+}
+
+// One block: total = sum of the bins; first pass: k = floor(fraction * total); the bin that holds rank k
+// and the rank inside it.  out[0] = total, out[1] = bin, out[2] = k - (sum of the bins below), out[3] = k
+// as used.  Integer arithmetic on the bins, fixed order: exact.
+__global__ void __launch_bounds__(1024) select_find_kernel(const unsigned long long* __restrict__ hist, int nbins,
+                                                           unsigned long long k_in, int first_pass, double fraction,
+                                                           unsigned long long* __restrict__ out) {
+  __shared__ unsigned long long part[1024];
+  __shared__ unsigned long long k_sh;
+  const int per = nbins > 1024 ? nbins / 1024 : 1;
+  const int b0 = (int)threadIdx.x * per;
+  unsigned long long s = 0;
+  for (int b = b0; b < b0 + per && b < nbins; ++b) s += hist[b];
+  part[threadIdx.x] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    unsigned long long run = 0;
+    for (int t = 0; t < 1024; ++t) { const unsigned long long v = part[t]; part[t] = run; run += v; }  // exclusive
+    out[0] = run;
+    unsigned long long k = k_in;
+    if (first_pass) k = (unsigned long long)floor(fraction * (double)run);
+    k_sh = k;
+    out[3] = k;
+    if (k >= run) { out[1] = (unsigned long long)(nbins - 1); out[2] = k; }  // caller: everything removed / last bin
+  }
+  __syncthreads();
+  const unsigned long long k = k_sh, below = part[threadIdx.x];
+  if (k >= below && k < below + s) {
+    unsigned long long rem = k - below;
+    int b = b0;
+    while (b < b0 + per - 1 && b < nbins - 1 && rem >= hist[b]) { rem -= hist[b]; ++b; }
+    out[1] = (unsigned long long)b;
+    out[2] = rem;
+  }
+}
+
 template <typename T> __device__ __forceinline__ bool kept(T v, T tau) { return v != T(0) && !(fabs(v) < tau); }
 
 // N holds rows [row0, row0 + n_rows) of a tensor of n_total rows (the whole tensor: row0 = 0, n_total =
@@ -597,12 +678,31 @@ int mt_launch_select_hist(mt_ctx* ctx, const void* N, int dtype, int64_t n, int6
   const int64_t need = (6 * n_rows * n + (1LL << 30) - 1) >> 30;
   if (blocks < need) blocks = need;
   const unsigned grid = (unsigned)min(blocks, 6 * n_rows);
+  if (width > kDigitBits) {  // wide digit: global histogram, prefix-matching elements only
+    if (dtype == MT_F32)
+      select_hist_wide_kernel<float><<<grid, 512, 0, ctx->stream>>>((const float*)N, n, n_rows, ld, (uint32_t)prefix,
+                                                                    prefix_shift, shift, width, hist);
+    else
+      select_hist_wide_kernel<double><<<grid, 512, 0, ctx->stream>>>((const double*)N, n, n_rows, ld, prefix,
+                                                                     prefix_shift, shift, width, hist);
+    ctx->launches++;
+    MT_CUDA_OK(ctx, cudaGetLastError());
+    return MT_OK;
+  }
   if (dtype == MT_F32)
     select_hist_kernel<float><<<grid, 512, 0, ctx->stream>>>((const float*)N, n, n_rows, ld, (uint32_t)prefix,
                                                              prefix_shift, shift, width, hist);
   else
     select_hist_kernel<double><<<grid, 512, 0, ctx->stream>>>((const double*)N, n, n_rows, ld, prefix, prefix_shift,
                                                               shift, width, hist);
+  ctx->launches++;
+  MT_CUDA_OK(ctx, cudaGetLastError());
+  return MT_OK;
+}
+
+int mt_launch_select_find(mt_ctx* ctx, const unsigned long long* hist, int nbins, unsigned long long k, int first_pass,
+                          double fraction, unsigned long long* out4) {
+  select_find_kernel<<<1, 1024, 0, ctx->stream>>>(hist, nbins, k, first_pass, fraction, out4);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   return MT_OK;

@@ -128,6 +128,46 @@ def config3(n1: int = 32, batch: int = 1, dtype: str = "f32") -> Workload:
                             extra={"rtol": 1e-6, "atol": 1e-8, "dt0": 1e-3, "torque_tol": 1e-5, "t_end": 200.0})
 
 
+def sp3_cube(n1: int, L: float, kind: str) -> Workload:
+    """µmag standard problem 3 shape as the paper ran it: a cube of side L exchange
+    lengths, n1^3 tiles, K_u = 0.1 K_m along z, started in a `flower`-like state (m along z, tilted
+    outwards/inwards with height) or a `vortex`-like state (m circulating about the x axis with an
+    x core).  Only the seeds of the two relaxations; the states themselves come out of the integrator."""
+    edge = L / n1
+    n = n1**3
+    center, _ = cuboid_grid(n1, n1, n1, edge)
+    r = center / L - 0.5                      # in [-0.5, 0.5]^3
+    m = np.zeros((1, 3, n))
+    if kind == "flower":
+        m[0, 0] = 0.4 * r[:, 0] * r[:, 2]
+        m[0, 1] = 0.4 * r[:, 1] * r[:, 2]
+        m[0, 2] = 1.0
+    elif kind == "vortex":
+        rho = np.sqrt(r[:, 1] ** 2 + r[:, 2] ** 2) + 1e-12
+        core = np.exp(-(rho / 0.15) ** 2)
+        m[0, 0] = core
+        m[0, 1] = -r[:, 2] / rho * (1.0 - core)
+        m[0, 2] = r[:, 1] / rho * (1.0 - core)
+    else:
+        raise ValueError(kind)
+    m /= np.linalg.norm(m, axis=1, keepdims=True)
+    return _cuboid_workload(f"sp3_{kind}_{n1}^3_L{L}", n1, n1, n1, edge, 1.0, m, nbr=grid_neighbours(n1, n1, n1),
+                            inv_d2=(1.0 / edge**2,) * 3, c_ex=1.0, c_an=0.1, easy=(0.0, 0.0, 1.0), gamma=1.0,
+                            alpha_ll=0.5, dtype="f64", extra={"rtol": 1e-6, "atol": 1e-8, "dt0": 1e-3})
+
+
+def sp2_film(d_over_lex: float, nx: int = 100, ny: int = 20, nz: int = 3) -> Workload:
+    """µmag standard problem 2 shape as the paper ran it: film of length L = 5 d, width
+    d, thickness d/10 on 100 x 20 x 3 tiles, no anisotropy, gamma = 0 (only the steady state matters),
+    dimensionless units (lengths in l_ex, fields in Ms); started saturated along [1, 1, 1]."""
+    d = float(d_over_lex)
+    edge = (5.0 * d / nx, d / ny, 0.1 * d / nz)
+    n = nx * ny * nz
+    m = np.full((1, 3, n), 1.0 / np.sqrt(3.0))
+    return _cuboid_workload(f"sp2_d{d}", nx, ny, nz, edge, 1.0, m, nbr=grid_neighbours(nx, ny, nz),
+                            inv_d2=tuple(1.0 / np.asarray(edge) ** 2), c_ex=1.0, gamma=0.0, alpha_ll=1.0, dtype="f32")
+
+
 def config5(nx: int = 64, ny: int = 64, nz: int = 16, batch: int = 8) -> Workload:
     """64x64x16 unit cubes (65,536 tiles), Ms = 1, eight seeded random unit states; fp32 tensor."""
     rng = rng_for(5)

@@ -200,6 +200,15 @@ def test_singular_geometry_sets_status_flag(ctx):
     tiles = H.dev_tiles(w)
     N, ld, status = H.assemble(ctx, tiles, "f64")
     assert status == 1
+    # the same through the ABI's own status check: MT_ERR_SINGULAR_GEOMETRY, and MT_OK for a clean flag
+    flag = torch.ones(1, dtype=torch.int32, device="cuda")
+    with pytest.raises(B.MtError) as ei:
+        B.mt_check_status(ctx, flag)
+    assert ei.value.code == B.MT_ERR_SINGULAR_GEOMETRY
+    flag.zero_()
+    assert B.mt_check_status(ctx, flag) == B.MT_OK
+    flag.fill_(2)
+    assert B.mt_check_status(ctx, flag, allow=(B.MT_ERR_INVALID_ARG,)) == B.MT_ERR_INVALID_ARG
 
 
 # ---- small mixed tetrahedra + octree mesh (config 4 shape) ------------------------------------------
@@ -297,6 +306,87 @@ def test_torque_stop_and_max_steps(ctx):
     m, _, res, rc = run_gpu_integrate(ctx, prob, m0, 1, method=B.MT_DP45, dt=1e-2, t_end=100.0, max_steps=5,
                                       allow=(B.MT_ERR_MAX_STEPS,))
     assert rc == B.MT_ERR_MAX_STEPS and res["accepted"] + res["rejected"] == 5
+
+
+def test_dp45_device_controller_equals_host_controller(oracle):
+    """mt_set_step_control: the one-thread controller kernel replayed from a CUDA graph (default for small
+    problems) against the host controller (one read per attempted step) and the oracle on an 8^3 replica of
+    config 3: same accept / reject sequence, same sample times, states and samples to rounding, with the
+    stop by the torque test, by t_end, and by max_steps, and sample rows capped by sample_cap."""
+    w = W.config3(8, batch=2)
+    x = w.extra
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=True)
+    runs = {}
+    for mode in (1, 2):
+        c = B.mt_create(0)
+        B.mt_set_step_control(c, mode)
+        tiles = H.dev_tiles(w)
+        N, ld, _ = H.assemble(c, tiles, "f64")
+        prob = H.dev_problem(w, tiles, N, "f64", ld)
+        out = []
+        for kw in (dict(t_end=2.0, sample_dt=0.25, sample_cap=16),
+                   dict(t_end=40.0, sample_dt=1.0, sample_cap=5, torque_tol=2e-2),
+                   dict(t_end=2.0, max_steps=37, allow=(B.MT_ERR_MAX_STEPS,))):
+            out.append(run_gpu_integrate(c, prob, w.m, 2, method=B.MT_DP45, dt=x["dt0"], rtol=x["rtol"], atol=x["atol"], **kw))
+        runs[mode] = out
+        c.close()
+    for (m1, s1, r1, rc1), (m2, s2, r2, rc2) in zip(runs[1], runs[2]):
+        assert rc1 == rc2
+        for key in ("accepted", "rejected", "rhs_calls", "n_samples"):
+            assert r1[key] == r2[key], key
+        # (the device takes err^(-1/5) from CUDA's pow, the host from the C library's: a last-bit difference
+        # in one dt feeds back through the next error estimate, so step sizes agree to ~1e-10, not to the bit)
+        assert abs(r1["t"] - r2["t"]) <= 1e-12 and abs(r1["dt_last"] - r2["dt_last"]) <= 1e-6 * r1["dt_last"]
+        assert abs(r1["max_torque"] - r2["max_torque"]) <= 1e-6 * r1["max_torque"]
+        assert np.array_equal(s1[:, 0], s2[:, 0]) and (s1.size == 0 or np.max(np.abs(s1 - s2)) < 1e-9)
+        assert np.max(np.abs(m1 - m2)) < 1e-9
+    (_, s, r, _), (_, s_t, r_t, _), (_, _, r_m, rc_m) = runs[2]
+    assert r["t"] == 2.0 and r["rejected"] > 0 and np.array_equal(s[:, 0], 0.25 * np.arange(1, 9))
+    assert r_t["max_torque"] <= 2e-2 and r_t["t"] < 40.0 and r_t["n_samples"] == 5
+    assert rc_m == B.MT_ERR_MAX_STEPS and r_m["accepted"] + r_m["rejected"] == 37
+    m_o, s_o, r_o = oracle.integrate(H.oracle_problem(oracle, w, N_ref), w.m[0], method=oracle.DP45, dt=x["dt0"],
+                                     rtol=x["rtol"], atol=x["atol"], t_end=2.0, sample_dt=0.25, sample_cap=16, weights=w.vol)
+    # (batch of two states shares the step sequence: the controller sees the maximum over both; compare a
+    # single-state device run with the oracle)
+    c = B.mt_create(0)
+    B.mt_set_step_control(c, 2)
+    tiles = H.dev_tiles(w)
+    N, ld, _ = H.assemble(c, tiles, "f64")
+    m, s, r, _ = run_gpu_integrate(c, H.dev_problem(w, tiles, N, "f64", ld), w.m[:1], 1, method=B.MT_DP45, dt=x["dt0"],
+                                   rtol=x["rtol"], atol=x["atol"], t_end=2.0, sample_dt=0.25, sample_cap=16)
+    c.close()
+    assert (r["accepted"], r["rejected"]) == (r_o["accepted"], r_o["rejected"])
+    assert np.array_equal(s[:, 0], s_o[:, 0]) and np.max(np.abs(s[:, 1:] - s_o[:, 1:])) < 1e-9
+    assert np.max(np.abs(m[0] - m_o)) < 1e-8
+
+
+def test_rk4_stop_test_inside_a_replayed_chunk(ctx, oracle):
+    """RK4 with the torque stop test (Eq. 2): the device runs chunks of steps from a CUDA
+    graph, every step leaving the torque of its start state in its own word, and the host reads a
+    chunk's words at once; a satisfied test inside a chunk sends the state back to the chunk's start and
+    repeats the steps before it.  Against the oracle's per-step test: same number of steps, same state,
+    with the stop falling well inside a replayed chunk (after the eager first chunk), with and without
+    sampling."""
+    w = W.config3(4)
+    tiles = H.dev_tiles(w)
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=True)
+    N, ld, _ = H.assemble(ctx, tiles, "f64")
+    prob = H.dev_problem(w, tiles, N, "f64", ld)
+    base = dict(dt=0.02, t_end=400.0)
+    # torque of a relaxing 4^3 cube falls steadily: pick the tolerance it crosses after ~200 steps
+    m_o, _, r_probe = oracle.integrate(H.oracle_problem(oracle, w, N_ref), w.m[0], method=oracle.RK4, dt=0.02, t_end=4.0,
+                                       torque_tol=1e-30)
+    tol = 0.999 * r_probe["max_torque"]
+    for extra in (dict(), dict(sample_every=16, sample_cap=64)):
+        m_o, s_o, r_o = oracle.integrate(H.oracle_problem(oracle, w, N_ref), w.m[0], method=oracle.RK4,
+                                         torque_tol=tol, weights=w.vol, **base, **extra)
+        m, s, r, rc = run_gpu_integrate(ctx, prob, w.m[:1], 1, method=B.MT_RK4, torque_tol=tol, **base, **extra)
+        assert rc == 0 and r["accepted"] == r_o["accepted"] and 150 < r["accepted"] < 20000
+        assert r["accepted"] % 64 not in (0, 63) or extra  # not at a chunk boundary by luck
+        assert abs(r["t"] - r_o["t"]) < 1e-9 and r["max_torque"] <= tol
+        assert abs(r["max_torque"] - r_o["max_torque"]) <= 1e-9 * tol
+        assert np.max(np.abs(m[0] - m_o)) < 1e-10
+        assert len(s) == len(s_o) and (len(s) == 0 or np.max(np.abs(s - s_o)) < 1e-10)
 
 
 def test_batched_rk4_equals_individual_runs(ctx, oracle):
