@@ -41,8 +41,8 @@ NCU_CAPTURES = {
     },
     # DFMA + DADD + DMUL thread-instructions per tile pair of the assembly kernels
     "asm_fp64_inst_per_pair": {
-        "cuboid": {"value": 386.4, "source": "profiles/r05_assembly_ncu_full.md", "kernel_commit": "6521e8f"},
-        "tet": {"value": 502.6, "source": "profiles/r05_assembly_ncu_full.md", "kernel_commit": "6521e8f"},
+        "cuboid": {"value": 375.4, "source": "profiles/r05_assembly_ncu_full.md", "kernel_commit": "1b6588c"},
+        "tet": {"value": 444.8, "source": "profiles/r05_assembly_ncu_full.md", "kernel_commit": "1b6588c"},
     },
 }
 FLOORS_NOTE = "floor = tensor bytes / measured HBM peak (MEASURED_PEAKS.json hbm_gbs)"
@@ -532,12 +532,12 @@ def run_extras(R, args, out, w, tiles, N, ld, dtype, m_all, m1, Hd1, step_field,
                               "finite": bool(torch.isfinite(mi).all().item())}
     if nb >= 8:
         Hd8 = torch.empty((8, 3, rows), dtype=torch.float64, device=dev)
-        ms_b8, _, _ = R.timed(lambda: B.mt_demag_field(ctx, N, code, n, rows, ld, tiles.Ms, m_all, 8, Hd8),
-                              3, max(5, K // 4), tag="b8")
+        ms_b8, _, clk8 = R.timed(lambda: B.mt_demag_field(ctx, N, code, n, rows, ld, tiles.Ms, m_all, 8, Hd8),
+                                 3, max(20, K // 2), clocks=True, tag="b8")
         alg_b8 = tensor_bytes(rows, n, s, batch=8)
         out["batch8"] = {"state_evals_per_s": 8000.0 / ms_b8, "ms": ms_b8, "kernel_ms": kernel_ms["b8"],
                          "achieved_gbs": alg_b8 / (kernel_ms["b8"] * 1e-3) / 1e9,
-                         "frac": alg_b8 / (kernel_ms["b8"] * 1e-3) / 1e9 / peak,
+                         "frac": alg_b8 / (kernel_ms["b8"] * 1e-3) / 1e9 / peak, "clocks": clk8,
                          "kernel": "demag_tma_mma_kernel (3xTF32 mma.sync, fp64 drain)" if dtype == "f32" else "demag_tma_kernel<double, 8>"}
         del Hd8
     if world == 1 and w.grid is not None and n >= 4096:

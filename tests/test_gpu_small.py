@@ -325,7 +325,7 @@ def test_dp45_device_controller_equals_host_controller(oracle):
         prob = H.dev_problem(w, tiles, N, "f64", ld)
         out = []
         for kw in (dict(t_end=2.0, sample_dt=0.25, sample_cap=16),
-                   dict(t_end=40.0, sample_dt=1.0, sample_cap=5, torque_tol=2e-2),
+                   dict(t_end=40.0, sample_dt=1.0, sample_cap=5, torque_tol=0.5),
                    dict(t_end=2.0, max_steps=37, allow=(B.MT_ERR_MAX_STEPS,))):
             out.append(run_gpu_integrate(c, prob, w.m, 2, method=B.MT_DP45, dt=x["dt0"], rtol=x["rtol"], atol=x["atol"], **kw))
         runs[mode] = out
@@ -342,7 +342,7 @@ def test_dp45_device_controller_equals_host_controller(oracle):
         assert np.max(np.abs(m1 - m2)) < 1e-9
     (_, s, r, _), (_, s_t, r_t, _), (_, _, r_m, rc_m) = runs[2]
     assert r["t"] == 2.0 and r["rejected"] > 0 and np.array_equal(s[:, 0], 0.25 * np.arange(1, 9))
-    assert r_t["max_torque"] <= 2e-2 and r_t["t"] < 40.0 and r_t["n_samples"] == 5
+    assert r_t["max_torque"] <= 0.5 and 5.0 < r_t["t"] < 40.0 and r_t["n_samples"] == 5
     assert rc_m == B.MT_ERR_MAX_STEPS and r_m["accepted"] + r_m["rejected"] == 37
     m_o, s_o, r_o = oracle.integrate(H.oracle_problem(oracle, w, N_ref), w.m[0], method=oracle.DP45, dt=x["dt0"],
                                      rtol=x["rtol"], atol=x["atol"], t_end=2.0, sample_dt=0.25, sample_cap=16, weights=w.vol)
