@@ -503,9 +503,12 @@ __global__ void __launch_bounds__(WARPS * 32, 1)
 //     H[(i,a), b] = sum_{(j,c)} N^{ac}_{ij} M[(j,c), b]           (3 n_rows x 3 n) x (3 n x 8),
 // and runs on the tensor cores (north_star allows them "if the batched form is a real dense
 // contraction that holds accuracy").  Accuracy: TF32 alone (10-bit mantissa) cannot hold the 1e-5
-// gate, so both operands are split, x = x_hi + x_lo with x_hi = RN_tf32(x) and x_lo = RN_tf32(x - x_hi)
-// (the subtraction is exact), and three products are accumulated: hi*hi + hi*lo + lo*hi; what is
-// dropped (lo*lo and the rounding of x_lo) is ~2^-22 relative per product, unbiased.  Products of
+// gate, so both operands are split, x = x_hi + x_lo: for the staged M (re-laid out once per call) x_hi =
+// RN_tf32(x), x_lo = RN_tf32(x - x_hi); for the streamed tensor x_hi = trunc_tf32(x) — the tensor core reads
+// only the top 19 bits of an fp32 operand, so the raw register is the hi operand — and x_lo = x - x_hi (the
+// subtraction is exact; r05 A/B: 18.2 -> 17.9 ms against rounding x_hi in software, error 1.21e-7 -> 1.33e-7).
+// Three products are accumulated: lo*hi + hi*lo + hi*hi; what is dropped (lo*lo and the truncation of x_lo)
+// is ~2^-21 relative per product.  Products of
 // tf32 operands are exact in the tensor core; its fp32 accumulator is drained into per-lane fp64
 // sums every kMmaFlush tiles (<= 2 x 9 x 3 mma per accumulator in between).
 // Shape: RT = 64 rows x CT = 32 columns per stage; the tensor box lands in shared memory with the
@@ -671,16 +674,13 @@ __global__ void __launch_bounds__(kMmaWarps * 32, 1)
 #pragma unroll
       for (int p = 0; p < 6; ++p) {
         constexpr int prow[6] = {0, 0, 0, 1, 1, 2}, pcol[6] = {0, 1, 2, 1, 2, 2};
-        uint32_t hi[4], lo[4];
+        // x_hi = trunc_tf32(x): the tensor core reads the top 19 bits of an fp32 operand, so x itself is
+        // passed as the hi operand (no instruction); x_lo = x - trunc(x) is exact and is truncated the same way
+        uint32_t lo[4];
+        const uint32_t* hi = raw[q][p];
 #pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          hi[i] = tf32_rn(raw[q][p][i]);
-#ifdef MT_MMA_LO_NOMASK
-          lo[i] = __float_as_uint(__uint_as_float(raw[q][p][i]) - __uint_as_float(hi[i]));  // the mma reads 19 bits
-#else
-          lo[i] = __float_as_uint(__uint_as_float(raw[q][p][i]) - __uint_as_float(hi[i])) & 0xffffe000u;
-#endif
-        }
+        for (int i = 0; i < 4; ++i)
+          lo[i] = __float_as_uint(__uint_as_float(raw[q][p][i]) - __uint_as_float(raw[q][p][i] & 0xffffe000u));
         const int ra = prow[p], ca = pcol[p];
         const float4* b = bq[q];
         // small terms first, the dominant hi*hi product last
@@ -722,225 +722,6 @@ __global__ void __launch_bounds__(kMmaWarps * 32, 1)
 #pragma unroll
           for (int cc = 0; cc < 3; ++cc) {
             // (dynamic index i: pick without spilling acc to local memory)
-            double v = i == 0 ? acc[cc][0] : i == 1 ? acc[cc][1] : i == 2 ? acc[cc][2] : acc[cc][3];
-#pragma unroll
-            for (int w = 0; w < KS - 1; ++w) v += exch[((w * 3 + cc) * 4 + i) * 128 + rb * 32 + lane];
-            s3[cc] = v;
-          }
-          if (b < e.batch && row < a.n_rows) {
-            if (head_in_range && group_done) {
-              const double hd[3] = {-s3[0], -s3[1], -s3[2]};
-              row_epilogue(e, row, b, hd);
-            } else {
-              const int slot = (g == g_first) ? 0 : 1;
-              double* pp = a.partial + ((((int64_t)c * 2 + slot) * RT + rg) * e.batch + b) * 3;
-              pp[0] = s3[0]; pp[1] = s3[1]; pp[2] = s3[2];
-            }
-          }
-        }
-      }
-      __syncthreads();
-#pragma unroll
-      for (int cc = 0; cc < 3; ++cc)
-#pragma unroll
-        for (int i = 0; i < 4; ++i) acc[cc][i] = 0.0;
-    }
-    if (group_done) { k = 0; ++g; head_in_range = true; } else { ++k; }
-  }
-}
-
-// ---- variant of the tensor-core kernel with the two correction products in bf16 (k = 16) --------------
-// x_hi x_hi stays a TF32 product (exact); the corrections x_lo m and x m_lo only need ~8 significant bits
-// each (they are 2^-11 of the result), so they run as bf16 m16n8k16: one mma covers two 8-column slabs, i.e.
-// 9 + 9 bf16 mma per 16 columns instead of 18 + 18 tf32 ones: 36 mma per 16 columns instead of 54.  The k
-// index of the bf16 fragments is a PERMUTATION of the 16 columns chosen so that the fp32 registers ldmatrix
-// delivered for the two tf32 slabs pack pairwise without any shuffle: k = 2t, 2t+1 <-> columns t, t+4 of
-// slab 0, k = 2t+8, 2t+9 <-> columns t, t+4 of slab 1 (a dot product does not care, as long as M is packed
-// the same way: mmab_stage_kernel).  Error of a corrected product ~2^-19 relative, unbiased (round to
-// nearest); measured against the fp64 tensor in DESIGN.md section 7.  8 warps: 4 row blocks x 2 column
-// halves of the 64 x 32 tile.
-constexpr int kMbWarps = 8, kMbKS = 2, kMbSPW = 2;
-struct MmabCfg {
-  static constexpr int WARPS = kMbWarps, RT = kMmaRT, CT = kMmaCT;
-  static constexpr size_t tensor_bytes = MmaCfg::tensor_bytes, m_bytes = MmaCfg::m_bytes, stage_bytes = MmaCfg::stage_bytes;
-  static constexpr size_t exch_bytes = (size_t)(kMbKS - 1) * 12 * 4 * 32 * sizeof(double);
-  static constexpr size_t smem_bytes = kMmaStages * stage_bytes + exch_bytes + 2 * kMmaStages * sizeof(uint64_t) + 1024;
-};
-
-__device__ __forceinline__ uint32_t pack_bf16(float lo_half, float hi_half) {
-  uint32_t r;
-  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(hi_half), "f"(lo_half));
-  return r;
-}
-__device__ __forceinline__ void mma_bf16(float d[4], const uint32_t a[4], uint32_t b0, uint32_t b1) {
-  asm volatile(
-      "mma.sync.aligned.m16n8k16.row.col.f32.bf16.bf16.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
-      : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
-      : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
-}
-
-// plain staged M [MT_MAX_BATCH][3][npad] fp32 -> Mq[3][npad/8][8 states][4] x {hi(t), hi(t+4) as tf32,
-// bf16x2(m(t), m(t+4)), bf16x2(lo(t), lo(t+4))}, lo = m - hi
-__global__ void __launch_bounds__(256) mmab_stage_kernel(const float* __restrict__ M, int64_t npad, float4* __restrict__ Mq) {
-  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // (comp, slab, g, t)
-  const int64_t slabs = npad / 8;
-  if (idx >= 3 * slabs * 32) return;
-  const int t = (int)(idx & 3), g = (int)((idx >> 2) & 7);
-  const int64_t slab = (idx >> 5) % slabs;
-  const int comp = (int)((idx >> 5) / slabs);
-  const float* src = M + ((int64_t)g * 3 + comp) * npad + slab * 8 + t;
-  const float v0 = src[0], v1 = src[4];
-  const uint32_t h0 = tf32_rn(__float_as_uint(v0)), h1 = tf32_rn(__float_as_uint(v1));
-  const float l0 = v0 - __uint_as_float(h0), l1 = v1 - __uint_as_float(h1);
-  Mq[idx] = make_float4(__uint_as_float(h0), __uint_as_float(h1), __uint_as_float(pack_bf16(v0, v1)),
-                        __uint_as_float(pack_bf16(l0, l1)));
-}
-
-__global__ void __launch_bounds__(kMbWarps * 32, 1)
-    demag_tma_mmab_kernel(const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmM, TmaArgs a,
-                          EpiArgs e) {
-  typedef MmabCfg Cfg;
-  constexpr int RT = kMmaRT, CT = kMmaCT, STAGES = kMmaStages, KS = kMbKS, SPW = kMbSPW;
-  extern __shared__ __align__(1024) unsigned char smem_raw[];
-  unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-  double* exch = (double*)(smem + STAGES * Cfg::stage_bytes);
-  uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::stage_bytes + Cfg::exch_bytes);
-  const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int64_t P = gridDim.x, c = blockIdx.x;
-  if (e.active_dev && !*e.active_dev) return;  // replayed attempt of a finished device-controlled DP45 run
-  const int64_t t0 = range_begin(a.tiles, P, c), t1 = range_begin(a.tiles, P, c + 1);
-
-  if (threadIdx.x == 0) {
-    for (int s = 0; s < STAGES; ++s) {
-      mbar_init(full0 + 8 * s, 1);
-      mbar_init(empty0 + 8 * s, kMbWarps);
-    }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  __syncthreads();
-  if (t0 >= t1) return;
-
-  // producer (lane 0 of warp 0), as in demag_tma_kernel
-  uint64_t pol_stream = 0, pol_keep = 0;
-  int p_stage = 0;
-  uint32_t p_phase = 0;
-  int64_t p_t = t0, p_g = t0 / a.chunks, p_k = t0 % a.chunks;
-  const bool is_producer = (threadIdx.x == 0);
-  if (is_producer) {
-    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
-    asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
-  }
-  auto top_up = [&](int64_t must) {
-    while (p_t < t1) {
-      if (!mbar_test(empty0 + 8 * p_stage, p_phase ^ 1)) {
-        if (p_t > must) break;
-        mbar_wait(empty0 + 8 * p_stage, p_phase ^ 1);
-      }
-      const uint32_t dst = smem_u32(smem + (size_t)p_stage * Cfg::stage_bytes);
-      mbar_expect_tx(full0 + 8 * p_stage, (uint32_t)Cfg::stage_bytes);
-      tma_load_3d(dst, &tmN, (int)(p_k * CT), (int)(p_g * RT), 0, full0 + 8 * p_stage, pol_stream);
-      tma_load_3d(dst + (uint32_t)Cfg::tensor_bytes, &tmM, 0, (int)(p_k * (CT / 8)), 0, full0 + 8 * p_stage, pol_keep);
-      if (++p_stage == STAGES) { p_stage = 0; p_phase ^= 1; }
-      if (++p_k == a.chunks) { p_k = 0; ++p_g; }
-      ++p_t;
-    }
-  };
-
-  const int rb = warp & 3, ks = warp >> 2;
-  const int g8 = lane >> 2, tig = lane & 3;
-  const int lm_r = lane & 7, lm_j = lane >> 3;
-  const uint32_t lm_row_off = (uint32_t)(rb * 16 + lm_r + 8 * (lm_j & 1)) * 128u;
-  uint32_t lm_chunk[SPW];
-#pragma unroll
-  for (int q = 0; q < SPW; ++q) lm_chunk[q] = (uint32_t)(((2 * (SPW * ks + q) + (lm_j >> 1)) ^ lm_r) << 4);
-
-  float d[3][4];
-  double acc[3][4];
-#pragma unroll
-  for (int cc = 0; cc < 3; ++cc)
-#pragma unroll
-    for (int i = 0; i < 4; ++i) { d[cc][i] = 0.f; acc[cc][i] = 0.0; }
-  int stage = 0;
-  uint32_t phase = 0;
-  int64_t g = t0 / a.chunks, k = t0 % a.chunks;
-  const int64_t g_first = g;
-  bool head_in_range = (k == 0);
-  for (int64_t t = t0; t < t1; ++t) {
-    if (is_producer) top_up(t);
-    __syncwarp();
-    mbar_wait(full0 + 8 * stage, phase);
-    const uint32_t tile = smem_u32(smem + (size_t)stage * Cfg::stage_bytes);
-    const float4* mq = (const float4*)(smem + (size_t)stage * Cfg::stage_bytes + Cfg::tensor_bytes);
-    uint32_t raw[SPW][6][4];
-    float4 bq[SPW][3];
-#pragma unroll
-    for (int q = 0; q < SPW; ++q) {
-#pragma unroll
-      for (int p = 0; p < 6; ++p)
-        asm volatile("ldmatrix.sync.aligned.m8n8.x4.shared.b16 {%0,%1,%2,%3}, [%4];"
-                     : "=r"(raw[q][p][0]), "=r"(raw[q][p][1]), "=r"(raw[q][p][2]), "=r"(raw[q][p][3])
-                     : "r"(tile + (uint32_t)p * (RT * 128u) + lm_row_off + lm_chunk[q]));
-#pragma unroll
-      for (int cc = 0; cc < 3; ++cc) bq[q][cc] = mq[(cc * (CT / 8) + SPW * ks + q) * 32 + lane];
-    }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(empty0 + 8 * stage);
-#pragma unroll
-    for (int p = 0; p < 6; ++p) {
-      constexpr int prow[6] = {0, 0, 0, 1, 1, 2}, pcol[6] = {0, 1, 2, 1, 2, 2};
-      const int ra = prow[p], ca = pcol[p];
-      uint32_t hi[SPW][4], alo[4], ax[4];  // tf32 hi per slab; bf16 pairs of x_lo and of x over the two slabs
-#pragma unroll
-      for (int q = 0; q < SPW; ++q) {
-        float lo[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          hi[q][i] = tf32_rn(raw[q][p][i]);
-          lo[i] = __uint_as_float(raw[q][p][i]) - __uint_as_float(hi[q][i]);
-        }
-        // tf32 fragment registers: 0 = (row g, col t), 1 = (row g+8, col t), 2 = (row g, col t+4), 3 = (row g+8, col t+4)
-        alo[2 * q + 0] = pack_bf16(lo[0], lo[2]);
-        alo[2 * q + 1] = pack_bf16(lo[1], lo[3]);
-        ax[2 * q + 0] = pack_bf16(__uint_as_float(raw[q][p][0]), __uint_as_float(raw[q][p][2]));
-        ax[2 * q + 1] = pack_bf16(__uint_as_float(raw[q][p][1]), __uint_as_float(raw[q][p][3]));
-      }
-      // small terms first: x_lo m and x m_lo over both slabs (bf16, k = 16), then x_hi m_hi per slab (tf32)
-      mma_bf16(d[ra], alo, __float_as_uint(bq[0][ca].z), __float_as_uint(bq[1][ca].z));
-      mma_bf16(d[ra], ax, __float_as_uint(bq[0][ca].w), __float_as_uint(bq[1][ca].w));
-      if (ra != ca) {
-        mma_bf16(d[ca], alo, __float_as_uint(bq[0][ra].z), __float_as_uint(bq[1][ra].z));
-        mma_bf16(d[ca], ax, __float_as_uint(bq[0][ra].w), __float_as_uint(bq[1][ra].w));
-      }
-#pragma unroll
-      for (int q = 0; q < SPW; ++q) {
-        mma_tf32(d[ra], hi[q], __float_as_uint(bq[q][ca].x), __float_as_uint(bq[q][ca].y));
-        if (ra != ca) mma_tf32(d[ca], hi[q], __float_as_uint(bq[q][ra].x), __float_as_uint(bq[q][ra].y));
-      }
-    }
-    if (++stage == STAGES) { stage = 0; phase ^= 1; }
-    const bool group_done = (k + 1 == a.chunks);
-    const bool emit = group_done || t + 1 == t1;
-#pragma unroll
-    for (int cc = 0; cc < 3; ++cc)
-#pragma unroll
-      for (int i = 0; i < 4; ++i) { acc[cc][i] += (double)d[cc][i]; d[cc][i] = 0.f; }
-    if (emit) {
-      if (ks > 0) {
-#pragma unroll
-        for (int cc = 0; cc < 3; ++cc)
-#pragma unroll
-          for (int i = 0; i < 4; ++i) exch[(((ks - 1) * 3 + cc) * 4 + i) * 128 + rb * 32 + lane] = acc[cc][i];
-      }
-      __syncthreads();
-      if (ks == 0) {
-#pragma unroll 1
-        for (int i = 0; i < 4; ++i) {
-          const int rg = rb * 16 + g8 + 8 * (i >> 1), b = 2 * tig + (i & 1);
-          const int64_t row = g * RT + rg;
-          double s3[3];
-#pragma unroll
-          for (int cc = 0; cc < 3; ++cc) {
             double v = i == 0 ? acc[cc][0] : i == 1 ? acc[cc][1] : i == 2 ? acc[cc][2] : acc[cc][3];
 #pragma unroll
             for (int w = 0; w < KS - 1; ++w) v += exch[((w * 3 + cc) * 4 + i) * 128 + rb * 32 + lane];
@@ -1206,7 +987,7 @@ int launch_T(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, i
 // (too few tiles to give every SM a share); the dispatcher then falls back to it.
 int mt_launch_demag_tma(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
                         const void* Mst, int64_t npad, const EpiArgs& e) {
-  if (ctx->variant != 2 && ctx->variant != 3) {
+  if (ctx->variant < 2) {
     const int64_t tiles = ((n_rows + 7) / 8) * ((n * (dtype == MT_F32 ? 4 : 8) + 1023) / 1024);
     if (tiles < 16LL * ctx->num_sms) return MT_ERR_UNIMPLEMENTED;
   }
