@@ -146,13 +146,17 @@ struct TmaCfg {
   static_assert(tensor_bytes % 128 == 0 && m_bytes % 128 == 0, "TMA destinations must stay 128-byte aligned");
 };
 
-template <typename T, int B, int RW, int CT, int STAGES>
+// NBOX > 1: a tile is NBOX boxes side by side (a TMA box is at most 256 elements wide), each laid out
+// [plane][row][CT / NBOX] in the stage, so that a row-plane contributes NBOX contiguous kilobytes per tile
+template <typename T, int B, int RW, int CT, int STAGES, int NBOX = 1>
 __global__ void __launch_bounds__(kThreads, 1)
     demag_tma_kernel(const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmM, TmaArgs a,
                      EpiArgs e) {
   typedef TmaCfg<T, B, RW, CT, STAGES> Cfg;
   typedef typename Vec<T>::type V;
   constexpr int RT = Cfg::RT, VPL = Cfg::VPL;
+  constexpr int BW = CT / NBOX;  // box width in elements
+  static_assert(CT % NBOX == 0 && BW <= 256 && BW % (32 * Cfg::W) == 0, "box width");
   extern __shared__ __align__(128) unsigned char smem_raw[];
   // (generic pointer on purpose: with the provenance-preserving form below the tile reads become LDS,
   // measured 0.5 % slower for this HBM-bound kernel — A/B on one box, r02 — while the packed-FMA kernel
@@ -195,8 +199,13 @@ __global__ void __launch_bounds__(kThreads, 1)
       }
       const uint32_t dst = smem_u32(smem + (size_t)p_stage * Cfg::stage_bytes);
       mbar_expect_tx(full0 + 8 * p_stage, (uint32_t)Cfg::stage_bytes);
-      tma_load_3d(dst, &tmN, (int)(p_k * CT), (int)(p_g * RT), 0, full0 + 8 * p_stage, pol_stream);
-      tma_load_2d(dst + (uint32_t)Cfg::tensor_bytes, &tmM, (int)(p_k * CT), 0, full0 + 8 * p_stage, pol_keep);
+#pragma unroll
+      for (int bx = 0; bx < NBOX; ++bx) {
+        tma_load_3d(dst + (uint32_t)(bx * (Cfg::tensor_bytes / NBOX)), &tmN, (int)(p_k * CT + bx * BW), (int)(p_g * RT), 0,
+                    full0 + 8 * p_stage, pol_stream);
+        tma_load_2d(dst + (uint32_t)(Cfg::tensor_bytes + bx * (Cfg::m_bytes / NBOX)), &tmM, (int)(p_k * CT + bx * BW), 0,
+                    full0 + 8 * p_stage, pol_keep);
+      }
       if (++p_stage == STAGES) { p_stage = 0; p_phase ^= 1; }
       if (++p_k == a.chunks) { p_k = 0; ++p_g; }
       ++p_t;
@@ -236,18 +245,22 @@ __global__ void __launch_bounds__(kThreads, 1)
     }
 #pragma unroll
     for (int v = 0; v < VPL; ++v) {
-      const int col = (v * 32 + lane) * Cfg::W;
+      const int colt = (v * 32 + lane) * Cfg::W;          // column in the tile
+      const int bx = (v * 32 * Cfg::W) / BW;                // its box (compile-time per v)
+      const int col = colt - bx * BW;
+      const T* tbox = tile + (size_t)bx * (6 * RT * BW);
+      const T* mbox = mt + (size_t)bx * (3 * B * BW);
       V tv[RW][6];
 #pragma unroll
       for (int r = 0; r < RW; ++r)
 #pragma unroll
         for (int cc = 0; cc < 6; ++cc)
-          tv[r][cc] = *(const V*)(tile + ((size_t)cc * RT + (warp * RW + r)) * CT + col);
+          tv[r][cc] = *(const V*)(tbox + ((size_t)cc * RT + (warp * RW + r)) * BW + col);
 #pragma unroll
       for (int b = 0; b < B; ++b) {
         V mv[3];
 #pragma unroll
-        for (int cc = 0; cc < 3; ++cc) mv[cc] = *(const V*)(mt + (size_t)(b * 3 + cc) * CT + col);
+        for (int cc = 0; cc < 3; ++cc) mv[cc] = *(const V*)(mbox + (size_t)(b * 3 + cc) * BW + col);
 #pragma unroll
         for (int r = 0; r < RW; ++r) fma3(run_of(r, b), tv[r], mv);
       }
@@ -831,7 +844,7 @@ int make_map(mt_ctx* ctx, CUtensorMap* out, int dtype, const void* base, int ran
 // Cfg = tile geometry; kern = the kernel instantiated for it; m_rows = rows of the staged-M box (3 B)
 template <typename T, typename Cfg, typename Kern>
 int launch_tiles(mt_ctx* ctx, Kern kern, unsigned char* attr_set, int m_rows, const void* N, int dtype, int64_t n,
-                 int64_t n_rows, int64_t ld, const void* Mst, int64_t npad, const EpiArgs& e) {
+                 int64_t n_rows, int64_t ld, const void* Mst, int64_t npad, const EpiArgs& e, int nbox = 1) {
   constexpr int RT = Cfg::RT;
   static_assert(Cfg::smem_bytes <= 227 * 1024, "ring does not fit shared memory");
   const int64_t P = ctx->num_sms;
@@ -848,14 +861,14 @@ int launch_tiles(mt_ctx* ctx, Kern kern, unsigned char* attr_set, int m_rows, co
   {
     const uint64_t dims[3] = {(uint64_t)n, (uint64_t)n_rows, 6};
     const uint64_t strides[2] = {(uint64_t)ld * sizeof(T), (uint64_t)n_rows * (uint64_t)ld * sizeof(T)};
-    const uint32_t box[3] = {(uint32_t)Cfg::CT, (uint32_t)RT, 6};
+    const uint32_t box[3] = {(uint32_t)(Cfg::CT / nbox), (uint32_t)RT, 6};
     if ((rc = make_map(ctx, &tmN, dtype, N, 3, dims, strides, box))) return rc;
   }
   {
     // the staged-M buffers always hold MT_MAX_BATCH states (rows beyond 3*batch: zero or stale, unused)
     const uint64_t dims[2] = {(uint64_t)npad, (uint64_t)(3 * MT_MAX_BATCH)};
     const uint64_t strides[1] = {(uint64_t)npad * sizeof(T)};
-    const uint32_t box[2] = {(uint32_t)Cfg::CT, (uint32_t)m_rows};
+    const uint32_t box[2] = {(uint32_t)(Cfg::CT / nbox), (uint32_t)m_rows};
     if ((rc = make_map(ctx, &tmM, dtype, Mst, 2, dims, strides, box))) return rc;
   }
   // the attribute is per DEVICE (a second mt_ctx on another device of the same process needs its own
@@ -875,12 +888,12 @@ int launch_tiles(mt_ctx* ctx, Kern kern, unsigned char* attr_set, int m_rows, co
   return MT_OK;
 }
 
-template <typename T, int B, int RW, int CT, int STAGES>
+template <typename T, int B, int RW, int CT, int STAGES, int NBOX = 1>
 int launch_cfg(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
                int64_t npad, const EpiArgs& e) {
   static unsigned char attr_set[kMaxDevices] = {};
-  return launch_tiles<T, TmaCfg<T, B, RW, CT, STAGES>>(ctx, demag_tma_kernel<T, B, RW, CT, STAGES>, attr_set, 3 * B,
-                                                        N, dtype, n, n_rows, ld, Mst, npad, e);
+  return launch_tiles<T, TmaCfg<T, B, RW, CT, STAGES>>(ctx, demag_tma_kernel<T, B, RW, CT, STAGES, NBOX>, attr_set, 3 * B,
+                                                        N, dtype, n, n_rows, ld, Mst, npad, e, NBOX);
 }
 
 // fp32, 5 <= batch <= 8: packed-FMA kernel (states beyond `batch` are computed on unused rows of M
@@ -962,7 +975,17 @@ template <typename T>
 int launch_T(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
              int64_t npad, const EpiArgs& e) {
   constexpr int CT1 = 1024 / sizeof(T);  // 1 KB of one row-plane per tile
-  if (e.batch == 1) return launch_cfg<T, 1, 1, CT1, 4>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+  // batches of 1 and 2: tiles of two boxes side by side (2 KB of every row-plane per tile, 96 KB per stage,
+  // two stages) — r05 A/B at config 5, batch 1: 14.94 ms with one-box tiles in four stages, 13.97 ms with
+  // two-box tiles in two (7.38 TB/s: the rate of the read-only stream microbenchmark)
+#ifndef MT_B1_NBOX
+#define MT_B1_NBOX 2
+#define MT_B1_STAGES 2
+#endif
+  if (e.batch == 1) return launch_cfg<T, 1, 1, CT1 * MT_B1_NBOX, MT_B1_STAGES, MT_B1_NBOX>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
+  // (batch 2 on fp32 tensors is no faster with them: 14.61 vs 14.58 ms; on fp64 tensors 7.36 vs 7.47 ms at config 3)
+  if (e.batch == 2 && sizeof(T) == 8)
+    return launch_cfg<T, 2, 1, CT1 * MT_B1_NBOX, MT_B1_STAGES, MT_B1_NBOX>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
   if (e.batch == 2) return launch_cfg<T, 2, 1, CT1, 4>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
   if (e.batch >= 3 && e.batch <= MT_MAX_BATCH) {
     if constexpr (sizeof(T) == 4) {
