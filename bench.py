@@ -36,8 +36,8 @@ NCU_CAPTURES = {
     # dram__bytes_read.sum + dram__bytes_write.sum per launch of the batch-1 field kernel;
     # key = (config, tensor dtype, n_gpus)
     "traffic_bytes": {
-        (5, "f32", 1): {"value": 103.082146e9 + 5.291520e6, "source": "profiles/r02_ncu_full_summaries.md",
-                        "kernel_commit": "45b85d2 (demag_tma_kernel unchanged since)"},
+        (5, "f32", 1): {"value": 103.082073e9 + 5.633280e6, "source": "profiles/r05_b1_ncu_full.md",
+                        "kernel_commit": "edb8245"},
     },
     # DFMA + DADD + DMUL thread-instructions per tile pair of the assembly kernels
     "asm_fp64_inst_per_pair": {
