@@ -40,8 +40,7 @@ constexpr int kMaxDevices = 64;  // device ordinals tracked by the per-device at
 #endif
 #ifndef MT_B4_WARPS
 #define MT_B4_WARPS 8
-#define MT_B4_CT 128
-#define MT_B4_STAGES 4
+#define MT_B4_CT 128 /* box width; a tile is two boxes */
 #endif
 constexpr int kThreads = kConsumerWarps * 32;
 
@@ -346,7 +345,7 @@ template <int NP> struct PairVec;
 template <> struct PairVec<1> { unsigned long long p[1]; };
 template <> struct alignas(16) PairVec<2> { unsigned long long p[2]; };
 
-template <int B, int WARPS, int CT, int STAGES>
+template <int B, int WARPS, int CT, int STAGES, int NBOX = 1>
 __global__ void __launch_bounds__(WARPS * 32, 1)
     demag_tma_f32x2_kernel(const __grid_constant__ CUtensorMap tmN, const __grid_constant__ CUtensorMap tmM,
                            TmaArgs a, EpiArgs e) {
@@ -354,8 +353,9 @@ __global__ void __launch_bounds__(WARPS * 32, 1)
   constexpr int RT = Cfg::RT, RW = kPackRW;
   constexpr int NV = RW * B * 3;                 // fp32 sums per lane
   constexpr int kOwnShift = (B == 8) ? 1 : 2;    // lane l ends up owning (row, state) index l >> kOwnShift
-  constexpr int NP = CT / 64;            // column pairs per lane
-  constexpr int kFlush = 96 / (3 * NP);  // tiles per fp32 run: <= 96 terms per accumulator
+  constexpr int BW = CT / NBOX;          // box width (a tile is NBOX boxes side by side, as in demag_tma_kernel)
+  constexpr int NP = BW / 64;            // column pairs per lane per box
+  constexpr int kFlush = 96 / (3 * NP * NBOX);  // tiles per fp32 run: <= 96 terms per accumulator
   static_assert((NP == 1 || NP == 2) && (B == 4 || B == 8), "lane mapping of the transposing butterfly");
   typedef PairVec<NP> PV;
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -398,8 +398,13 @@ __global__ void __launch_bounds__(WARPS * 32, 1)
       }
       const uint32_t dst = smem_u32(smem + (size_t)p_stage * Cfg::stage_bytes);
       mbar_expect_tx(full0 + 8 * p_stage, (uint32_t)Cfg::stage_bytes);
-      tma_load_3d(dst, &tmN, (int)(p_k * CT), (int)(p_g * RT), 0, full0 + 8 * p_stage, pol_stream);
-      tma_load_2d(dst + (uint32_t)Cfg::tensor_bytes, &tmM, (int)(p_k * CT), 0, full0 + 8 * p_stage, pol_keep);
+#pragma unroll
+      for (int bx = 0; bx < NBOX; ++bx) {
+        tma_load_3d(dst + (uint32_t)(bx * (Cfg::tensor_bytes / NBOX)), &tmN, (int)(p_k * CT + bx * BW), (int)(p_g * RT), 0,
+                    full0 + 8 * p_stage, pol_stream);
+        tma_load_2d(dst + (uint32_t)(Cfg::tensor_bytes + bx * (Cfg::m_bytes / NBOX)), &tmM, (int)(p_k * CT + bx * BW), 0,
+                    full0 + 8 * p_stage, pol_keep);
+      }
       if (++p_stage == STAGES) { p_stage = 0; p_phase ^= 1; }
       if (++p_k == a.chunks) { p_k = 0; ++p_g; }
       ++p_t;
@@ -425,17 +430,21 @@ __global__ void __launch_bounds__(WARPS * 32, 1)
     const float* tile = (const float*)(smem + (size_t)stage * Cfg::stage_bytes);
     const float* mt = (const float*)(smem + (size_t)stage * Cfg::stage_bytes + Cfg::tensor_bytes);
     const int col = lane * (2 * NP);
+#pragma unroll
+    for (int bx = 0; bx < NBOX; ++bx) {
+    const float* tbox = tile + (size_t)bx * (6 * RT * BW);
+    const float* mbox = mt + (size_t)bx * (3 * B * BW);
     PV tv[RW][6];
 #pragma unroll
     for (int r = 0; r < RW; ++r)
 #pragma unroll
       for (int cc = 0; cc < 6; ++cc)
-        tv[r][cc] = *(const PV*)(tile + ((size_t)cc * RT + (warp * RW + r)) * CT + col);
+        tv[r][cc] = *(const PV*)(tbox + ((size_t)cc * RT + (warp * RW + r)) * BW + col);
 #pragma unroll
     for (int b = 0; b < B; ++b) {
       PV mv[3];
 #pragma unroll
-      for (int cc = 0; cc < 3; ++cc) mv[cc] = *(const PV*)(mt + (size_t)(b * 3 + cc) * CT + col);
+      for (int cc = 0; cc < 3; ++cc) mv[cc] = *(const PV*)(mbox + (size_t)(b * 3 + cc) * BW + col);
 #pragma unroll
       for (int r = 0; r < RW; ++r)
 #pragma unroll
@@ -451,6 +460,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1)
           ffma2(run[r][b][1], tv[r][4].p[q], mv[2].p[q]);
           ffma2(run[r][b][2], tv[r][5].p[q], mv[2].p[q]);
         }
+    }
     }
     __syncwarp();
     if (lane == 0) mbar_arrive(empty0 + 8 * stage);
@@ -898,12 +908,12 @@ int launch_cfg(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows,
 
 // fp32, 5 <= batch <= 8: packed-FMA kernel (states beyond `batch` are computed on unused rows of M
 // and dropped)
-template <int B, int WARPS, int CT, int STAGES>
+template <int B, int WARPS, int CT, int STAGES, int NBOX = 1>
 int launch_f32x2_shape(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
                        int64_t npad, const EpiArgs& e) {
   static unsigned char attr_set[kMaxDevices] = {};
   return launch_tiles<float, TmaCfg<float, B, kPackRW, CT, STAGES, WARPS>>(
-      ctx, demag_tma_f32x2_kernel<B, WARPS, CT, STAGES>, attr_set, 3 * B, N, MT_F32, n, n_rows, ld, Mst, npad, e);
+      ctx, demag_tma_f32x2_kernel<B, WARPS, CT, STAGES, NBOX>, attr_set, 3 * B, N, MT_F32, n, n_rows, ld, Mst, npad, e, NBOX);
 }
 
 // fp32, 5 <= batch <= 8: tensor-core kernel (error-compensated TF32); states beyond `batch` are
@@ -965,7 +975,9 @@ int launch_mma(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld
 // unused rows of M and dropped)
 int launch_f32x2(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld, const void* Mst, int64_t npad,
                  const EpiArgs& e) {
-  if (e.batch <= 4) return launch_f32x2_shape<4, MT_B4_WARPS, MT_B4_CT, MT_B4_STAGES>(ctx, N, n, n_rows, ld, Mst, npad, e);
+  // two boxes of MT_B4_CT columns side by side per tile, two stages (r05 A/B at config 5: batches of 3 and 4
+  // 16.4-16.7 -> 15.5-15.6 ms against one-box tiles in four stages)
+  if (e.batch <= 4) return launch_f32x2_shape<4, MT_B4_WARPS, MT_B4_CT * 2, 2, 2>(ctx, N, n, n_rows, ld, Mst, npad, e);
   // variant 3 keeps the packed-FFMA2 kernel for A/B comparisons; the default is the tensor-core kernel
   if (ctx->variant != 3) return launch_mma(ctx, N, n, n_rows, ld, Mst, npad, e);
   return launch_f32x2_shape<8, MT_B8_WARPS, MT_B8_CT, MT_B8_STAGES>(ctx, N, n, n_rows, ld, Mst, npad, e);
