@@ -124,6 +124,7 @@ struct TmaArgs {
   int64_t chunks;   // ceil(n / CT)
   int64_t tiles;    // groups * chunks
   double* partial;  // [P][2][RT][B][3]
+  double* exch;     // tensor-core kernel: [P][MmaCfg::exch_doubles] column parts of a row block
 };
 
 __host__ __device__ __forceinline__ int64_t range_begin(int64_t tiles, int64_t P, int64_t c) {
@@ -554,7 +555,12 @@ __global__ void __launch_bounds__(WARPS * 32, 1)
 #ifndef MT_MMA_FLUSH_TILES
 #define MT_MMA_FLUSH_TILES 1  /* measured (N = 32,768, 8 states, vs the fp64 tensor): 1 -> 2.0e-7, 2 -> 4.3e-7, 8 -> 1.8e-6 */
 #endif
-constexpr int kMmaWarps = MT_MMA_WARPS, kMmaRT = 64, kMmaCT = 32, kMmaStages = 3;
+#ifndef MT_MMA_NBOX
+#define MT_MMA_NBOX 2 /* swizzled boxes of 32 columns side by side in a tile (1: three stages of 54 KB, 2: two of 108 KB; r05 A/B at config 5, eight states: 17.7 -> 16.45 ms) */
+#endif
+constexpr int kMmaNBox = MT_MMA_NBOX;
+constexpr int kMmaWarps = MT_MMA_WARPS, kMmaRT = 64, kMmaCT = 32 * kMmaNBox, kMmaStages = kMmaNBox == 1 ? 3 : 2;
+constexpr uint32_t kMmaBoxBytes = 6u * kMmaRT * 128u;  // one swizzled box: 6 planes x 64 rows x 128 bytes
 constexpr int kMmaKS = kMmaWarps / 4;           // warps that share a row block (column split of a tile)
 constexpr int kMmaSPW = (kMmaCT / 8) / kMmaKS;  // 8-column slabs per warp per tile
 constexpr int kMmaFlush = MT_MMA_FLUSH_TILES;
@@ -564,8 +570,10 @@ struct MmaCfg {
   static constexpr size_t tensor_bytes = (size_t)6 * kMmaRT * kMmaCT * 4;          // 49,152
   static constexpr size_t m_bytes = (size_t)3 * (kMmaCT / 8) * 128 * 4;           // 6,144
   static constexpr size_t stage_bytes = tensor_bytes + m_bytes;                  // 55,296 = 54 KB
-  static constexpr size_t exch_bytes = (size_t)(kMmaKS - 1) * 12 * 4 * 32 * sizeof(double);
-  static constexpr size_t smem_bytes = kMmaStages * stage_bytes + exch_bytes + 2 * kMmaStages * sizeof(uint64_t) + 1024;
+  // column parts of a row block meet in a per-CTA global scratch at the end of a row group (rare: once per
+  // 64 rows x n columns), not in shared memory: the ring may use all of it
+  static constexpr size_t exch_doubles = (size_t)(kMmaKS - 1) * 12 * 4 * 32;
+  static constexpr size_t smem_bytes = kMmaStages * stage_bytes + 2 * kMmaStages * sizeof(uint64_t) + 1024;
   static_assert(stage_bytes % 1024 == 0, "swizzled tiles must start on 1 KB boundaries");
 };
 
@@ -600,12 +608,12 @@ __global__ void __launch_bounds__(kMmaWarps * 32, 1)
   constexpr int RT = kMmaRT, CT = kMmaCT, STAGES = kMmaStages, KS = kMmaKS, SPW = kMmaSPW;
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-  double* exch = (double*)(smem + STAGES * Cfg::stage_bytes);
-  uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::stage_bytes + Cfg::exch_bytes);
+  uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::stage_bytes);
   const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t P = gridDim.x, c = blockIdx.x;
   if (e.active_dev && !*e.active_dev) return;  // replayed attempt of a finished device-controlled DP45 run
+  double* exch = a.exch + (size_t)c * Cfg::exch_doubles;
   const int64_t t0 = range_begin(a.tiles, P, c), t1 = range_begin(a.tiles, P, c + 1);
 
   if (threadIdx.x == 0) {
@@ -636,7 +644,10 @@ __global__ void __launch_bounds__(kMmaWarps * 32, 1)
       }
       const uint32_t dst = smem_u32(smem + (size_t)p_stage * Cfg::stage_bytes);
       mbar_expect_tx(full0 + 8 * p_stage, (uint32_t)Cfg::stage_bytes);
-      tma_load_3d(dst, &tmN, (int)(p_k * CT), (int)(p_g * RT), 0, full0 + 8 * p_stage, pol_stream);
+#pragma unroll
+      for (int bx = 0; bx < kMmaNBox; ++bx)
+        tma_load_3d(dst + (uint32_t)bx * kMmaBoxBytes, &tmN, (int)(p_k * CT + bx * 32), (int)(p_g * RT), 0,
+                    full0 + 8 * p_stage, pol_stream);
       tma_load_3d(dst + (uint32_t)Cfg::tensor_bytes, &tmM, 0, (int)(p_k * (CT / 8)), 0, full0 + 8 * p_stage, pol_keep);
       if (++p_stage == STAGES) { p_stage = 0; p_phase ^= 1; }
       if (++p_k == a.chunks) { p_k = 0; ++p_g; }
@@ -653,7 +664,10 @@ __global__ void __launch_bounds__(kMmaWarps * 32, 1)
   const uint32_t lm_row_off = (uint32_t)(rb * 16 + lm_r + 8 * (lm_j & 1)) * 128u;
   uint32_t lm_chunk[SPW];
 #pragma unroll
-  for (int q = 0; q < SPW; ++q) lm_chunk[q] = (uint32_t)(((2 * (SPW * ks + q) + (lm_j >> 1)) ^ lm_r) << 4);
+  for (int q = 0; q < SPW; ++q) {
+    const int sl = SPW * ks + q;  // slab of the tile: box sl >> 2, 16-byte chunks 2 (sl & 3), 2 (sl & 3) + 1 of the row
+    lm_chunk[q] = (uint32_t)(sl >> 2) * kMmaBoxBytes + (uint32_t)(((2 * (sl & 3) + (lm_j >> 1)) ^ lm_r) << 4);
+  }
 
   float d[3][4];
   double acc[3][4];
@@ -867,6 +881,7 @@ int launch_tiles(mt_ctx* ctx, Kern kern, unsigned char* attr_set, int m_rows, co
   int rc = mt_ensure_ws(ctx, (void**)&ctx->partial, &ctx->partial_bytes, need);
   if (rc) return rc;
   a.partial = ctx->partial;
+  a.exch = nullptr;
   alignas(64) CUtensorMap tmN, tmM;
   {
     const uint64_t dims[3] = {(uint64_t)n, (uint64_t)n_rows, 6};
@@ -929,9 +944,12 @@ int launch_mma(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld
   a.groups = (n_rows + RT - 1) / RT;
   a.chunks = (n + Cfg::CT - 1) / Cfg::CT;
   a.tiles = a.groups * a.chunks;
-  int rc = mt_ensure_ws(ctx, (void**)&ctx->partial, &ctx->partial_bytes, (size_t)P * 2 * RT * e.batch * 3 * sizeof(double));
+  const size_t partial_doubles = (size_t)P * 2 * RT * e.batch * 3;
+  int rc = mt_ensure_ws(ctx, (void**)&ctx->partial, &ctx->partial_bytes,
+                        (partial_doubles + (size_t)P * Cfg::exch_doubles) * sizeof(double));
   if (rc) return rc;
   a.partial = ctx->partial;
+  a.exch = ctx->partial + partial_doubles;
   // M re-laid out for the B fragments: hi/lo split, [3][npad/8][8 states][4][4] fp32
   const size_t mq_bytes = (size_t)3 * (npad / 8) * 32 * sizeof(float4);
   if ((rc = mt_ensure_ws(ctx, &ctx->Mq, &ctx->Mq_bytes, mq_bytes))) return rc;
@@ -945,7 +963,7 @@ int launch_mma(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld
   {
     const uint64_t dims[3] = {(uint64_t)n, (uint64_t)n_rows, 6};
     const uint64_t strides[2] = {(uint64_t)ld * 4, (uint64_t)n_rows * (uint64_t)ld * 4};
-    const uint32_t box[3] = {(uint32_t)Cfg::CT, (uint32_t)RT, 6};
+    const uint32_t box[3] = {32, (uint32_t)RT, 6};  // one swizzle span wide; a tile is kMmaNBox of them
     if ((rc = make_map(ctx, &tmN, MT_F32, N, 3, dims, strides, box, /*swizzle128=*/true))) return rc;
   }
   {
