@@ -59,6 +59,12 @@ def parse_args():
     ap.add_argument("--protocol", action="store_true", help="also run the config's own workload as BASELINE.json states it")
     ap.add_argument("--protocol-t-end", type=float, default=0.0, help="config 3 protocol: stop time (default 200)")
     ap.add_argument("--grid", type=str, default="", help="override nx,ny,nz (debug only; marks the line invalid)")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"], help="torch.distributed backend for --gpus N (gloo: debug)")
+    ap.add_argument("--force-dist", action="store_true",
+                    help="debug only: initialise torch.distributed and run the exchange steps even with one rank "
+                         "(under torchrun --nproc-per-node 1: exercises the NCCL calls of the N > 1 path on a 1-GPU box)")
+    ap.add_argument("--one-device", action="store_true",
+                    help="debug only, with --grid: every rank uses cuda:0 (functional check of the N > 1 path on a 1-GPU box)")
     ap.add_argument("--variant", type=int, default=0, help="demag kernel variant (0 auto, 1 LDG, 2 TMA)")
     ap.add_argument("--f4", action="store_true", help="also run the F4 report (SP2-shaped sweep, SP3 flower/vortex energies)")
     ap.add_argument("--skip-extras", action="store_true", help="only the headline metric (used under ncu)")
@@ -246,13 +252,19 @@ class Runner:
         self.rank = int(os.environ.get("RANK", "0"))
         self.local_rank = int(os.environ.get("LOCAL_RANK", "0"))
         self.dist = None
-        if self.world > 1:
+        if args.one_device and not args.grid:
+            raise SystemExit("--one-device is a debug switch and needs --grid")
+        self.device_index = 0 if args.one_device else self.local_rank
+        if self.world > 1 or args.force_dist:
             import torch.distributed as dist
-            dist.init_process_group("nccl", device_id=torch.device(f"cuda:{self.local_rank}"))
+            if args.backend == "nccl":
+                dist.init_process_group("nccl", device_id=torch.device(f"cuda:{self.device_index}"))
+            else:
+                dist.init_process_group("gloo")
             self.dist = dist
-        torch.cuda.set_device(self.local_rank)
-        self.dev = f"cuda:{self.local_rank}"
-        self.ctx = B.mt_create(self.local_rank)
+        torch.cuda.set_device(self.device_index)
+        self.dev = f"cuda:{self.device_index}"
+        self.ctx = B.mt_create(self.device_index)
         if args.variant:
             B.mt_set_demag_variant(self.ctx, args.variant)
         self.kernel_ms = {}
@@ -274,7 +286,7 @@ class Runner:
         for _ in range(warmup):
             fn()
         self.barrier()
-        sampler = ClockSampler(self.local_rank) if (clocks and self.rank == 0) else None
+        sampler = ClockSampler(self.device_index) if (clocks and self.rank == 0) else None
         e0, e1 = self.ev(), self.ev()
         l0 = ctx.launches
         if tag:
@@ -509,13 +521,13 @@ def run_extras(R, args, out, w, tiles, N, ld, dtype, m_all, m1, Hd1, step_field,
     # ---- fused right-hand side (A4-A6) and the batched variant (A7) ---------------------------------
     prob = H.dev_problem(w, tiles, N, dtype, ld)
     shard = None
-    if world > 1:
+    if dist is not None:
         shard = B.Shard(rank, world, n, 1, dev, S.dist_exchange(dist, rank))
         prob.shard = shard
     k1 = torch.empty_like(m1)
     ms_rhs, _, _ = R.timed(lambda: B.mt_llg_rhs(ctx, prob, m1, 1, k1, None), 3, max(5, K // 2))
     out["llg_rhs"] = {"evals_per_s": 1000.0 / ms_rhs, "ms": ms_rhs}
-    if world > 1:
+    if dist is not None:
         # the simulation loop, row-sharded (mt.h section 8(e)): RK4 steps of mt_integrate, one in-place
         # all-gather of the next stage state per right-hand side
         mi = m1.clone()
@@ -876,7 +888,7 @@ def main():
     Hd1 = torch.empty((1, 3, rows), dtype=torch.float64, device=dev)
     # the one real exchange step of the sharded field: all-gather of the ranks' slices through
     # preallocated, equally padded blocks (nothing allocated or reassembled inside the timed step)
-    gather = S.FieldGather(dist, rank, world, n, 1, dev) if world > 1 else None
+    gather = S.FieldGather(dist, rank, world, n, 1, dev) if dist is not None else None
 
     def step_field():
         B.mt_demag_field(ctx, N, code, n, rows, ld, tiles.Ms, m1, 1, Hd1)
@@ -893,7 +905,7 @@ def main():
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong", "vs_baseline": None,
         "dtype": dtype, "data": "synthetic",
-        "config": {"workload": wname, "parallelism": f"row-sharded x{world}" if world > 1 else "single GPU",
+        "config": {"workload": wname, "parallelism": f"row-sharded x{world}" if dist is not None else "single GPU",
                    "l2": ("tensor (12.6 MB) is L2-resident by design of this config: no flush, the HBM roofline does not apply"
                           if l2_resident else
                           "tensor streamed per step is far larger than the 126 MB L2: no flush needed"),

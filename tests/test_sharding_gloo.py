@@ -32,6 +32,21 @@ def test_row_bands_tile_the_rows_in_rank_order():
         S.row_band(2, 2, 10)
 
 
+def test_blocks_reassemble_through_the_precomputed_index():
+    """pack [world, B, 3, pad] (block g = rows of rank g, padded to the widest band) -> [B, 3, n]: the torch
+    mirror of the library's scatter kernel, for even and uneven bands."""
+    for world, n in ((1, 5), (2, 90), (3, 40), (4, 7), (8, 65536)):
+        pad = S.max_band_rows(world, n)
+        full = torch.arange(2 * 3 * n, dtype=torch.float64).reshape(2, 3, n)
+        pack = torch.full((world, 2, 3, pad), -1.0, dtype=torch.float64)
+        for g in range(world):
+            a, b = S.row_band(g, world, n)
+            pack[g, :, :, : b - a] = full[:, :, a:b]
+        assert torch.equal(S.unpack(pack, n), full)
+        idx = S.unpack_index(world, n, pad)
+        assert idx.shape == (n,) and int(idx.max()) < world * pad and len(set(idx.tolist())) == n
+
+
 def _free_port() -> int:
     with socket.socket() as s:
         s.bind(("127.0.0.1", 0))

@@ -1,5 +1,6 @@
 """-m "not gpu": host logic of the seeded input generators (no method arithmetic)."""
 import numpy as np
+import pytest
 
 from paper_2107_05364_b200 import workloads as W
 
@@ -124,3 +125,24 @@ def test_fields_of_a_reordered_problem_are_the_permuted_fields(oracle):
     k_w, _ = oracle.llg_rhs(H.oracle_problem(oracle, w, N_w), w.m)
     k_r, _ = oracle.llg_rhs(H.oracle_problem(oracle, r, N_r), r.m)
     assert np.max(np.abs(k_r - k_w[:, :, perm])) <= 1e-13 * np.max(np.abs(k_w))
+
+
+def test_sp2_and_sp3_shaped_seeds():
+    """The report-only F4 workloads (PAPER.md:163-199 shapes): unit vectors, the stated tile counts and aspect
+    ratios, Neumann neighbour tables; the flower seed points along z, the vortex seed circulates about x."""
+    w = W.sp2_film(10.0)
+    assert w.n == 6000 and w.grid == (100, 20, 3) and w.gamma == 0.0
+    L = np.array(w.grid) * w.size[0]
+    assert np.allclose(L, [50.0, 10.0, 1.0])          # L = 5 d, d, d / 10 in exchange lengths
+    assert np.allclose(np.linalg.norm(w.m, axis=1), 1.0) and np.allclose(w.m[0, :, 0], 1 / np.sqrt(3))
+    for kind in ("flower", "vortex"):
+        c = W.sp3_cube(8, 8.5, kind)
+        assert c.n == 512 and np.allclose(np.linalg.norm(c.m, axis=1), 1.0, atol=1e-14)
+        assert np.allclose(c.size, 8.5 / 8) and c.c_an == 0.1 and tuple(c.easy) == (0.0, 0.0, 1.0)
+    f, v = W.sp3_cube(8, 8.5, "flower"), W.sp3_cube(8, 8.5, "vortex")
+    assert f.m[0, 2].min() > 0.9 and abs(f.m[0, 0].mean()) < 1e-12
+    r = v.center / 8.5 - 0.5
+    circ = (r[:, 1] * v.m[0, 2] - r[:, 2] * v.m[0, 1]).sum()   # x component of sum r x m: the circulation
+    assert circ > 0.5 * np.sqrt(r[:, 1] ** 2 + r[:, 2] ** 2).sum() * 0.5
+    with pytest.raises(ValueError):
+        W.sp3_cube(4, 8.0, "onion")
