@@ -120,7 +120,9 @@ int mt_set_assembly_mode(mt_ctx* ctx, int mode);
  * N is [6][n_rows][ld] (n_rows == n for the full tensor; a row band gives the band's field),
  * Ms [n], m [batch][3][n], Hd [batch][3][n_rows], 1 <= batch <= 8.  For MT_F32 the product
  * Ms*m is rounded to fp32 once, products are fp32 and accumulation is fp32 over at most 128
- * consecutive terms per lane then fp64 (Q19); for MT_F64 everything is fp64.  The
+ * consecutive terms per lane then fp64 (Q19); batches of 5..8 states on an MT_F32 tensor run
+ * as an error-compensated 3xTF32 tensor-core contraction (operands split hi + lo, three products, fp32
+ * accumulation over one tile then fp64: ~2e-7 relative); for MT_F64 everything is fp64.  The
  * reduction order is fixed: results are bitwise reproducible run to run.
  * Errors: MT_ERR_INVALID_ARG, MT_ERR_CUDA.                                                        */
 int mt_demag_field(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
