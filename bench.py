@@ -538,10 +538,15 @@ def run_extras(R, args, out, w, tiles, N, ld, dtype, m_all, m1, Hd1, step_field,
         t, res, ms, launches = integrate_timed(R, prob, mi, 1, method=B.MT_RK4, dt=dt_rk, t_end=steps_rk * dt_rk)
         tt = torch.tensor([ms], device=dev)
         dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        ref0 = mi.clone()
+        dist.broadcast(ref0, src=0)                      # every rank must hold the same state, bit for bit
+        same = torch.tensor([1.0 if torch.equal(ref0, mi) else 0.0], device=dev)
+        dist.all_reduce(same, op=dist.ReduceOp.MIN)
         out["sharded_rk4"] = {"rhs_calls": res["rhs_calls"], "ms_per_rhs": float(tt.item()) / res["rhs_calls"],
                               "rhs_evals_per_s": 1000.0 * res["rhs_calls"] / float(tt.item()),
-                              "exchange": "one all_gather_into_tensor (NCCL) of the next stage state per right-hand side",
-                              "finite": bool(torch.isfinite(mi).all().item())}
+                              "exchange": f"one all_gather_into_tensor ({args.backend}) of the next stage state per right-hand side",
+                              "finite": bool(torch.isfinite(mi).all().item()),
+                              "ranks_hold_identical_state": bool(same.item() == 1.0)}
     if nb >= 8:
         Hd8 = torch.empty((8, 3, rows), dtype=torch.float64, device=dev)
         ms_b8, _, clk8 = R.timed(lambda: B.mt_demag_field(ctx, N, code, n, rows, ld, tiles.Ms, m_all, 8, Hd8),
