@@ -180,10 +180,9 @@ int mt_create(mt_ctx** out, int device, void* cuda_stream) {
     return MT_ERR_CUDA;
   }
   c->num_sms = prop.multiProcessorCount;
-  // device scalars: [0] err bits, [1] torque bits, [2..5] the selection's bin search, [8 + 2048 ..] 256
-  // per-step torque words of an RK4 chunk; the pinned mirror holds
-  // the two words, the search result or the chunk's torques
-  if (cudaMalloc((void**)&c->dscal, (8 + 2048 + 256) * sizeof(unsigned long long)) != cudaSuccess ||
+  // device scalars: [0] err bits, [1] torque bits, [2..5] the selection's bin search, [8 ..] 256 per-step
+  // torque words of an RK4 chunk; the pinned mirror holds the two words, the search result or the chunk's torques
+  if (cudaMalloc((void**)&c->dscal, (8 + 256) * sizeof(unsigned long long)) != cudaSuccess ||
       cudaMallocHost((void**)&c->hscal, 2048 * sizeof(unsigned long long)) != cudaSuccess) {
     cudaFree(c->dscal);
     delete c;
@@ -892,7 +891,7 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       int64_t chunk = o->sample_every > 0 ? o->sample_every : 64;
       if (chunk > 256) chunk = 256;
       while (o->sample_every > 0 && o->sample_every % chunk) chunk--;  // chunk divides sample_every
-      unsigned long long* slots = ctx->dscal + 8 + 2048;
+      unsigned long long* slots = ctx->dscal + 8;
       cudaGraph_t graph = nullptr;
       cudaGraphExec_t exec = nullptr;
       int64_t graph_launches = 0;
