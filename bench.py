@@ -42,7 +42,7 @@ NCU_CAPTURES = {
     # DFMA + DADD + DMUL thread-instructions per tile pair of the assembly kernels
     "asm_fp64_inst_per_pair": {
         "cuboid": {"value": 375.4, "source": "profiles/r05_assembly_ncu_full.md", "kernel_commit": "1b6588c"},
-        "tet": {"value": 444.8, "source": "profiles/r05_assembly_ncu_full.md", "kernel_commit": "1b6588c"},
+        "tet": {"value": 479.9, "source": "profiles/r05_assembly_ncu_full.md", "kernel_commit": "60a614f"},
     },
 }
 FLOORS_NOTE = "floor = tensor bytes / measured HBM peak (MEASURED_PEAKS.json hbm_gbs)"
