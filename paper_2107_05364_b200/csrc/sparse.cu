@@ -544,12 +544,21 @@ __device__ __forceinline__ void index_load(const T* __restrict__ vals, const uin
 // beg/end: the plane row's range in vals/cols (read by the caller for all six planes up front).  The
 // next block's values and columns are requested before the current block's gathers are issued, so a
 // warp keeps two blocks of kIdxUnroll * 32 entries (2 x 1.5 KB) in flight towards HBM.
-template <typename T, int B, int P>
+// BP = 0: M is the plain staged layout [B][3][npad] (one gather per state and component: fine for 1-2 states).
+// BP = 4 / 8: M is interleaved [3][npad][BP] (interleave_stage_kernel), so that ONE gather of BP values serves
+// all states of a batch: the per-entry cost of a batch of 8 is two 32-byte loads instead of sixteen scalar ones.
+template <typename T, int BP> struct StateVec;
+template <> struct StateVec<float, 4> { float4 v[1]; };
+template <> struct StateVec<float, 8> { float4 v[2]; };
+template <> struct StateVec<double, 4> { double2 v[2]; };
+template <> struct StateVec<double, 8> { double2 v[4]; };
+
+template <typename T, int B, int P, int BP>
 __device__ __forceinline__ void index_panel(const SparseArgs& a, const uint16_t* __restrict__ cols, int64_t beg,
                                             int64_t end, int64_t col0, int lane, double (&acc)[B][3]) {
   constexpr int R = PlaneRC<P>::r, Cc = PlaneRC<P>::c;
   const T* __restrict__ vals = (const T*)a.vals;
-  const T* __restrict__ M = (const T*)a.Mst + col0;
+  const T* __restrict__ M = (const T*)a.Mst + (BP ? col0 * BP : col0);
   T vn[kIdxUnroll];
   int cn[kIdxUnroll];
   int64_t kb = beg;  // warp-uniform block start
@@ -565,13 +574,30 @@ __device__ __forceinline__ void index_panel(const SparseArgs& a, const uint16_t*
       for (int u = 0; u < kIdxUnroll; ++u) { v[u] = vn[u]; col[u] = cn[u]; }
       kb += 32 * kIdxUnroll;
       index_load<T>(vals, cols, kb + lane, end, vn, cn);
+      if constexpr (BP == 0) {
 #pragma unroll
-      for (int b = 0; b < B; ++b) {
-        const T* Mb = M + (int64_t)b * 3 * a.npad;
+        for (int b = 0; b < B; ++b) {
+          const T* Mb = M + (int64_t)b * 3 * a.npad;
+#pragma unroll
+          for (int u = 0; u < kIdxUnroll; ++u) {
+            runR[b] = fma(v[u], __ldg(Mb + (int64_t)Cc * a.npad + col[u]), runR[b]);
+            if (R != Cc) runC[b] = fma(v[u], __ldg(Mb + (int64_t)R * a.npad + col[u]), runC[b]);
+          }
+        }
+      } else {
+        typedef StateVec<T, BP> SV;
 #pragma unroll
         for (int u = 0; u < kIdxUnroll; ++u) {
-          runR[b] = fma(v[u], __ldg(Mb + (int64_t)Cc * a.npad + col[u]), runR[b]);
-          if (R != Cc) runC[b] = fma(v[u], __ldg(Mb + (int64_t)R * a.npad + col[u]), runC[b]);
+          const SV mc = *reinterpret_cast<const SV*>(M + ((int64_t)Cc * a.npad + col[u]) * BP);
+          const T* pc = reinterpret_cast<const T*>(&mc);
+#pragma unroll
+          for (int b = 0; b < B; ++b) runR[b] = fma(v[u], pc[b], runR[b]);
+          if (R != Cc) {
+            const SV mr = *reinterpret_cast<const SV*>(M + ((int64_t)R * a.npad + col[u]) * BP);
+            const T* pr = reinterpret_cast<const T*>(&mr);
+#pragma unroll
+            for (int b = 0; b < B; ++b) runC[b] = fma(v[u], pr[b], runC[b]);
+          }
         }
       }
     }
@@ -584,23 +610,33 @@ __device__ __forceinline__ void index_panel(const SparseArgs& a, const uint16_t*
 }
 
 // A plane row = its column panels in turn (PANELS = false, n <= 65,536: the one panel, nothing extra).
-template <typename T, int B, int P, bool PANELS>
+template <typename T, int B, int P, bool PANELS, int BP>
 __device__ __forceinline__ void index_plane(const SparseArgs& a, const uint16_t* __restrict__ cols, int64_t row,
                                             int64_t beg, int64_t end, int lane, double (&acc)[B][3]) {
   if (!PANELS) {
-    index_panel<T, B, P>(a, cols, beg, end, 0, lane, acc);
+    index_panel<T, B, P, BP>(a, cols, beg, end, 0, lane, acc);
     return;
   }
   const int64_t* pp = a.panel_ptr + ((int64_t)P * a.n_rows + row) * (a.npanels - 1);
   int64_t b = beg;
   for (int q = 0; q < a.npanels; ++q) {
     const int64_t e = q + 1 < a.npanels ? __ldg(pp + q) : end;
-    index_panel<T, B, P>(a, cols, b, e, (int64_t)q << 16, lane, acc);
+    index_panel<T, B, P, BP>(a, cols, b, e, (int64_t)q << 16, lane, acc);
     b = e;
   }
 }
 
-template <typename T, int B, bool PANELS>
+// M[b][c][j] (plain staged layout, MT_MAX_BATCH states) -> Mi[c][j][b], b < BP
+template <typename T, int BP>
+__global__ void __launch_bounds__(256) interleave_stage_kernel(const T* __restrict__ M, int64_t npad, T* __restrict__ Mi) {
+  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;  // (c, j)
+  if (idx >= 3 * npad) return;
+  const int64_t c = idx / npad, j = idx % npad;
+#pragma unroll
+  for (int b = 0; b < BP; ++b) Mi[idx * BP + b] = M[((int64_t)b * 3 + c) * npad + j];
+}
+
+template <typename T, int B, bool PANELS, int BP = 0>
 __global__ void __launch_bounds__(256, (B <= 2 ? 4 : 2)) demag_index_kernel(SparseArgs a, const uint16_t* __restrict__ cols, EpiArgs e) {
   const int64_t row = (int64_t)blockIdx.x * 8 + (threadIdx.x >> 5);
   const int lane = threadIdx.x & 31;
@@ -616,7 +652,7 @@ __global__ void __launch_bounds__(256, (B <= 2 ? 4 : 2)) demag_index_kernel(Spar
     nbeg = __ldg(rp + (int64_t)(P + 1) * a.n_rows);            \
     nend = __ldg(rp + (int64_t)(P + 1) * a.n_rows + 1);        \
   }                                                            \
-  index_plane<T, B, P, PANELS>(a, cols, row, beg, end, lane, acc); \
+  index_plane<T, B, P, PANELS, BP>(a, cols, row, beg, end, lane, acc); \
   beg = nbeg;                                                  \
   end = nend;
   MT_INDEX_PLANE(0)
@@ -643,11 +679,24 @@ __global__ void __launch_bounds__(256, (B <= 2 ? 4 : 2)) demag_index_kernel(Spar
 }
 
 template <typename T, int B>
-int launch_index_B(mt_ctx* ctx, const SparseArgs& a, const uint16_t* cols, const EpiArgs& e) {
+int launch_index_B(mt_ctx* ctx, const SparseArgs& a0, const uint16_t* cols, const EpiArgs& e) {
+  constexpr int BP = B <= 2 ? 0 : B <= 4 ? 4 : 8;
+  SparseArgs a = a0;
+  if constexpr (BP != 0) {
+    // batches of 3..8: the staged M re-laid out with the states innermost, once per evaluation
+    const size_t need = (size_t)3 * a.npad * BP * sizeof(T);
+    int rc = mt_ensure_ws(ctx, &ctx->Mq, &ctx->Mq_bytes, need);
+    if (rc) return rc;
+    const int64_t tot = 3 * a.npad;
+    interleave_stage_kernel<T, BP><<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>((const T*)a.Mst, a.npad, (T*)ctx->Mq);
+    ctx->launches++;
+    MT_CUDA_OK(ctx, cudaGetLastError());
+    a.Mst = ctx->Mq;
+  }
   if (a.npanels > 1)
-    demag_index_kernel<T, B, true><<<(unsigned)((a.n_rows + 7) / 8), 256, 0, ctx->stream>>>(a, cols, e);
+    demag_index_kernel<T, B, true, BP><<<(unsigned)((a.n_rows + 7) / 8), 256, 0, ctx->stream>>>(a, cols, e);
   else
-    demag_index_kernel<T, B, false><<<(unsigned)((a.n_rows + 7) / 8), 256, 0, ctx->stream>>>(a, cols, e);
+    demag_index_kernel<T, B, false, BP><<<(unsigned)((a.n_rows + 7) / 8), 256, 0, ctx->stream>>>(a, cols, e);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   return MT_OK;

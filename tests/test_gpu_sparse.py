@@ -104,7 +104,7 @@ def test_threshold_value_and_bitmap_rows_are_exact(ctx, oracle, grid, dtype):
         assert torch.equal(Hi, Hi2)
 
 
-@pytest.mark.parametrize("batch", [1, 5, 8])
+@pytest.mark.parametrize("batch", [1, 4, 5, 8])
 def test_sparse_field_batches_match_dense_path_on_truncated_tensor(ctx, oracle, batch):
     """Dense kernels on the truncated tensor and the bitmap kernel on its compressed form agree."""
     w = W.config5(20, 10, 2, batch=batch)
