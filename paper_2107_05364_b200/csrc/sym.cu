@@ -5,9 +5,12 @@
 // of the full tensor.  Bound: HBM (3 flop/B fp32), same roofline as A4.
 //
 // One CTA (8 warps) walks the tiles of a row block I and then of its mirror block nrb-1-I, so every
-// CTA streams the same number of tiles.  Inside a tile warp w owns 4W columns for all 32 rows:
-// lane l holds, for g = 0..3, the W-column vector of row 8g + l/4 of the six planes (24 x 16-byte loads
-// in flight per lane, each warp-wide load 512 contiguous bytes).
+// CTA streams the same number of tiles.  A tile is 96 KiB of CONTIGUOUS storage (sym_layout.cuh), so
+// since r05 it is fetched by three 32 KiB bulk copies (cp.async.bulk, L2 evict-first) into a two-stage
+// shared-memory ring guarded by full/empty mbarriers — the access pattern of the read-only stream
+// microbenchmark — instead of 24 x 16-byte register loads per lane.  Inside a tile warp w owns 4W columns
+// for all 32 rows: lane l reads, for g = 0..3, the W-column vector of row 8g + l/4 of the six planes (each
+// warp-wide read 512 contiguous bytes of shared memory: conflict-free).
 //   * row part:    racc[g] += N_ij M_j over the lane's W columns; summed over the tiles of the row block
 //                  in registers (fp32 runs of <= 96 terms, then fp64), reduced over the 4 lanes of a row
 //                  and the 8 warps once per row block (shared memory, fixed order);
@@ -18,6 +21,7 @@
 // The 32 x 32 diagonal block is stored whole and used for the row part only; the entries left of it
 // are zero in storage and masked here.  Results are bitwise reproducible.
 #include "epilogue.cuh"
+#include "mbar.cuh"
 #include "sym_layout.cuh"
 
 namespace {
@@ -49,22 +53,72 @@ struct SymArgs {
   void* colpart;     // [nrb][3][ncolpad] in the tensor's dtype
 };
 
+constexpr int kSymStages = 2;
+constexpr uint32_t kSymTileBytes = 6u * 32u * 32u * 16u;  // 98,304 for both dtypes (TW = 32 W, W = 16 / sizeof(T))
+constexpr size_t kSymSmemBytes = (size_t)kSymStages * kSymTileBytes + 2 * kSymStages * sizeof(uint64_t) + 128;
+
 template <typename T>
 __global__ void __launch_bounds__(256, 1) sym_field_kernel(SymArgs a) {
   typedef SymCfg<T> Cfg;
   typedef typename SymVec<T>::type V;
   constexpr int W = Cfg::W, TW = Cfg::TW;
   constexpr int kFlushTiles = 96 / (3 * W);  // fp32: 8 tiles of 12 terms per accumulator
+  static_assert(Cfg::kTileElems * sizeof(T) == kSymTileBytes, "tile size");
   __shared__ double red[8][32][3];
+  extern __shared__ __align__(128) unsigned char sym_smem_raw[];
+  unsigned char* ring = sym_smem_raw + ((128u - (smem_u32(sym_smem_raw) & 127u)) & 127u);
+  uint64_t* bars = (uint64_t*)(ring + (size_t)kSymStages * kSymTileBytes);
+  const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + kSymStages);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int rl = lane >> 2, cq = lane & 3;  // row-lane (0..7), column quad (0..3)
   const T* M = (const T*)a.Mst;
   T* colpart = (T*)a.colpart;
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < kSymStages; ++s) {
+      mbar_init(full0 + 8 * s, 1);
+      mbar_init(empty0 + 8 * s, 8);
+    }
+    mbar_fence_init();
+  }
+  __syncthreads();
+  // the CTA's tile sequence: all tiles of row block I0 = blockIdx.x, then all of its mirror block I1
+  const int64_t I0 = blockIdx.x, I1 = a.nrb - 1 - (int64_t)blockIdx.x;
+  const int64_t cnt0 = a.ntc - (32 * I0) / TW;
+  const int64_t cnt1 = I1 > I0 ? a.ntc - (32 * I1) / TW : 0;
+  const int64_t start0 = sym_tile_prefix(I0, a.ntc, Cfg::kBlocksPerTile);
+  const int64_t start1 = cnt1 ? sym_tile_prefix(I1, a.ntc, Cfg::kBlocksPerTile) : 0;
+  const int64_t total = cnt0 + cnt1;
+  // producer (thread 0): tops the ring up before each of its own tiles, as in demag_tma.cu
+  const bool is_producer = threadIdx.x == 0;
+  uint64_t policy = 0;
+  if (is_producer) policy = l2_policy_evict_first();
+  int64_t p_q = 0;
+  int p_stage = 0;
+  uint32_t p_phase = 0;
+  auto top_up = [&](int64_t must) {
+    while (p_q < total) {
+      if (!mbar_test(empty0 + 8 * p_stage, p_phase ^ 1)) {
+        if (p_q > must) break;
+        mbar_wait(empty0 + 8 * p_stage, p_phase ^ 1);
+      }
+      const int64_t tile = p_q < cnt0 ? start0 + p_q : start1 + (p_q - cnt0);
+      const unsigned char* src = (const unsigned char*)a.data + tile * (int64_t)kSymTileBytes;
+      const uint32_t dst = smem_u32(ring + (size_t)p_stage * kSymTileBytes);
+      mbar_expect_tx(full0 + 8 * p_stage, kSymTileBytes);
+#pragma unroll
+      for (int c = 0; c < 3; ++c)
+        bulk_load_1d(dst + c * (kSymTileBytes / 3), src + c * (kSymTileBytes / 3), kSymTileBytes / 3, full0 + 8 * p_stage, policy);
+      if (++p_stage == kSymStages) { p_stage = 0; p_phase ^= 1; }
+      ++p_q;
+    }
+  };
+  int stage = 0;
+  uint32_t phase = 0;
+  int64_t q = 0;
   for (int pass = 0; pass < 2; ++pass) {
-    const int64_t I = pass == 0 ? (int64_t)blockIdx.x : a.nrb - 1 - (int64_t)blockIdx.x;
-    if (pass == 1 && I <= (int64_t)blockIdx.x) break;  // odd count: the middle block was done in pass 0
+    const int64_t I = pass == 0 ? I0 : I1;
+    if (pass == 1 && cnt1 == 0) break;  // odd count: the middle block was done in pass 0
     const int64_t Jd = (32 * I) / TW;
-    const int64_t tile0 = sym_tile_prefix(I, a.ntc, Cfg::kBlocksPerTile);
     T Mi[4][3];
 #pragma unroll
     for (int g = 0; g < 4; ++g)
@@ -77,13 +131,19 @@ __global__ void __launch_bounds__(256, 1) sym_field_kernel(SymArgs a) {
 #pragma unroll
       for (int c = 0; c < 3; ++c) { racc[g][c] = 0.0; rrun[g][c] = T(0); }
     int since = 0;
-    for (int64_t J = Jd; J < a.ntc; ++J) {
-      const V* tp = (const V*)((const T*)a.data + (tile0 + (J - Jd)) * Cfg::kTileElems) + warp * 32 + lane;
+    for (int64_t J = Jd; J < a.ntc; ++J, ++q) {
+      if (is_producer) top_up(q);
+      __syncwarp();
+      mbar_wait(full0 + 8 * stage, phase);
+      const V* tp = (const V*)(ring + (size_t)stage * kSymTileBytes) + warp * 32 + lane;
       V v[6][4];
 #pragma unroll
       for (int p = 0; p < 6; ++p)
 #pragma unroll
-        for (int g = 0; g < 4; ++g) v[p][g] = ld_stream(tp + (p * 4 + g) * 256);
+        for (int g = 0; g < 4; ++g) v[p][g] = tp[(p * 4 + g) * 256];
+      __syncwarp();
+      if (lane == 0) mbar_arrive(empty0 + 8 * stage);  // the tile is in registers: hand the stage back
+      if (++stage == kSymStages) { stage = 0; phase ^= 1; }
       const int64_t j0 = J * TW + warp * 4 * W + cq * W;
       const int64_t jb = j0 >> 5;
       const bool use_row = jb >= I, use_col = jb > I;
@@ -194,9 +254,14 @@ int launch_sym_T(mt_ctx* ctx, const mt_sym_tensor* S, const void* Mst, int64_t n
   a.rowpart = (double*)ctx->sym_ws;
   a.colpart = (char*)ctx->sym_ws + row_bytes;
   const unsigned grid = (unsigned)((a.nrb + 1) / 2);
+  static unsigned char attr_set[64] = {};  // per device ordinal (the attribute is per device)
+  if (!attr_set[ctx->device & 63]) {
+    MT_CUDA_OK(ctx, cudaFuncSetAttribute(sym_field_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSymSmemBytes));
+    attr_set[ctx->device & 63] = 1;
+  }
   for (int b = 0; b < e.batch; ++b) {  // states one after the other: each streams the half once
     a.Mst = (const T*)Mst + (int64_t)b * 3 * npad;
-    sym_field_kernel<T><<<grid, 256, 0, ctx->stream>>>(a);
+    sym_field_kernel<T><<<grid, 256, kSymSmemBytes, ctx->stream>>>(a);
     ctx->launches++;
     MT_CUDA_OK(ctx, cudaGetLastError());
     sym_finish_kernel<T><<<(unsigned)((S->n + 255) / 256), 256, 0, ctx->stream>>>(a, b, e);
