@@ -58,16 +58,15 @@ __device__ __forceinline__ double log_ratio_fast(double a, double b) {
 
 // sqrt(x) for positive normal x without the library's special-case branch (whose convergence barriers
 // keep the compiler from interleaving the eight independent square roots of a pair): 64-bit MUFU seed
-// of 1/sqrt(x) (20 bits), two coupled Goldschmidt steps (g -> sqrt(x), h -> 1/(2 sqrt(x))), one residual
-// correction: <= 1 ulp.  x = 0 gives NaN (inf * 0): a target on a source corner is singular anyway.
+// of 1/sqrt(x) (20 bits), ONE coupled Goldschmidt step (g -> sqrt(x), h -> 1/(2 sqrt(x)): 40 bits) and one
+// residual correction g += (x - g^2) h, which squares the error once more: <= 1 ulp (checked against long
+// double on 2e6 arguments with seed errors up to 2^-20: worst 0.999 x 2^-53 relative).  x = 0 gives NaN
+// (inf * 0): a target on a source corner is singular anyway.
 __device__ __forceinline__ double sqrt_pos(double x) {
   double y;
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   double g = x * y, h = 0.5 * y;
-  double e = fma(-h, g, 0.5);
-  g = fma(g, e, g);
-  h = fma(h, e, h);
-  e = fma(-h, g, 0.5);
+  const double e = fma(-h, g, 0.5);
   g = fma(g, e, g);
   h = fma(h, e, h);
   return fma(fma(-g, g, x), h, g);
