@@ -41,8 +41,8 @@ NCU_CAPTURES = {
     },
     # DFMA + DADD + DMUL thread-instructions per tile pair of the assembly kernels
     "asm_fp64_inst_per_pair": {
-        "cuboid": {"value": 375.4, "source": "profiles/r05_assembly_ncu_full.md", "kernel_commit": "1b6588c"},
-        "tet": {"value": 479.9, "source": "profiles/r05_assembly_ncu_full.md", "kernel_commit": "60a614f"},
+        "cuboid": {"value": 351.2, "source": "profiles/r05_assembly_ncu_full.md (r05d)", "kernel_commit": "0994392"},
+        "tet": {"value": 467.7, "source": "profiles/r05_assembly_ncu_full.md (r05d)", "kernel_commit": "0994392"},
     },
 }
 FLOORS_NOTE = "floor = tensor bytes / measured HBM peak (MEASURED_PEAKS.json hbm_gbs)"
