@@ -320,6 +320,42 @@ def test_index_rows_beyond_65536_columns(ctx, oracle):
         assert H.rel_l2(Hi[b].cpu().numpy(), ref[b]) <= 1e-5
 
 
+def test_stream_calls_tau_given_and_argument_errors(ctx):
+    """mt_sparse_stream_count / _fill (the streamed build as two library calls): a threshold handed in
+    (fraction < 0) skips the selection and reproduces the selected build; bad arguments come back as
+    MT_ERR_INVALID_ARG with a message, nothing is launched."""
+    import ctypes as C
+    w = W.config5(9, 6, 2, batch=1)
+    tiles = H.dev_tiles(w)
+    A = B.mt_sparse_build_streamed(ctx, tiles, B.MT_F32, 0.6, 32)
+    G = B.mt_sparse_build_streamed(ctx, tiles, B.MT_F32, 0.0, 50, tau=A.tau)
+    torch.cuda.synchronize()
+    assert G.tau == A.tau and G.nnz == A.nnz and torch.equal(G.row_ptr, A.row_ptr)
+    assert torch.equal(G.mask, A.mask) and torch.equal(G.vals, A.vals)
+    n = w.n
+    ld = W.leading_dim(n, "f32")
+    band = torch.empty(6 * 16 * ld, dtype=torch.float32, device="cuda")
+    row_ptr = torch.empty(6 * n + 1, dtype=torch.int64, device="cuda")
+    t = tiles._c()
+    tau, nnz = C.c_double(0.0), C.c_int64(0)
+
+    def count(fraction, r0, r1, band_rows, band_ptr=band.data_ptr(), rp=row_ptr.data_ptr()):
+        return ctx.lib.mt_sparse_stream_count(ctx.h, C.byref(t), B.MT_F32, fraction, r0, r1, band_ptr, band_rows, ld, rp,
+                                              None, B.ALLREDUCE_FN(), None, None, C.byref(tau), C.byref(nnz))
+
+    l0 = ctx.launches
+    assert count(1.5, 0, n, 16) == B.MT_ERR_INVALID_ARG and b"fraction" in ctx.lib.mt_last_error(ctx.h)
+    assert count(0.5, 5, 5, 16) == B.MT_ERR_INVALID_ARG        # empty band
+    assert count(0.5, 0, n + 1, 16) == B.MT_ERR_INVALID_ARG    # beyond the tiles
+    assert count(0.5, 0, n, 0) == B.MT_ERR_INVALID_ARG         # no band rows
+    assert count(0.5, 0, n, 16, band_ptr=None) == B.MT_ERR_INVALID_ARG
+    assert count(0.5, 0, n, 16, rp=None) == B.MT_ERR_INVALID_ARG
+    assert ctx.lib.mt_sparse_stream_fill(ctx.h, C.byref(t), B.MT_F32, 0.1, 0, n, band.data_ptr(), 16, ld, row_ptr.data_ptr(),
+                                         None, None, None, None, None) == B.MT_ERR_INVALID_ARG   # no output arrays
+    assert ctx.launches == l0
+    assert count(0.6, 0, n, 16) == B.MT_OK and tau.value == A.tau and nnz.value == A.nnz
+
+
 def test_streamed_thresholding_row_sharded_with_histogram_allreduce(ctx, oracle):
     """DESIGN.md section 9 on F1: two "ranks" (threads with their own mt_ctx and stream on this one GPU)
     each build the thresholded rows of their half, exchanging only the selection histogram after every
