@@ -197,6 +197,34 @@ def test_sharded_rk4_tma_bands_fp32():
         assert np.max(np.abs(np.linalg.norm(m[0], axis=0) - 1.0)) < 1e-14
 
 
+def test_sharded_rk4_on_a_row_sharded_thresholded_tensor():
+    """The thresholded tensor (F1) shards by rows like the dense one: every rank compresses its band with the
+    whole tensor's threshold (index rows) and runs the sharded RK4 on it; the result equals the single-context
+    run on the whole thresholded tensor."""
+    w = W.config3(8, batch=1)
+    kw = dict(method=B.MT_RK4, dt=2e-3, t_end=0.04)
+
+    def with_sparse(ctx, prob, rank, tau_box=[None]):
+        n = w.n
+        rows = prob.N.shape[1]
+        if tau_box[0] is None:          # the single-context call comes first and fixes the threshold
+            tau_box[0], _ = B.mt_threshold_value(ctx, prob.N, B.MT_F64, n, rows, prob.ld, 0.5)
+        S = B.mt_sparse_build(ctx, prob.N, B.MT_F64, n, rows, prob.ld, tau_box[0])
+        B.mt_sparse_index(ctx, S, drop_mask=True)
+        prob.N_sparse, prob.N = S, None
+        return integrate_fn(w, 1, **kw)(ctx, prob, rank)
+
+    m1, _, r1, _ = run_single(w, "f64", with_sparse)
+    outs, xch = run_sharded(2, w, "f64", with_sparse)
+    for m, _, r, _ in outs:
+        assert r["accepted"] == 20
+        assert np.max(np.abs(m - m1)) < 1e-12
+    assert np.array_equal(outs[0][0], outs[1][0]) and xch.calls[S.GATHER_STATE] == 80
+    # and thresholding did change the dynamics a little (the test is not run on an untouched tensor)
+    m0, _, _, _ = run_single(w, "f64", integrate_fn(w, 1, **kw))
+    assert 1e-9 < np.max(np.abs(m0 - m1)) < 1e-2
+
+
 def test_sharded_argument_errors():
     w = W.config3(4)
     ctx = B.mt_create(0)
