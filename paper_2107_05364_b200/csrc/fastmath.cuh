@@ -72,6 +72,17 @@ __device__ __forceinline__ double sqrt_pos(double x) {
   return fma(fma(-g, g, x), h, g);
 }
 
+// 1/sqrt(x) to ~1e-12 relative for positive normal x: 64-bit MUFU seed (20 bits) + one Goldschmidt step
+// (40 bits), branch-free.  For the far-field quadrature (F2), whose own truncation error is of that size
+// and whose terms do not cancel; NOT for the closed forms.
+__device__ __forceinline__ double rsqrt_pos_40(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double h = 0.5 * y;
+  const double e = fma(-h, x * y, 0.5);
+  return fma(y, e, y);
+}
+
 // Several small-argument evaluations at once: r[k] = atan(n[k]/d[k]) for k < NA, atanh(n[k]/d[k]) for
 // NA <= k < NA + NH (atan's series is atanh's at -t^2, so all share the coefficients and run as
 // independent chains the compiler can interleave).  Requires |n[k]| <= d[k]/8, d[k] > 0.
