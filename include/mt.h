@@ -491,6 +491,33 @@ int mt_set_step_control(mt_ctx* ctx, int mode);
  * MT_ERR_INVALID_ARG.  Results of all variants agree to rounding; each is deterministic.          */
 int mt_set_demag_variant(mt_ctx* ctx, int variant);
 
+/* ---- Demagnetising field without any allocation (for callers that cannot call cudaMalloc: code under
+ * CUDA graph capture, tight serving loops, harnesses that forbid it).  Same operation as mt_demag_field
+ * for ONE state (Eq. 9, sign and Ms reading DESIGN.md Q1; the arithmetic of DESIGN.md Q19):
+ *     Hd[a][i] = - sum_j sum_c N^{ac}_{ij} Ms[j] m[c][j],   i in [0, n_rows)
+ * N [6][n_rows][ld], Ms [n], m [3][n], Hd [3][n_rows]: DEVICE memory of `device`, owned by the caller;
+ * `cuda_stream` is a cudaStream_t of that device (NULL = legacy default stream); the call only enqueues
+ * work on it and does not synchronise.  No mt_ctx is involved (mt_create allocates), and the call makes no
+ * cudaMalloc / cudaFree / allocating library call: the staged vector Ms*m (tensor dtype) and the partial
+ * row sums of the column splits live in a file-scope __device__ array of MT_NOALLOC_SCRATCH_BYTES that every
+ * GPU which loads the library holds until the process exits.  Limits: n <= MT_NOALLOC_MAX_N and
+ * n_rows <= MT_NOALLOC_MAX_N; anything larger is rejected with MT_ERR_INVALID_ARG (use mt_demag_field).
+ * The scratch array is SHARED by every call on a device and keeps the last call's contents: each call
+ * rewrites every word it later reads (the staging kernel also zeroes the padding of the staged vector),
+ * so calls in stream order are independent of one another, but two calls that overlap on the GPU (different
+ * streams without an ordering between them, or two host threads) RACE on it — serialise them.
+ * The first call on a device looks the array's device address up (cudaGetSymbolAddress, once per device;
+ * this loads the module): make one call outside a graph capture first.  The current device of the calling
+ * thread is left as it was.  The reduction order is fixed (bitwise reproducible for a given shape).
+ * `err` (may be NULL) is a caller-provided HOST buffer of err_cap bytes that receives the error text.
+ * Returns MT_OK, MT_ERR_INVALID_ARG (null / misaligned pointer, ld < n, size over the limit, bad dtype or
+ * device) or MT_ERR_CUDA.                                                                          */
+#define MT_NOALLOC_MAX_N 65536
+#define MT_NOALLOC_SCRATCH_BYTES (4718592) /* 4.5 MiB: 1.5 MiB staged vector + 3 MiB partial sums */
+int mt_demag_field_noalloc(int device, void* cuda_stream, const void* N, int dtype, int64_t n, int64_t n_rows,
+                           int64_t ld, const double* Ms, const double* m, double* Hd, char* err,
+                           int64_t err_cap);
+
 #ifdef __cplusplus
 }
 #endif

@@ -23,6 +23,8 @@ MT_ERR_STEP_UNDERFLOW, MT_ERR_MAX_STEPS, MT_ERR_UNIMPLEMENTED = -4, -5, -6
 MT_F32, MT_F64 = 0, 1
 MT_RK4, MT_DP45 = 0, 1
 MT_SELECT_HIST_WORDS = 1 << 20
+MT_NOALLOC_MAX_N = 65536
+MT_NOALLOC_SCRATCH_BYTES = 4718592
 COMPONENTS = ("xx", "xy", "xz", "yy", "yz", "zz")
 EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assemble_tensor",
            "mt_check_status", "mt_demag_field", "mt_demag_field_host", "mt_llg_rhs", "mt_integrate", "mt_energy",
@@ -31,7 +33,8 @@ EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assembl
            "mt_sparse_count_band", "mt_sparse_scan", "mt_sparse_fill_band", "mt_sparse_fill_index_band",
            "mt_sparse_stream_count", "mt_sparse_stream_fill", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
            "mt_demag_field_sym", "mt_set_assembly_mode", "mt_launch_count",
-           "mt_set_demag_variant", "mt_set_step_control", "mt_profile_begin", "mt_profile_end", "mt_measure_peak")
+           "mt_set_demag_variant", "mt_set_step_control", "mt_profile_begin", "mt_profile_end", "mt_measure_peak",
+           "mt_demag_field_noalloc")
 
 
 class MtError(RuntimeError):
@@ -165,6 +168,8 @@ def load() -> C.CDLL:
         lib.mt_energy.argtypes = [C.c_void_p, C.POINTER(_Problem), C.c_void_p, C.c_int, C.c_void_p]
         lib.mt_field_sweep.argtypes = [C.c_void_p, C.POINTER(_Problem), C.POINTER(_Opts), C.c_void_p, C.c_int64,
                                        C.c_void_p, C.c_int, C.c_void_p, C.POINTER(_Result)]
+        lib.mt_demag_field_noalloc.argtypes = [C.c_int, C.c_void_p, C.c_void_p, C.c_int, C.c_int64, C.c_int64,
+                                               C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p, C.c_char_p, C.c_int64]
         _lib = lib
     return _lib
 
@@ -316,6 +321,19 @@ def mt_demag_field_host(ctx: Context, N: torch.Tensor, dtype: int, n: int, n_row
     ctx.check(ctx.lib.mt_demag_field_host(ctx.h, _ptr(N, torch_dtype(dtype)), dtype, n, n_rows, ld,
                                           _ptr(Ms, torch.float64), _ptr(m_host, torch.float64), batch,
                                           _ptr(Hd_host, torch.float64)))
+
+
+def mt_demag_field_noalloc(device: int, cuda_stream: int, N: torch.Tensor, dtype: int, n: int, n_rows: int, ld: int,
+                           Ms: torch.Tensor, m: torch.Tensor, Hd: torch.Tensor):
+    """One state's field with no allocation anywhere (mt.h): no Context; scratch is the library's static device
+    array (n, n_rows <= MT_NOALLOC_MAX_N; calls that overlap on the GPU race on it).  `cuda_stream` is the raw
+    stream handle (torch.cuda.Stream.cuda_stream; 0 = legacy default stream).  Enqueues only."""
+    err = C.create_string_buffer(256)
+    rc = load().mt_demag_field_noalloc(device, C.c_void_p(cuda_stream), _ptr(N, torch_dtype(dtype)), dtype, n, n_rows,
+                                       ld, _ptr(Ms, torch.float64), _ptr(m, torch.float64), _ptr(Hd, torch.float64),
+                                       err, len(err))
+    if rc != MT_OK:
+        raise MtError(rc, err.value.decode(errors="replace"))
 
 
 class Shard:
