@@ -199,6 +199,7 @@ int mt_destroy(mt_ctx* c) {
   cudaFree(c->Mst[0]);
   cudaFree(c->Mst[1]);
   cudaFree(c->partial);
+  cudaFree(c->split_count);
   cudaFree(c->Mq);
   cudaFree(c->rk);
   cudaFree(c->edens);

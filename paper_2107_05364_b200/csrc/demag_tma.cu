@@ -21,8 +21,10 @@
 // on fp32 tensors use `demag_tma_f32x2_kernel` below (packed FFMA2, the only way to the full FP32
 // rate on sm_100a: a three-register FFMA issues every other cycle per scheduler).  Lanes are combined
 // with a fixed xor butterfly; a group finished inside one CTA goes straight to the fused epilogue
-// (epilogue.cuh); a group split between CTAs leaves per-CTA partial sums that a small second kernel
-// adds in CTA order — no atomics, bitwise reproducible for a given (n, n_rows, #SMs).
+// (epilogue.cuh); a group split between CTAs leaves per-CTA partial sums, and the CTA that completes the
+// group's chunk count adds them in CTA order and runs the epilogue (finish_split_group: nobody waits, the
+// order of the sum does not depend on who arrives last) — bitwise reproducible for a given (n, n_rows,
+// #SMs), in ONE launch (a second, fix-up launch cost 5-10 us per call: r06, problems of 1,000-8,000 tiles).
 #include <cuda.h>
 #include <string.h>
 
@@ -93,10 +95,64 @@ struct TmaArgs {
   int64_t tiles;    // groups * chunks
   double* partial;  // [P][2][RT][B][3]
   double* exch;     // tensor-core kernel: [P][MmaCfg::exch_doubles] column parts of a row block
+  int* count;       // [groups] chunks of a split row group summed so far; zero between launches
 };
 
+// first tile of CTA c: floor(tiles * c / P), c in [0, P]
 __host__ __device__ __forceinline__ int64_t range_begin(int64_t tiles, int64_t P, int64_t c) {
+  if (tiles < (int64_t(1) << 40) && P < (int64_t(1) << 20))  // every real shape: one 64-bit division
+    return (int64_t)((uint64_t)tiles * (uint64_t)c / (uint64_t)P);
   return (int64_t)(((unsigned __int128)tiles * (unsigned __int128)c) / (unsigned __int128)P);
+}
+
+// A row group split between CTAs.  Every CTA that covers part of it has left its partial sums in
+// a.partial (slot 0: the group its range starts in, slot 1: the group its range ends in) and now adds
+// the number of chunks it covered to the group's counter; the CTA whose addition completes the count
+// adds the parts in CTA order — the order is fixed whichever CTA arrives last: bitwise reproducible —
+// runs the epilogue and puts the counter back to zero for the next launch.  Nobody waits for anybody.
+// Called by ALL threads of the CTA after their partial stores; `sh` = 3 ints of shared memory.
+template <int RT>
+__device__ __forceinline__ void finish_split_group(const TmaArgs& a, int64_t P, int64_t c, const EpiArgs& e, int B,
+                                                   int64_t g, int mine, volatile int* sh) {
+  __threadfence();  // this thread's partial sums are visible device-wide before the count moves
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const int last = (atomicAdd(a.count + g, mine) + mine == (int)a.chunks) ? 1 : 0;
+    if (last) {
+      a.count[g] = 0;  // nobody else touches this word any more in this launch
+      const int64_t tb = g * a.chunks, te = tb + a.chunks;
+      int64_t lo = c, hi = c;
+      while (lo > 0 && range_begin(a.tiles, P, lo) > tb) --lo;
+      while (hi + 1 < P && range_begin(a.tiles, P, hi + 1) < te) ++hi;
+      sh[1] = (int)lo;
+      sh[2] = (int)hi;
+    }
+    sh[0] = last;
+  }
+  __syncthreads();
+  if (!sh[0]) return;
+  __threadfence();
+  const int lo = sh[1], hi = sh[2];
+  for (int idx = threadIdx.x; idx < RT * B; idx += blockDim.x) {
+    const int rg = idx / B, b = idx - rg * B;
+    const int64_t row = g * RT + rg;
+    if (row >= a.n_rows) continue;
+    double s[3] = {0.0, 0.0, 0.0};
+    int64_t cb = range_begin(a.tiles, P, lo);
+    for (int cc = lo; cc <= hi; ++cc) {
+      const int64_t ce = range_begin(a.tiles, P, cc + 1);
+      if (cb < ce) {
+        const int slot = (cb / a.chunks == g) ? 0 : 1;
+        const double* p = a.partial + ((((int64_t)cc * 2 + slot) * RT + rg) * B + b) * 3;
+        s[0] += __ldcg(p);  // written by other SMs in this launch: read from L2
+        s[1] += __ldcg(p + 1);
+        s[2] += __ldcg(p + 2);
+      }
+      cb = ce;
+    }
+    const double hd[3] = {-s[0], -s[1], -s[2]};
+    row_epilogue(e, row, b, hd);
+  }
 }
 
 template <typename T, int B, int RW, int CT_, int STAGES, int WARPS_ = kConsumerWarps>
@@ -109,7 +165,7 @@ struct TmaCfg {
   static constexpr size_t tensor_bytes = (size_t)6 * RT * CT * sizeof(T);
   static constexpr size_t m_bytes = (size_t)3 * B * CT * sizeof(T);
   static constexpr size_t stage_bytes = tensor_bytes + m_bytes;
-  static constexpr size_t smem_bytes = STAGES * stage_bytes + 2 * STAGES * sizeof(uint64_t) + 128;
+  static constexpr size_t smem_bytes = STAGES * stage_bytes + 2 * STAGES * sizeof(uint64_t) + 16 + 128;  // ring, barriers, finish_split_group's words, alignment slack
   static_assert(CT % 64 == 0, "tile width must be a whole number of warp-wide 8-byte vectors");
   static_assert(tensor_bytes % 128 == 0 && m_bytes % 128 == 0, "TMA destinations must stay 128-byte aligned");
 };
@@ -131,6 +187,7 @@ __global__ void __launch_bounds__(kThreads, 1)
   // gains 2.7 % at B = 8 from it)
   unsigned char* smem = (unsigned char*)(((uintptr_t)smem_raw + 127) & ~(uintptr_t)127);
   uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::stage_bytes);
+  volatile int* fin = (volatile int*)(bars + 2 * STAGES);  // finish_split_group's three words
   const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t P = gridDim.x, c = blockIdx.x;
@@ -278,6 +335,7 @@ __global__ void __launch_bounds__(kThreads, 1)
           }
         }
       }
+      if (!whole) finish_split_group<RT>(a, P, c, e, B, g, (int)(t + 1 - max(t0, g * a.chunks)), fin);
 #pragma unroll
       for (int r = 0; r < RW; ++r)
 #pragma unroll
@@ -288,7 +346,7 @@ __global__ void __launch_bounds__(kThreads, 1)
 }
 
 // ---- fp32 tensors, batches of 5..8 states: packed-FMA consumer -------------------------------------
-// Same ring, same work split, same fix-up as above; what differs is the arithmetic of a tile.  At
+// Same ring, same work split, same finish of split groups as above; what differs is the arithmetic of a tile.  At
 // B = 8 a tile block (24 B) carries 72 FMAs: at the HBM rate that is 67 FMA/clk/SM, above what
 // three-register FFMA sustains (64/clk/SM), so the products are issued as FFMA2 (fma.rn.f32x2): the
 // two halves of a 64-bit register pair are two adjacent source columns, so an LDS.128 of a plane row
@@ -333,6 +391,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1)
   // instead of generic LD (which queue behind the global-memory path: r02 ncu, lg_throttle stalls)
   unsigned char* smem = smem_raw + ((128u - (smem_u32(smem_raw) & 127u)) & 127u);
   uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::stage_bytes);
+  volatile int* fin = (volatile int*)(bars + 2 * STAGES);  // finish_split_group's three words
   const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t P = gridDim.x, c = blockIdx.x;
@@ -481,6 +540,8 @@ __global__ void __launch_bounds__(WARPS * 32, 1)
           p[0] = acc[0]; p[1] = acc[1]; p[2] = acc[2];
         }
       }
+      if (!(head_in_range && group_done))
+        finish_split_group<RT>(a, P, c, e, e.batch, g, (int)(t + 1 - max(t0, g * a.chunks)), fin);
       acc[0] = acc[1] = acc[2] = 0.0;
     }
     if (group_done) { k = 0; ++g; head_in_range = true; } else { ++k; }
@@ -541,7 +602,7 @@ struct MmaCfg {
   // column parts of a row block meet in a per-CTA global scratch at the end of a row group (rare: once per
   // 64 rows x n columns), not in shared memory: the ring may use all of it
   static constexpr size_t exch_doubles = (size_t)(kMmaKS - 1) * 12 * 4 * 32;
-  static constexpr size_t smem_bytes = kMmaStages * stage_bytes + 2 * kMmaStages * sizeof(uint64_t) + 1024;
+  static constexpr size_t smem_bytes = kMmaStages * stage_bytes + 2 * kMmaStages * sizeof(uint64_t) + 16 + 1024;
   static_assert(stage_bytes % 1024 == 0, "swizzled tiles must start on 1 KB boundaries");
 };
 
@@ -577,6 +638,7 @@ __global__ void __launch_bounds__(kMmaWarps * 32, 1)
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   uint64_t* bars = (uint64_t*)(smem + STAGES * Cfg::stage_bytes);
+  volatile int* fin = (volatile int*)(bars + 2 * STAGES);  // finish_split_group's three words
   const uint32_t full0 = smem_u32(bars), empty0 = smem_u32(bars + STAGES);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int64_t P = gridDim.x, c = blockIdx.x;
@@ -745,6 +807,8 @@ __global__ void __launch_bounds__(kMmaWarps * 32, 1)
         }
       }
       __syncthreads();
+      if (!(head_in_range && group_done))
+        finish_split_group<RT>(a, P, c, e, e.batch, g, (int)(t + 1 - max(t0, g * a.chunks)), fin);
 #pragma unroll
       for (int cc = 0; cc < 3; ++cc)
 #pragma unroll
@@ -752,37 +816,6 @@ __global__ void __launch_bounds__(kMmaWarps * 32, 1)
     }
     if (group_done) { k = 0; ++g; head_in_range = true; } else { ++k; }
   }
-}
-
-// second pass: groups that were split between CTAs — add the per-CTA partial sums in CTA order
-template <int RT>
-__global__ void __launch_bounds__(256) demag_tma_fixup_kernel(TmaArgs a, int64_t P, int B, EpiArgs e) {
-  const int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= a.n_rows * B) return;
-  const int b = (int)(idx / a.n_rows);
-  const int64_t row = idx % a.n_rows;
-  const int64_t g = row / RT;
-  const int rg = (int)(row % RT);
-  const int64_t tb = g * a.chunks, te = tb + a.chunks;  // tiles of this group
-  // CTA that owns tile t: the c with begin(c) <= t < begin(c+1)
-  auto owner = [&](int64_t t) {
-    int64_t c = (int64_t)(((unsigned __int128)t * (unsigned __int128)P) / (unsigned __int128)a.tiles);
-    while (c + 1 < P && range_begin(a.tiles, P, c + 1) <= t) ++c;
-    while (c > 0 && range_begin(a.tiles, P, c) > t) --c;
-    return c;
-  };
-  const int64_t c_lo = owner(tb), c_hi = owner(te - 1);
-  if (c_lo == c_hi) return;  // finished inside one CTA: epilogue already done there
-  double s[3] = {0.0, 0.0, 0.0};
-  for (int64_t c = c_lo; c <= c_hi; ++c) {
-    const int64_t cb = range_begin(a.tiles, P, c), ce = range_begin(a.tiles, P, c + 1);
-    if (cb >= ce) continue;
-    const int slot = (cb / a.chunks == g) ? 0 : 1;
-    const double* p = a.partial + ((((int64_t)c * 2 + slot) * RT + rg) * B + b) * 3;
-    s[0] += p[0]; s[1] += p[1]; s[2] += p[2];
-  }
-  const double hd[3] = {-s[0], -s[1], -s[2]};
-  row_epilogue(e, row, b, hd);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -833,6 +866,16 @@ int make_map(mt_ctx* ctx, CUtensorMap* out, int dtype, const void* base, int ran
   return MT_OK;
 }
 
+// the split-group counters (finish_split_group): zeroed when allocated, left at zero by every launch
+int ensure_count(mt_ctx* ctx, int64_t groups) {
+  const size_t need = (size_t)(groups > 16384 ? groups : 16384) * sizeof(int);
+  if (ctx->split_count && ctx->split_count_bytes >= need) return MT_OK;
+  int rc = mt_ensure_ws(ctx, (void**)&ctx->split_count, &ctx->split_count_bytes, need);
+  if (rc) return rc;
+  MT_CUDA_OK(ctx, cudaMemsetAsync(ctx->split_count, 0, need, ctx->stream));
+  return MT_OK;
+}
+
 // Cfg = tile geometry; kern = the kernel instantiated for it; m_rows = rows of the staged-M box (3 B)
 template <typename T, typename Cfg, typename Kern>
 int launch_tiles(mt_ctx* ctx, Kern kern, unsigned char* attr_set, int m_rows, const void* N, int dtype, int64_t n,
@@ -850,6 +893,8 @@ int launch_tiles(mt_ctx* ctx, Kern kern, unsigned char* attr_set, int m_rows, co
   if (rc) return rc;
   a.partial = ctx->partial;
   a.exch = nullptr;
+  if ((rc = ensure_count(ctx, a.groups))) return rc;
+  a.count = ctx->split_count;
   alignas(64) CUtensorMap tmN, tmM;
   {
     const uint64_t dims[3] = {(uint64_t)n, (uint64_t)n_rows, 6};
@@ -872,10 +917,6 @@ int launch_tiles(mt_ctx* ctx, Kern kern, unsigned char* attr_set, int m_rows, co
     attr_set[dev] = 1;
   }
   kern<<<(unsigned)P, Cfg::WARPS * 32, Cfg::smem_bytes, ctx->stream>>>(tmN, tmM, a, e);
-  ctx->launches++;
-  MT_CUDA_OK(ctx, cudaGetLastError());
-  const int64_t tot = n_rows * e.batch;
-  demag_tma_fixup_kernel<RT><<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(a, P, e.batch, e);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   return MT_OK;
@@ -918,6 +959,8 @@ int launch_mma(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld
   if (rc) return rc;
   a.partial = ctx->partial;
   a.exch = ctx->partial + partial_doubles;
+  if ((rc = ensure_count(ctx, a.groups))) return rc;
+  a.count = ctx->split_count;
   // M re-laid out for the B fragments: hi/lo split, [3][npad/8][8 states][4][4] fp32
   const size_t mq_bytes = (size_t)3 * (npad / 8) * 32 * sizeof(float4);
   if ((rc = mt_ensure_ws(ctx, &ctx->Mq, &ctx->Mq_bytes, mq_bytes))) return rc;
@@ -948,10 +991,6 @@ int launch_mma(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld
     attr_set[dev] = 1;
   }
   demag_tma_mma_kernel<<<(unsigned)P, Cfg::WARPS * 32, Cfg::smem_bytes, ctx->stream>>>(tmN, tmM, a, e);
-  ctx->launches++;
-  MT_CUDA_OK(ctx, cudaGetLastError());
-  const int64_t tot = n_rows * e.batch;
-  demag_tma_fixup_kernel<RT><<<(unsigned)((tot + 255) / 256), 256, 0, ctx->stream>>>(a, P, e.batch, e);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   return MT_OK;

@@ -28,6 +28,8 @@ struct mt_ctx {
   size_t Mst_bytes;
   double* partial;
   size_t partial_bytes;
+  int* split_count;  // demag_tma.cu: chunks summed so far per split row group (zero between launches)
+  size_t split_count_bytes;
   void* Mq;  // staged M re-laid out for the tensor-core kernel's B fragments (demag_tma.cu)
   size_t Mq_bytes;
   double* rk;  // integrator stages + scratch states
