@@ -743,7 +743,8 @@ def threshold_curve(R, cfg: int, K: int):
 
 def integrators_small_n(R):
     """Per-right-hand-side cost INSIDE mt_integrate where the step is launch-bound (configs 1 and 2):
-    RK4 (CUDA-graph replay) and DP45 with the controller on the host (one 16-byte read per attempted step)
+    RK4 (CUDA-graph replay of the per-stage launches, and the tensor-resident cooperative kernel where the
+    tensor fits in shared memory) and DP45 with the controller on the host (one 16-byte read per attempted step)
     and on the device (mt_set_step_control: graph replay, the default at these sizes)."""
     import torch
     from paper_2107_05364_b200 import workloads as W
@@ -759,9 +760,16 @@ def integrators_small_n(R):
         prob = H.dev_problem(w, tiles, N, dtype, ld)
         dt = float(w.extra["dt"]) if cfg == 2 else 1e-2
         m = torch.from_numpy(w.m[:1].copy()).to(dev)
-        integrate_timed(R, prob, m, 1, method=B.MT_RK4, dt=dt, t_end=130 * dt)   # warm-up incl. graph capture
-        t, r, ms, _ = integrate_timed(R, prob, m, 1, method=B.MT_RK4, dt=dt, t_end=2048 * dt)
-        entry = {"n": n, "rk4": {"steps": r["accepted"], "us_per_rhs": 1e3 * ms / r["rhs_calls"]}}
+        entry = {"n": n}
+        # mode 1: the per-stage launches replayed from a CUDA graph; mode 0: the default, which at config 1
+        # (tensor fits in the SMs' shared memory) is one cooperative launch per chunk of steps (resident.cu)
+        for mode, key in ((1, "rk4_staged_launches_graph"), (0, "rk4")):
+            B.mt_set_resident_mode(ctx, mode)
+            m = torch.from_numpy(w.m[:1].copy()).to(dev)
+            integrate_timed(R, prob, m, 1, method=B.MT_RK4, dt=dt, t_end=130 * dt)   # warm-up incl. graph capture
+            t, r, ms, nl = integrate_timed(R, prob, m, 1, method=B.MT_RK4, dt=dt, t_end=2048 * dt)
+            entry[key] = {"steps": r["accepted"], "us_per_rhs": 1e3 * ms / r["rhs_calls"], "launches": nl}
+        B.mt_set_resident_mode(ctx, 0)
         # long enough that the one-off graph capture of the device-controlled run is amortised (config 1 has
         # no exchange term: a tight tolerance keeps the steps short)
         t_end = 400 * dt if cfg == 2 else 60.0

@@ -485,6 +485,20 @@ int mt_measure_peak(mt_ctx* ctx, int kind, const void* buf, int64_t bytes, doubl
  * Returns MT_OK or MT_ERR_INVALID_ARG.                                                              */
 int mt_set_step_control(mt_ctx* ctx, int mode);
 
+/* RK4 (A8) with the tensor resident in shared memory.  A dense, unsharded problem whose n x n x 6 tensor
+ * fits in the shared memory of the device's SMs together (one CTA per SM holding ceil(n / SMs) <= 8 rows of
+ * the six planes: N <= ~740 tiles fp64, ~1,100 fp32 on a B200 — the sizes the paper runs)
+ * is integrated a chunk of steps per COOPERATIVE launch: the tensor is read once per launch, every stage
+ * multiplies the resident rows with the staged Ms*m, runs the same fused epilogue as the other field
+ * kernels and ends at a grid barrier; no launch between right-hand sides.
+ * mode 0 (default): used whenever the problem qualifies; 1: never (the per-stage launches replayed from a
+ * CUDA graph); 2: required — mt_integrate(MT_RK4) fails with MT_ERR_INVALID_ARG when the problem does not
+ * qualify.  Same arithmetic per term as the streaming kernels (fp32 tensors: fp32 products and partial
+ * sums, then fp64), another summation order: results agree to rounding (1e-12 relative on fp64 tensors);
+ * deterministic.  Sampling, the stop test (torque words per step, read once per chunk) and the result
+ * counters behave as in the other path.  Returns MT_OK or MT_ERR_INVALID_ARG.                          */
+int mt_set_resident_mode(mt_ctx* ctx, int mode);
+
 /* Tuning / A-B testing hook: selects the demag kernel variant (0 = default choice by shape,
  * 1 = register-streaming LDG kernel, 2 = TMA bulk-tensor pipeline, 3 = as 2 but batches of 5..8
  * states on fp32 tensors use the packed-FFMA2 kernel instead of the tensor-core one).  Returns MT_OK or

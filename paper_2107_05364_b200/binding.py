@@ -33,7 +33,7 @@ EXPORTS = ("mt_create", "mt_destroy", "mt_last_error", "mt_version", "mt_assembl
            "mt_sparse_count_band", "mt_sparse_scan", "mt_sparse_fill_band", "mt_sparse_fill_index_band",
            "mt_sparse_stream_count", "mt_sparse_stream_fill", "mt_demag_field_sparse", "mt_sym_tensor_elems", "mt_assemble_tensor_sym",
            "mt_demag_field_sym", "mt_set_assembly_mode", "mt_launch_count",
-           "mt_set_demag_variant", "mt_set_step_control", "mt_profile_begin", "mt_profile_end", "mt_measure_peak",
+           "mt_set_demag_variant", "mt_set_step_control", "mt_set_resident_mode", "mt_profile_begin", "mt_profile_end", "mt_measure_peak",
            "mt_demag_field_noalloc")
 
 
@@ -120,6 +120,7 @@ def load() -> C.CDLL:
         lib.mt_set_demag_variant.argtypes = [C.c_void_p, C.c_int]
         lib.mt_set_assembly_mode.argtypes = [C.c_void_p, C.c_int]
         lib.mt_set_step_control.argtypes = [C.c_void_p, C.c_int]
+        lib.mt_set_resident_mode.argtypes = [C.c_void_p, C.c_int]
         lib.mt_check_status.argtypes = [C.c_void_p, C.c_void_p]
         lib.mt_profile_begin.argtypes = [C.c_void_p]
         lib.mt_measure_peak.argtypes = [C.c_void_p, C.c_int, C.c_void_p, C.c_int64, C.POINTER(C.c_double)]
@@ -250,6 +251,11 @@ def mt_set_demag_variant(ctx: Context, variant: int):
 def mt_set_step_control(ctx: Context, mode: int):
     """DP45 controller: 0 auto (device for small unsharded problems), 1 host, 2 device."""
     ctx.check(ctx.lib.mt_set_step_control(ctx.h, mode))
+
+
+def mt_set_resident_mode(ctx: Context, mode: int):
+    """RK4 with the tensor resident in shared memory: 0 auto (when it fits), 1 never, 2 required."""
+    ctx.check(ctx.lib.mt_set_resident_mode(ctx.h, mode))
 
 
 def mt_profile_begin(ctx: Context):

@@ -16,7 +16,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(HERE, "libmagtile.so")
-SOURCES = ("api.cu", "demag.cu", "demag_tma.cu", "assemble.cu", "sparse.cu", "sym.cu", "peaks.cu", "noalloc.cu")
+SOURCES = ("api.cu", "demag.cu", "demag_tma.cu", "assemble.cu", "sparse.cu", "sym.cu", "peaks.cu", "noalloc.cu", "resident.cu")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I", INCLUDE]
 

@@ -180,7 +180,8 @@ int mt_create(mt_ctx** out, int device, void* cuda_stream) {
     return MT_ERR_CUDA;
   }
   c->num_sms = prop.multiProcessorCount;
-  // device scalars: [0] err bits, [1] torque bits, [2..5] the selection's bin search, [8 ..] 256 per-step
+  // device scalars: [0] err bits, [1] torque bits, [2..5] the selection's bin search, [6] the resident RK4
+  // kernel's grid-barrier counter, [8 ..] 256 per-step
   // torque words of an RK4 chunk; the pinned mirror holds the two words, the search result or the chunk's torques
   if (cudaMalloc((void**)&c->dscal, (8 + 256) * sizeof(unsigned long long)) != cudaSuccess ||
       cudaMallocHost((void**)&c->hscal, 2048 * sizeof(unsigned long long)) != cudaSuccess) {
@@ -256,6 +257,12 @@ int mt_profile_end(mt_ctx* c, double* total_ms, int64_t* launches) {
 int mt_set_demag_variant(mt_ctx* c, int variant) {
   if (!c || variant < 0 || variant > 3) return MT_ERR_INVALID_ARG;
   c->variant = variant;
+  return MT_OK;
+}
+
+int mt_set_resident_mode(mt_ctx* c, int mode) {
+  if (!c || mode < 0 || mode > 2) return MT_ERR_INVALID_ARG;
+  c->resident_mode = mode;
   return MT_OK;
 }
 
@@ -826,39 +833,47 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
     bool hit_max = false;
     if (o->max_steps > 0 && nsteps > o->max_steps) { nsteps = o->max_steps; hit_max = true; }
     const bool want_tq = o->torque_tol > 0;
-    auto stage1 = [&](unsigned long long* tq) -> int {  // k1 = f(m); ya = m + dt/2 k1
+    // the four stages of a step as epilogue descriptors (stage s reads the staged M of buffer src[s]):
+    //   1: k1 = f(m),  ya = m + dt/2 k1      2: k2 = f(ya), yb = m + dt/2 k2
+    //   3: k3 = f(yb), ya = m + dt k3        4: k4 = f(ya), m <- m + dt/6 (k1 + 2 k2 + 2 k3 + k4), renormalised
+    void* const Mbuf[2] = {has_demag(p) ? ctx->Mst[0] : nullptr, has_demag(p) ? ctx->Mst[1] : nullptr};
+    double* const y_in[4] = {m, ya, yb, ya};
+    double* const y_to[4] = {ya, yb, ya, m};
+    const int src_of[4] = {0, 1, 0, 1};
+    auto make_stage = [&](int s, unsigned long long* tq) -> EpiArgs {
       EpiArgs e = base;
-      e.y = m; e.k_out = k[0]; e.torque_bits = tq;
-      e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[0]; e.coef[0] = 1.0; e.base = m; e.h = 0.5 * dt;
-      void* Md = has_demag(p) ? ctx->Mst[1] : nullptr;
-      route(e, ya, Md);
-      int r = eval_rhs(ctx, p, npad, 0, e);
-      return r ? r : finish(ya, Md);
+      e.y = y_in[s]; e.k_out = k[s]; e.torque_bits = s == 0 ? tq : nullptr;
+      e.do_comb = 1; e.base = m;
+      if (s < 3) {
+        e.ncomb = 1; e.kptr[0] = k[s]; e.coef[0] = 1.0; e.h = s < 2 ? 0.5 * dt : dt;
+      } else {
+        e.ncomb = 4;
+        for (int j = 0; j < 4; ++j) e.kptr[j] = k[j];
+        e.coef[0] = 1.0; e.coef[1] = 2.0; e.coef[2] = 2.0; e.coef[3] = 1.0;
+        e.h = dt / 6.0; e.renorm = o->renormalize;
+      }
+      route(e, y_to[s], Mbuf[src_of[s] ^ 1]);
+      return e;
     };
+    auto run_stage = [&](int s, unsigned long long* tq) -> int {
+      const EpiArgs e = make_stage(s, tq);
+      int r = eval_rhs(ctx, p, npad, src_of[s], e);
+      return r ? r : finish(y_to[s], Mbuf[src_of[s] ^ 1]);
+    };
+    auto stage1 = [&](unsigned long long* tq) -> int { return run_stage(0, tq); };
     auto stages234 = [&]() -> int {
       int r;
-      EpiArgs e = base;  // stage 2: k2 = f(ya); yb = m + dt/2 k2
-      e.y = ya; e.k_out = k[1];
-      e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[1]; e.coef[0] = 1.0; e.base = m; e.h = 0.5 * dt;
-      void* M0 = has_demag(p) ? ctx->Mst[0] : nullptr;
-      void* M1 = has_demag(p) ? ctx->Mst[1] : nullptr;
-      route(e, yb, M0);
-      if ((r = eval_rhs(ctx, p, npad, 1, e)) || (r = finish(yb, M0))) return r;
-      e = base;  // stage 3: k3 = f(yb); ya = m + dt k3
-      e.y = yb; e.k_out = k[2];
-      e.do_comb = 1; e.ncomb = 1; e.kptr[0] = k[2]; e.coef[0] = 1.0; e.base = m; e.h = dt;
-      route(e, ya, M1);
-      if ((r = eval_rhs(ctx, p, npad, 0, e)) || (r = finish(ya, M1))) return r;
-      e = base;  // stage 4: k4 = f(ya); m <- m + dt/6 (k1 + 2 k2 + 2 k3 + k4), renormalised, restaged
-      e.y = ya; e.k_out = k[3];
-      e.do_comb = 1; e.ncomb = 4;
-      for (int s = 0; s < 4; ++s) e.kptr[s] = k[s];
-      e.coef[0] = 1.0; e.coef[1] = 2.0; e.coef[2] = 2.0; e.coef[3] = 1.0;
-      e.base = m; e.h = dt / 6.0; e.renorm = o->renormalize;
-      route(e, m, M0);
-      if ((r = eval_rhs(ctx, p, npad, 1, e))) return r;
-      return finish(m, M0);
+      if ((r = run_stage(1, nullptr)) || (r = run_stage(2, nullptr))) return r;
+      return run_stage(3, nullptr);
     };
+    // Tensor resident in shared memory (resident.cu): dense, unsharded problems small enough for the SMs
+    // to hold the tensor between them run a whole chunk of steps in ONE cooperative launch.
+    const bool res_ok = p->N && !p->N_sparse && !p->N_sym && !sh && mt_resident_fits(ctx, p->dtype, n, batch) &&
+                        round_up(n, p->dtype == MT_F32 ? 4 : 2) <= p->ld;
+    if (ctx->resident_mode == 2 && !res_ok)
+      return mt_fail(ctx, MT_ERR_INVALID_ARG, "resident RK4 required (mt_set_resident_mode 2) but the problem does not qualify "
+                     "(dense unsharded tensor that fits in the SMs' shared memory)");
+    const bool resident = res_ok && ctx->resident_mode != 1;
     auto sample_if_due = [&](int64_t done) -> int {
       if (o->sample_every > 0 && done % o->sample_every == 0 && samples && res->n_samples < sample_cap) {
         int r = mt_launch_mean(ctx, m, p->vol, batch, n, t0 + (double)done * dt, samples + res->n_samples * stride);
@@ -898,6 +913,9 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       int64_t graph_launches = 0;
       bool stopped = false;
       auto run_steps = [&](int64_t count, bool with_tq) -> int {
+        if (resident)
+          return mt_launch_rk4_resident(ctx, p->N, p->dtype, n, p->ld, base, m, ya, yb, dt, o->renormalize,
+                                        with_tq ? slots : nullptr, (unsigned int*)(ctx->dscal + 6), count);
         int r = MT_OK;
         for (int64_t s = 0; s < count && !r; ++s) {
           r = stage1(with_tq ? slots + s : nullptr);
@@ -906,7 +924,8 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
         return r;
       };
       while (done < nsteps && !rc && !stopped) {
-        const bool use_graph = !sh && done >= chunk && done % chunk == 0 && nsteps - done >= chunk;  // (exchange callbacks are host calls)
+        // (exchange callbacks are host calls; a resident chunk already is a single launch)
+        const bool use_graph = !sh && !resident && done >= chunk && done % chunk == 0 && nsteps - done >= chunk;
         int64_t kk = chunk - done % chunk;
         if (kk > nsteps - done) kk = nsteps - done;
         if (want_tq) {

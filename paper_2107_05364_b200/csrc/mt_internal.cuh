@@ -17,6 +17,7 @@ struct mt_ctx {
   cudaStream_t cap_stream;  // private stream for CUDA-graph capture
   int num_sms;
   int step_control;  // DP45 controller: 0 auto (device for small problems), 1 host, 2 device
+  int resident_mode; // RK4 with the tensor resident in shared memory (resident.cu): 0 auto (when it fits), 1 never, 2 required
   DpState* dp_dev;   // device copy of the controller state (lazily allocated)
   DpState* dp_host;  // pinned mirror
   int variant;  // 0 auto, 1 LDG, 2 TMA, 3 TMA with the packed-FFMA2 kernel for batches of 5..8
@@ -158,6 +159,11 @@ int mt_launch_stage_M(mt_ctx* ctx, int dtype, const double* Ms, const double* m,
 int mt_launch_demag(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
                     const void* Mst, int64_t npad, const EpiArgs& epi);
 int mt_launch_local_only(mt_ctx* ctx, const EpiArgs& epi);  // N == NULL: H_d = 0
+// resident.cu: a chunk of RK4 steps in one cooperative launch, the dense tensor held in shared memory
+bool mt_resident_fits(mt_ctx* ctx, int dtype, int64_t n, int batch);
+int mt_launch_rk4_resident(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t ld, const EpiArgs& prob,
+                           double* m, double* ya, double* yb, double dt, int renorm,
+                           unsigned long long* tq_slots, unsigned int* bar, int64_t count);
 int mt_launch_combine(mt_ctx* ctx, const EpiArgs& epi);     // stage combine without a field evaluation
 // row-sharded problems: blocks [world][B][3][pad] of the gathered stage state -> full state y[B][3][n]
 // and (M_out non-NULL) the staged Ms*y in the tensor's dtype
