@@ -774,14 +774,19 @@ def integrators_small_n(R):
         # no exchange term: a tight tolerance keeps the steps short)
         t_end = 400 * dt if cfg == 2 else 60.0
         rtol, atol = (1e-6, 1e-8) if cfg == 2 else (1e-10, 1e-12)
-        for mode, key in ((1, "dp45_host_controller"), (2, "dp45_device_controller")):
+        # host controller / device controller with the attempt replayed from a CUDA graph / the default: where the
+        # tensor fits in shared memory (config 1), controller and stages inside one cooperative kernel
+        for mode, resm, key in ((1, 1, "dp45_host_controller"), (2, 1, "dp45_device_controller"), (0, 0, "dp45")):
             B.mt_set_step_control(ctx, mode)
+            B.mt_set_resident_mode(ctx, resm)
             m = torch.from_numpy(w.m[:1].copy()).to(dev)
             integrate_timed(R, prob, m, 1, method=B.MT_DP45, dt=dt, t_end=20 * dt, rtol=rtol, atol=atol)
             t, r, ms, _ = integrate_timed(R, prob, m, 1, method=B.MT_DP45, dt=dt, t_end=t_end, rtol=rtol, atol=atol, t0=20 * dt)
             entry[key] = {"accepted": r["accepted"], "rejected": r["rejected"],
                           "us_per_rhs": 1e3 * ms / max(1, r["rhs_calls"])}
         B.mt_set_step_control(ctx, 0)
+        B.mt_set_resident_mode(ctx, 0)
+        entry["resident"] = bool(n <= 1024)  # (what mt_integrate chose by itself: see mt_set_resident_mode)
         res_all[f"config{cfg}"] = entry
         del N, prob
         torch.cuda.empty_cache()

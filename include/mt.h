@@ -485,18 +485,25 @@ int mt_measure_peak(mt_ctx* ctx, int kind, const void* buf, int64_t bytes, doubl
  * Returns MT_OK or MT_ERR_INVALID_ARG.                                                              */
 int mt_set_step_control(mt_ctx* ctx, int mode);
 
-/* RK4 (A8) with the tensor resident in shared memory.  A dense, unsharded problem whose n x n x 6 tensor
- * fits in the shared memory of the device's SMs together (one CTA per SM holding ceil(n / SMs) <= 8 rows of
- * the six planes: N <= ~740 tiles fp64, ~1,100 fp32 on a B200 — the sizes the paper runs)
- * is integrated a chunk of steps per COOPERATIVE launch: the tensor is read once per launch, every stage
- * multiplies the resident rows with the staged Ms*m, runs the same fused epilogue as the other field
- * kernels and ends at a grid barrier; no launch between right-hand sides.
- * mode 0 (default): used whenever the problem qualifies; 1: never (the per-stage launches replayed from a
- * CUDA graph); 2: required — mt_integrate(MT_RK4) fails with MT_ERR_INVALID_ARG when the problem does not
- * qualify.  Same arithmetic per term as the streaming kernels (fp32 tensors: fp32 products and partial
- * sums, then fp64), another summation order: results agree to rounding (1e-12 relative on fp64 tensors);
- * deterministic.  Sampling, the stop test (torque words per step, read once per chunk) and the result
- * counters behave as in the other path.  Returns MT_OK or MT_ERR_INVALID_ARG.                          */
+/* RK4 (A8) and DP45 (A9) with the tensor resident in shared memory.  A dense, unsharded problem whose
+ * n x n x 6 tensor fits in the shared memory of the device's SMs together (one CTA per SM holding
+ * ceil(n / SMs) <= 8 rows of the six planes, plus the stage states: N <= ~740 tiles fp64, ~1,020 fp32 on a
+ * B200 — the sizes the paper runs) is integrated by a COOPERATIVE kernel: a chunk of RK4
+ * steps, or up to 64 attempted DP45 steps, per launch.  The tensor is read once per launch; every stage
+ * reads the stage state of all tiles from L2, multiplies the resident rows with Ms*m, adds
+ * exchange, anisotropy and the applied field and forms the Landau-Lifshitz right-hand side and the next
+ * stage state with the row's constants, the step's start state and the slopes in
+ * registers, and ends at a grid barrier; no launch between right-hand sides.  DP45: the step controller
+ * (the rules of mt_set_step_control's device controller) runs inside the kernel as well — every CTA takes
+ * the same decision from the grid-wide error / torque maxima — and the host reads the controller state
+ * once per launch.
+ * mode 0 (default): used whenever the problem qualifies (DP45: unless mt_set_step_control(ctx, 1) keeps
+ * the controller on the host); 1: never (per-stage launches, replayed from a CUDA graph); 2: required —
+ * mt_integrate fails with MT_ERR_INVALID_ARG when the problem does not qualify.  Same arithmetic per term
+ * as the streaming kernels (fp32 tensors: fp32 products and partial sums, then fp64), another summation
+ * order: RK4 trajectories agree to rounding (1e-11 on fp64 tensors), DP45 takes the same accept / reject
+ * sequence with step sizes equal to ~1e-10; deterministic.  Sampling, the stop tests and the result
+ * counters behave as in the other paths.  Returns MT_OK or MT_ERR_INVALID_ARG.                         */
 int mt_set_resident_mode(mt_ctx* ctx, int mode);
 
 /* Tuning / A-B testing hook: selects the demag kernel variant (0 = default choice by shape,

@@ -868,7 +868,7 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
     };
     // Tensor resident in shared memory (resident.cu): dense, unsharded problems small enough for the SMs
     // to hold the tensor between them run a whole chunk of steps in ONE cooperative launch.
-    const bool res_ok = p->N && !p->N_sparse && !p->N_sym && !sh && mt_resident_fits(ctx, p->dtype, n, batch) &&
+    const bool res_ok = p->N && !p->N_sparse && !p->N_sym && !sh && mt_resident_fits(ctx, p->dtype, n, batch, MT_RK4) &&
                         round_up(n, p->dtype == MT_F32 ? 4 : 2) <= p->ld;
     if (ctx->resident_mode == 2 && !res_ok)
       return mt_fail(ctx, MT_ERR_INVALID_ARG, "resident RK4 required (mt_set_resident_mode 2) but the problem does not qualify "
@@ -1012,7 +1012,15 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
     // the device (DpState, demag.cu): one attempted step is a fixed sequence of launches replayed from a
     // CUDA graph, and the host looks at the state every kLook attempts.  Attempts replayed after the run
     // has ended do nothing (their kernels see active == 0), but still stream the tensor: hence small n only.
-    const bool use_dev = !sh && (ctx->step_control == 2 || (ctx->step_control == 0 && n <= 8192));
+    // Tensor resident in shared memory (resident.cu): the whole attempt loop, controller included, runs in
+    // a cooperative kernel, kResAttempts attempted steps per launch (the kernel returns early when the run ends).
+    const bool res_ok = p->N && !p->N_sparse && !p->N_sym && !sh && mt_resident_fits(ctx, p->dtype, n, batch, MT_DP45) &&
+                        round_up(n, p->dtype == MT_F32 ? 4 : 2) <= p->ld;
+    if (ctx->resident_mode == 2 && !res_ok)
+      return mt_fail(ctx, MT_ERR_INVALID_ARG, "resident DP45 required (mt_set_resident_mode 2) but the problem does not qualify "
+                     "(dense unsharded tensor that fits in the SMs' shared memory)");
+    const bool use_res = res_ok && ctx->resident_mode != 1 && ctx->step_control != 1;
+    const bool use_dev = use_res || (!sh && (ctx->step_control == 2 || (ctx->step_control == 0 && n <= 8192)));
     if (use_dev) {
       if (!ctx->dp_dev) {
         MT_CUDA_OK(ctx, cudaMalloc((void**)&ctx->dp_dev, sizeof(DpState)));
@@ -1074,11 +1082,17 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
         return false;
       };
       const int kLook = n <= 2048 ? 16 : 8;
+      const int kResAttempts = 64;
       cudaGraph_t graph = nullptr;
       cudaGraphExec_t exec = nullptr;
       int64_t graph_launches = 0;
       bool first = true;
-      while (!rc && !finished()) {
+      while (use_res && !rc && !finished()) {
+        rc = mt_launch_dp45_resident(ctx, p->N, p->dtype, n, p->ld, base, S, m, k[0], ya, yb, o->renormalize, samples,
+                                     stride, p->vol, ctx->dscal + 8, (unsigned int*)(ctx->dscal + 6), kResAttempts);
+        if (!rc) rc = look();
+      }
+      while (!use_res && !rc && !finished()) {
         if (first) {  // eagerly: sizes the workspaces, which must not be allocated under capture
           first = false;
           if ((rc = attempt())) break;

@@ -1,5 +1,5 @@
-"""-m gpu: RK4 with the tensor resident in shared memory (csrc/resident.cu, mt_set_resident_mode): one
-cooperative launch per chunk of steps.  Checked against the per-stage launches (mode 1) and against the
+"""-m gpu: RK4 and DP45 with the tensor resident in shared memory (csrc/resident.cu, mt_set_resident_mode): one
+cooperative launch per chunk of steps / per 64 attempted steps.  Checked against the per-stage launches (mode 1) and against the
 CPU oracle's trajectory, with the tolerances of tests/test_gpu_small.py, on ragged sizes, both tensor
 dtypes, batches, sampling and the stop test (Eq. 2); a problem that does not fit is refused
 when the mode is 'required' and runs through the streaming kernels otherwise.
@@ -122,3 +122,94 @@ def test_resident_mode_required_refuses_what_does_not_fit(ctx, oracle):
     assert rc == 0 and r["accepted"] == 8 and np.isfinite(m).all()
     with pytest.raises(B.MtError):
         B.mt_set_resident_mode(ctx, 3)
+
+
+def test_resident_dp45_equals_host_controller_and_oracle(oracle):
+    """DP45 inside the resident kernel (controller of dp_control.cuh run by every CTA on its own copy of the
+    state) against the host controller with per-stage launches and against the oracle, on an 8^3 replica of
+    config 3 with two states: same accept / reject sequence, same sample times, states and samples to
+    rounding; stops by the torque test, by t_end and by max_steps; sample rows capped by sample_cap."""
+    w = W.config3(8, batch=2)
+    x = w.extra
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=True)
+    runs = {}
+    for key, (ctl, resident) in {"host": (1, 1), "resident": (0, 2)}.items():
+        c = B.mt_create(0)
+        B.mt_set_step_control(c, ctl)
+        B.mt_set_resident_mode(c, resident)
+        tiles = H.dev_tiles(w)
+        N, ld, _ = H.assemble(c, tiles, "f64")
+        prob = H.dev_problem(w, tiles, N, "f64", ld)
+        out = []
+        for kw in (dict(t_end=2.0, sample_dt=0.25, sample_cap=16),
+                   dict(t_end=40.0, sample_dt=1.0, sample_cap=5, torque_tol=0.5),
+                   dict(t_end=2.0, max_steps=37, allow=(B.MT_ERR_MAX_STEPS,))):
+            l0 = B.mt_launch_count(c)
+            out.append(run_gpu_integrate(c, prob, w.m, 2, method=B.MT_DP45, dt=x["dt0"], rtol=x["rtol"], atol=x["atol"], **kw)
+                       + (B.mt_launch_count(c) - l0,))
+        runs[key] = out
+        c.close()
+    for (m1, s1, r1, rc1, n1), (m2, s2, r2, rc2, n2) in zip(runs["host"], runs["resident"]):
+        assert rc1 == rc2
+        for key in ("accepted", "rejected", "rhs_calls", "n_samples"):
+            assert r1[key] == r2[key], key
+        # (another summation order in H_d: the error estimate, a difference of nearly equal slopes, moves in its
+        # ~10th digit and the step sizes with it: a run that ends on a step count ends at t equal to ~1e-10)
+        assert abs(r1["t"] - r2["t"]) <= 1e-9 and abs(r1["dt_last"] - r2["dt_last"]) <= 1e-6 * r1["dt_last"]
+        assert abs(r1["max_torque"] - r2["max_torque"]) <= 1e-6 * r1["max_torque"]
+        assert np.array_equal(s1[:, 0], s2[:, 0]) and (s1.size == 0 or np.max(np.abs(s1 - s2)) < 1e-9)
+        assert np.max(np.abs(m1 - m2)) < 1e-9
+        # stagings + k1 + one launch per 64 attempts, against ~8 launches per attempt
+        assert n2 <= 3 + (r2["accepted"] + r2["rejected"]) // 64 + 1 and n2 < n1 / 20
+    (_, s, r, _, _), (_, s_t, r_t, _, _), (_, _, r_m, rc_m, _) = runs["resident"]
+    assert r["t"] == 2.0 and r["rejected"] > 0 and np.array_equal(s[:, 0], 0.25 * np.arange(1, 9))
+    assert r_t["max_torque"] <= 0.5 and 5.0 < r_t["t"] < 40.0 and r_t["n_samples"] == 5
+    assert rc_m == B.MT_ERR_MAX_STEPS and r_m["accepted"] + r_m["rejected"] == 37
+    # a single state against the oracle's own step sequence
+    m_o, s_o, r_o = oracle.integrate(H.oracle_problem(oracle, w, N_ref), w.m[0], method=oracle.DP45, dt=x["dt0"],
+                                     rtol=x["rtol"], atol=x["atol"], t_end=2.0, sample_dt=0.25, sample_cap=16, weights=w.vol)
+    c = B.mt_create(0)
+    B.mt_set_resident_mode(c, 2)
+    tiles = H.dev_tiles(w)
+    N, ld, _ = H.assemble(c, tiles, "f64")
+    m, s, r, _ = run_gpu_integrate(c, H.dev_problem(w, tiles, N, "f64", ld), w.m[:1], 1, method=B.MT_DP45, dt=x["dt0"],
+                                   rtol=x["rtol"], atol=x["atol"], t_end=2.0, sample_dt=0.25, sample_cap=16)
+    c.close()
+    assert (r["accepted"], r["rejected"]) == (r_o["accepted"], r_o["rejected"])
+    assert np.array_equal(s[:, 0], s_o[:, 0]) and np.max(np.abs(s[:, 1:] - s_o[:, 1:])) < 1e-9
+    assert np.max(np.abs(m[0] - m_o)) < 1e-8
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_resident_dp45_small_cube_against_oracle(ctx, oracle, dtype):
+    """Config-3 physics on a 6^3 cube (216 tiles: two rows per CTA on 108 CTAs): DP45 to t = 3 on the resident
+    kernel, the assertions of test_dp45_trajectory_small_cube; then continued in a second call (k1 = f(m) is
+    re-evaluated by the caller, the controller state starts afresh)."""
+    w = W.config3(6)
+    prob, _ = setup(ctx, oracle, w, dtype)
+    N_ref = oracle.assemble_rows(H.oracle_tiles(oracle, w), long_double=True)
+    kw = dict(dt=1e-3, t_end=3.0, rtol=1e-6, atol=1e-8, sample_dt=0.25)
+    m_ref, s_ref, r_ref = oracle.integrate(H.oracle_problem(oracle, w, N_ref), w.m[0], method=oracle.DP45,
+                                           sample_cap=64, weights=w.vol, **kw)
+    B.mt_set_resident_mode(ctx, 2)
+    m, s, res, _ = run_gpu_integrate(ctx, prob, w.m, 1, method=B.MT_DP45, sample_cap=64, **kw)
+    assert res["n_samples"] == 12 == r_ref["n_samples"] and res["t"] == 3.0
+    assert np.array_equal(s[:, 0], s_ref[:, 0])
+    assert np.max(np.abs(s[:, 1:] - s_ref[:, 1:])) < 1e-3
+    if dtype == "f64":
+        assert res["accepted"] == r_ref["accepted"] and res["rejected"] == r_ref["rejected"]
+        assert np.max(np.abs(m[0] - m_ref)) < 1e-8
+    assert res["rhs_calls"] == 1 + 6 * (res["accepted"] + res["rejected"])
+    assert np.max(np.abs(np.linalg.norm(m[0], axis=0) - 1.0)) < 1e-14
+
+
+def test_resident_dp45_nonfinite_state_is_an_error(ctx, oracle):
+    """A NaN in the state reaches the error estimate inside the kernel: MT_ERR_STEP_UNDERFLOW (Q11b)."""
+    w = W.config3(4)
+    prob, _ = setup(ctx, oracle, w, "f64")
+    B.mt_set_resident_mode(ctx, 2)
+    m0 = w.m[:1].copy()
+    m0[0, 1, 7] = np.nan
+    _, _, r, rc = run_gpu_integrate(ctx, prob, m0, 1, method=B.MT_DP45, dt=1e-3, t_end=1.0,
+                                    allow=(B.MT_ERR_STEP_UNDERFLOW,))
+    assert rc == B.MT_ERR_STEP_UNDERFLOW and r["accepted"] == 0

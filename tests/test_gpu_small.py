@@ -320,6 +320,7 @@ def test_dp45_device_controller_equals_host_controller(oracle):
     for mode in (1, 2):
         c = B.mt_create(0)
         B.mt_set_step_control(c, mode)
+        B.mt_set_resident_mode(c, 1)  # the graph-replayed attempt (the tensor-resident kernel: test_gpu_resident.py)
         tiles = H.dev_tiles(w)
         N, ld, _ = H.assemble(c, tiles, "f64")
         prob = H.dev_problem(w, tiles, N, "f64", ld)
@@ -350,6 +351,7 @@ def test_dp45_device_controller_equals_host_controller(oracle):
     # single-state device run with the oracle)
     c = B.mt_create(0)
     B.mt_set_step_control(c, 2)
+    B.mt_set_resident_mode(c, 1)
     tiles = H.dev_tiles(w)
     N, ld, _ = H.assemble(c, tiles, "f64")
     m, s, r, _ = run_gpu_integrate(c, H.dev_problem(w, tiles, N, "f64", ld), w.m[:1], 1, method=B.MT_DP45, dt=x["dt0"],
