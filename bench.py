@@ -435,6 +435,22 @@ def run_protocol(R, args, w, tiles, N, ld, dtype):
         if args.config != 5:
             ms = block(lambda: B.mt_llg_rhs(ctx, prob, m1, 1, k1, None), count)
             out["llg_rhs"] = {"calls": count, "total_ms": ms, "ms_per_call": ms / count}
+        if args.config == 1:
+            # the same tensor inside the integrators: resident in shared memory (one cooperative launch per
+            # chunk of RK4 steps / per 64 attempted DP45 steps), beside the per-stage launches
+            for resm, key in ((1, "staged_launches"), (0, "resident")):
+                B.mt_set_resident_mode(ctx, resm)
+                mm = m1.clone()
+                integrate_timed(R, prob, mm, 1, method=B.MT_RK4, dt=1e-2, t_end=1.3)
+                _, r, ms, nl = integrate_timed(R, prob, mm, 1, method=B.MT_RK4, dt=1e-2, t_end=20.48)
+                out[f"rk4_{key}"] = {"steps": r["accepted"], "us_per_rhs": 1e3 * ms / r["rhs_calls"], "launches": nl}
+                mm = m1.clone()
+                kw = dict(method=B.MT_DP45, dt=1e-2, rtol=1e-10, atol=1e-12)
+                integrate_timed(R, prob, mm, 1, t_end=0.2, **kw)
+                _, r, ms, nl = integrate_timed(R, prob, mm, 1, t_end=60.0, t0=0.2, **kw)
+                out[f"dp45_{key}"] = {"accepted": r["accepted"], "rejected": r["rejected"],
+                                      "us_per_rhs": 1e3 * ms / max(1, r["rhs_calls"]), "launches": nl}
+            B.mt_set_resident_mode(ctx, 0)
         else:
             m8 = torch.from_numpy(w.m).to(dev)
             Hd8 = torch.empty((8, 3, n), dtype=torch.float64, device=dev)
