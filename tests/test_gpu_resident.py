@@ -213,3 +213,34 @@ def test_resident_dp45_nonfinite_state_is_an_error(ctx, oracle):
     _, _, r, rc = run_gpu_integrate(ctx, prob, m0, 1, method=B.MT_DP45, dt=1e-3, t_end=1.0,
                                     allow=(B.MT_ERR_STEP_UNDERFLOW,))
     assert rc == B.MT_ERR_STEP_UNDERFLOW and r["accepted"] == 0
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+@pytest.mark.parametrize("grid", [(1, 1, 1), (3, 1, 1), (2, 2, 1)])
+def test_resident_tiny_problems_with_padded_rows(ctx, oracle, grid, dtype):
+    """One to four tiles (one CTA row each, vectors mostly padding) on a tensor with extra row padding filled
+    with NaN beyond column n: both integrators equal the per-stage launches."""
+    nx, ny, nz = grid
+    n = nx * ny * nz
+    rng = np.random.default_rng(10 + n)
+    edge = (1.0, 0.8, 1.2)
+    w = W._cuboid_workload("tiny", nx, ny, nz, edge, 1.0, W.random_unit_states(rng, 2, n),
+                           nbr=W.grid_neighbours(nx, ny, nz), inv_d2=tuple(1.0 / e**2 for e in edge), c_ex=0.2,
+                           c_an=0.3, easy=(0.0, 0.6, 0.8), H_a=(0.1, 0.0, 0.05), gamma=1.0, alpha_ll=0.4)
+    tiles = H.dev_tiles(w)
+    ld = W.leading_dim(n, dtype) + 8
+    N, ld, status = H.assemble(ctx, tiles, dtype, ld=ld)
+    assert status == 0
+    N[:, :, n:] = float("nan")  # what lies beyond column n must never be used
+    prob = H.dev_problem(w, tiles, N, dtype, ld)
+    tol = 1e-11 if dtype == "f64" else 2e-5
+    for kw in (dict(method=B.MT_RK4, dt=0.01, t_end=1.0, sample_every=25, sample_cap=8),
+               dict(method=B.MT_DP45, dt=1e-3, t_end=1.0, rtol=1e-7, atol=1e-9, sample_dt=0.25, sample_cap=8)):
+        out = {}
+        for mode in (1, 2):
+            B.mt_set_resident_mode(ctx, mode)
+            out[mode] = run_gpu_integrate(ctx, prob, w.m, 2, **kw)
+        (m1, s1, r1, _), (m2, s2, r2, _) = out[1], out[2]
+        assert np.isfinite(m2).all() and r1["n_samples"] == r2["n_samples"] == 4
+        assert (r1["accepted"], r1["rejected"]) == (r2["accepted"], r2["rejected"])
+        assert np.max(np.abs(m2 - m1)) < tol and np.max(np.abs(s2 - s1)) < tol
