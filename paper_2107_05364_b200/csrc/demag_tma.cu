@@ -88,6 +88,14 @@ __device__ __forceinline__ void fma3(double acc[3], const double2 v[6], const do
 template <typename T, bool Direct> struct RunSel { typedef T type; };
 template <typename T> struct RunSel<T, true> { typedef char type; };
 
+#ifndef MT_TMA_MIN_TILES_PER_SM
+#define MT_TMA_MIN_TILES_PER_SM 9LL
+#endif
+#ifndef MT_KEEP_L2_MB
+#define MT_KEEP_L2_MB 100
+#endif
+constexpr size_t kKeepL2Bytes = (size_t)MT_KEEP_L2_MB << 20;  // tensors up to this size are kept in the 126 MB L2 between calls
+
 struct TmaArgs {
   int64_t n_rows;
   int64_t groups;   // ceil(n_rows / RT)
@@ -96,6 +104,7 @@ struct TmaArgs {
   double* partial;  // [P][2][RT][B][3]
   double* exch;     // tensor-core kernel: [P][MmaCfg::exch_doubles] column parts of a row block
   int* count;       // [groups] chunks of a split row group summed so far; zero between launches
+  int keep_l2;      // the tensor fits in L2: load it with the evict-last policy (it is read again at the next right-hand side)
 };
 
 // first tile of CTA c: floor(tiles * c / P), c in [0, P]
@@ -213,6 +222,7 @@ __global__ void __launch_bounds__(kThreads, 1)
   if (is_producer) {
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+    if (a.keep_l2) pol_stream = pol_keep;
   }
   // issues tiles until the ring is full or a slot is still being read; `must` = tile index that has to
   // be in flight on return (blocking wait for its slot if necessary)
@@ -417,6 +427,7 @@ __global__ void __launch_bounds__(WARPS * 32, 1)
   if (is_producer) {
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+    if (a.keep_l2) pol_stream = pol_keep;
   }
   auto top_up = [&](int64_t must) {
     while (p_t < t1) {
@@ -665,6 +676,7 @@ __global__ void __launch_bounds__(kMmaWarps * 32, 1)
   if (is_producer) {
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol_stream));
     asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol_keep));
+    if (a.keep_l2) pol_stream = pol_keep;
   }
   auto top_up = [&](int64_t must) {
     while (p_t < t1) {
@@ -895,6 +907,7 @@ int launch_tiles(mt_ctx* ctx, Kern kern, unsigned char* attr_set, int m_rows, co
   a.exch = nullptr;
   if ((rc = ensure_count(ctx, a.groups))) return rc;
   a.count = ctx->split_count;
+  a.keep_l2 = 6 * (size_t)n_rows * (size_t)ld * sizeof(T) <= kKeepL2Bytes;
   alignas(64) CUtensorMap tmN, tmM;
   {
     const uint64_t dims[3] = {(uint64_t)n, (uint64_t)n_rows, 6};
@@ -961,6 +974,7 @@ int launch_mma(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld
   a.exch = ctx->partial + partial_doubles;
   if ((rc = ensure_count(ctx, a.groups))) return rc;
   a.count = ctx->split_count;
+  a.keep_l2 = 6 * (size_t)n_rows * (size_t)ld * sizeof(float) <= kKeepL2Bytes;
   // M re-laid out for the B fragments: hi/lo split, [3][npad/8][8 states][4][4] fp32
   const size_t mq_bytes = (size_t)3 * (npad / 8) * 32 * sizeof(float4);
   if ((rc = mt_ensure_ws(ctx, &ctx->Mq, &ctx->Mq_bytes, mq_bytes))) return rc;
@@ -1049,7 +1063,7 @@ int mt_launch_demag_tma(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_
                         const void* Mst, int64_t npad, const EpiArgs& e) {
   if (ctx->variant < 2) {
     const int64_t tiles = ((n_rows + 7) / 8) * ((n * (dtype == MT_F32 ? 4 : 8) + 1023) / 1024);
-    if (tiles < 16LL * ctx->num_sms) return MT_ERR_UNIMPLEMENTED;
+    if (tiles < MT_TMA_MIN_TILES_PER_SM * ctx->num_sms) return MT_ERR_UNIMPLEMENTED;
   }
   if (dtype == MT_F32) return launch_T<float>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
   return launch_T<double>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
