@@ -25,6 +25,7 @@ namespace {
 
 constexpr int kResThreads = 256;
 constexpr int kResWarps = kResThreads / 32;
+constexpr int kColQ = 5;  // columns per thread of the stage state: n <= kColQ * kResThreads = 1,280
 
 struct ResArgs {
   const void* N;  // [6][n][ld]
@@ -98,12 +99,12 @@ __device__ __forceinline__ void grid_barrier(unsigned int* ctr, unsigned int tar
 }
 
 // The resident machinery both integrators share.  Shared memory:
-//   tens[R][6][ldS] T | Msh[B][3][ldS] T | ysh[B][3][n] double | Mss[n] double | red[B][8][3] double | extra
+//   tens[R][6][ldS] T | Msh[B][3][ldS] T | ysh[B][3][n] double | red[B][8][3] double | extra
 template <typename T>
 struct Resident {
   typedef typename Vec<T>::type V;
   static constexpr int W = Vec<T>::W;
-  V* tens; V* Msh; double* ysh; double* Mss; double* red; unsigned char* extra;
+  V* tens; V* Msh; double* ysh; double* red; unsigned char* extra;
   const V* trow;
   int64_t n, ldS, nv, r0, v0, v1, i;
   int B, R, rows, wpr, row, tid, warp, lane, er, eb;
@@ -111,6 +112,7 @@ struct Resident {
   // the row's constants (epilogue threads)
   int32_t nb[6];
   double cex, can, ax[3], ha[3];
+  double msj[kColQ];  // Ms of the columns tid + 256 q (every thread: the stage state's staging)
 
   // carve the shared memory, load the CTA's rows of the six planes (columns >= n read as zero), Ms, zero M
   __device__ __forceinline__ void init(unsigned char* smem, const void* Nptr, int64_t n_, int64_t ld, int64_t ldS_, int R_,
@@ -123,8 +125,7 @@ struct Resident {
     tens = reinterpret_cast<V*>(smem);
     Msh = tens + (int64_t)R * 6 * nv;
     ysh = reinterpret_cast<double*>(Msh + (int64_t)B * 3 * nv);
-    Mss = ysh + (int64_t)B * 3 * n;
-    red = Mss + n;
+    red = ysh + (int64_t)B * 3 * n;
     extra = reinterpret_cast<unsigned char*>(red + (int64_t)B * kResWarps * 3);
     const T* N = (const T*)Nptr;
     const int64_t plane = n * ld;
@@ -136,7 +137,8 @@ struct Resident {
       const V x = __ldcs(reinterpret_cast<const V*>(N + c * plane + (r0 + r) * ld) + v);
       tens[((int64_t)r * 6 + c) * nv + v] = zero_from(x, v * W, n);
     }
-    for (int64_t j = tid; j < n; j += kResThreads) Mss[j] = e.Ms[j];
+#pragma unroll
+    for (int q = 0; q < kColQ; ++q) msj[q] = tid + q * kResThreads < n ? e.Ms[tid + q * kResThreads] : 0.0;
     T* Mz = reinterpret_cast<T*>(Msh);
     for (int64_t idx = tid; idx < (int64_t)B * 3 * ldS; idx += kResThreads) Mz[idx] = T(0);
     epi = tid < rows * B;
@@ -173,46 +175,52 @@ struct Resident {
   // L2, not L1).  Epilogue threads return mi = the state of their tile, k = dm/dt (Eq. 1) and |m x H_eff|.
   __device__ __forceinline__ void rhs(const double* yin, const EpiArgs& e, double mi[3], double k[3], double& torque) {
     {
-      // Ms*m in the tensor's dtype, rounded once (Q19); eight loads in flight per thread: the stage
-      // costs one L2 round trip, not one per element
+      // Ms*m in the tensor's dtype, rounded once (Q19).  A thread owns the columns tid + 256 q: a
+      // state's 3 x kColQ loads are in flight together (the stage costs one L2 round trip per state, not one
+      // per element) and Ms of those columns stays in registers for the whole launch.
       T* Ms_ = reinterpret_cast<T*>(Msh);
-      const int n32 = (int)n, ld32 = (int)ldS, total = 3 * B * n32;
-      for (int base0 = 0; base0 < total; base0 += kResThreads * 8) {
-        double yv[8];
+      const int n32 = (int)n, ld32 = (int)ldS;
+      for (int b = 0; b < B; ++b) {
+        const double* src = yin + (int64_t)b * 3 * n;
+        double yv[3][kColQ];
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
-          const int idx = base0 + u * kResThreads + tid;
-          yv[u] = idx < total ? __ldcg(yin + idx) : 0.0;
-        }
+        for (int c = 0; c < 3; ++c)
 #pragma unroll
-        for (int u = 0; u < 8; ++u) {
-          const int idx = base0 + u * kResThreads + tid;
-          if (idx < total) {
-            const int bc = idx / n32, j = idx - bc * n32;
-            ysh[idx] = yv[u];
-            Ms_[bc * ld32 + j] = (T)(Mss[j] * yv[u]);
+          for (int q = 0; q < kColQ; ++q) {
+            const int j = tid + q * kResThreads;
+            yv[c][q] = j < n32 ? __ldcg(src + c * n32 + j) : 0.0;
           }
-        }
+#pragma unroll
+        for (int c = 0; c < 3; ++c)
+#pragma unroll
+          for (int q = 0; q < kColQ; ++q) {
+            const int j = tid + q * kResThreads;
+            if (j < n32) {
+              ysh[(b * 3 + c) * n32 + j] = yv[c][q];
+              Ms_[(b * 3 + c) * ld32 + j] = (T)(msj[q] * yv[c][q]);
+            }
+          }
       }
     }
     __syncthreads();
     if (row < rows) {
       // up to four states per pass over the row: the tensor's shared-memory rows are read once per pass
+      const int nv32 = (int)nv, v0i = (int)v0, v1i = (int)v1;
       for (int b0 = 0; b0 < B; b0 += 4) {
         T acc[4][3];
 #pragma unroll
         for (int bb = 0; bb < 4; ++bb) acc[bb][0] = acc[bb][1] = acc[bb][2] = T(0);
-        for (int64_t v = v0 + lane; v < v1; v += 32) {
+        for (int v = v0i + lane; v < v1i; v += 32) {
           V t[6];
 #pragma unroll
-          for (int c = 0; c < 6; ++c) t[c] = trow[c * nv + v];
+          for (int c = 0; c < 6; ++c) t[c] = trow[c * nv32 + v];
 #pragma unroll
           for (int bb = 0; bb < 4; ++bb)
             if (b0 + bb < B) {
-              const V* Mb = Msh + (int64_t)(b0 + bb) * 3 * nv;
+              const V* Mb = Msh + (b0 + bb) * 3 * nv32;
               V m[3];
 #pragma unroll
-              for (int c = 0; c < 3; ++c) m[c] = Mb[c * nv + v];
+              for (int c = 0; c < 3; ++c) m[c] = Mb[c * nv32 + v];
               vec3(acc[bb], t, m);
             }
         }
@@ -533,7 +541,7 @@ size_t resident_smem(int dtype, int64_t n, int R, int batch, size_t extra, int64
   const size_t sz = dtype == MT_F32 ? 4 : 8;
   const int64_t ldS = (n + W - 1) / W * W;
   if (ldS_out) *ldS_out = ldS;
-  return ((size_t)R * 6 + (size_t)batch * 3) * ldS * sz + ((size_t)batch * 3 + 1) * n * sizeof(double) +
+  return ((size_t)R * 6 + (size_t)batch * 3) * ldS * sz + (size_t)batch * 3 * n * sizeof(double) +
          (size_t)batch * kResWarps * 3 * sizeof(double) + extra;
 }
 constexpr size_t kDpExtra = 2 * kResThreads * sizeof(double);  // the sample's reduction tree
@@ -547,7 +555,7 @@ static_assert(sizeof(DpState) <= kDpStatic, "static shared memory of the DP45 ke
 // Can the dense n x n tensor of this dtype stay resident in shared memory across the GPU (one CTA per SM,
 // ceil(n / SMs) <= 8 rows each) together with `batch` stage states?  method: MT_RK4 or MT_DP45.
 bool mt_resident_fits(mt_ctx* ctx, int dtype, int64_t n, int batch, int method) {
-  if (n <= 0 || n > 65536 || batch < 1 || batch > MT_MAX_BATCH) return false;
+  if (n <= 0 || n > kColQ * kResThreads || batch < 1 || batch > MT_MAX_BATCH) return false;
   const int R = (int)((n + ctx->num_sms - 1) / ctx->num_sms);
   if (R > kResWarps || R * batch > kResThreads) return false;
   int dev_smem = 0, coop = 0;
