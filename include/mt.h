@@ -497,6 +497,10 @@ int mt_set_step_control(mt_ctx* ctx, int mode);
  * (the rules of mt_set_step_control's device controller) runs inside the kernel as well — every CTA takes
  * the same decision from the grid-wide error / torque maxima — and the host reads the controller state
  * once per launch.
+ * A tensor too large for that but of at most 100 MB (it stays in the 126 MB L2 between right-hand sides: up to
+ * ~2,000 tiles fp32, ~1,450 fp64) runs the same persistent kernels with the CTA's rows (at most 32) read from
+ * L2 at every stage instead of from shared memory; everything else — stage state, epilogue, barrier,
+ * controller — is unchanged.
  * mode 0 (default): used whenever the problem qualifies (DP45: unless mt_set_step_control(ctx, 1) keeps
  * the controller on the host); 1: never (per-stage launches, replayed from a CUDA graph); 2: required —
  * mt_integrate fails with MT_ERR_INVALID_ARG when the problem does not qualify.  Same arithmetic per term

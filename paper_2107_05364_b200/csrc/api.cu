@@ -868,8 +868,9 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
     };
     // Tensor resident in shared memory (resident.cu): dense, unsharded problems small enough for the SMs
     // to hold the tensor between them run a whole chunk of steps in ONE cooperative launch.
-    const bool res_ok = p->N && !p->N_sparse && !p->N_sym && !sh && mt_resident_fits(ctx, p->dtype, n, batch, MT_RK4) &&
-                        round_up(n, p->dtype == MT_F32 ? 4 : 2) <= p->ld;
+    const int res_mode = (p->N && !p->N_sparse && !p->N_sym && !sh && round_up(n, p->dtype == MT_F32 ? 4 : 2) <= p->ld)
+                             ? mt_resident_fits(ctx, p->dtype, n, p->ld, batch, MT_RK4) : MT_RES_NONE;
+    const bool res_ok = res_mode != MT_RES_NONE;
     if (ctx->resident_mode == 2 && !res_ok)
       return mt_fail(ctx, MT_ERR_INVALID_ARG, "resident RK4 required (mt_set_resident_mode 2) but the problem does not qualify "
                      "(dense unsharded tensor that fits in the SMs' shared memory)");
@@ -914,7 +915,7 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       bool stopped = false;
       auto run_steps = [&](int64_t count, bool with_tq) -> int {
         if (resident)
-          return mt_launch_rk4_resident(ctx, p->N, p->dtype, n, p->ld, base, m, ya, yb, dt, o->renormalize,
+          return mt_launch_rk4_resident(ctx, res_mode, p->N, p->dtype, n, p->ld, base, m, ya, yb, dt, o->renormalize,
                                         with_tq ? slots : nullptr, (unsigned int*)(ctx->dscal + 6), count);
         int r = MT_OK;
         for (int64_t s = 0; s < count && !r; ++s) {
@@ -1014,8 +1015,9 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
     // has ended do nothing (their kernels see active == 0), but still stream the tensor: hence small n only.
     // Tensor resident in shared memory (resident.cu): the whole attempt loop, controller included, runs in
     // a cooperative kernel, kResAttempts attempted steps per launch (the kernel returns early when the run ends).
-    const bool res_ok = p->N && !p->N_sparse && !p->N_sym && !sh && mt_resident_fits(ctx, p->dtype, n, batch, MT_DP45) &&
-                        round_up(n, p->dtype == MT_F32 ? 4 : 2) <= p->ld;
+    const int res_mode = (p->N && !p->N_sparse && !p->N_sym && !sh && round_up(n, p->dtype == MT_F32 ? 4 : 2) <= p->ld)
+                             ? mt_resident_fits(ctx, p->dtype, n, p->ld, batch, MT_DP45) : MT_RES_NONE;
+    const bool res_ok = res_mode != MT_RES_NONE;
     if (ctx->resident_mode == 2 && !res_ok)
       return mt_fail(ctx, MT_ERR_INVALID_ARG, "resident DP45 required (mt_set_resident_mode 2) but the problem does not qualify "
                      "(dense unsharded tensor that fits in the SMs' shared memory)");
@@ -1088,7 +1090,7 @@ int mt_integrate(mt_ctx* ctx, const mt_problem* p, const mt_integrator_opts* o, 
       int64_t graph_launches = 0;
       bool first = true;
       while (use_res && !rc && !finished()) {
-        rc = mt_launch_dp45_resident(ctx, p->N, p->dtype, n, p->ld, base, S, m, k[0], ya, yb, o->renormalize, samples,
+        rc = mt_launch_dp45_resident(ctx, res_mode, p->N, p->dtype, n, p->ld, base, S, m, k[0], ya, yb, o->renormalize, samples,
                                      stride, p->vol, ctx->dscal + 8, (unsigned int*)(ctx->dscal + 6), kResAttempts);
         if (!rc) rc = look();
       }

@@ -160,11 +160,14 @@ int mt_launch_demag(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_
                     const void* Mst, int64_t npad, const EpiArgs& epi);
 int mt_launch_local_only(mt_ctx* ctx, const EpiArgs& epi);  // N == NULL: H_d = 0
 // resident.cu: a chunk of RK4 steps in one cooperative launch, the dense tensor held in shared memory
-bool mt_resident_fits(mt_ctx* ctx, int dtype, int64_t n, int batch, int method);
-int mt_launch_rk4_resident(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t ld, const EpiArgs& prob,
+#define MT_RES_NONE 0
+#define MT_RES_SMEM 1 /* tensor resident in shared memory */
+#define MT_RES_L2 2   /* tensor read from L2 at every stage by the same persistent kernel */
+int mt_resident_fits(mt_ctx* ctx, int dtype, int64_t n, int64_t ld, int batch, int method);
+int mt_launch_rk4_resident(mt_ctx* ctx, int mode, const void* N, int dtype, int64_t n, int64_t ld, const EpiArgs& prob,
                            double* m, double* ya, double* yb, double dt, int renorm,
                            unsigned long long* tq_slots, unsigned int* bar, int64_t count);
-int mt_launch_dp45_resident(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t ld, const EpiArgs& prob,
+int mt_launch_dp45_resident(mt_ctx* ctx, int mode, const void* N, int dtype, int64_t n, int64_t ld, const EpiArgs& prob,
                             DpState* S, double* m, double* k1, double* ya, double* yb, int renorm,
                             double* samples, int64_t stride, const double* vol, unsigned long long* words,
                             unsigned int* bar, int attempts);

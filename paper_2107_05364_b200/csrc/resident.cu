@@ -14,6 +14,8 @@
 // stage — the only thing left between two right-hand sides.  The tensor is read from HBM/L2 once per launch
 // instead of once per right-hand side; per stage a CTA moves 24 n bytes per state from L2 and 24 bytes per
 // row to it.  The arithmetic of a row is that of epilogue.cuh's row_epilogue / stage_combine, term by term.
+// Tensors too large for shared memory but small enough to stay in L2 (<= 100 MB) run the same kernels with
+// STREAM = true: the CTA's rows (<= 32) are read from L2 at every stage, everything else is unchanged.
 //
 // Deterministic: a row's columns are split over WPR warps, lanes stride the columns, fixed xor butterfly,
 // the warps' parts added in warp order.  fp32 tensors: fp32 products and per-lane partial sums over at most
@@ -25,6 +27,7 @@ namespace {
 
 constexpr int kResThreads = 256;
 constexpr int kResWarps = kResThreads / 32;
+constexpr int kStreamUnroll = 2;  // row vectors in flight per lane when the tensor is read from L2 (A/B: 1..4)
 constexpr int kColQ = 5;  // columns per thread of the stage state: n <= kColQ * kResThreads = 1,280
 
 struct ResArgs {
@@ -99,13 +102,19 @@ __device__ __forceinline__ void grid_barrier(unsigned int* ctr, unsigned int tar
 }
 
 // The resident machinery both integrators share.  Shared memory:
-//   tens[R][6][ldS] T | Msh[B][3][ldS] T | ysh[B][3][n] double | red[B][8][3] double | extra
-template <typename T>
+//   STREAM = false (tensor resident in shared memory):
+//     tens[R][6][ldS] T | Msh[B][3][ldS] T | ysh[B][3][n] double | red[B][8][3] double | extra
+//   STREAM = true (tensor too large for shared memory but small enough for L2: the rows are read from L2 at every
+//   stage by all eight warps, one row after the other; nothing else changes):
+//     Msh[B][3][ldS] T | ysh[B][3][n] double | Mss[n] double | red[B][R][8][3] double | extra
+template <typename T, bool STREAM>
 struct Resident {
   typedef typename Vec<T>::type V;
   static constexpr int W = Vec<T>::W;
-  V* tens; V* Msh; double* ysh; double* red; unsigned char* extra;
+  V* tens; V* Msh; double* ysh; double* red; double* Mss; unsigned char* extra;
   const V* trow;
+  const T* Ng;     // STREAM: the tensor in global memory
+  int64_t ldg;     //         and its row pitch
   int64_t n, ldS, nv, r0, v0, v1, i;
   int B, R, rows, wpr, row, tid, warp, lane, er, eb;
   bool epi;  // this thread finishes (row i = r0 + er, state eb)
@@ -123,22 +132,29 @@ struct Resident {
     r0 = (int64_t)blockIdx.x * R;
     rows = (int)min((int64_t)R, n - r0);
     tens = reinterpret_cast<V*>(smem);
-    Msh = tens + (int64_t)R * 6 * nv;
+    Msh = STREAM ? tens : tens + (int64_t)R * 6 * nv;
     ysh = reinterpret_cast<double*>(Msh + (int64_t)B * 3 * nv);
-    red = ysh + (int64_t)B * 3 * n;
-    extra = reinterpret_cast<unsigned char*>(red + (int64_t)B * kResWarps * 3);
-    const T* N = (const T*)Nptr;
-    const int64_t plane = n * ld;
-    const int64_t tot = (int64_t)rows * 6 * nv;
-    for (int64_t idx = tid; idx < tot; idx += kResThreads) {
-      const int64_t v = idx % nv;
-      const int c = (int)((idx / nv) % 6);
-      const int r = (int)(idx / (6 * nv));
-      const V x = __ldcs(reinterpret_cast<const V*>(N + c * plane + (r0 + r) * ld) + v);
-      tens[((int64_t)r * 6 + c) * nv + v] = zero_from(x, v * W, n);
-    }
+    Mss = ysh + (int64_t)B * 3 * n;
+    red = STREAM ? Mss + n : Mss;
+    extra = reinterpret_cast<unsigned char*>(red + (int64_t)B * (STREAM ? R : 1) * kResWarps * 3);
+    Ng = (const T*)Nptr;
+    ldg = ld;
+    if constexpr (!STREAM) {
+      const T* N = (const T*)Nptr;
+      const int64_t plane = n * ld;
+      const int64_t tot = (int64_t)rows * 6 * nv;
+      for (int64_t idx = tid; idx < tot; idx += kResThreads) {
+        const int64_t v = idx % nv;
+        const int c = (int)((idx / nv) % 6);
+        const int r = (int)(idx / (6 * nv));
+        const V x = __ldcs(reinterpret_cast<const V*>(N + c * plane + (r0 + r) * ld) + v);
+        tens[((int64_t)r * 6 + c) * nv + v] = zero_from(x, v * W, n);
+      }
 #pragma unroll
-    for (int q = 0; q < kColQ; ++q) msj[q] = tid + q * kResThreads < n ? e.Ms[tid + q * kResThreads] : 0.0;
+      for (int q = 0; q < kColQ; ++q) msj[q] = tid + q * kResThreads < n ? e.Ms[tid + q * kResThreads] : 0.0;
+    } else {
+      for (int64_t j = tid; j < n; j += kResThreads) Mss[j] = e.Ms[j];
+    }
     T* Mz = reinterpret_cast<T*>(Msh);
     for (int64_t idx = tid; idx < (int64_t)B * 3 * ldS; idx += kResThreads) Mz[idx] = T(0);
     epi = tid < rows * B;
@@ -162,7 +178,7 @@ struct Resident {
         ha[c] = e.H_a ? e.H_a[3 * i + c] : e.H_a_c[c];
       }
     }
-    row = warp / wpr;
+    row = warp / wpr;  // (STREAM: the warp's slot within a round of kResWarps / wpr rows)
     const int seg = warp % wpr;
     const int64_t per = (nv + wpr - 1) / wpr;
     v0 = (int64_t)seg * per;
@@ -182,28 +198,79 @@ struct Resident {
       const int n32 = (int)n, ld32 = (int)ldS;
       for (int b = 0; b < B; ++b) {
         const double* src = yin + (int64_t)b * 3 * n;
-        double yv[3][kColQ];
+        for (int q0 = 0; q0 == 0 || (STREAM && q0 * kResThreads < n32); q0 += kColQ) {  // (one pass unless STREAM and n > 1,280)
+          double yv[3][kColQ];
 #pragma unroll
-        for (int c = 0; c < 3; ++c)
+          for (int c = 0; c < 3; ++c)
 #pragma unroll
-          for (int q = 0; q < kColQ; ++q) {
-            const int j = tid + q * kResThreads;
-            yv[c][q] = j < n32 ? __ldcg(src + c * n32 + j) : 0.0;
-          }
-#pragma unroll
-        for (int c = 0; c < 3; ++c)
-#pragma unroll
-          for (int q = 0; q < kColQ; ++q) {
-            const int j = tid + q * kResThreads;
-            if (j < n32) {
-              ysh[(b * 3 + c) * n32 + j] = yv[c][q];
-              Ms_[(b * 3 + c) * ld32 + j] = (T)(msj[q] * yv[c][q]);
+            for (int q = 0; q < kColQ; ++q) {
+              const int j = tid + (q0 + q) * kResThreads;
+              yv[c][q] = j < n32 ? __ldcg(src + c * n32 + j) : 0.0;
             }
-          }
+#pragma unroll
+          for (int c = 0; c < 3; ++c)
+#pragma unroll
+            for (int q = 0; q < kColQ; ++q) {
+              const int j = tid + (q0 + q) * kResThreads;
+              if (j < n32) {
+                ysh[(b * 3 + c) * n32 + j] = yv[c][q];
+                Ms_[(b * 3 + c) * ld32 + j] = (T)((STREAM ? Mss[j] : msj[q]) * yv[c][q]);
+              }
+            }
+        }
       }
     }
     __syncthreads();
-    if (row < rows) {
+    if constexpr (STREAM) {
+      // the CTA's rows one after the other, every warp an eighth of the columns; the row comes from L2
+      // (read-only for the kernel: non-coherent loads), columns >= n of its last vector read as zero
+      const int nv32 = (int)nv, v0i = (int)v0, v1i = (int)v1;
+      const int64_t plane = n * ldg;
+      const int per_round = kResWarps / wpr;  // rows in flight: wpr warps stream one row, each its share of the columns
+      const int64_t pv = plane / W;           // vectors per plane
+      for (int r = row; r < rows; r += per_round) {
+        const V* g = reinterpret_cast<const V*>(Ng + (r0 + r) * ldg);
+        for (int b0 = 0; b0 < B; b0 += 4) {
+          T acc[4][3];
+#pragma unroll
+          for (int bb = 0; bb < 4; ++bb) acc[bb][0] = acc[bb][1] = acc[bb][2] = T(0);
+#pragma unroll kStreamUnroll
+          for (int v = v0i + lane; v < v1i; v += 32) {
+            V t[6];
+#pragma unroll
+            for (int c = 0; c < 6; ++c) t[c] = __ldg(g + c * pv + v);
+            if (v == nv32 - 1) {
+#pragma unroll
+              for (int c = 0; c < 6; ++c) t[c] = zero_from(t[c], (int64_t)v * W, n);
+            }
+#pragma unroll
+            for (int bb = 0; bb < 4; ++bb)
+              if (b0 + bb < B) {
+                const V* Mb = Msh + (b0 + bb) * 3 * nv32;
+                V m[3];
+#pragma unroll
+                for (int c = 0; c < 3; ++c) m[c] = Mb[c * nv32 + v];
+                vec3(acc[bb], t, m);
+              }
+          }
+#pragma unroll
+          for (int bb = 0; bb < 4; ++bb)
+            if (b0 + bb < B) {
+              double d[3] = {(double)acc[bb][0], (double)acc[bb][1], (double)acc[bb][2]};
+#pragma unroll
+              for (int c = 0; c < 3; ++c)
+#pragma unroll
+                for (int off = 16; off > 0; off >>= 1) d[c] += __shfl_xor_sync(0xffffffffu, d[c], off);
+              if (lane == 0) {
+                double* o = red + (((int64_t)(b0 + bb) * R + r) * kResWarps + (warp % wpr)) * 3;
+                o[0] = d[0];
+                o[1] = d[1];
+                o[2] = d[2];
+              }
+            }
+        }
+      }
+    } else if (row < rows) {
       // up to four states per pass over the row: the tensor's shared-memory rows are read once per pass
       const int nv32 = (int)nv, v0i = (int)v0, v1i = (int)v1;
       for (int b0 = 0; b0 < B; b0 += 4) {
@@ -246,7 +313,7 @@ struct Resident {
     // H_d = -N.M, the warps' column parts added in warp order
     double H[3] = {0.0, 0.0, 0.0};
     for (int w = 0; w < wpr; ++w) {
-      const double* o = red + ((int64_t)eb * kResWarps + er * wpr + w) * 3;
+      const double* o = red + (STREAM ? ((int64_t)eb * R + er) * kResWarps + w : (int64_t)eb * kResWarps + er * wpr + w) * 3;
 #pragma unroll
       for (int c = 0; c < 3; ++c) H[c] += o[c];
     }
@@ -299,10 +366,10 @@ __device__ __forceinline__ void renormalise(double yo[3]) {
   }
 }
 
-template <typename T>
+template <typename T, bool STREAM>
 __global__ void __launch_bounds__(kResThreads, 1) rk4_resident_kernel(const __grid_constant__ ResArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  Resident<T> rs;
+  Resident<T, STREAM> rs;
   rs.init(smem_raw, a.N, a.n, a.ld, a.ldS, a.R, a.wpr, a.batch, a.prob);
   const EpiArgs& e = a.prob;
   double base[3] = {0.0, 0.0, 0.0}, ks[3][3];
@@ -387,11 +454,11 @@ __device__ const double kDpE[7] = {35.0 / 384 - 5179.0 / 57600,       0.0,
                                    -2187.0 / 6784 + 92097.0 / 339200, 11.0 / 84 - 187.0 / 2100,
                                    -1.0 / 40};
 
-template <typename T>
+template <typename T, bool STREAM>
 __global__ void __launch_bounds__(kResThreads, 1) dp45_resident_kernel(const __grid_constant__ DpResArgs a) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
   __shared__ DpState S;
-  Resident<T> rs;
+  Resident<T, STREAM> rs;
   rs.init(smem_raw, a.N, a.n, a.ld, a.ldS, a.R, a.wpr, a.batch, a.prob);
   const EpiArgs& e = a.prob;
   const int64_t n = a.n;
@@ -536,14 +603,25 @@ __global__ void __launch_bounds__(kResThreads, 1) dp45_resident_kernel(const __g
   if (blockIdx.x == 0 && threadIdx.x == 0) *a.S = S;
 }
 
-size_t resident_smem(int dtype, int64_t n, int R, int batch, size_t extra, int64_t* ldS_out) {
+size_t resident_smem(int dtype, int64_t n, int R, int batch, size_t extra, bool stream, int64_t* ldS_out) {
   const int64_t W = dtype == MT_F32 ? 4 : 2;
   const size_t sz = dtype == MT_F32 ? 4 : 8;
   const int64_t ldS = (n + W - 1) / W * W;
   if (ldS_out) *ldS_out = ldS;
+  if (stream)  // Msh | ysh | Mss | red[B][R][8][3]
+    return (size_t)batch * 3 * ldS * sz + ((size_t)batch * 3 + 1) * n * sizeof(double) +
+           (size_t)batch * R * kResWarps * 3 * sizeof(double) + extra;
   return ((size_t)R * 6 + (size_t)batch * 3) * ldS * sz + (size_t)batch * 3 * n * sizeof(double) +
          (size_t)batch * kResWarps * 3 * sizeof(double) + extra;
 }
+// Rows read from L2: one warp per row keeps the longest streams in flight; two warps per row when that takes fewer
+// rounds of eight warps (9..12 rows: 3 half-rounds instead of 2 rounds).  Four and eight warps per row measured slower.
+inline int stream_wpr(int R) {
+  const int rounds1 = (R + kResWarps - 1) / kResWarps, rounds2 = (R + kResWarps / 2 - 1) / (kResWarps / 2);
+  return rounds2 < 2 * rounds1 ? 2 : 1;
+}
+constexpr int kStreamMaxRows = 32;                      // rows per CTA when the tensor is read from L2 at every stage
+constexpr size_t kStreamMaxBytes = (size_t)100 << 20;   // ... which pays while the tensor stays in the 126 MB L2
 constexpr size_t kDpExtra = 2 * kResThreads * sizeof(double);  // the sample's reduction tree
 constexpr size_t kDpStatic = 1024;                             // the CTA's copy of the controller state
 
@@ -552,20 +630,29 @@ static_assert(sizeof(DpState) <= kDpStatic, "static shared memory of the DP45 ke
 
 }  // namespace
 
-// Can the dense n x n tensor of this dtype stay resident in shared memory across the GPU (one CTA per SM,
-// ceil(n / SMs) <= 8 rows each) together with `batch` stage states?  method: MT_RK4 or MT_DP45.
-bool mt_resident_fits(mt_ctx* ctx, int dtype, int64_t n, int batch, int method) {
-  if (n <= 0 || n > kColQ * kResThreads || batch < 1 || batch > MT_MAX_BATCH) return false;
-  const int R = (int)((n + ctx->num_sms - 1) / ctx->num_sms);
-  if (R > kResWarps || R * batch > kResThreads) return false;
+// How can the integrators keep the dense n x n tensor of this dtype on the chip?  MT_RES_SMEM: resident in shared
+// memory across the GPU (one CTA per SM, ceil(n / SMs) <= 8 rows each) together with `batch` stage states;
+// MT_RES_L2: too large for that but at most 100 MB, read from L2 at every stage by a persistent kernel of the same
+// structure (<= 32 rows per CTA); MT_RES_NONE otherwise.  method: MT_RK4 or MT_DP45.
+int mt_resident_fits(mt_ctx* ctx, int dtype, int64_t n, int64_t ld, int batch, int method) {
+  if (n <= 0 || batch < 1 || batch > MT_MAX_BATCH) return MT_RES_NONE;
   int dev_smem = 0, coop = 0;
   if (cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->device) != cudaSuccess ||
       cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, ctx->device) != cudaSuccess || !coop) {
     cudaGetLastError();
-    return false;
+    return MT_RES_NONE;
   }
+  const int R = (int)((n + ctx->num_sms - 1) / ctx->num_sms);
   const size_t extra = method == MT_DP45 ? kDpExtra + kDpStatic : 0;
-  return resident_smem(dtype, n, R, batch, extra, nullptr) <= (size_t)dev_smem;
+  if (R * batch > kResThreads) return MT_RES_NONE;
+  if (n <= kColQ * kResThreads && R <= kResWarps &&
+      resident_smem(dtype, n, R, batch, extra, false, nullptr) <= (size_t)dev_smem)
+    return MT_RES_SMEM;
+  const size_t bytes = 6 * (size_t)n * (size_t)ld * (dtype == MT_F32 ? 4 : 8);
+  if (R <= kStreamMaxRows && bytes <= kStreamMaxBytes &&
+      resident_smem(dtype, n, R, batch, extra, true, nullptr) <= (size_t)dev_smem)
+    return MT_RES_L2;
+  return MT_RES_NONE;
 }
 
 static int launch_cooperative(mt_ctx* ctx, const void* fn, unsigned grid, size_t smem, void* arg) {
@@ -582,7 +669,7 @@ static int launch_cooperative(mt_ctx* ctx, const void* fn, unsigned grid, size_t
 }
 
 // `count` RK4 steps of m (in place); ya, yb: two scratch states [B][3][n]; `prob`: fill_problem's constants.
-int mt_launch_rk4_resident(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t ld, const EpiArgs& prob,
+int mt_launch_rk4_resident(mt_ctx* ctx, int mode, const void* N, int dtype, int64_t n, int64_t ld, const EpiArgs& prob,
                            double* m, double* ya, double* yb, double dt, int renorm,
                            unsigned long long* tq_slots, unsigned int* bar, int64_t count) {
   if (count <= 0) return MT_OK;
@@ -604,16 +691,20 @@ int mt_launch_rk4_resident(mt_ctx* ctx, const void* N, int dtype, int64_t n, int
   a.y_in[2] = yb; a.y_to[2] = ya; a.h[2] = dt;
   a.y_in[3] = ya; a.y_to[3] = m;  a.h[3] = dt / 6.0;
   a.prob = prob;
-  const size_t smem = resident_smem(dtype, n, a.R, a.batch, 0, &a.ldS);
+  const bool stream = mode == MT_RES_L2;
+  if (stream) a.wpr = stream_wpr(a.R);
+  const size_t smem = resident_smem(dtype, n, a.R, a.batch, 0, stream, &a.ldS);
   if (a.ldS > ld) return mt_fail(ctx, MT_ERR_INVALID_ARG, "resident RK4: ld must cover whole 16-byte vectors");
-  const void* fn = dtype == MT_F32 ? (const void*)rk4_resident_kernel<float> : (const void*)rk4_resident_kernel<double>;
+  const void* fn = dtype == MT_F32
+                       ? (stream ? (const void*)rk4_resident_kernel<float, true> : (const void*)rk4_resident_kernel<float, false>)
+                       : (stream ? (const void*)rk4_resident_kernel<double, true> : (const void*)rk4_resident_kernel<double, false>);
   MT_CUDA_OK(ctx, cudaMemsetAsync(bar, 0, sizeof(unsigned int), ctx->stream));
   return launch_cooperative(ctx, fn, (unsigned)((n + a.R - 1) / a.R), smem, &a);
 }
 
 // Up to `attempts` attempted DP45 steps of m (in place) under the controller state S (device); k1 holds
 // f(m) on entry and the FSAL slope of the state on exit; words: 4 device words, bar: 1 (zeroed here).
-int mt_launch_dp45_resident(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t ld, const EpiArgs& prob,
+int mt_launch_dp45_resident(mt_ctx* ctx, int mode, const void* N, int dtype, int64_t n, int64_t ld, const EpiArgs& prob,
                             DpState* S, double* m, double* k1, double* ya, double* yb, int renorm,
                             double* samples, int64_t stride, const double* vol, unsigned long long* words,
                             unsigned int* bar, int attempts) {
@@ -640,9 +731,13 @@ int mt_launch_dp45_resident(mt_ctx* ctx, const void* N, int dtype, int64_t n, in
   a.stride = stride;
   a.vol = vol;
   a.prob = prob;
-  const size_t smem = resident_smem(dtype, n, a.R, a.batch, kDpExtra, &a.ldS);
+  const bool stream = mode == MT_RES_L2;
+  if (stream) a.wpr = stream_wpr(a.R);
+  const size_t smem = resident_smem(dtype, n, a.R, a.batch, kDpExtra, stream, &a.ldS);
   if (a.ldS > ld) return mt_fail(ctx, MT_ERR_INVALID_ARG, "resident DP45: ld must cover whole 16-byte vectors");
-  const void* fn = dtype == MT_F32 ? (const void*)dp45_resident_kernel<float> : (const void*)dp45_resident_kernel<double>;
+  const void* fn = dtype == MT_F32
+                       ? (stream ? (const void*)dp45_resident_kernel<float, true> : (const void*)dp45_resident_kernel<float, false>)
+                       : (stream ? (const void*)dp45_resident_kernel<double, true> : (const void*)dp45_resident_kernel<double, false>);
   MT_CUDA_OK(ctx, cudaMemsetAsync(bar, 0, sizeof(unsigned int), ctx->stream));
   MT_CUDA_OK(ctx, cudaMemsetAsync(words, 0, 4 * sizeof(unsigned long long), ctx->stream));
   return launch_cooperative(ctx, fn, (unsigned)((n + a.R - 1) / a.R), smem, &a);

@@ -244,3 +244,36 @@ def test_resident_tiny_problems_with_padded_rows(ctx, oracle, grid, dtype):
         assert np.isfinite(m2).all() and r1["n_samples"] == r2["n_samples"] == 4
         assert (r1["accepted"], r1["rejected"]) == (r2["accepted"], r2["rejected"])
         assert np.max(np.abs(m2 - m1)) < tol and np.max(np.abs(s2 - s1)) < tol
+
+
+@pytest.mark.parametrize("grid,dtype,batch", [((40, 30, 1), "f32", 1), ((30, 30, 1), "f64", 2), ((11, 11, 11), "f32", 3)])
+def test_l2_streamed_persistent_kernel_equals_staged_launches(ctx, oracle, grid, dtype, batch):
+    """Tensors too large for shared memory but at most 100 MB (1,200 / 1,331 tiles fp32, 900 tiles fp64) run the same
+    persistent kernels with the rows read from L2 at every stage: RK4 and DP45 against the per-stage launches, with
+    NaN in the row padding, odd n (1,331: ragged last vector) and batches."""
+    nx, ny, nz = grid
+    w = W.config2(nx, ny, batch=batch, phase="dynamics") if nz == 1 else W.config3(nx, batch=batch, dtype=dtype)
+    n = w.n
+    tiles = H.dev_tiles(w)
+    ld = W.leading_dim(n, dtype) + 4
+    N, ld, status = H.assemble(ctx, tiles, dtype, ld=ld)
+    assert status == 0
+    N[:, :, n:] = float("nan")
+    prob = H.dev_problem(w, tiles, N, dtype, ld)
+    film = nz == 1
+    rk = dict(method=B.MT_RK4, dt=1e-13 if film else 0.005, sample_every=10, sample_cap=8)
+    rk["t_end"] = 40 * rk["dt"]
+    dp = dict(method=B.MT_DP45, dt=1e-13 if film else 1e-3, rtol=1e-6, atol=1e-8, sample_cap=8)
+    dp["t_end"], dp["sample_dt"] = (40e-13, 10e-13) if film else (0.2, 0.05)
+    tol = 1e-11 if dtype == "f64" else 2e-5
+    for kw in (rk, dp):
+        out = {}
+        for mode in (1, 2):
+            B.mt_set_resident_mode(ctx, mode)
+            l0 = B.mt_launch_count(ctx)
+            out[mode] = run_gpu_integrate(ctx, prob, w.m, batch, **kw) + (B.mt_launch_count(ctx) - l0,)
+        (m1, s1, r1, _, n1), (m2, s2, r2, _, n2) = out[1], out[2]
+        assert np.isfinite(m2).all() and r1["n_samples"] == r2["n_samples"] == 4
+        assert (r1["accepted"], r1["rejected"]) == (r2["accepted"], r2["rejected"]) and r2["accepted"] >= 4
+        assert np.max(np.abs(m2 - m1)) < tol and np.max(np.abs(s2[:, 1:] - s1[:, 1:])) < tol
+        assert n2 <= 12 and n2 < n1 / 8  # a handful of cooperative launches against several per right-hand side
