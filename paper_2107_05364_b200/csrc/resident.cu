@@ -621,7 +621,10 @@ inline int stream_wpr(int R) {
   return rounds2 < 2 * rounds1 ? 2 : 1;
 }
 constexpr int kStreamMaxRows = 32;                      // rows per CTA when the tensor is read from L2 at every stage
-constexpr size_t kStreamMaxBytes = (size_t)100 << 20;   // ... which pays while the tensor stays in the 126 MB L2
+#ifndef MT_STREAM_MAX_MB
+#define MT_STREAM_MAX_MB 100
+#endif
+constexpr size_t kStreamMaxBytes = (size_t)MT_STREAM_MAX_MB << 20;   // ... which pays while the tensor stays in the 126 MB L2
 constexpr size_t kDpExtra = 2 * kResThreads * sizeof(double);  // the sample's reduction tree
 constexpr size_t kDpStatic = 1024;                             // the CTA's copy of the controller state
 
