@@ -767,14 +767,19 @@ def integrators_small_n(R):
     from tests import harness as H
     B, ctx, dev = R.B, R.ctx, R.dev
     res_all = {}
-    for cfg in (1, 2):
-        w, name, dtype = config_workload(cfg, batch=1)
+    # configs 1 and 2, and config 2's film at the 80 x 20 resolution (the paper's SP4 grid at n = 4, PAPER.md:209:
+    # 1,600 tiles, 61 MB: fits in L2 but not in shared memory -> the persistent kernel with rows read from L2)
+    for cfg in (1, 2, "film_80x20"):
+        if cfg == "film_80x20":
+            w, name, dtype = W.config2(80, 20, batch=1), "config 2 physics on 80x20x1 tiles, fp32 tensor 61 MB", "f32"
+        else:
+            w, name, dtype = config_workload(cfg, batch=1)
         n, code = w.n, H.dtype_code(dtype)
         tiles = H.dev_tiles(w, dev)
         ld = W.leading_dim(n, dtype)
         N, _, _ = R.assemble(tiles, code, 0, n, ld)
         prob = H.dev_problem(w, tiles, N, dtype, ld)
-        dt = float(w.extra["dt"]) if cfg == 2 else 1e-2
+        dt = float(w.extra["dt"]) if cfg != 1 else 1e-2
         m = torch.from_numpy(w.m[:1].copy()).to(dev)
         entry = {"n": n}
         # mode 1: the per-stage launches replayed from a CUDA graph; mode 0: the default, which at config 1
@@ -788,8 +793,8 @@ def integrators_small_n(R):
         B.mt_set_resident_mode(ctx, 0)
         # long enough that the one-off graph capture of the device-controlled run is amortised (config 1 has
         # no exchange term: a tight tolerance keeps the steps short)
-        t_end = 400 * dt if cfg == 2 else 60.0
-        rtol, atol = (1e-6, 1e-8) if cfg == 2 else (1e-10, 1e-12)
+        t_end = 400 * dt if cfg != 1 else 60.0
+        rtol, atol = (1e-6, 1e-8) if cfg != 1 else (1e-10, 1e-12)
         # host controller / device controller with the attempt replayed from a CUDA graph / the default: where the
         # tensor fits in shared memory (config 1), controller and stages inside one cooperative kernel
         for mode, resm, key in ((1, 1, "dp45_host_controller"), (2, 1, "dp45_device_controller"), (0, 0, "dp45")):
@@ -802,8 +807,11 @@ def integrators_small_n(R):
                           "us_per_rhs": 1e3 * ms / max(1, r["rhs_calls"])}
         B.mt_set_step_control(ctx, 0)
         B.mt_set_resident_mode(ctx, 0)
-        entry["resident"] = bool(n <= 1024)  # (what mt_integrate chose by itself: see mt_set_resident_mode)
-        res_all[f"config{cfg}"] = entry
+        # (what mt_integrate chose by itself in the default mode: see mt_set_resident_mode)
+        entry["default_path"] = ("tensor resident in shared memory" if n <= 1024 else
+                                 "persistent kernel, rows read from L2" if 6.0 * n * ld * (4 if dtype == "f32" else 8) <= 100 * 2**20
+                                 else "per-stage launches (CUDA graph)")
+        res_all[f"config{cfg}" if cfg != "film_80x20" else cfg] = entry
         del N, prob
         torch.cuda.empty_cache()
     return res_all
