@@ -105,7 +105,7 @@ __device__ __forceinline__ void grid_barrier(unsigned int* ctr, unsigned int tar
 //   STREAM = false (tensor resident in shared memory):
 //     tens[R][6][ldS] T | Msh[B][3][ldS] T | ysh[B][3][n] double | red[B][8][3] double | extra
 //   STREAM = true (tensor too large for shared memory but small enough for L2: the rows are read from L2 at every
-//   stage by all eight warps, one row after the other; nothing else changes):
+//   stage, one or two warps per row, kResWarps / wpr rows at a time; nothing else changes):
 //     Msh[B][3][ldS] T | ysh[B][3][n] double | Mss[n] double | red[B][R][8][3] double | extra
 template <typename T, bool STREAM>
 struct Resident {
@@ -222,8 +222,9 @@ struct Resident {
     }
     __syncthreads();
     if constexpr (STREAM) {
-      // the CTA's rows one after the other, every warp an eighth of the columns; the row comes from L2
-      // (read-only for the kernel: non-coherent loads), columns >= n of its last vector read as zero
+      // kResWarps / wpr of the CTA's rows at a time, wpr (1 or 2) warps per row; the row comes from L2 (read-only
+      // for the kernel: non-coherent loads), columns >= n of its last vector read as zero.  fp32: a lane's partial
+      // sum covers at most 4 * ceil(n / 128) <= 68 terms at the 100 MB limit (Q19 allows 128)
       const int nv32 = (int)nv, v0i = (int)v0, v1i = (int)v1;
       const int64_t plane = n * ldg;
       const int per_round = kResWarps / wpr;  // rows in flight: wpr warps stream one row, each its share of the columns
