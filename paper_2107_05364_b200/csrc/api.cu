@@ -313,10 +313,6 @@ int mt_demag_field(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_r
   if (batch < 1 || batch > MT_MAX_BATCH) return mt_fail(ctx, MT_ERR_INVALID_ARG, "batch must be in [1, %d]", MT_MAX_BATCH);
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
   const int64_t npad = round_up(n, MT_COL_CHUNK);
-  rc = ensure_Mst(ctx, dtype, batch, npad);
-  if (rc) return rc;
-  rc = mt_launch_stage_M(ctx, dtype, Ms, m, batch, n, npad, ctx->Mst[0]);
-  if (rc) return rc;
   EpiArgs e;
   memset(&e, 0, sizeof(e));
   e.mode = 0;
@@ -324,6 +320,13 @@ int mt_demag_field(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_r
   e.n = n;
   e.n_rows = n_rows;
   e.Hd = Hd;
+  // small problems: one launch, the field kernel forms Ms*m itself (same bits as the staged M)
+  if (mt_demag_can_fuse(ctx, dtype, n, n_rows, Ms, m))
+    return mt_launch_demag(ctx, N, dtype, n, n_rows, ld, nullptr, npad, e, Ms, m);
+  rc = ensure_Mst(ctx, dtype, batch, npad);
+  if (rc) return rc;
+  rc = mt_launch_stage_M(ctx, dtype, Ms, m, batch, n, npad, ctx->Mst[0]);
+  if (rc) return rc;
   return mt_launch_demag(ctx, N, dtype, n, n_rows, ld, ctx->Mst[0], npad, e);
 }
 
@@ -354,17 +357,20 @@ int mt_llg_rhs(mt_ctx* ctx, const mt_problem* p, const double* m, int batch, dou
   if (!m || !dmdt) return mt_fail(ctx, MT_ERR_INVALID_ARG, "m and dmdt must be non-NULL");
   MT_CUDA_OK(ctx, cudaSetDevice(ctx->device));
   const int64_t npad = round_up(p->n, MT_COL_CHUNK);
+  EpiArgs e;
+  fill_problem(e, p, batch);
+  e.y = m;
+  e.k_out = dmdt;
+  e.heff_out = Heff;
+  // small dense problems: one launch, the field kernel forms Ms*m itself (same bits as the staged M)
+  if (p->N && !p->N_sparse && !p->N_sym && mt_demag_can_fuse(ctx, p->dtype, p->n, e.n_rows, p->Ms, m))
+    return mt_launch_demag(ctx, p->N, p->dtype, p->n, e.n_rows, p->ld, nullptr, npad, e, p->Ms, m);
   if (has_demag(p)) {
     rc = ensure_Mst(ctx, demag_dtype(p), batch, npad);
     if (rc) return rc;
     rc = mt_launch_stage_M(ctx, demag_dtype(p), p->Ms, m, batch, p->n, npad, ctx->Mst[0]);
     if (rc) return rc;
   }
-  EpiArgs e;
-  fill_problem(e, p, batch);
-  e.y = m;
-  e.k_out = dmdt;
-  e.heff_out = Heff;
   return eval_rhs(ctx, p, npad, 0, e);
 }
 

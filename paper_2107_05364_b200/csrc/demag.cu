@@ -90,12 +90,32 @@ struct DemagArgs {
   int64_t vec_per_split;         // full vectors per column split
   int nsplit;
   double* partial;               // [nsplit][B][3][n_rows] when nsplit > 1
+  const double* Ms;              // FUSE: M is formed on the fly as (T)(Ms[j] * y[b][c][j]) — the same expression,
+  const double* y;               // hence the same bits, as stage_M_kernel's — instead of read from the staged M
 };
+
+// FUSE: the 16 bytes of M a lane needs, from Ms and the state (n a multiple of the vector width: no tail)
+__device__ __forceinline__ void fused_ms(const double* Ms, int64_t v, double (&ms)[4]) {
+  const double2 a = __ldg(reinterpret_cast<const double2*>(Ms) + 2 * v), b = __ldg(reinterpret_cast<const double2*>(Ms) + 2 * v + 1);
+  ms[0] = a.x; ms[1] = a.y; ms[2] = b.x; ms[3] = b.y;
+}
+__device__ __forceinline__ void fused_ms(const double* Ms, int64_t v, double (&ms)[2]) {
+  const double2 a = __ldg(reinterpret_cast<const double2*>(Ms) + v);
+  ms[0] = a.x; ms[1] = a.y;
+}
+__device__ __forceinline__ float4 fused_m(const double* yrow, int64_t v, const double (&ms)[4]) {
+  const double2 a = __ldg(reinterpret_cast<const double2*>(yrow) + 2 * v), b = __ldg(reinterpret_cast<const double2*>(yrow) + 2 * v + 1);
+  return make_float4((float)(ms[0] * a.x), (float)(ms[1] * a.y), (float)(ms[2] * b.x), (float)(ms[3] * b.y));
+}
+__device__ __forceinline__ double2 fused_m(const double* yrow, int64_t v, const double (&ms)[2]) {
+  const double2 a = __ldg(reinterpret_cast<const double2*>(yrow) + v);
+  return make_double2(ms[0] * a.x, ms[1] * a.y);
+}
 
 constexpr int kWarps = 8;
 constexpr int kFlush = 8;  // fp32: vector iterations per fp32 run
 
-template <typename T, int B>
+template <typename T, int B, bool FUSE>
 __global__ void __launch_bounds__(kWarps * 32) demag_ldg_kernel(DemagArgs<T> a, EpiArgs e) {
   typedef typename VecOf<T>::type V;
   constexpr int W = VecOf<T>::W;
@@ -128,11 +148,16 @@ __global__ void __launch_bounds__(kWarps * 32) demag_ldg_kernel(DemagArgs<T> a, 
         V t[6];
 #pragma unroll
         for (int c = 0; c < 6; ++c) t[c] = ld_stream(p[c] + v);
+        double ms[W];
+        if constexpr (FUSE) fused_ms(a.Ms, v, ms);
 #pragma unroll
         for (int b = 0; b < B; ++b) {
           V m[3];
 #pragma unroll
-          for (int c = 0; c < 3; ++c) m[c] = __ldg(mp + (b * 3 + c) * mstride + v);
+          for (int c = 0; c < 3; ++c) {
+            if constexpr (FUSE) m[c] = fused_m(a.y + (int64_t)(b * 3 + c) * a.n, v, ms);
+            else m[c] = __ldg(mp + (b * 3 + c) * mstride + v);
+          }
           vec_fma(run[b], t, m);
         }
       }
@@ -359,7 +384,8 @@ __global__ void energy_total_kernel(int batch, double* __restrict__ out) {
 template <typename T, int B>
 int launch_ldg_T(mt_ctx* ctx, const DemagArgs<T>& a, const EpiArgs& e) {
   dim3 grid((unsigned)((a.n_rows + kWarps - 1) / kWarps), (unsigned)a.nsplit);
-  demag_ldg_kernel<T, B><<<grid, kWarps * 32, 0, ctx->stream>>>(a, e);
+  if (a.y) demag_ldg_kernel<T, B, true><<<grid, kWarps * 32, 0, ctx->stream>>>(a, e);
+  else demag_ldg_kernel<T, B, false><<<grid, kWarps * 32, 0, ctx->stream>>>(a, e);
   ctx->launches++;
   MT_CUDA_OK(ctx, cudaGetLastError());
   if (a.nsplit > 1) {
@@ -373,7 +399,7 @@ int launch_ldg_T(mt_ctx* ctx, const DemagArgs<T>& a, const EpiArgs& e) {
 
 template <typename T>
 int launch_ldg(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld, const void* Mst,
-               int64_t npad, const EpiArgs& e) {
+               int64_t npad, const EpiArgs& e, const double* Ms_fuse, const double* y_fuse) {
   constexpr int W = VecOf<T>::W;
   DemagArgs<T> a;
   a.N = (const T*)N;
@@ -383,6 +409,8 @@ int launch_ldg(mt_ctx* ctx, const void* N, int64_t n, int64_t n_rows, int64_t ld
   a.plane = n_rows * ld;
   a.M = (const T*)Mst;
   a.npad = npad;
+  a.Ms = Ms_fuse;
+  a.y = y_fuse;
   // split the columns when the rows alone cannot fill the machine twice over
   const int64_t ctas = (n_rows + kWarps - 1) / kWarps;
   const int64_t want = 2LL * ctx->num_sms;
@@ -436,21 +464,35 @@ int mt_launch_stage_M(mt_ctx* ctx, int dtype, const double* Ms, const double* m,
 }
 
 static int launch_demag_variant(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
-                                const void* Mst, int64_t npad, const EpiArgs& epi) {
+                                const void* Mst, int64_t npad, const EpiArgs& epi, const double* Ms_fuse,
+                                const double* y_fuse) {
+  if (y_fuse) {  // the caller checked mt_demag_can_fuse: register-streaming kernel, M formed on the fly
+    if (dtype == MT_F32) return launch_ldg<float>(ctx, N, n, n_rows, ld, nullptr, npad, epi, Ms_fuse, y_fuse);
+    return launch_ldg<double>(ctx, N, n, n_rows, ld, nullptr, npad, epi, Ms_fuse, y_fuse);
+  }
   if (ctx->variant != 1) {
     int rc = mt_launch_demag_tma(ctx, N, dtype, n, n_rows, ld, Mst, npad, epi);
     if (rc != MT_ERR_UNIMPLEMENTED) return rc;
     if (ctx->variant >= 2) return rc;
   }
-  if (dtype == MT_F32) return launch_ldg<float>(ctx, N, n, n_rows, ld, Mst, npad, epi);
-  return launch_ldg<double>(ctx, N, n, n_rows, ld, Mst, npad, epi);
+  if (dtype == MT_F32) return launch_ldg<float>(ctx, N, n, n_rows, ld, Mst, npad, epi, nullptr, nullptr);
+  return launch_ldg<double>(ctx, N, n, n_rows, ld, Mst, npad, epi, nullptr, nullptr);
+}
+
+// Small problems (the register-streaming kernel's range) with n a multiple of the 16-byte vector: the field
+// kernel can form Ms*m itself — one launch per call instead of two (staging + field), same bits.
+bool mt_demag_can_fuse(mt_ctx* ctx, int dtype, int64_t n, int64_t n_rows, const double* Ms, const double* y) {
+  const int64_t W = dtype == MT_F32 ? 4 : 2;
+  if (n % W || ((uintptr_t)Ms & 15) || ((uintptr_t)y & 15) || (n & 1)) return false;
+  if (ctx->variant != 0) return false;  // (a forced variant keeps the staged M: mt_set_demag_variant(ctx, 1) is the A/B)
+  return !mt_demag_tma_takes(ctx, dtype, n, n_rows);
 }
 
 int mt_launch_demag(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
-                    const void* Mst, int64_t npad, const EpiArgs& epi) {
+                    const void* Mst, int64_t npad, const EpiArgs& epi, const double* Ms_fuse, const double* y_fuse) {
   const bool prof = ctx->prof_on && ctx->prof_ev && ctx->prof_count < MT_PROF_CAP;
   if (prof) MT_CUDA_OK(ctx, cudaEventRecord(ctx->prof_ev[2 * ctx->prof_count], ctx->stream));
-  const int rc = launch_demag_variant(ctx, N, dtype, n, n_rows, ld, Mst, npad, epi);
+  const int rc = launch_demag_variant(ctx, N, dtype, n, n_rows, ld, Mst, npad, epi, Ms_fuse, y_fuse);
   if (prof) {
     MT_CUDA_OK(ctx, cudaEventRecord(ctx->prof_ev[2 * ctx->prof_count + 1], ctx->stream));
     ctx->prof_count++;

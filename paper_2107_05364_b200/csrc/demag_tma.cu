@@ -1057,13 +1057,17 @@ int launch_T(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, i
 
 }  // namespace
 
+bool mt_demag_tma_takes(mt_ctx* ctx, int dtype, int64_t n, int64_t n_rows) {
+  const int64_t tiles = ((n_rows + 7) / 8) * ((n * (dtype == MT_F32 ? 4 : 8) + 1023) / 1024);
+  return tiles >= MT_TMA_MIN_TILES_PER_SM * ctx->num_sms;
+}
+
 // Returns MT_ERR_UNIMPLEMENTED when the shape is better served by the register-streaming kernel
 // (too few tiles to give every SM a share); the dispatcher then falls back to it.
 int mt_launch_demag_tma(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
                         const void* Mst, int64_t npad, const EpiArgs& e) {
   if (ctx->variant < 2) {
-    const int64_t tiles = ((n_rows + 7) / 8) * ((n * (dtype == MT_F32 ? 4 : 8) + 1023) / 1024);
-    if (tiles < MT_TMA_MIN_TILES_PER_SM * ctx->num_sms) return MT_ERR_UNIMPLEMENTED;
+    if (!mt_demag_tma_takes(ctx, dtype, n, n_rows)) return MT_ERR_UNIMPLEMENTED;
   }
   if (dtype == MT_F32) return launch_T<float>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);
   return launch_T<double>(ctx, N, dtype, n, n_rows, ld, Mst, npad, e);

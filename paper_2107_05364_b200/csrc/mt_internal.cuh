@@ -156,8 +156,12 @@ int mt_launch_mean_cond(mt_ctx* ctx, const DpState* st, const double* m, const d
 // launchers (demag.cu)
 int mt_launch_stage_M(mt_ctx* ctx, int dtype, const double* Ms, const double* m, int batch, int64_t n,
                       int64_t npad, void* M_out);
+// Ms_fuse / y_fuse non-NULL (only after mt_demag_can_fuse said yes): Mst is not read, the kernel forms Ms*y itself
 int mt_launch_demag(mt_ctx* ctx, const void* N, int dtype, int64_t n, int64_t n_rows, int64_t ld,
-                    const void* Mst, int64_t npad, const EpiArgs& epi);
+                    const void* Mst, int64_t npad, const EpiArgs& epi, const double* Ms_fuse = nullptr,
+                    const double* y_fuse = nullptr);
+bool mt_demag_can_fuse(mt_ctx* ctx, int dtype, int64_t n, int64_t n_rows, const double* Ms, const double* y);
+bool mt_demag_tma_takes(mt_ctx* ctx, int dtype, int64_t n, int64_t n_rows);  // demag_tma.cu: the default choice by shape
 int mt_launch_local_only(mt_ctx* ctx, const EpiArgs& epi);  // N == NULL: H_d = 0
 // resident.cu: a chunk of RK4 steps in one cooperative launch, the dense tensor held in shared memory
 #define MT_RES_NONE 0

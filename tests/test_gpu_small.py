@@ -422,3 +422,28 @@ def test_dp45_nonfinite_state_is_an_error_and_zero_m_stays_zero(ctx):
         m, _, res, rc = run_gpu_integrate(ctx, prob, zero, 1, method=method, dt=1e-2, t_end=0.5)
         assert rc == 0 and np.all(m[0][:, 1] == 0.0) and np.all(np.isfinite(m))
         assert np.allclose(np.linalg.norm(m[0][:, [0, 2]], axis=0), 1.0, atol=1e-14)
+
+
+@pytest.mark.parametrize("dtype", ["f64", "f32"])
+def test_small_problem_field_in_one_launch_equals_staged_path_bitwise(ctx, cfg1, dtype):
+    """Where the register-streaming kernel is the default and n is a multiple of the 16-byte vector, mt_demag_field and
+    mt_llg_rhs form Ms*m inside the field kernel (one launch per call); forcing the same kernel with
+    mt_set_demag_variant(1) keeps the staging launch: the two agree to the bit (same expression for Ms*m)."""
+    w, _ = cfg1
+    tiles = H.dev_tiles(w)
+    N, ld, _ = H.assemble(ctx, tiles, dtype)
+    prob = H.dev_problem(w, tiles, N, dtype, ld)
+    m = torch.from_numpy(w.m).cuda()
+    out = {}
+    for variant in (0, 1):
+        B.mt_set_demag_variant(ctx, variant)
+        Hd, k = torch.empty_like(m), torch.empty_like(m)
+        l0 = B.mt_launch_count(ctx)
+        B.mt_demag_field(ctx, N, H.dtype_code(dtype), w.n, w.n, ld, tiles.Ms, m, m.shape[0], Hd)
+        l1 = B.mt_launch_count(ctx)
+        B.mt_llg_rhs(ctx, prob, m, m.shape[0], k, None)
+        torch.cuda.synchronize()
+        out[variant] = (Hd, k, l1 - l0, B.mt_launch_count(ctx) - l1)
+    B.mt_set_demag_variant(ctx, 0)
+    assert torch.equal(out[0][0], out[1][0]) and torch.equal(out[0][1], out[1][1])
+    assert out[0][2:] == (1, 1) and out[1][2:] == (2, 2)
